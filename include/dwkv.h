@@ -1,0 +1,172 @@
+/* dwkv.h -- C ABI of the B200-native DepthWeave-KV decode-attention hot path.
+ *
+ * The library computes decode-time softmax attention directly over the cross-layer low-rank KV cache of
+ * DepthWeave-KV (arxiv/paper_2607_06523) without materialising K-hat / V-hat ("reconstructed KV tensors are not
+ * written back to global memory").  Cache content follows PAPER.md:47-56, Eq. (1)
+ *     X-hat[l,h,t] = A[l,h,t] . B[m(l),h]  +  g . R[l,h,t]
+ * in the reading BASELINE.json `north_star` fixes (readings A1-A21):
+ *     K-hat[t,:] = gK[l,h,:] * ( sum_{j<r_t} cK[l,h,t,j] * BK[m(l),h,j,:] ) + f_t * deq(RK[l,h,t])      (same for V)
+ *     deq(R)[i]  = code[i] * scale[i/16]       int4 two's-complement codes, fp16 scale per group of 16 channels
+ *     m(l) = l / group_size ;  query head hq uses kv head hq / (n_q_heads / n_kv_heads)
+ *     o[hq,:] = sum_t softmax_t( q[hq,:] . K-hat[t,:] * softmax_scale ) * V-hat[t,:]
+ * Basis, coefficients, gates and q are bf16; accumulation is fp32; outputs are fp32.
+ *
+ * Conventions
+ *   - Every pointer argument is caller-owned.  "dev" = device pointer on cfg.device, "host" = host pointer.
+ *     The library copies what it keeps (basis, gates) and owns all cache pages.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls enqueue work and return;
+ *     host arrays are consumed before the call returns.  dwkv_decode_attention never synchronises the host
+ *     unless it has to grow a scratch buffer (first call / larger batch).
+ *   - Return value: 0 = DWKV_OK, negative = error (see enum).  No exceptions or aborts cross the ABI.
+ *     dwkv_last_error() returns a thread-local message for the last non-zero return.
+ *   - One cache per handle; a handle is not thread-safe.  seq_ids within one call must be distinct.
+ *   - Limits of this build: d_head in {64, 128}; tier ranks multiples of 8, ascending, last == basis rank <= 64;
+ *     n_q_heads / n_kv_heads <= 8.
+ */
+#ifndef DWKV_H_
+#define DWKV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DWKV_MAX_TIERS 4
+
+enum {
+  DWKV_OK = 0,
+  DWKV_E_INVALID = -1,  /* bad config / NULL pointer / tier >= n_tiers / bad layer or sequence id            */
+  DWKV_E_STATE = -2,    /* append before basis+gates set; basis or gates changed after tokens exist; bad gate  */
+  DWKV_E_CAPACITY = -3, /* sequence slots, tokens per sequence, or arena pages exhausted                       */
+  DWKV_E_EMPTY = -4,    /* decode on a sequence with no tokens (softmax over nothing); nothing is launched     */
+  DWKV_E_CUDA = -5      /* a CUDA runtime call failed; message in dwkv_last_error()                            */
+};
+
+typedef struct dwkv_cache dwkv_cache; /* opaque; owned by the library */
+
+typedef struct {
+  int32_t n_layers;                  /* L                                                                      */
+  int32_t group_size;                /* w layers per depth window; L % w == 0                    */
+  int32_t n_kv_heads;                /* H_kv                                                                   */
+  int32_t n_q_heads;                 /* H_q, multiple of H_kv, H_q / H_kv <= 8                                 */
+  int32_t d_head;                    /* 64 or 128                                                              */
+  int32_t n_tiers;                   /* 1..DWKV_MAX_TIERS rank tiers                                           */
+  int32_t tier_rank[DWKV_MAX_TIERS]; /* ascending, multiples of 8; tier_rank[n_tiers-1] == basis rank r        */
+  int32_t max_seqs;                  /* sequence slots: valid seq ids are 0..max_seqs-1                        */
+  int64_t max_tokens_per_seq;        /* capacity per sequence                                                  */
+  float softmax_scale;               /* 0 => 1/sqrt(d_head)  (reading A9)                                      */
+  int32_t device;                    /* CUDA device ordinal                                                    */
+  void* arena;                       /* optional caller-owned device memory for the cache pages (256-B aligned) */
+  uint64_t arena_bytes;              /* size of `arena`; if arena == NULL: bytes to cudaMalloc (0 => worst case) */
+} dwkv_config;
+
+/* Create a cache. *out receives the handle. Errors: INVALID (config), CUDA (allocation). */
+int dwkv_create(const dwkv_config* cfg, dwkv_cache** out);
+
+/* Free everything the library owns (synchronises the device first). dwkv_destroy(NULL) is a no-op. */
+void dwkv_destroy(dwkv_cache* c);
+
+/* Shared per-(depth window, head) channel bases B^K, B^V: dev bf16 [L/w, H_kv, r, d], rows assumed
+ * orthonormal, used as stored. Copied. Errors: STATE if any sequence already holds tokens (reading A19). */
+int dwkv_set_basis(dwkv_cache* c, const void* Bk, const void* Bv, void* stream);
+
+/* Per-layer per-channel gates (reading A8): dev bf16 [L, H_kv, d]. Copied. Synchronises `stream` to validate that
+ * every entry is finite and non-zero (STATE otherwise). STATE if any sequence already holds tokens. */
+int dwkv_set_gates(dwkv_cache* c, const void* gK, const void* gV, void* stream);
+
+/* Append/compress ("projecting the original cache vector onto the current basis"; readings A13, A14):
+ * for every new token, layer, kv head and Z in {K,V}:  c = bf16(B[:r_t] . (x / g));  if flagged, the residual
+ * e = x - g * (c . B[:r_t]) is quantised to int4 / group 16 / fp16 scale.  Entries go to the pages of class
+ * (tier, flag); slot = number of earlier tokens of the sequence in that class.
+ *   seq_ids, n_new : host int32 [n_seqs]      k_new, v_new : dev bf16 [sum(n_new), L, H_kv, d], sequences in call order
+ *   tier, flag     : host uint8 [sum(n_new)]  (tier index 0..n_tiers-1, residual flag 0/1)
+ * Errors: INVALID, STATE (basis/gates not set), CAPACITY (state is unchanged when CAPACITY is returned). */
+int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, const int32_t* n_new,
+                         const void* k_new, const void* v_new, const uint8_t* tier, const uint8_t* flag, void* stream);
+
+/* Fused decode attention: q pre-projection into basis space,
+ * split-T online-softmax scan over the tier-segregated pages, split-combine + back-projection through B^V and gV.
+ *   layer   : 0..L-1, or -1 = all layers in one call
+ *   seq_ids : host int32 [n_seqs], distinct
+ *   q       : dev bf16 [n_seqs, H_q, d]  (layer >= 0)   or [n_seqs, L, H_q, d]  (layer == -1)
+ *   out     : dev fp32, same shape as q; fully overwritten
+ * The query attends to all tokens of the sequence present at call time, no mask (reading A10).
+ * Errors: INVALID, STATE, EMPTY (some sequence has no tokens; nothing launched), CUDA. */
+int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids, const void* q,
+                          float* out, void* stream);
+
+/* ---- auxiliaries used by tests and bench (not on the hot path) ------------------------------------------------ */
+
+/* Pre-compressed, token-ordered entries of ONE sequence (device pointers). Residual arrays hold rows for the FLAGGED
+ * tokens only, in token order. Exactly one residual mode is used when any token is flagged:
+ *   mode A: residK/residV fp32 [n_flagged, L, H_kv, d] -> the library quantises them (reading A14, bit-exact)
+ *   mode B: codeK/codeV u8 [n_flagged, L, H_kv, d/2], byte i = channel 2i in the low nibble, 2i+1 in the high nibble,
+ *           two's complement;  scaleK/scaleV fp16 [n_flagged, L, H_kv, d/16]                            (reading A7) */
+typedef struct {
+  const void* coefK;  /* bf16 [n, L, H_kv, r]; entries at j >= r_t are ignored */
+  const void* coefV;
+  const float* residK;
+  const float* residV;
+  const uint8_t* codeK;
+  const uint8_t* codeV;
+  const void* scaleK;
+  const void* scaleV;
+} dwkv_raw_tokens;
+
+int dwkv_append_raw(dwkv_cache* c, int32_t seq_id, int32_t n, const uint8_t* tier /*host*/, const uint8_t* flag /*host*/,
+                    const dwkv_raw_tokens* data, void* stream);
+
+/* Token-ordered dump of tokens [t0, t0+n) of one sequence (device pointers; any may be NULL). Synchronous. */
+typedef struct {
+  uint8_t* tier;  /* [n] */
+  uint8_t* flag;  /* [n] */
+  int32_t* slot;  /* [n] slot within the token's class */
+  void* coefK;    /* bf16 [n, L, H_kv, r], zero beyond r_t */
+  void* coefV;
+  uint8_t* codeK; /* u8 [n, L, H_kv, d/2] canonical nibble order; zero rows for unflagged tokens */
+  uint8_t* codeV;
+  void* scaleK;   /* fp16 [n, L, H_kv, d/16]; zero rows for unflagged tokens */
+  void* scaleV;
+  float* deqK;    /* fp32 [n, L, H_kv, d] dequantised residual code*scale; zero rows for unflagged tokens */
+  float* deqV;
+} dwkv_token_dump;
+
+int dwkv_export_tokens(dwkv_cache* c, int32_t seq_id, int64_t t0, int64_t n, const dwkv_token_dump* out, void* stream);
+
+/* Drop all tokens of a sequence and return its pages to the pool. */
+int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id);
+
+/* Number of cached tokens of a sequence (negative = error code). */
+int64_t dwkv_seq_len(const dwkv_cache* c, int32_t seq_id);
+
+/* used = sum over tokens of 4*r_t + f_t*2*(d/2+d/8) bytes times L*H_kv (the compressed footprint, pin P13);
+ * reserved = bytes of arena pages currently allocated to sequences; dense_equiv = tokens * L * H_kv * 2*d*2. */
+int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved_bytes, uint64_t* dense_equiv_bytes);
+
+/* Tuning knobs for experiments (bench / tests): key in {"max_unit_blocks", "scan_variant", "time_scan"}; see DESIGN.md section 6. */
+int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);
+
+/* Measurement aid: with option "time_scan" = 1 every dwkv_decode_attention brackets its split-T scan launches (step a2)
+ * with CUDA events on `stream`; dwkv_get_stat(c, "scan_ms") waits for the last bracket and returns its duration in
+ * milliseconds (negative = none recorded / error). */
+double dwkv_get_stat(dwkv_cache* c, const char* key);
+
+/* Kernels launched by this handle since creation (bench's gpu_launches claim). */
+int64_t dwkv_launch_count(const dwkv_cache* c);
+
+const char* dwkv_last_error(void);
+
+/* ---- dense bf16 comparison kernel (BASELINE.json "from-scratch dense-bf16-cache decode kernel")
+ * Plain softmax attention over an uncompressed cache. K, V: dev bf16 [n_seqs, L, H_kv, T, d] (all sequences length T);
+ * q: dev bf16 [n_seqs, L, H_q, d]; out: dev fp32 [n_seqs, L, H_q, d]; workspace: dev, >= dwkv_dense_workspace_bytes(). */
+uint64_t dwkv_dense_workspace_bytes(int32_t n_seqs, int32_t n_layers, int32_t n_q_heads, int32_t d_head, int64_t T);
+int dwkv_dense_decode_attention(const void* K, const void* V, const void* q, float* out, void* workspace,
+                                int32_t n_seqs, int32_t n_layers, int32_t n_kv_heads, int32_t n_q_heads, int32_t d_head,
+                                int64_t T, float softmax_scale, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DWKV_H_ */

@@ -1,0 +1,235 @@
+// dwkv_cache_ops.cu -- cache construction side (SURVEY.md section 8a step a4 and the load / dump auxiliaries):
+//   compress_kernel     append/compress: project new K/V on the shared basis, quantise the residual, write tier pages
+//                       (readings A13, A14)
+//   scatter_raw_kernel  load pre-compressed token-ordered entries into the fragment-native pages
+//   gather_kernel       token-ordered dump of stored entries (bit-exact checks of routing and int4 dequantisation)
+#include "dwkv_internal.h"
+
+namespace dwkv {
+namespace {
+
+constexpr uint32_t kFull = 0xffffffffu;
+
+// Reading A14: fp32 IEEE, round-to-nearest-even, no FMA contraction, no reciprocal.
+//   s32 = amax / 7 ; s32 = min(s32, 65504) ; s = fp16_rn(s32) ; s == 0 -> 0 else clamp(rint(e / float(s)), -7, 7)
+__device__ __forceinline__ int quant_code(float e, float amax, __half* s_out) {
+  float s32 = __fdiv_rn(amax, 7.0f);
+  s32 = fminf(s32, 65504.0f);
+  const __half s = __float2half_rn(s32);
+  const float sf = __half2float(s);
+  *s_out = s;
+  if (sf == 0.f) return 0;
+  float r = rintf(__fdiv_rn(e, sf));
+  r = fminf(fmaxf(r, -7.f), 7.f);
+  return (int)r;
+}
+
+__device__ __forceinline__ float group16_amax(float a) {   // max over the 16 lanes of a half-warp
+  a = fmaxf(a, __shfl_xor_sync(kFull, a, 8));
+  a = fmaxf(a, __shfl_xor_sync(kFull, a, 4));
+  a = fmaxf(a, __shfl_xor_sync(kFull, a, 2));
+  a = fmaxf(a, __shfl_xor_sync(kFull, a, 1));
+  return a;
+}
+
+struct BlockPtr {
+  uint8_t* blk;
+  ClassLayout cl;
+  int rk;
+};
+
+__device__ __forceinline__ BlockPtr block_ptr(const uint8_t* arena, const CacheGeom& g, const TokDst& td, int lh) {
+  BlockPtr b;
+  b.rk = g.tier_rank[td.cls >> 1];
+  b.cl = make_class_layout(b.rk, td.cls & 1, g.d);
+  b.blk = const_cast<uint8_t*>(arena) + td.page_off + (size_t)lh * kPageLhBytes + (size_t)td.blk * b.cl.block_bytes;
+  return b;
+}
+
+__device__ __forceinline__ void store_code(uint8_t* region, int word_off, int bit, int code) {
+  atomicOr(reinterpret_cast<unsigned int*>(region + word_off), (unsigned int)((code + 8) & 15) << bit);
+}
+
+__device__ __forceinline__ int load_code(const uint8_t* region, int word_off, int bit) {
+  const unsigned int w = *reinterpret_cast<const unsigned int*>(region + word_off);
+  return (int)((w >> bit) & 15u) - 8;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) scatter_raw_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst,
+                                                          const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
+                                                          const float* residK, const float* residV,
+                                                          const uint8_t* codeK, const uint8_t* codeV,
+                                                          const __half* scaleK, const __half* scaleV) {
+  const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x;
+  const TokDst td = dst[tok];
+  const BlockPtr bp = block_ptr(arena, g, td, lh);
+  const size_t row = (size_t)tok * LH + lh;
+  if (tid < bp.rk) {
+    *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(td.slot, tid)) = coefK[row * g.r + tid];
+    *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(td.slot, tid)) = coefV[row * g.r + tid];
+  }
+  if (td.ridx < 0) return;
+  const size_t rrow = (size_t)td.ridx * LH + lh;
+  const int d = g.d, ng = d / 16;
+  if (tid < d) {
+    const int ch = tid, grp = ch >> 4;
+    for (int z = 0; z < 2; ++z) {
+      const float* resid = z ? residV : residK;
+      const uint8_t* codes = z ? codeV : codeK;
+      const __half* scales = z ? scaleV : scaleK;
+      int code;
+      __half s;
+      if (resid) {
+        const float e = resid[rrow * d + ch];
+        const float amax = group16_amax(fabsf(e));
+        code = quant_code(e, amax, &s);
+      } else {
+        const uint8_t byte = codes[rrow * (d / 2) + (ch >> 1)];
+        const int nib = (ch & 1) ? (byte >> 4) : (byte & 15);
+        code = (nib < 8) ? nib : nib - 16;
+        s = scales[rrow * ng + grp];
+      }
+      int wo, bit;
+      if (z == 0) kcode_nibble(td.slot, ch, d, &wo, &bit); else vcode_nibble(td.slot, ch, d, &wo, &bit);
+      store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
+      if ((ch & 15) == 0)
+        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(td.slot, grp, d)) = s;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a4: append / compress. One CTA per (new token, layer, kv head); both K and V.
+//   c = bf16( B[:r_t] . (x / g) )      e = x - g * (c . B[:r_t])      (readings A13, A14)
+__global__ void __launch_bounds__(128) compress_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst,
+                                                       const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
+                                                       const __nv_bfloat16* BK, const __nv_bfloat16* BV,
+                                                       const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
+  __shared__ float xn[128];
+  __shared__ float cf[64];
+  const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int l = lh / g.H, h = lh % g.H, d = g.d;
+  const TokDst td = dst[tok];
+  const BlockPtr bp = block_ptr(arena, g, td, lh);
+  const size_t row = (size_t)tok * LH + lh;
+  for (int z = 0; z < 2; ++z) {
+    const __nv_bfloat16* xs = (z ? v_new : k_new) + row * d;
+    const __nv_bfloat16* B = (z ? BV : BK) + ((size_t)(l / g.w) * g.H + h) * (size_t)g.r * d;
+    const __nv_bfloat16* gt = (z ? gV : gK) + (size_t)lh * d;
+    float x = 0.f, gate = 1.f;
+    if (tid < d) {
+      x = __bfloat162float(xs[tid]);
+      gate = __bfloat162float(gt[tid]);
+      xn[tid] = __fdiv_rn(x, gate);
+    }
+    __syncthreads();
+    for (int j = warp; j < bp.rk; j += 4) {
+      float acc = 0.f;
+      for (int i = lane; i < d; i += 32) acc = fmaf(__bfloat162float(B[(size_t)j * d + i]), xn[i], acc);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
+      if (lane == 0) {
+        const __nv_bfloat16 c = __float2bfloat16_rn(acc);
+        cf[j] = __bfloat162float(c);
+        const int off = z ? off_coefV(bp.cl) + vcoef_elem_off(td.slot, j) : off_coefK(bp.cl) + kcoef_elem_off(td.slot, j);
+        *reinterpret_cast<__nv_bfloat16*>(bp.blk + off) = c;
+      }
+    }
+    __syncthreads();
+    if (td.ridx >= 0 && tid < d) {
+      float rec = 0.f;
+      for (int j = 0; j < bp.rk; ++j) rec = fmaf(cf[j], __bfloat162float(B[(size_t)j * d + tid]), rec);
+      const float e = fmaf(-gate, rec, x);
+      const float amax = group16_amax(fabsf(e));
+      __half s;
+      const int code = quant_code(e, amax, &s);
+      int wo, bit;
+      if (z == 0) kcode_nibble(td.slot, tid, d, &wo, &bit); else vcode_nibble(td.slot, tid, d, &wo, &bit);
+      store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
+      if ((tid & 15) == 0)
+        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(td.slot, tid >> 4, d)) = s;
+    }
+    __syncthreads();
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst, DumpPtrs o) {
+  const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x;
+  const TokDst td = dst[tok];
+  const BlockPtr bp = block_ptr(arena, g, td, lh);
+  const size_t row = (size_t)tok * LH + lh;
+  const int d = g.d, ng = d / 16;
+  if (tid < g.r) {
+    const __nv_bfloat16 zero = __float2bfloat16_rn(0.f);
+    if (o.coefK)
+      o.coefK[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(td.slot, tid)) : zero;
+    if (o.coefV)
+      o.coefV[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(td.slot, tid)) : zero;
+  }
+  const bool fl = (td.cls & 1) != 0;
+  for (int z = 0; z < 2; ++z) {
+    uint8_t* codes = z ? o.codeV : o.codeK;
+    __half* scales = z ? o.scaleV : o.scaleK;
+    float* deq = z ? o.deqV : o.deqK;
+    const uint8_t* creg = bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl));
+    const uint8_t* sreg = bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl));
+    if (tid < d) {
+      int code = 0;
+      __half s = __float2half_rn(0.f);
+      if (fl) {
+        int wo, bit;
+        if (z == 0) kcode_nibble(td.slot, tid, d, &wo, &bit); else vcode_nibble(td.slot, tid, d, &wo, &bit);
+        code = load_code(creg, wo, bit);
+        s = *reinterpret_cast<const __half*>(sreg + scale_elem_off(td.slot, tid >> 4, d));
+      }
+      if (deq) deq[row * d + tid] = (float)code * __half2float(s);
+      if (scales && (tid & 15) == 0) scales[row * ng + (tid >> 4)] = s;
+      const int other = __shfl_down_sync(kFull, code, 1);
+      if (codes && (tid & 1) == 0) codes[row * (d / 2) + (tid >> 1)] = (uint8_t)((code & 15) | ((other & 15) << 4));
+    }
+  }
+}
+
+__global__ void gate_check_kernel(const __nv_bfloat16* g, int64_t n, int* bad) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) {
+    const float v = __bfloat162float(g[i]);
+    if (!(fabsf(v) > 0.f) || isinf(v) || isnan(v)) atomicOr(bad, 1);
+  }
+}
+
+}  // namespace
+
+int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const __nv_bfloat16* coefK,
+                       const __nv_bfloat16* coefV, const float* residK, const float* residV, const uint8_t* codeK,
+                       const uint8_t* codeV, const __half* scaleK, const __half* scaleV, cudaStream_t s) {
+  if (n <= 0) return 0;
+  dim3 grid(n, g.L * g.H);
+  scatter_raw_kernel<<<grid, 128, 0, s>>>(arena, g, dst, coefK, coefV, residK, residV, codeK, codeV, scaleK, scaleV);
+  return 1;
+}
+
+int launch_compress(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const __nv_bfloat16* k_new,
+                    const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
+                    const __nv_bfloat16* gK, const __nv_bfloat16* gV, cudaStream_t s) {
+  if (n <= 0) return 0;
+  dim3 grid(n, g.L * g.H);
+  compress_kernel<<<grid, 128, 0, s>>>(arena, g, dst, k_new, v_new, BK, BV, gK, gV);
+  return 1;
+}
+
+int launch_gather(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const DumpPtrs& o, cudaStream_t s) {
+  if (n <= 0) return 0;
+  dim3 grid(n, g.L * g.H);
+  gather_kernel<<<grid, 128, 0, s>>>(arena, g, dst, o);
+  return 1;
+}
+
+int launch_gate_check(const __nv_bfloat16* g, int64_t n, int* bad_flag, cudaStream_t s) {
+  gate_check_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(g, n, bad_flag);
+  return 1;
+}
+
+}  // namespace dwkv

@@ -1,0 +1,101 @@
+// dwkv_internal.h -- structs shared by the host runtime (dwkv_api.cu) and the kernels. Not part of the ABI.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "dwkv_layout.cuh"
+
+namespace dwkv {
+
+// One work unit of the split-T scan: a run of blocks of one (sequence, class) inside one page; the same unit is
+// processed for every (layer, kv head) by grid dimension y.
+struct __align__(16) Unit {
+  int64_t page_off;   // byte offset of the page in the arena
+  int32_t blk0;       // first block inside the page's (l,h) stripe
+  int32_t nblk;       // number of blocks (>= 1)
+  int32_t ntok;       // valid tokens in the unit (last block may be partial)
+  int16_t cls;        // class id = 2*tier + flag
+  int16_t b;          // index of the sequence in this call's seq_ids
+  int32_t epart;      // index into the residual-V partial buffer, -1 for unflagged classes
+  int32_t rk;         // rank of the class
+};
+
+struct ScanParams {
+  const uint8_t* arena;
+  const Unit* units;          // all units of the plan
+  int32_t unit0;              // first unit of the class handled by this launch
+  int32_t n_units_total;      // number of units in the plan (stride of the partial buffers)
+  int32_t n_eunits_total;     // number of flagged-class units in the plan
+  const __nv_bfloat16* qt_hi; // [n_seqs][Lsel][H][8][r]  q~ high part (bf16), rows >= G are zero
+  const __nv_bfloat16* qt_lo; // same shape, low part: q~ = hi + lo to 16 significant bits
+  const __nv_bfloat16* q;     // [n_seqs][Lq][Hq][d] raw queries (residual-K term)
+  float* part;                // [Lsel*H][n_units_total][G][2 + r]  (m, l, a[r]) per query head
+  float* epart;               // [Lsel*H][n_eunits_total][G][d]
+  int32_t Lsel, layer0, Lq;   // layers in this call, first absolute layer, layer stride of q (1 or L)
+  int32_t H, G, r, d;
+  float cscale;               // softmax_scale * log2(e)
+};
+
+struct CombineParams {
+  const Unit* units;
+  const int32_t* ulist;       // unit ids grouped by sequence
+  const int32_t* ustart;      // [n_seqs+1] ranges into ulist
+  const float* part;
+  const float* epart;
+  const __nv_bfloat16* BV;    // [M][H][r][d]
+  const __nv_bfloat16* gV;    // [L][H][d]
+  float* out;                 // [n_seqs][Lq][Hq][d]
+  int32_t n_units_total, n_eunits_total;
+  int32_t Lsel, layer0, Lq, w;
+  int32_t H, G, r, d;
+};
+
+struct QPrepParams {
+  const __nv_bfloat16* q;     // [n_seqs][Lq][Hq][d]
+  const __nv_bfloat16* BK;    // [M][H][r][d]
+  const __nv_bfloat16* gK;    // [L][H][d]
+  __nv_bfloat16* qt_hi;
+  __nv_bfloat16* qt_lo;
+  int32_t n_seqs, Lsel, layer0, Lq, w;
+  int32_t H, G, r, d;
+  float cscale;
+};
+
+// per-token destination for the scatter / gather kernels
+struct TokDst {
+  int64_t page_off;   // page of the token's class
+  int32_t blk;        // block inside the page stripe
+  int32_t slot;       // slot inside the block (0..31)
+  int32_t cls;        // class id
+  int32_t ridx;       // index among the flagged tokens of this call (-1 if unflagged)
+};
+
+struct CacheGeom {
+  int32_t L, w, H, G, r, d, n_tiers;
+  int32_t tier_rank[4];
+};
+
+// kernel launchers (dwkv_scan.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
+int launch_qprep(const QPrepParams& p, cudaStream_t s);
+int launch_scan(const ScanParams& p, int cls_rank, int resid, int n_units, int variant, cudaStream_t s);
+int launch_combine(const CombineParams& p, int n_seqs, cudaStream_t s);
+int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
+                       const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
+                       const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,
+                       const __half* scaleK, const __half* scaleV, cudaStream_t s);
+int launch_compress(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
+                    const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
+                    const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK, const __nv_bfloat16* gV,
+                    cudaStream_t s);
+struct DumpPtrs {
+  __nv_bfloat16 *coefK, *coefV;
+  uint8_t *codeK, *codeV;
+  __half *scaleK, *scaleV;
+  float *deqK, *deqV;
+};
+int launch_gather(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const DumpPtrs& o, cudaStream_t s);
+int launch_gate_check(const __nv_bfloat16* g, int64_t n, int* bad_flag, cudaStream_t s);
+
+}  // namespace dwkv

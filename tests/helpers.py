@@ -37,3 +37,32 @@ def oracle_load(oc, seq, inp):
 def rel_l2(a, b):
     a = np.asarray(a, np.float64); b = np.asarray(b, np.float64)
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def oracle_slice_from_kept(wl, consts, tier, flag, kept_lh, q_lh, l, h, scale=None):
+    """Oracle attention for one (layer, kv head) from the generator outputs kept on the host.
+    Returns (o [G,d], V-hat [T,d], (codeK, scaleK, codeV, scaleV) full-length arrays)."""
+    BK, BV, gK, gV = consts
+    T = len(tier)
+    ranks = np.asarray(wl.tier_ranks)[tier]
+    d = wl.d
+    cK_ = np.zeros((T, d), np.int8); cV_ = np.zeros((T, d), np.int8)
+    sK_ = np.zeros((T, d // 16), np.float16); sV_ = np.zeros((T, d // 16), np.float16)
+    idx = np.nonzero(flag)[0]
+    if len(idx):
+        cK_[idx], sK_[idx] = orc.quantize_int4_g16(kept_lh["rK"].numpy())
+        cV_[idx], sV_[idx] = orc.quantize_int4_g16(kept_lh["rV"].numpy())
+    scale = (1.0 / np.sqrt(d)) if scale is None else scale
+    o, _, V = orc.attention_slice(f64(kept_lh["cK"]), f64(kept_lh["cV"]), ranks, flag, cK_, sK_, cV_, sV_,
+                                  f64(BK)[l // wl.w, h], f64(BV)[l // wl.w, h], f64(gK)[l, h], f64(gV)[l, h],
+                                  q_lh, scale)
+    return o, V, (cK_, sK_, cV_, sV_)
+
+
+def check_output(o_gpu, o_ref, vmax, what=""):
+    """BASELINE.json north_star tolerance: max-abs <= 2e-3 * max|V-hat| and relative L2 <= 5e-3."""
+    err = float(np.abs(np.asarray(o_gpu, np.float64) - o_ref).max())
+    rel = rel_l2(o_gpu, o_ref)
+    assert err <= 2e-3 * vmax, f"{what}: max-abs {err:.3e} > 2e-3*{vmax:.3e}"
+    assert rel <= 5e-3, f"{what}: rel-L2 {rel:.3e} > 5e-3"
+    return err, rel

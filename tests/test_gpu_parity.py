@@ -1,0 +1,334 @@
+"""GPU parity: the CUDA path (through the C ABI / ctypes binding) against the CPU oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): tier routing and int4 dequantisation bit-exact; attention outputs within
+max-abs <= 2e-3 * max|V-hat| and relative L2 <= 5e-3 per (layer, sequence) block.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+import gen
+from oracle import dwkv_oracle as orc
+from helpers import f64, oracle_slice_from_kept, check_output, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mod():
+    from paper_2607_06523_b200 import binding, harness
+    return binding, harness
+
+
+def all_lh(wl):
+    return [(l, h) for l in range(wl.L) for h in range(wl.H_kv)]
+
+
+def load(harness, wl, routings, keep=None, chunk=1024, softmax_scale=0.0):
+    cache, consts = harness.make_cache(wl, n_seqs=len(routings), max_tokens=max(len(t) for t, _ in routings) + 256,
+                                       arena_bytes=harness.arena_bytes_for(wl, routings, 2), softmax_scale=softmax_scale)
+    keep = all_lh(wl) if keep is None else keep
+    kept = [harness.fill_sequence(cache, wl, s, s, t, f, chunk=chunk, keep=keep) for s, (t, f) in enumerate(routings)]
+    return cache, consts, kept
+
+
+def compare(wl, cache, consts, kept, routings, q, out, lhs=None, scale=None, what=""):
+    """q, out: [n_seq, L, Hq, d] tensors. Checks every (sequence, layer) block over the kv heads in `lhs`."""
+    o = out.double().cpu().numpy()
+    qn = f64(q)
+    worst = 0.0
+    lhs = all_lh(wl) if lhs is None else lhs
+    for s, (tier, flag) in enumerate(routings):
+        for l in sorted({l for l, _ in lhs}):
+            hs = [h for (ll, h) in lhs if ll == l]
+            ref = []; got = []; vmax = 0.0
+            for h in hs:
+                sl = slice(h * wl.G, (h + 1) * wl.G)
+                o_ref, V, _ = oracle_slice_from_kept(wl, consts, tier, flag, kept[s][(l, h)], qn[s, l, sl], l, h, scale)
+                ref.append(o_ref); got.append(o[s, l, sl]); vmax = max(vmax, float(np.abs(V).max()))
+            _, rel = check_output(np.concatenate(got), np.concatenate(ref), vmax, f"{what} seq {s} layer {l}")
+            worst = max(worst, rel)
+    return worst
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def test_tiny_config_all_layers_and_per_layer(mod):
+    """BASELINE.json configs[0], element by element, both launch modes, plus the peaked variants (pin P12)."""
+    binding, harness = mod
+    wl = gen.WORKLOADS["tiny"]
+    routings = [gen.make_routing(wl, 0)]
+    cache, consts, kept = load(harness, wl, routings)
+    for gain in (1.0, 8.0, 64.0):
+        q = gen.make_q(wl, device="cuda", gain=gain)
+        out = cache.decode_attention(-1, [0], q)
+        compare(wl, cache, consts, kept, routings, q, out, what=f"all-layers gain {gain}")
+        out2 = torch.stack([cache.decode_attention(l, [0], q[:, l].contiguous()) for l in range(wl.L)], dim=1)
+        compare(wl, cache, consts, kept, routings, q, out2, what=f"per-layer gain {gain}")
+        assert rel_l2(out2.cpu().numpy(), out.cpu().numpy()) < 1e-5
+    fp = cache.footprint()
+    assert fp["used_bytes"] == orc.footprint_bytes(*routings[0], wl.tier_ranks, wl.d, wl.L, wl.H_kv)
+    assert fp["dense_equiv_bytes"] == 512 * wl.L * wl.H_kv * 4 * wl.d
+    cache.destroy()
+
+
+def test_routing_and_dequant_bit_exact(mod):
+    """Export the stored entries: tier/flag/slot == oracle routing; coefficients, codes, scales and dequantised values
+    bit-exact against the oracle quantiser on the same fp32 residuals (reading A15 i, ii)."""
+    binding, harness = mod
+    wl = gen.WORKLOADS["tiny"]
+    tier, flag = gen.make_routing(wl, 0)
+    cache, consts, kept = load(harness, wl, [(tier, flag)], chunk=200)     # several appends: slots carry over
+    dump = cache.export_tokens(0, 0, len(tier))
+    cls, slot, _ = orc.route_slots(tier, flag, len(wl.tier_ranks))
+    assert np.array_equal(dump["tier"].cpu().numpy(), tier) and np.array_equal(dump["flag"].cpu().numpy(), flag)
+    assert np.array_equal(dump["slot"].cpu().numpy(), slot)
+    idx = np.nonzero(flag)[0]
+    for (l, h) in all_lh(wl):
+        k = kept[0][(l, h)]
+        for z in "KV":
+            got = dump["coef" + z][:, l, h].cpu().view(torch.int16).numpy()
+            want = k["c" + z].view(torch.int16).numpy()
+            assert np.array_equal(got, want)
+            codes, scales = orc.quantize_int4_g16(k["r" + z].numpy())
+            gc = dump["code" + z][:, l, h].cpu().numpy()
+            lo = (gc & 15).astype(np.int8); hi = (gc >> 4).astype(np.int8)
+            lo = np.where(lo > 7, lo - 16, lo); hi = np.where(hi > 7, hi - 16, hi)
+            dec = np.stack([lo, hi], axis=-1).reshape(len(tier), wl.d)
+            assert np.array_equal(dec[idx], codes) and not dec[flag == 0].any()
+            gs = dump["scale" + z][:, l, h].cpu().numpy()
+            assert np.array_equal(gs[idx].view(np.uint16), scales.view(np.uint16)) and not gs[flag == 0].view(np.uint16).any()
+            deq = dump["deq" + z][:, l, h].cpu().numpy()
+            assert np.array_equal(deq[idx].view(np.uint32), orc.dequant_int4_g16(codes, scales).view(np.uint32))
+    # partial export window
+    d2 = cache.export_tokens(0, 100, 37, want=("slot", "coefK"))
+    assert np.array_equal(d2["slot"].cpu().numpy(), slot[100:137])
+    cache.destroy()
+
+
+def test_raw_mode_b_codes_and_minus_eight(mod):
+    """Load codes + scales directly (canonical nibble order), including code -8; compare with the oracle."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(77,))
+    rng = np.random.default_rng(5)
+    T = 77
+    tier = rng.integers(0, 2, T).astype(np.uint8); flag = rng.integers(0, 2, T).astype(np.uint8)
+    nf = int(flag.sum())
+    cK, cV = gen.make_coef_chunk(wl, 0, 0, tier, device="cuda")
+    codes = {z: rng.integers(-8, 8, (nf, wl.L, wl.H_kv, wl.d)).astype(np.int8) for z in "KV"}
+    scales = {z: rng.uniform(0.001, 0.05, (nf, wl.L, wl.H_kv, wl.d // 16)).astype(np.float16) for z in "KV"}
+    packed = {z: ((codes[z][..., 0::2] & 15) | ((codes[z][..., 1::2] & 15) << 4)).astype(np.uint8) for z in "KV"}
+    cache, consts = harness.make_cache(wl, n_seqs=1, max_tokens=128)
+    dev = lambda a: torch.as_tensor(a).cuda()
+    cache.append_raw(0, tier, flag, cK, cV, codeK=dev(packed["K"]), codeV=dev(packed["V"]), scaleK=dev(scales["K"]), scaleV=dev(scales["V"]))
+    BK, BV, gK, gV = consts
+    oc = orc.OracleCache(wl.L, wl.w, wl.H_kv, wl.G, wl.d, wl.tier_ranks, f64(BK), f64(BV), f64(gK), f64(gV))
+    oc.append_raw(0, tier, flag, f64(cK), f64(cV), codeK=codes["K"], scaleK=scales["K"], codeV=codes["V"], scaleV=scales["V"])
+    dump = cache.export_tokens(0, 0, T, want=("codeK", "deqV"))
+    assert np.array_equal(dump["codeK"].cpu().numpy()[flag == 1], packed["K"])
+    assert np.array_equal(dump["deqV"].cpu().numpy()[flag == 1], orc.dequant_int4_g16(codes["V"], scales["V"]))
+    q = gen.make_q(wl, device="cuda")
+    out = cache.decode_attention(-1, [0], q).double().cpu().numpy()
+    ref = oc.decode_all_layers([0], f64(q))
+    for l in range(wl.L):
+        check_output(out[0, l], ref[0, l], oc.max_abs_vhat(0, l), f"mode B layer {l}")
+    cache.destroy()
+
+
+def test_split_invariance_p11(mod):
+    """Result independent of the work-list shape: one block per unit vs whole pages (pin P11)."""
+    binding, harness = mod
+    wl = gen.WORKLOADS["tiny"]
+    routings = [gen.make_routing(wl, 0)]
+    cache, consts, kept = load(harness, wl, routings)
+    q = gen.make_q(wl, device="cuda", gain=4.0)
+    outs = []
+    for ub in (1, 2, 1 << 20, 0):
+        cache.set_option("max_unit_blocks", ub)
+        outs.append(cache.decode_attention(-1, [0], q).double().cpu().numpy())
+    for o in outs[1:]:
+        assert rel_l2(o, outs[0]) < 2e-6
+    cache.destroy()
+
+
+@pytest.mark.parametrize("T", [1, 2, 31, 32, 33, 257])
+def test_short_and_ragged_lengths(mod, T):
+    """T = 1 gives o = V-hat[0] (pin P6); lengths around the 32-slot block and tile sizes (ragged tails)."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(T,), S0=0)
+    rng = np.random.default_rng(T)
+    tier = rng.integers(0, 2, T).astype(np.uint8); flag = (rng.random(T) < 0.4).astype(np.uint8)
+    cache, consts, kept = load(harness, wl, [(tier, flag)])
+    q = gen.make_q(wl, device="cuda", gain=3.0)
+    out = cache.decode_attention(-1, [0], q)
+    compare(wl, cache, consts, kept, [(tier, flag)], q, out, what=f"T={T}")
+    if T == 1:
+        o = out.double().cpu().numpy()
+        for (l, h) in all_lh(wl):
+            _, V, _ = oracle_slice_from_kept(wl, consts, tier, flag, kept[0][(l, h)], f64(q)[0, l, h * wl.G:(h + 1) * wl.G], l, h)
+            np.testing.assert_allclose(o[0, l, h * wl.G:(h + 1) * wl.G], np.broadcast_to(V[0], (wl.G, wl.d)), rtol=2e-3, atol=1e-6)
+    cache.destroy()
+
+
+def test_extreme_tier_patterns_multi_sequence(mod):
+    """All-lowest/no residual, all-top/all flagged, alternating tiers, and an ordinary mix decoded in ONE call
+    (BASELINE.json configs[4] extremes, small shape), also addressed through a permuted seq_ids list."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(300, 45, 131, 512),
+                             patterns=("all_low", "all_top_flag", "alternating", ""))
+    routings = [gen.make_routing(wl, s) for s in range(4)]
+    assert routings[0][0].max() == 0 and routings[1][1].all()
+    cache, consts, kept = load(harness, wl, routings)
+    q = gen.make_q(wl, device="cuda", gain=2.0)
+    out = cache.decode_attention(-1, [0, 1, 2, 3], q)
+    compare(wl, cache, consts, kept, routings, q, out, what="extremes")
+    perm = [2, 0, 3, 1]
+    out_p = cache.decode_attention(-1, perm, q[perm].contiguous())
+    assert rel_l2(out_p.cpu().numpy(), out[perm].cpu().numpy()) < 1e-6
+    cache.destroy()
+
+
+def test_llama8b_shape_d128_three_tiers_sampled(mod):
+    """Llama-3-8B shape (d=128, G=4, ranks 8/16/32), two ragged sequences spanning several pages of the flagged class and
+    a ragged tail; sampled (layer, head) slices against the oracle, per-layer launch included."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=4, T=(3000, 1237))
+    routings = [gen.make_routing(wl, s) for s in range(2)]
+    keep = [(0, 0), (1, 3), (3, 7), (2, 5)]
+    cache, consts, kept = load(harness, wl, routings, keep=keep, chunk=700)
+    for gain in (1.0, 8.0):
+        q = gen.make_q(wl, device="cuda", gain=gain)
+        out = cache.decode_attention(-1, [0, 1], q)
+        compare(wl, cache, consts, kept, routings, q, out, lhs=keep, what=f"8b gain {gain}")
+    out3 = cache.decode_attention(3, [0, 1], q[:, 3].contiguous())
+    assert rel_l2(out3.cpu().numpy(), out[:, 3].cpu().numpy()) < 1e-5
+    cache.destroy()
+
+
+def test_llama70b_shape_g8_ranks_8_24_48(mod):
+    """Llama-3-70B shape (G=8, w=4, ranks 8/24/48: odd numbers of 8-column chunks) with isolated top-tier singles."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["llama70b_128k_b1"], L=4, T=(2100,))
+    routings = [gen.make_routing(wl, 0)]
+    keep = [(0, 1), (3, 6)]
+    cache, consts, kept = load(harness, wl, routings, keep=keep, chunk=1000)
+    q = gen.make_q(wl, device="cuda", gain=2.0)
+    out = cache.decode_attention(-1, [0], q)
+    compare(wl, cache, consts, kept, routings, q, out, lhs=keep, what="70b")
+    cache.destroy()
+
+
+def test_append_compress_against_oracle(mod):
+    """dwkv_append_compress from dense K/V (reading A15 iii): coefficients within 1 bf16 ulp of the fp64 oracle on a tiny
+    fraction, codes within +-1 on <= 0.1 % of entries (and reconstruction within one scale there), attention within
+    tolerance; routing bit-exact; a second append continues the slots."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(96,))
+    cache, consts = harness.make_cache(wl, n_seqs=2, max_tokens=512)
+    BK, BV, gK, gV = consts
+    oc = orc.OracleCache(wl.L, wl.w, wl.H_kv, wl.G, wl.d, wl.tier_ranks, f64(BK), f64(BV), f64(gK), f64(gV))
+    rng = np.random.default_rng(3)
+    t0 = {0: 0, 1: 0}
+    for step in range(2):
+        n_new = [40, 23] if step == 0 else [9, 64]
+        tier = rng.integers(0, 2, sum(n_new)).astype(np.uint8); flag = (rng.random(sum(n_new)) < 0.5).astype(np.uint8)
+        ks, vs = [], []
+        for s, n in enumerate(n_new):
+            k, v = gen.make_dense_kv_chunk(wl, s, t0[s], n, BK, BV, gK, gV, device="cuda")
+            ks.append(k); vs.append(v); t0[s] += n
+        k_new, v_new = torch.cat(ks), torch.cat(vs)
+        cache.append_compress([0, 1], n_new, k_new, v_new, tier, flag)
+        off = 0
+        for s, n in enumerate(n_new):
+            oc.append_compress(s, f64(k_new[off:off + n]), f64(v_new[off:off + n]), tier[off:off + n], flag[off:off + n])
+            off += n
+    for s in (0, 1):
+        T = oc.seq_len(s)
+        assert cache.seq_len(s) == T
+        dump = cache.export_tokens(s, 0, T)
+        S = oc.seqs[s]
+        assert np.array_equal(dump["slot"].cpu().numpy(), S["slot"]) and np.array_equal(dump["tier"].cpu().numpy(), S["tier"])
+        for z in "KV":
+            got = dump["coef" + z].double().cpu().numpy()
+            want = S["c" + z]
+            ulp = np.maximum(np.abs(want), 2.0 ** -126) * 2.0 ** -7
+            assert np.all(np.abs(got - want) <= ulp)
+            assert np.mean(got != want) < 5e-3
+            gc = dump["code" + z].cpu().numpy()
+            lo = (gc & 15).astype(np.int8); hi = (gc >> 4).astype(np.int8)
+            lo = np.where(lo > 7, lo - 16, lo); hi = np.where(hi > 7, hi - 16, hi)
+            dec = np.stack([lo, hi], axis=-1).reshape(S["code" + z].shape)
+            diff = np.abs(dec.astype(np.int32) - S["code" + z])
+            fl = S["flag"].astype(bool)
+            assert diff.max() <= 1 and np.mean(diff[fl] != 0) <= 2e-3
+            assert not dec[~fl].any()
+            # where coefficients agree the scales must be identical or adjacent fp16 values
+            gs = dump["scale" + z].cpu().numpy().view(np.uint16).astype(np.int32)
+            ws = S["scale" + z].view(np.uint16).astype(np.int32)
+            assert np.abs(gs - ws).max() <= 1 and np.mean(gs != ws) <= 5e-3
+    q = gen.make_q(wl, device="cuda", n_seq=2)
+    out = cache.decode_attention(-1, [0, 1], q).double().cpu().numpy()
+    ref = oc.decode_all_layers([0, 1], f64(q))
+    for s in (0, 1):
+        for l in range(wl.L):
+            check_output(out[s, l], ref[s, l], oc.max_abs_vhat(s, l), f"append seq {s} layer {l}")
+    cache.destroy()
+
+
+def test_errors_and_reset(mod):
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(64,))
+    cache, consts = harness.make_cache(wl, n_seqs=2, max_tokens=100)
+    q = gen.make_q(wl, device="cuda", n_seq=1)
+    with pytest.raises(binding.DwkvError) as e:
+        cache.decode_attention(-1, [0], q)
+    assert e.value.code == binding.DWKV_E_EMPTY
+    tier, flag = gen.make_routing(wl, 0)
+    cK, cV = gen.make_coef_chunk(wl, 0, 0, tier, device="cuda")
+    rK, rV = gen.make_resid_chunk(wl, 0, 0, int(flag.sum()), device="cuda")
+    cache.append_raw(0, tier, flag, cK, cV, residK=rK, residV=rV)
+    with pytest.raises(binding.DwkvError) as e:      # capacity: 64 + 64 > 100, state unchanged
+        cache.append_raw(0, tier, flag, cK, cV, residK=rK, residV=rV)
+    assert e.value.code == binding.DWKV_E_CAPACITY and cache.seq_len(0) == 64
+    with pytest.raises(binding.DwkvError) as e:
+        cache.append_raw(0, np.full(1, 7, np.uint8), np.zeros(1, np.uint8), cK[:1].contiguous(), cV[:1].contiguous())
+    assert e.value.code == binding.DWKV_E_INVALID
+    with pytest.raises(binding.DwkvError) as e:      # basis frozen once tokens exist (reading A19)
+        cache.set_basis(consts[0], consts[1])
+    assert e.value.code == binding.DWKV_E_STATE
+    with pytest.raises(binding.DwkvError) as e:
+        cache.decode_attention(5, [0], q[:, 0].contiguous())
+    assert e.value.code == binding.DWKV_E_INVALID
+    out1 = cache.decode_attention(-1, [0], q).clone()
+    cache.reset_seq(0)
+    assert cache.seq_len(0) == 0 and cache.footprint()["reserved_bytes"] == 0
+    cache.append_raw(1, tier, flag, cK, cV, residK=rK, residV=rV)       # reuses the freed pages (zeroed on allocation)
+    out2 = cache.decode_attention(-1, [1], q)
+    assert torch.equal(out1, out2)
+    bad = consts[2].clone(); bad[0, 0, 0] = 0
+    c2 = binding.DwkvCache(wl.L, wl.w, wl.H_kv, wl.H_q, wl.d, list(wl.tier_ranks), 1, 64)
+    with pytest.raises(binding.DwkvError) as e:
+        c2.set_gates(bad, consts[3])
+    assert e.value.code == binding.DWKV_E_STATE
+    c2.destroy()
+    with pytest.raises(binding.DwkvError):
+        binding.DwkvCache(3, 2, 2, 4, 64, [8, 16], 1, 64)
+    cache.destroy()
+
+
+def test_dense_bf16_kernel_against_oracle_softmax(mod):
+    """The comparison kernel: plain attention over a dense bf16 cache vs the oracle's softmax_attention."""
+    binding, harness = mod
+    torch.manual_seed(0)
+    for (n_seq, L, H, G, d, T) in [(2, 2, 2, 4, 128, 1000), (1, 1, 2, 8, 128, 77), (1, 2, 2, 2, 64, 515)]:
+        K = (torch.randn(n_seq, L, H, T, d, device="cuda") * 0.3).to(torch.bfloat16)
+        V = (torch.randn(n_seq, L, H, T, d, device="cuda") * 0.3).to(torch.bfloat16)
+        q = (torch.randn(n_seq, L, H * G, d, device="cuda") * 2).to(torch.bfloat16)
+        out = binding.dense_decode_attention(K, V, q, H).double().cpu().numpy()
+        Kn, Vn, qn = f64(K), f64(V), f64(q)
+        for s in range(n_seq):
+            for l in range(L):
+                ref = np.concatenate([orc.softmax_attention(qn[s, l, h * G:(h + 1) * G], Kn[s, l, h], Vn[s, l, h], 1 / np.sqrt(d))
+                                      for h in range(H)])
+                check_output(out[s, l], ref, float(np.abs(Vn[s, l]).max()), f"dense {(n_seq, L, H, G, d, T)}")
