@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py -- decode-attention throughput of the DepthWeave-KV hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path (q pre-projection, split-T scan, combine: all layers) over one batch of
+synthetic cached sequences. Default workload: BASELINE.json configs[2] at batch 8 (Llama-3-8B shape, T = 65536).
+    python bench.py [--gpus N --steps K --warmup W] [--workload NAME] [--impl reference]
+Prints ONE JSON line (rank 0). N > 1 (torchrun): independent replicas, one per GPU, no data-path collective.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gen  # noqa: E402
+
+METRIC = "decode-attn cached tokens scanned/s (all layers; ms_per_step = ms/step) at 64K ctx"
+UNIT = "tokens/s"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples SM clocks and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake": 0x80, "sync_boost": 0x10, "applications_clocks": 0x2}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def __enter__(self):
+        if self.nv:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+def time_steps(fn, steps, warmup):
+    """CUDA-event timing on the current stream, sync on both sides; returns ms per step."""
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+def oracle_sample(wl, consts, tier, flag, kept, q_host, layers, budget_s=25.0):
+    """Time the CPU oracle as it stands on (layer, kv head) slices of sequence 0; returns (token-layers/s, sample text,
+    threads, worst rel-L2 vs `gpu_out` if given)."""
+    from oracle import dwkv_oracle as orc
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        threads = os.cpu_count() or 1
+    f64 = lambda t: t.detach().double().cpu().numpy()
+    BK, BV, gK, gV = [f64(x) for x in consts]
+    T = len(tier)
+    ranks = np.asarray(wl.tier_ranks)[tier]
+    idx = np.nonzero(flag)[0]
+    outs = {}
+    t0 = time.perf_counter()
+    done_layers = 0
+    for l in layers:
+        for h in range(wl.H_kv):
+            k = kept[(l, h)]
+            cK_ = np.zeros((T, wl.d), np.int8); cV_ = np.zeros((T, wl.d), np.int8)
+            sK_ = np.zeros((T, wl.d // 16), np.float16); sV_ = np.zeros((T, wl.d // 16), np.float16)
+            if len(idx):
+                cK_[idx], sK_[idx] = orc.quantize_int4_g16(k["rK"].numpy())
+                cV_[idx], sV_[idx] = orc.quantize_int4_g16(k["rV"].numpy())
+            o, _, V = orc.attention_slice(f64(k["cK"]), f64(k["cV"]), ranks, flag, cK_, sK_, cV_, sV_, BK[l // wl.w, h],
+                                          BV[l // wl.w, h], gK[l, h], gV[l, h], q_host[l, h * wl.G:(h + 1) * wl.G],
+                                          1.0 / np.sqrt(wl.d))
+            outs[(l, h)] = (o, float(np.abs(V).max()))
+        done_layers += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return done_layers * T / dt, done_layers, dt, threads, outs
+
+
+def run_reference(args, wl):
+    """--impl reference: the CPU oracle on the host cores, on a bounded sample of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    tier, flag = gen.make_routing(wl, 0)
+    consts = gen.make_basis(wl) + gen.make_gates(wl)
+    n_layers = 1
+    keep = [(l, h) for l in range(n_layers) for h in range(wl.H_kv)]
+    kept = {lh: dict(cK=[], cV=[], rK=[], rV=[]) for lh in keep}
+    chunk = 8192
+    for t0 in range(0, len(tier), chunk):      # generate only the sampled slices' worth of data, chunk by chunk
+        tr, fl = tier[t0:t0 + chunk], flag[t0:t0 + chunk]
+        wl1 = wl
+        cK, cV = gen.make_coef_chunk(wl1, 0, t0, tr, device="cpu")
+        nf = int(fl.sum())
+        rK, rV = gen.make_resid_chunk(wl1, 0, t0, nf, device="cpu") if nf else (None, None)
+        for (l, h) in keep:
+            kept[(l, h)]["cK"].append(cK[:, l, h].clone()); kept[(l, h)]["cV"].append(cV[:, l, h].clone())
+            if nf:
+                kept[(l, h)]["rK"].append(rK[:, l, h].clone()); kept[(l, h)]["rV"].append(rV[:, l, h].clone())
+    kept = {lh: {k: (torch.cat(v) if v else None) for k, v in d.items()} for lh, d in kept.items()}
+    q = gen.make_q(wl, n_seq=1).double().numpy()[0]
+    vals = []
+    for i in range(args.warmup + args.steps):
+        tps, nl, dt, threads, _ = oracle_sample(wl, consts, tier, flag, kept, q, range(n_layers), budget_s=1e9)
+        if i >= args.warmup:
+            vals.append((tps, dt))
+    tps = float(np.mean([v[0] for v in vals]))
+    ms = float(np.mean([v[1] for v in vals])) * 1e3
+    sample = f"{n_layers} layer x {wl.H_kv} kv heads x T={len(tier)} of sequence 0 per step (1/{wl.L * wl.n_seq} of the workload step)"
+    line = {"impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "note": "CPU oracle (oracle/dwkv_oracle.py) as it stands, bounded sample"},
+            "cpu_baseline": {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": tps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="llama8b_64k_b8")
+    ap.add_argument("--no-dense", action="store_true", help="skip the dense-bf16 comparison kernel")
+    ap.add_argument("--no-extra", action="store_true", help="skip batch 1/4, per-layer mode and the CPU baseline")
+    args = ap.parse_args()
+    wl = gen.WORKLOADS[args.workload]
+    if args.impl == "reference":
+        return run_reference(args, wl)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2607_06523_b200 import harness, binding
+
+    # ---- build the cache (every rank: its own replica of the batch, different seeds would not change the timing) ----
+    routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
+    cache, consts = harness.make_cache(wl, arena_bytes=harness.arena_bytes_for(wl, routings, 1), device=local)
+    sample_layers = [0]
+    keep = [(l, h) for l in sample_layers for h in range(wl.H_kv)] if (rank == 0 and not args.no_extra) else []
+    kept0 = None
+    t_fill = time.perf_counter()
+    for s, (tier, flag) in enumerate(routings):
+        k = harness.fill_sequence(cache, wl, s, s, tier, flag, device=local, chunk=4096, keep=keep if s == 0 else [])
+        if s == 0:
+            kept0 = k
+    torch.cuda.synchronize()
+    t_fill = time.perf_counter() - t_fill
+    fp = cache.footprint()
+    n_seq, L = wl.n_seq, wl.L
+    seq_ids = list(range(n_seq))
+    tokens_per_step = sum(wl.T) * L
+    nq = 4
+    qs = [gen.make_q(wl, step=i, device=dev) for i in range(nq)]
+    out = torch.empty(n_seq, L, wl.H_q, wl.d, dtype=torch.float32, device=dev)
+    it = [0]
+
+    def step():
+        cache.decode_attention(-1, seq_ids, qs[it[0] % nq], out)
+        it[0] += 1
+
+    # ---- timed region: K steps, inputs resident in HBM ------------------------------------------------------------
+    step(); torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    l0 = cache.launch_count()
+    with ClockSampler(local) as cs:
+        ms = time_steps(step, args.steps, args.warmup)
+    launches = (cache.launch_count() - l0) * args.steps // (args.steps + args.warmup)
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = tokens_per_step * world / (ms * 1e-3)
+
+    # ---- e2e: host q -> device, decode, result -> host, every step ------------------------------------------------
+    q_host = [q.cpu().pin_memory() for q in qs]
+    q_dev = torch.empty_like(qs[0])
+    out_host = torch.empty(out.shape, dtype=out.dtype).pin_memory()
+
+    def step_e2e():
+        q_dev.copy_(q_host[it[0] % nq], non_blocking=True)
+        cache.decode_attention(-1, seq_ids, q_dev, out)
+        out_host.copy_(out, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        it[0] += 1
+
+    for _ in range(args.warmup):
+        step_e2e()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e = {"value": tokens_per_step * world / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+           "h2d_bytes_per_step": q_dev.numel() * 2, "d2h_bytes_per_step": out.numel() * 4}
+
+    # ---- roofline of the dominant kernel group (split-T scan), CUDA events inside the library on the launch stream --
+    cache.set_option("time_scan", 1)
+    scan_ms = []
+    for i in range(args.steps):
+        step()
+        scan_ms.append(cache.get_stat("scan_ms"))
+    cache.set_option("time_scan", 0)
+    scan_ms = float(np.mean(scan_ms))
+    peak, peak_src = peaks()
+    alg_bytes = fp["used_bytes"]                      # compressed records: 4 r_t + f_t*2*(d/2+d/8) per (l, h, token)
+    achieved = alg_bytes / (scan_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "kernel": "scan_kernel<NK,RESID,D,PF> (all class launches of one step)",
+                "scan_ms": scan_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
+                "frac_of_8TBps_nominal": achieved / 8000.0, "step_frac_of_peak": alg_bytes / (ms * 1e-3) / 1e9 / peak}
+
+    extra = {"fill_s": t_fill, "footprint": fp, "compression_ratio": fp["dense_equiv_bytes"] / fp["used_bytes"],
+             "us_per_step": ms * 1e3}
+    cpu_baseline = None
+    if rank == 0 and not args.no_extra:
+        # batch 1 and 4 on the same cache; per-layer launch mode
+        for nb in (1, 4):
+            if nb < n_seq:
+                ids = seq_ids[:nb]
+                qb = [q[:nb].contiguous() for q in qs]
+                ob = torch.empty(nb, L, wl.H_q, wl.d, dtype=torch.float32, device=dev)
+                msb = time_steps(lambda: cache.decode_attention(-1, ids, qb[0], ob), args.steps, args.warmup)
+                extra[f"batch{nb}_us_per_step"] = msb * 1e3
+                extra[f"batch{nb}_frac_of_peak"] = alg_bytes * nb / n_seq / (msb * 1e-3) / 1e9 / peak
+        ql = [qs[0][:, l].contiguous() for l in range(L)]
+        ol = [torch.empty(n_seq, wl.H_q, wl.d, dtype=torch.float32, device=dev) for l in range(L)]
+
+        def per_layer():
+            for l in range(L):
+                cache.decode_attention(l, seq_ids, ql[l], ol[l])
+        extra["per_layer_mode_us_per_step"] = time_steps(per_layer, max(3, args.steps // 2), args.warmup) * 1e3
+        # CPU oracle on the host cores: bounded sample, and parity of the sampled slices at full size
+        tier, flag = routings[0]
+        o_gpu = out.clone()
+        cache.decode_attention(-1, seq_ids, qs[0], o_gpu)
+        torch.cuda.synchronize()
+        tps, nl, dt, threads, outs = oracle_sample(wl, consts, tier, flag, kept0, qs[0][0].double().cpu().numpy(),
+                                                   sample_layers, budget_s=25.0)
+        og = o_gpu[0].double().cpu().numpy()
+        rels = []
+        for (l, h), (o_ref, vmax) in outs.items():
+            got = og[l, h * wl.G:(h + 1) * wl.G]
+            rels.append(float(np.linalg.norm(got - o_ref) / np.linalg.norm(o_ref)))
+        cpu_baseline = {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": f"{nl} layer(s) x {wl.H_kv} kv heads x T={len(tier)} of sequence 0 ({dt:.1f} s)",
+                        "sampled_parity_rel_l2_max": max(rels)}
+
+    # ---- dense bf16 comparison kernel on the same shapes ------------------------------------------------------------
+    if rank == 0 and not args.no_dense:
+        try:
+            T = wl.T[0]
+            free, _ = torch.cuda.mem_get_info()
+            need = 2 * n_seq * L * wl.H_kv * T * wl.d * 2
+            nb = n_seq
+            while need * nb // n_seq > free - (4 << 30) and nb > 1:
+                nb //= 2
+            K = torch.empty(nb, L, wl.H_kv, T, wl.d, dtype=torch.bfloat16, device=dev)
+            V = torch.empty_like(K)
+            for s in range(nb):
+                K[s].normal_(0, 0.17); V[s].normal_(0, 0.17)
+            qd = qs[0][:nb].contiguous()
+            od = torch.empty(nb, L, wl.H_q, wl.d, dtype=torch.float32, device=dev)
+            ws = torch.empty(binding.lib.dwkv_dense_workspace_bytes(nb, L, wl.H_q, wl.d, T), dtype=torch.uint8, device=dev)
+            dms = time_steps(lambda: binding.dense_decode_attention(K, V, qd, wl.H_kv, workspace=ws, out=od),
+                             max(3, args.steps // 2), args.warmup)
+            dense_bytes = 2 * K.numel() * 2
+            comp_ms_same_batch = ms if nb == n_seq else extra.get(f"batch{nb}_us_per_step", ms * 1e3 * nb / n_seq) / 1e3
+            extra["dense"] = {"batch": nb, "us_per_step": dms * 1e3, "GBps": dense_bytes / (dms * 1e-3) / 1e9,
+                              "frac_of_peak": dense_bytes / (dms * 1e-3) / 1e9 / peak,
+                              "speedup_compressed_vs_dense": dms / comp_ms_same_batch,
+                              "required_speedup_0.7x_ratio": 0.7 * extra["compression_ratio"]}
+            del K, V
+        except Exception as ex:  # pragma: no cover
+            extra["dense"] = {"error": repr(ex)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+                "data": "synthetic",
+                "config": {"workload": wl.name, "shape": f"L={wl.L} w={wl.w} H_kv={wl.H_kv} G={wl.G} d={wl.d} r={wl.r}",
+                           "batch": n_seq, "T": wl.T[0], "tiers": list(wl.tier_ranks), "tier_frac": list(wl.tier_frac),
+                           "resid_frac": wl.resid_frac, "launch_mode": "all layers in one call (layer = -1)",
+                           "l2_policy": "inputs larger than L2 (compressed cache %.2f GB >> 126 MB)" % (fp["used_bytes"] / 1e9),
+                           "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"},
+                "clocks": cs.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "cpu_baseline": cpu_baseline, "extra": extra}
+        print(json.dumps(line))
+    cache.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
