@@ -178,6 +178,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llama8b_64k_b8")
+    ap.add_argument("--variant", type=int, default=0, help="scan_variant option of the library (A/B experiments)")
     ap.add_argument("--no-dense", action="store_true", help="skip the dense-bf16 comparison kernel")
     ap.add_argument("--no-extra", action="store_true", help="skip batch 1/4, per-layer mode and the CPU baseline")
     args = ap.parse_args()
@@ -199,6 +200,8 @@ def main():
     # ---- build the cache (every rank: its own replica of the batch, different seeds would not change the timing) ----
     routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
     cache, consts = harness.make_cache(wl, arena_bytes=harness.arena_bytes_for(wl, routings, 1), device=local)
+    if args.variant:
+        cache.set_option("scan_variant", args.variant)
     sample_layers = [0]
     keep = [(l, h) for l in sample_layers for h in range(wl.H_kv)] if (rank == 0 and not args.no_extra) else []
     kept0 = None

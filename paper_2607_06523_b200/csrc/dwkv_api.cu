@@ -112,7 +112,8 @@ struct Plan {
   uint64_t version = ~0ull;
   int n_units = 0, n_eunits = 0;
   int cls_unit0[kMaxClasses], cls_units[kMaxClasses];
-  size_t off_ulist = 0, off_ustart = 0;
+  int n_flag_units = 0;           // flagged-class units come first in the unit list
+  size_t off_ulist = 0, off_ustart = 0, off_wstart = 0;
   bool valid = false;
 };
 
@@ -140,6 +141,7 @@ struct dwkv_cache {
   uint64_t version = 0;
   // scratch
   DevBuf qt, part, epart, plan_dev, tokdst_dev, meta_dev;
+  int n_sms = 148;
   StagingRing ring;
   Plan plan;
   // options
@@ -248,6 +250,7 @@ int dwkv_create(const dwkv_config* cfg, dwkv_cache** out) {
     if (f.tier_rank[k] <= 0 || f.tier_rank[k] % 8 || f.tier_rank[k] > 64 || f.tier_rank[k] > f.d_head)
       return fail(DWKV_E_INVALID, "tier ranks must be multiples of 8, <= 64 and <= d_head");
     if (k && f.tier_rank[k] <= f.tier_rank[k - 1]) return fail(DWKV_E_INVALID, "tier ranks must ascend");
+    if (f.tier_rank[k] == 40 || f.tier_rank[k] == 56) return fail(DWKV_E_INVALID, "tier ranks 40 and 56 are not instantiated");
   }
   if (f.max_seqs <= 0 || f.max_seqs > 32767 || f.max_tokens_per_seq <= 0) return fail(DWKV_E_INVALID, "bad max_seqs / max_tokens_per_seq");
   if ((int64_t)f.n_layers * f.n_kv_heads > 65535) return fail(DWKV_E_INVALID, "n_layers * n_kv_heads > 65535");
@@ -255,6 +258,7 @@ int dwkv_create(const dwkv_config* cfg, dwkv_cache** out) {
 
   dwkv_cache* c = new dwkv_cache();
   c->cfg = f;
+  if (cudaDeviceGetAttribute(&c->n_sms, cudaDevAttrMultiProcessorCount, f.device) != cudaSuccess || c->n_sms <= 0) c->n_sms = 148;
   c->geom.L = f.n_layers; c->geom.w = f.group_size; c->geom.H = f.n_kv_heads; c->geom.G = f.n_q_heads / f.n_kv_heads;
   c->geom.r = f.tier_rank[f.n_tiers - 1]; c->geom.d = f.d_head; c->geom.n_tiers = f.n_tiers;
   for (int k = 0; k < 4; ++k) c->geom.tier_rank[k] = k < f.n_tiers ? f.tier_rank[k] : 0;
@@ -531,14 +535,14 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
       std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids))
     return DWKV_OK;
   P.valid = false;
-  // bytes per (layer, head) over the whole call -> target unit size
+  // bytes per (layer, head) over the whole call -> target unit size: about 16 items per warp of the persistent scan
   double total_bytes = 0;
   for (int b = 0; b < n_seqs; ++b)
     for (int k = 0; k < c->n_classes; ++k)
       total_bytes += (double)((c->seqs[seq_ids[b]].count[k] + kBlockTok - 1) / kBlockTok) * c->cl[k].block_bytes;
-  const double target_ctas = 148.0 * 24.0;
-  const double units_needed = std::max(1.0, std::ceil(target_ctas / ((double)n_lsel * c->geom.H)));
-  double unit_bytes = total_bytes / units_needed;
+  const int W = scan2_num_warps(c->n_sms);
+  const int LHsel = n_lsel * c->geom.H;
+  double unit_bytes = total_bytes * LHsel / ((double)W * 16.0);
   unit_bytes = std::min(std::max(unit_bytes, 8192.0), (double)kPageLhBytes);
 
   std::vector<Unit> units_by_cls[kMaxClasses];
@@ -548,7 +552,7 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
       if (S.count[k] == 0) continue;
       const ClassLayout& cl = c->cl[k];
       int64_t ub = c->opt_max_unit_blocks > 0 ? c->opt_max_unit_blocks
-                                              : std::max<int64_t>(cl.resid ? 1 : 4, (int64_t)(unit_bytes / cl.block_bytes));
+                                              : std::max<int64_t>(1, (int64_t)(unit_bytes / cl.block_bytes));
       ub = std::min<int64_t>(ub, cl.blocks_per_page);
       const int64_t tpp = cl.tokens_per_page;
       for (size_t pi = 0; pi < S.pages[k].size(); ++pi) {
@@ -573,15 +577,21 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
       }
     }
   }
+  // unit order: flagged classes first (highest rank first), then unflagged (highest rank first)
   std::vector<Unit> units;
   int n_e = 0;
-  for (int k = 0; k < kMaxClasses; ++k) {
-    P.cls_unit0[k] = (int)units.size();
-    P.cls_units[k] = (int)units_by_cls[k].size();
-    for (Unit& u : units_by_cls[k]) {
-      if (k & 1) u.epart = n_e++;
-      units.push_back(u);
+  for (int k = 0; k < kMaxClasses; ++k) { P.cls_unit0[k] = 0; P.cls_units[k] = 0; }
+  for (int fl = 1; fl >= 0; --fl) {
+    for (int tr = c->cfg.n_tiers - 1; tr >= 0; --tr) {
+      const int k = 2 * tr + fl;
+      P.cls_unit0[k] = (int)units.size();
+      P.cls_units[k] = (int)units_by_cls[k].size();
+      for (Unit& u : units_by_cls[k]) {
+        if (fl) u.epart = n_e++;
+        units.push_back(u);
+      }
     }
+    if (fl) P.n_flag_units = (int)units.size();
   }
   P.n_units = (int)units.size();
   P.n_eunits = n_e;
@@ -592,12 +602,40 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
     std::vector<int32_t> fill(ustart.begin(), ustart.end() - 1);
     for (int i = 0; i < (int)units.size(); ++i) ulist[fill[units[i].b]++] = i;
   }
-  // one blob: units | ulist | ustart
+  // byte-balanced slices of the item list (item = unit * LHsel + lh) for the warps of the persistent scan.
+  // scan_variant 1 hands the unflagged classes to the per-class v1 kernels, so only flagged items are sliced.
+  const int n_slice_units = c->opt_scan_variant == 1 ? P.n_flag_units : (int)units.size();
+  std::vector<int32_t> wstart(W + 1, 0);
+  {
+    const double kItemOverhead = 1024.0;     // prologue / epilogue of an item, in byte-equivalents
+    std::vector<double> cum(n_slice_units + 1, 0.0);
+    for (int i = 0; i < n_slice_units; ++i)
+      cum[i + 1] = cum[i] + ((double)units[i].nblk * c->cl[units[i].cls].block_bytes + kItemOverhead) * LHsel;
+    const double C = cum[n_slice_units];
+    int u = 0;
+    for (int k = 0; k <= W; ++k) {
+      const double target = C * (double)k / (double)W;
+      while (u < n_slice_units && cum[u + 1] <= target) ++u;
+      int64_t pos;
+      if (u >= n_slice_units) pos = (int64_t)n_slice_units * LHsel;
+      else {
+        const double per = (cum[u + 1] - cum[u]) / LHsel;
+        pos = (int64_t)u * LHsel + std::min<int64_t>(LHsel, (int64_t)std::floor((target - cum[u]) / per + 0.5));
+      }
+      wstart[k] = (int32_t)pos;
+    }
+    wstart[0] = 0;
+    wstart[W] = n_slice_units * LHsel;
+    for (int k = 1; k <= W; ++k) wstart[k] = std::max(wstart[k], wstart[k - 1]);
+  }
+  // one blob: units | ulist | ustart | wstart
   const size_t sz_units = units.size() * sizeof(Unit);
   P.off_ulist = (sz_units + 15) & ~(size_t)15;
   P.off_ustart = (P.off_ulist + ulist.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  const size_t total = P.off_ustart + ustart.size() * sizeof(int32_t);
+  P.off_wstart = (P.off_ustart + ustart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
+  const size_t total = P.off_wstart + wstart.size() * sizeof(int32_t);
   std::vector<uint8_t> blob(total, 0);
+  memcpy(blob.data() + P.off_wstart, wstart.data(), wstart.size() * sizeof(int32_t));
   memcpy(blob.data(), units.data(), sz_units);
   memcpy(blob.data() + P.off_ulist, ulist.data(), ulist.size() * sizeof(int32_t));
   memcpy(blob.data() + P.off_ustart, ustart.data(), ustart.size() * sizeof(int32_t));
@@ -655,13 +693,24 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
     if (!c->ev_scan0) { CU_OK(cudaEventCreate(&c->ev_scan0)); CU_OK(cudaEventCreate(&c->ev_scan1)); }
     CU_OK(cudaEventRecord(c->ev_scan0, st));
   }
-  // fattest classes first: they have the longest units
-  for (int k = c->n_classes - 1; k >= 0; --k) {
-    if (P.cls_units[k] == 0) continue;
-    sp.unit0 = P.cls_unit0[k];
-    const int n = launch_scan(sp, g.tier_rank[k >> 1], k & 1, P.cls_units[k], (int)c->opt_scan_variant, st);
-    if (n == 0) return fail(DWKV_E_INVALID, "no scan kernel for this class");
-    c->launches += n;
+  {
+    Scan2Params s2;
+    s2.arena = c->arena; s2.units = sp.units;
+    s2.wstart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_wstart);
+    s2.n_units_total = P.n_units; s2.n_eunits_total = P.n_eunits;
+    s2.qt_hi = sp.qt_hi; s2.qt_lo = sp.qt_lo; s2.q = sp.q; s2.part = sp.part; s2.epart = sp.epart;
+    s2.Lsel = Lsel; s2.layer0 = layer0; s2.Lq = Lq; s2.LH = Lsel * g.H; s2.H = g.H; s2.G = g.G; s2.r = g.r; s2.d = g.d;
+    s2.cscale = cscale;
+    if (c->opt_scan_variant != 1 || P.n_flag_units > 0) c->launches += launch_scan2(s2, c->n_sms, st);
+  }
+  if (c->opt_scan_variant == 1) {   // A/B: unflagged classes through the one-CTA-per-unit kernels, one launch per class
+    for (int k = c->n_classes - 2; k >= 0; k -= 2) {
+      if (P.cls_units[k] == 0) continue;
+      sp.unit0 = P.cls_unit0[k];
+      const int n = launch_scan(sp, g.tier_rank[k >> 1], 0, P.cls_units[k], 0, st);
+      if (n == 0) return fail(DWKV_E_INVALID, "no scan kernel for this class");
+      c->launches += n;
+    }
   }
   if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_scan1, st)); c->scan_timed = true; }
   CombineParams cp;

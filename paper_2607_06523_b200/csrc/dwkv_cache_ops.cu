@@ -33,7 +33,8 @@ __device__ __forceinline__ float group16_amax(float a) {   // max over the 16 la
 }
 
 struct BlockPtr {
-  uint8_t* blk;
+  uint8_t* blk;     // start of the sub-block that holds the token
+  int slot;         // slot inside the sub-block
   ClassLayout cl;
   int rk;
 };
@@ -42,7 +43,9 @@ __device__ __forceinline__ BlockPtr block_ptr(const uint8_t* arena, const CacheG
   BlockPtr b;
   b.rk = g.tier_rank[td.cls >> 1];
   b.cl = make_class_layout(b.rk, td.cls & 1, g.d);
-  b.blk = const_cast<uint8_t*>(arena) + td.page_off + (size_t)lh * kPageLhBytes + (size_t)td.blk * b.cl.block_bytes;
+  b.blk = const_cast<uint8_t*>(arena) + td.page_off + (size_t)lh * kPageLhBytes + (size_t)td.blk * b.cl.block_bytes +
+          sub_off(b.cl, td.slot);
+  b.slot = sub_slot(b.cl, td.slot);
   return b;
 }
 
@@ -66,8 +69,8 @@ __global__ void __launch_bounds__(128) scatter_raw_kernel(const uint8_t* arena, 
   const BlockPtr bp = block_ptr(arena, g, td, lh);
   const size_t row = (size_t)tok * LH + lh;
   if (tid < bp.rk) {
-    *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(td.slot, tid)) = coefK[row * g.r + tid];
-    *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(td.slot, tid)) = coefV[row * g.r + tid];
+    *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(bp.slot, tid, bp.cl.tb)) = coefK[row * g.r + tid];
+    *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(bp.slot, tid, bp.cl.tb)) = coefV[row * g.r + tid];
   }
   if (td.ridx < 0) return;
   const size_t rrow = (size_t)td.ridx * LH + lh;
@@ -91,10 +94,10 @@ __global__ void __launch_bounds__(128) scatter_raw_kernel(const uint8_t* arena, 
         s = scales[rrow * ng + grp];
       }
       int wo, bit;
-      if (z == 0) kcode_nibble(td.slot, ch, d, &wo, &bit); else vcode_nibble(td.slot, ch, d, &wo, &bit);
+      if (z == 0) kcode_nibble(bp.slot, ch, d, &wo, &bit); else vcode_nibble(bp.slot, ch, d, &wo, &bit);
       store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
       if ((ch & 15) == 0)
-        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(td.slot, grp, d)) = s;
+        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(bp.slot, grp, d)) = s;
     }
   }
 }
@@ -132,7 +135,7 @@ __global__ void __launch_bounds__(128) compress_kernel(const uint8_t* arena, Cac
       if (lane == 0) {
         const __nv_bfloat16 c = __float2bfloat16_rn(acc);
         cf[j] = __bfloat162float(c);
-        const int off = z ? off_coefV(bp.cl) + vcoef_elem_off(td.slot, j) : off_coefK(bp.cl) + kcoef_elem_off(td.slot, j);
+        const int off = z ? off_coefV(bp.cl) + vcoef_elem_off(bp.slot, j, bp.cl.tb) : off_coefK(bp.cl) + kcoef_elem_off(bp.slot, j, bp.cl.tb);
         *reinterpret_cast<__nv_bfloat16*>(bp.blk + off) = c;
       }
     }
@@ -145,10 +148,10 @@ __global__ void __launch_bounds__(128) compress_kernel(const uint8_t* arena, Cac
       __half s;
       const int code = quant_code(e, amax, &s);
       int wo, bit;
-      if (z == 0) kcode_nibble(td.slot, tid, d, &wo, &bit); else vcode_nibble(td.slot, tid, d, &wo, &bit);
+      if (z == 0) kcode_nibble(bp.slot, tid, d, &wo, &bit); else vcode_nibble(bp.slot, tid, d, &wo, &bit);
       store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
       if ((tid & 15) == 0)
-        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(td.slot, tid >> 4, d)) = s;
+        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(bp.slot, tid >> 4, d)) = s;
     }
     __syncthreads();
   }
@@ -164,9 +167,9 @@ __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, Cache
   if (tid < g.r) {
     const __nv_bfloat16 zero = __float2bfloat16_rn(0.f);
     if (o.coefK)
-      o.coefK[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(td.slot, tid)) : zero;
+      o.coefK[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(bp.slot, tid, bp.cl.tb)) : zero;
     if (o.coefV)
-      o.coefV[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(td.slot, tid)) : zero;
+      o.coefV[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(bp.slot, tid, bp.cl.tb)) : zero;
   }
   const bool fl = (td.cls & 1) != 0;
   for (int z = 0; z < 2; ++z) {
@@ -180,9 +183,9 @@ __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, Cache
       __half s = __float2half_rn(0.f);
       if (fl) {
         int wo, bit;
-        if (z == 0) kcode_nibble(td.slot, tid, d, &wo, &bit); else vcode_nibble(td.slot, tid, d, &wo, &bit);
+        if (z == 0) kcode_nibble(bp.slot, tid, d, &wo, &bit); else vcode_nibble(bp.slot, tid, d, &wo, &bit);
         code = load_code(creg, wo, bit);
-        s = *reinterpret_cast<const __half*>(sreg + scale_elem_off(td.slot, tid >> 4, d));
+        s = *reinterpret_cast<const __half*>(sreg + scale_elem_off(bp.slot, tid >> 4, d));
       }
       if (deq) deq[row * d + tid] = (float)code * __half2float(s);
       if (scales && (tid & 15) == 0) scales[row * ng + (tid >> 4)] = s;

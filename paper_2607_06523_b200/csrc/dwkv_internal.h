@@ -38,6 +38,21 @@ struct ScanParams {
   float cscale;               // softmax_scale * log2(e)
 };
 
+struct Scan2Params {            // persistent scan (dwkv_scan2.cu)
+  const uint8_t* arena;
+  const Unit* units;
+  const int32_t* wstart;       // [n_warps + 1] item positions; item = unit * LH + (lsel * H + h)
+  int32_t n_units_total, n_eunits_total;
+  const __nv_bfloat16* qt_hi;
+  const __nv_bfloat16* qt_lo;
+  const __nv_bfloat16* q;
+  float* part;
+  float* epart;
+  int32_t Lsel, layer0, Lq, LH;
+  int32_t H, G, r, d;
+  float cscale;
+};
+
 struct CombineParams {
   const Unit* units;
   const int32_t* ulist;       // unit ids grouped by sequence
@@ -80,6 +95,8 @@ struct CacheGeom {
 // kernel launchers (dwkv_scan.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
 int launch_qprep(const QPrepParams& p, cudaStream_t s);
 int launch_scan(const ScanParams& p, int cls_rank, int resid, int n_units, int variant, cudaStream_t s);
+int scan2_num_warps(int n_sms);
+int launch_scan2(const Scan2Params& p, int n_sms, cudaStream_t s);
 int launch_combine(const CombineParams& p, int n_seqs, cudaStream_t s);
 int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
