@@ -113,7 +113,7 @@ struct Plan {
   int n_units = 0, n_eunits = 0;
   int cls_unit0[kMaxClasses], cls_units[kMaxClasses];
   int n_flag_units = 0;           // flagged-class units come first in the unit list
-  size_t off_ulist = 0, off_ustart = 0, off_wstart = 0;
+  size_t off_ulist = 0, off_ustart = 0, off_wstart[2] = {0, 0};   // wstart[0]: unflagged items, [1]: flagged items
   bool valid = false;
 };
 
@@ -540,7 +540,7 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
   for (int b = 0; b < n_seqs; ++b)
     for (int k = 0; k < c->n_classes; ++k)
       total_bytes += (double)((c->seqs[seq_ids[b]].count[k] + kBlockTok - 1) / kBlockTok) * c->cl[k].block_bytes;
-  const int W = scan2_num_warps(c->n_sms);
+  const int W = scan2_num_warps(c->n_sms, 0);
   const int LHsel = n_lsel * c->geom.H;
   double unit_bytes = total_bytes * LHsel / ((double)W * 16.0);
   unit_bytes = std::min(std::max(unit_bytes, 8192.0), (double)kPageLhBytes);
@@ -602,40 +602,46 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
     std::vector<int32_t> fill(ustart.begin(), ustart.end() - 1);
     for (int i = 0; i < (int)units.size(); ++i) ulist[fill[units[i].b]++] = i;
   }
-  // byte-balanced slices of the item list (item = unit * LHsel + lh) for the warps of the persistent scan.
-  // scan_variant 1 hands the unflagged classes to the per-class v1 kernels, so only flagged items are sliced.
-  const int n_slice_units = c->opt_scan_variant == 1 ? P.n_flag_units : (int)units.size();
-  std::vector<int32_t> wstart(W + 1, 0);
-  {
+  // byte-balanced slices of the item list (item = unit * LHsel + lh) for the warps of the persistent scan kernels:
+  // one table over the flagged units [0, n_flag_units), one over the unflagged units [n_flag_units, n_units).
+  std::vector<int32_t> wtab[2];
+  for (int fl = 0; fl < 2; ++fl) {
+    const int u_lo = fl ? 0 : P.n_flag_units, u_hi = fl ? P.n_flag_units : (int)units.size();
+    const int Wk = scan2_num_warps(c->n_sms, fl);
+    std::vector<int32_t>& wstart = wtab[fl];
+    wstart.assign(Wk + 1, u_lo * LHsel);
+    const int n = u_hi - u_lo;
     const double kItemOverhead = 1024.0;     // prologue / epilogue of an item, in byte-equivalents
-    std::vector<double> cum(n_slice_units + 1, 0.0);
-    for (int i = 0; i < n_slice_units; ++i)
-      cum[i + 1] = cum[i] + ((double)units[i].nblk * c->cl[units[i].cls].block_bytes + kItemOverhead) * LHsel;
-    const double C = cum[n_slice_units];
+    std::vector<double> cum(n + 1, 0.0);
+    for (int i = 0; i < n; ++i)
+      cum[i + 1] = cum[i] + ((double)units[u_lo + i].nblk * c->cl[units[u_lo + i].cls].block_bytes + kItemOverhead) * LHsel;
+    const double C = cum[n];
     int u = 0;
-    for (int k = 0; k <= W; ++k) {
-      const double target = C * (double)k / (double)W;
-      while (u < n_slice_units && cum[u + 1] <= target) ++u;
+    for (int k = 0; k <= Wk; ++k) {
+      const double target = C * (double)k / (double)Wk;
+      while (u < n && cum[u + 1] <= target) ++u;
       int64_t pos;
-      if (u >= n_slice_units) pos = (int64_t)n_slice_units * LHsel;
+      if (u >= n) pos = (int64_t)n * LHsel;
       else {
         const double per = (cum[u + 1] - cum[u]) / LHsel;
         pos = (int64_t)u * LHsel + std::min<int64_t>(LHsel, (int64_t)std::floor((target - cum[u]) / per + 0.5));
       }
-      wstart[k] = (int32_t)pos;
+      wstart[k] = (int32_t)((int64_t)u_lo * LHsel + pos);
     }
-    wstart[0] = 0;
-    wstart[W] = n_slice_units * LHsel;
-    for (int k = 1; k <= W; ++k) wstart[k] = std::max(wstart[k], wstart[k - 1]);
+    wstart[0] = u_lo * LHsel;
+    wstart[Wk] = u_hi * LHsel;
+    for (int k = 1; k <= Wk; ++k) wstart[k] = std::max(wstart[k], wstart[k - 1]);
   }
   // one blob: units | ulist | ustart | wstart
   const size_t sz_units = units.size() * sizeof(Unit);
   P.off_ulist = (sz_units + 15) & ~(size_t)15;
   P.off_ustart = (P.off_ulist + ulist.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  P.off_wstart = (P.off_ustart + ustart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  const size_t total = P.off_wstart + wstart.size() * sizeof(int32_t);
+  P.off_wstart[0] = (P.off_ustart + ustart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
+  P.off_wstart[1] = (P.off_wstart[0] + wtab[0].size() * sizeof(int32_t) + 15) & ~(size_t)15;
+  const size_t total = P.off_wstart[1] + wtab[1].size() * sizeof(int32_t);
   std::vector<uint8_t> blob(total, 0);
-  memcpy(blob.data() + P.off_wstart, wstart.data(), wstart.size() * sizeof(int32_t));
+  memcpy(blob.data() + P.off_wstart[0], wtab[0].data(), wtab[0].size() * sizeof(int32_t));
+  memcpy(blob.data() + P.off_wstart[1], wtab[1].data(), wtab[1].size() * sizeof(int32_t));
   memcpy(blob.data(), units.data(), sz_units);
   memcpy(blob.data() + P.off_ulist, ulist.data(), ulist.size() * sizeof(int32_t));
   memcpy(blob.data() + P.off_ustart, ustart.data(), ustart.size() * sizeof(int32_t));
@@ -696,12 +702,18 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
   {
     Scan2Params s2;
     s2.arena = c->arena; s2.units = sp.units;
-    s2.wstart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_wstart);
     s2.n_units_total = P.n_units; s2.n_eunits_total = P.n_eunits;
     s2.qt_hi = sp.qt_hi; s2.qt_lo = sp.qt_lo; s2.q = sp.q; s2.part = sp.part; s2.epart = sp.epart;
     s2.Lsel = Lsel; s2.layer0 = layer0; s2.Lq = Lq; s2.LH = Lsel * g.H; s2.H = g.H; s2.G = g.G; s2.r = g.r; s2.d = g.d;
     s2.cscale = cscale;
-    if (c->opt_scan_variant != 1 || P.n_flag_units > 0) c->launches += launch_scan2(s2, c->n_sms, st);
+    if (P.n_flag_units > 0) {                       // flagged classes: the register-hungry kernel, 8 warps per SM
+      s2.wstart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_wstart[1]);
+      c->launches += launch_scan2(s2, 1, c->n_sms, st);
+    }
+    if (c->opt_scan_variant != 1 && P.n_units > P.n_flag_units) {
+      s2.wstart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_wstart[0]);
+      c->launches += launch_scan2(s2, 0, c->n_sms, st);
+    }
   }
   if (c->opt_scan_variant == 1) {   // A/B: unflagged classes through the one-CTA-per-unit kernels, one launch per class
     for (int k = c->n_classes - 2; k >= 0; k -= 2) {

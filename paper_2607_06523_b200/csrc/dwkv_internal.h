@@ -95,8 +95,8 @@ struct CacheGeom {
 // kernel launchers (dwkv_scan.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
 int launch_qprep(const QPrepParams& p, cudaStream_t s);
 int launch_scan(const ScanParams& p, int cls_rank, int resid, int n_units, int variant, cudaStream_t s);
-int scan2_num_warps(int n_sms);
-int launch_scan2(const Scan2Params& p, int n_sms, cudaStream_t s);
+int scan2_num_warps(int n_sms, int resid);
+int launch_scan2(const Scan2Params& p, int resid, int n_sms, cudaStream_t s);
 int launch_combine(const CombineParams& p, int n_seqs, cudaStream_t s);
 int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,

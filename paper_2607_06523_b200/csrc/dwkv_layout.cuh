@@ -20,8 +20,9 @@
 //             q = 4x+s = (group q>>1, half b = q&1): offset-binary codes (code+8) of slot 8j+g, channels
 //             16*grp + 8*b + 2t (low half-word) and +1 (high half-word)
 //   [K scale] word (j, t, grp) = fp16x2 ( scale[slot 8j+2t][grp], scale[slot 8j+2t+1][grp] )
-//   [V code]  lane (g,t): d/4 bytes = d/16 words; register q = 4x+s = (n-tile c = q>>1, b = q&1):
-//             codes of slots 8b+2t (low) and +1 (high), channel 8c+g
+//   [V code]  lane (g,t): d/4 bytes = d/16 words; word grp, nibble pair a (bits 4a.. and 16+4a..) is A-fragment register a
+//             of the transposed value MMA e^T += codeV^T . (P*scaleV): offset-binary codes of slots 8*(a>>1)+2t (low
+//             half-word) and +1 (high), channel 16*grp + 8*(a&1) + g
 //   [V scale] same arrangement as [K scale]
 #pragma once
 #include <stdint.h>
@@ -96,10 +97,11 @@ DWKV_HD void kcode_nibble(int s, int ch, int d, int* word_off, int* bit) {   // 
   *bit = 4 * (q & 3) + 16 * hi;
 }
 DWKV_HD void vcode_nibble(int s, int ch, int d, int* word_off, int* bit) {   // inside [V code] (s in 0..15)
-  const int b = (s >> 3) & 1, p = s & 7, t = p >> 1, hi = p & 1, c = ch >> 3, g = ch & 7;
-  const int q = 2 * c + b;
-  *word_off = (4 * g + t) * (d / 4) + (q >> 2) * 4;
-  *bit = 4 * (q & 3) + 16 * hi;
+  const int tile = (s >> 3) & 1, p = s & 7, t = p >> 1, hi = p & 1;
+  const int grp = ch >> 4, wi = ch & 15, g = wi & 7, upper = wi >> 3;
+  const int a = upper + 2 * tile;        // A-fragment register index of the transposed value MMA
+  *word_off = (4 * g + t) * (d / 4) + grp * 4;
+  *bit = 4 * a + 16 * hi;
 }
 DWKV_HD int scale_elem_off(int s, int grp, int d) {   // byte offset of the fp16 element inside [K scale] / [V scale]
   const int j = s >> 3, p = s & 7, t = p >> 1, hi = p & 1, ng = d / 16;

@@ -15,7 +15,8 @@ namespace dwkv {
 namespace {
 using namespace dwkv::dev;
 
-constexpr int kWarps = 16;
+constexpr int kWarpsPlain = 16;    // unflagged classes: 16 warps x <= 128 registers
+constexpr int kWarpsResid = 8;     // flagged classes: 8 warps x <= 255 registers (32 + 16 accumulators, 48 query registers)
 constexpr int kRing = 13824;       // ring bytes per warp (3 stages of the 4.5 KB flagged r=32 sub-block)
 constexpr int kMaxStages = 8;
 constexpr float kLazy = 8.0f;      // rescale when a score exceeds the reference by more than this (log2 units)
@@ -61,6 +62,18 @@ __device__ __forceinline__ void mma16816q(float (&d)[4], const uint32_t (&a)[4],
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
+__device__ __forceinline__ void mma1688q(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
+  asm("mma.sync.aligned.m16n8k8.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a0), "r"(a1), "r"(b0));
+}
+// D = A . B with C = 0: fresh outputs, rows 8..15 discarded by the caller
+__device__ __forceinline__ void mma16816z(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
+      : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "f"(0.f));
+}
+
 __device__ __forceinline__ Unit load_unit(const Unit* u) {
   const uint4 a = __ldg(reinterpret_cast<const uint4*>(u));
   const uint4 b = __ldg(reinterpret_cast<const uint4*>(u) + 1);
@@ -76,34 +89,35 @@ template <int NK, bool RESID, int D>
 struct Geo {
   static constexpr int TB = RESID ? 2 : 4;
   static constexpr int SUBTOK = 8 * TB;
-  static constexpr int COEF = NK * 128 * TB;                      // bytes of [K coef] (= [V coef])
-  static constexpr int SB = 2 * COEF + (RESID ? 20 * D : 0);      // stage bytes = one sub-block
+  static constexpr int COEF = NK * 128 * TB;                      // bytes of [K coef] (= [V coef]) of a sub-block
+  static constexpr int SB1 = 2 * COEF + (RESID ? 20 * D : 0);     // bytes of one sub-block
+  static constexpr int BPS = (!RESID && NK == 1) ? 2 : 1;         // sub-blocks per stage (amortises the per-stage work)
+  static constexpr int SB = SB1 * BPS;                            // stage bytes
   static constexpr int NS = (kRing / SB) < kMaxStages ? ((kRing / SB) < 1 ? 1 : (kRing / SB)) : kMaxStages;
   static constexpr int NG = D / 16;
-  static constexpr int NE = RESID ? D / 8 : 1;
 };
 
 template <int NK, bool RESID, int D>
 struct State {
   float m, l;
-  float acc[NK][4];                                  // rows 8..15 (acc[i][2..3]) stay zero
-  float eacc[Geo<NK, RESID, D>::NE][2];
+  float acc[NK][4];                         // a[row g][8i + 2t + {0,1}]; rows 8..15 (acc[i][2..3]) stay zero
+  float eacc[RESID ? D / 16 : 1][4];        // TRANSPOSED: e[head 2t+{0,1}][channel 16grp + g (+8)]
 };
 
-// Query-side operands of one item, in MMA A-fragment order (rows 8..15 explicit zeros).
+// Query-side operands of one item, in MMA A-fragment order.
 template <int NK, bool RESID, int D>
 struct QFrag {
-  static constexpr int NP = (NK + 1) / 2;            // k16 steps over the rank columns
-  uint32_t hi[NP][4];                                // NK == 1: the single quad is [hi | lo]
-  uint32_t lo[NP][4];                                // odd NK: last hi quad is [hi_last | lo_last], last lo quad unused
-  uint32_t qa[RESID ? D / 16 : 1][2];
-  float qbias[RESID ? D / 16 : 1];
+  static constexpr int NP = NK / 2;                  // k16 steps over pairs of 8-column chunks; odd NK adds two k8 steps
+  uint32_t hi[NP > 0 ? NP : 1][4];
+  uint32_t lo[NP > 0 ? NP : 1][4];
+  uint32_t hi_last, lo_last;                         // odd NK: last chunk, used with m16n8k8
+  uint32_t qa[RESID ? D / 16 : 1][4];                // raw q, group grp: {k 0..7, 0, k 8..15, 0}
 };
 
-// One stage (sub-block) from shared memory (32-bit shared address sp).
+// One sub-block from shared memory (32-bit shared address sp).
 template <int NK, bool RESID, int D>
-__device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uint32_t sp, const int nv, const int lane,
-                                              const bool first, const QFrag<NK, RESID, D>& qf, const float cscale) {
+__device__ __forceinline__ void process_sub(State<NK, RESID, D>& st, const uint32_t sp, const int nv, const int lane,
+                                            const bool first, const QFrag<NK, RESID, D>& qf, const float cscale) {
   using G = Geo<NK, RESID, D>;
   constexpr int TB = G::TB, NG = G::NG, NP = QFrag<NK, RESID, D>::NP;
   const int t = lane & 3;
@@ -122,7 +136,7 @@ __device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uin
       vw[i][0] = b.x; vw[i][1] = b.y;
     }
   }
-  // ---- scores relative to the reference: s' = q~ . cK - m_ref ------------------------------------------------------
+  // ---- scores relative to the reference: s' = q~ . cK - m_ref  (q~ = hi + lo) ----------------------------------------
   const float cinit = first ? 0.f : -st.m;
   float s[TB][4];
 #pragma unroll
@@ -130,12 +144,15 @@ __device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uin
     s[j][0] = cinit; s[j][1] = cinit; s[j][2] = 0.f; s[j][3] = 0.f;
 #pragma unroll
     for (int pi = 0; pi < NP; ++pi) {
-      const int i0 = 2 * pi, i1 = (2 * pi + 1 < NK) ? 2 * pi + 1 : 2 * pi;
-      mma16816q(s[j], qf.hi[pi], kw[i0][j], kw[i1][j]);              // odd tail: A = [hi | lo], B = [cK | cK]
-      if (2 * pi + 1 < NK) mma16816q(s[j], qf.lo[pi], kw[i0][j], kw[i1][j]);
+      mma16816q(s[j], qf.hi[pi], kw[2 * pi][j], kw[2 * pi + 1][j]);
+      mma16816q(s[j], qf.lo[pi], kw[2 * pi][j], kw[2 * pi + 1][j]);
+    }
+    if constexpr (NK & 1) {
+      mma1688q(s[j], qf.hi_last, 0u, kw[NK - 1][j]);
+      mma1688q(s[j], qf.lo_last, 0u, kw[NK - 1][j]);
     }
   }
-  // ---- residual-K term: integer-code dot on the tensor cores, fp32 group scales afterwards -------------------------
+  // ---- residual-K term: exact integer-code dot on the tensor cores, fp32 group scales afterwards -----------------------
   if constexpr (RESID) {
     const uint32_t codeK = sp + 2 * G::COEF;
     const uint32_t scaleK = codeK + 8 * D;
@@ -157,13 +174,12 @@ __device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uin
       float sr0 = 0.f, sr1 = 0.f;
 #pragma unroll
       for (int grp = 0; grp < NG; ++grp) {
-        float c0 = qf.qbias[grp], c1 = qf.qbias[grp];  // -136 * sum_i q_i cancels the offset of the biased codes
         const int q = 2 * grp;
-        mma16816(c0, c1, qf.qa[grp][0], qf.qa[grp][1], nib_to_bf16x2_biased(w[q >> 2], q & 3),
-                 nib_to_bf16x2_biased(w[q >> 2], (q & 3) + 1));
+        float c[4];
+        mma16816z(c, qf.qa[grp], nib_to_bf16x2(w[q >> 2], q & 3), nib_to_bf16x2(w[q >> 2], (q & 3) + 1));
         const float2 f = h2f2(sc[grp]);
-        sr0 = fmaf(c0, f.x, sr0);
-        sr1 = fmaf(c1, f.y, sr1);
+        sr0 = fmaf(c[0], f.x, sr0);
+        sr1 = fmaf(c[1], f.y, sr1);
       }
       s[j][0] = fmaf(cscale, sr0, s[j][0]);
       s[j][1] = fmaf(cscale, sr1, s[j][1]);
@@ -184,14 +200,17 @@ __device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uin
     mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 1));
     mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 2));
     const float up = first ? mx : fmaxf(mx, 0.f);      // new reference = old reference + up (never lowered later)
-    const float corr = first ? 1.f : ex2(-up);         // nothing accumulated yet on the first stage
+    const float corr = first ? 1.f : ex2(-up);         // nothing accumulated yet on the first sub-block
     st.m = (first ? 0.f : st.m) + up;
     st.l *= corr;
 #pragma unroll
     for (int i = 0; i < NK; ++i) { st.acc[i][0] *= corr; st.acc[i][1] *= corr; }
-    if constexpr (RESID) {
+    if constexpr (RESID) {   // e is held transposed: this lane's entries belong to heads 2t and 2t+1
+      const float c0 = __shfl_sync(kFull, corr, 8 * t), c1 = __shfl_sync(kFull, corr, 8 * t + 4);
 #pragma unroll
-      for (int c = 0; c < G::NE; ++c) { st.eacc[c][0] *= corr; st.eacc[c][1] *= corr; }
+      for (int grp = 0; grp < NG; ++grp) {
+        st.eacc[grp][0] *= c0; st.eacc[grp][1] *= c1; st.eacc[grp][2] *= c0; st.eacc[grp][3] *= c1;
+      }
     }
 #pragma unroll
     for (int j = 0; j < TB; ++j) { s[j][0] -= up; s[j][1] -= up; }
@@ -214,11 +233,11 @@ __device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uin
 #pragma unroll
     for (int i = 0; i < NK; ++i) mma16816q(st.acc[i], pa, vw[i][2 * ks], vw[i][2 * ks + 1]);
   }
-  // ---- e += (P * scaleV) . codeV ----------------------------------------------------------------------------------------
+  // ---- e^T += codeV^T . (P * scaleV): channels on the MMA m dimension, no padding rows ------------------------------------
   if constexpr (RESID) {
     const uint32_t codeV = sp + 2 * G::COEF + 10 * D;
     const uint32_t scaleV = codeV + 8 * D;
-    uint32_t w[D / 16], sc0[NG], sc1[NG];
+    uint32_t w[NG], sc0[NG], sc1[NG];
     if constexpr (D == 128) {
       const uint4 c0 = lds128(codeV + lane * 32);
       const uint4 c1 = lds128(codeV + lane * 32 + 16);
@@ -235,17 +254,18 @@ __device__ __forceinline__ void process_stage(State<NK, RESID, D>& st, const uin
       sc0[0] = x0.x; sc0[1] = x0.y; sc0[2] = x0.z; sc0[3] = x0.w;
       sc1[0] = y0.x; sc1[1] = y0.y; sc1[2] = y0.z; sc1[3] = y0.w;
     }
+    const uint32_t neg136[4] = {0xC308C308u, 0xC308C308u, 0xC308C308u, 0xC308C308u};   // bf16 pairs of -136
 #pragma unroll
     for (int grp = 0; grp < NG; ++grp) {
       const float2 f0 = h2f2(sc0[grp]);
       const float2 f1 = h2f2(sc1[grp]);
-      const uint32_t a0 = pack_bf16x2(pr[0][0] * f0.x, pr[0][1] * f0.y);
-      const uint32_t a2 = pack_bf16x2(pr[1][0] * f1.x, pr[1][1] * f1.y);
+      const uint32_t b0 = pack_bf16x2(pr[0][0] * f0.x, pr[0][1] * f0.y);
+      const uint32_t b1 = pack_bf16x2(pr[1][0] * f1.x, pr[1][1] * f1.y);
+      uint32_t a[4];
 #pragma unroll
-      for (int cc = 0; cc < 2; ++cc) {
-        const int c = 2 * grp + cc, q = 2 * c;
-        mma16816(st.eacc[c][0], st.eacc[c][1], a0, a2, nib_to_bf16x2(w[q >> 2], q & 3), nib_to_bf16x2(w[q >> 2], (q & 3) + 1));
-      }
+      for (int x = 0; x < 4; ++x) a[x] = nib_to_bf16x2_biased(w[grp], x);     // 136 + code, exact
+      mma16816q(st.eacc[grp], a, b0, b1);
+      mma16816q(st.eacc[grp], neg136, b0, b1);                                // removes the 136 offset on the tensor pipe
     }
   }
 }
@@ -263,41 +283,42 @@ template <int NK, bool RESID, int D>
 __device__ __forceinline__ int run_class(const Scan2Params& p, WarpCtx& cx, int& u, int& lh, Unit& un, const int n_items) {
   using G = Geo<NK, RESID, D>;
   using QF = QFrag<NK, RESID, D>;
-  constexpr int SB = G::SB, NS = G::NS, NG = G::NG;
-  constexpr int kBlockBytes = SB * (kBlockTok / G::SUBTOK);
+  constexpr int SB1 = G::SB1, BPS = G::BPS, NS = G::NS, NG = G::NG;
+  constexpr int kBlockBytes = SB1 * (kBlockTok / G::SUBTOK);
   const int lane = cx.lane, g = lane >> 2, t = lane & 3;
   const int cls = un.cls;
-  auto nstages = [](const Unit& x) { return RESID ? (x.ntok + 15) >> 4 : x.nblk; };
+  auto nsubs = [](const Unit& x) { return RESID ? (x.ntok + 15) >> 4 : x.nblk; };
   auto item_base = [&](const Unit& x, int lhx) {
     return p.arena + x.page_off + (size_t)(p.layer0 * p.H + lhx) * kPageLhBytes + (size_t)x.blk0 * kBlockBytes;
   };
 
   // ---- fetch stream (runs up to NS stages ahead of the compute stream) --------------------------------------------------
-  int u_f = u, lh_f = lh, st_f = 0, k_f = 0, left_f = n_items;
+  int u_f = u, lh_f = lh, k_f = 0, left_f = n_items;
   Unit un_f = un;
-  int nst_f = nstages(un_f);
+  int sub_left_f = nsubs(un_f);
   const uint8_t* src_f = item_base(un_f, lh_f);
   bool f_on = true;
   auto fetch_one = [&]() {
     if (!f_on) return;
+    const int nb = (BPS == 1) ? 1 : min(BPS, sub_left_f);
     if (lane == 0) {
       const uint32_t bar = cx.bar0 + 8 * k_f;
-      mbar_expect_tx(bar, SB);
-      bulk_g2s(cx.ring_s + k_f * SB, src_f, SB, bar);
+      mbar_expect_tx(bar, nb * SB1);
+      bulk_g2s(cx.ring_s + k_f * G::SB, src_f, nb * SB1, bar);
     }
-    src_f += SB;
+    src_f += nb * SB1;
     k_f = (k_f + 1 == NS) ? 0 : k_f + 1;
-    if (++st_f == nst_f) {
-      st_f = 0;
+    sub_left_f -= nb;
+    if (sub_left_f == 0) {
       if (--left_f == 0) {
         f_on = false;
       } else {
         if (++lh_f == p.LH) {
           lh_f = 0;
           un_f = load_unit(p.units + (++u_f));
-          nst_f = nstages(un_f);
           if (un_f.cls != cls) f_on = false;
         }
+        sub_left_f = nsubs(un_f);
         src_f = item_base(un_f, lh_f);
       }
     }
@@ -320,27 +341,23 @@ __device__ __forceinline__ int run_class(const Scan2Params& p, WarpCtx& cx, int&
       }
 #pragma unroll
       for (int pi = 0; pi < QF::NP; ++pi) {
-        const bool pair = 2 * pi + 1 < NK;
-        qf.hi[pi][0] = qh[2 * pi]; qf.hi[pi][1] = 0u; qf.hi[pi][2] = pair ? qh[2 * pi + 1] : ql[2 * pi]; qf.hi[pi][3] = 0u;
-        qf.lo[pi][0] = ql[2 * pi]; qf.lo[pi][1] = 0u; qf.lo[pi][2] = pair ? ql[2 * pi + 1] : 0u; qf.lo[pi][3] = 0u;
+        qf.hi[pi][0] = qh[2 * pi]; qf.hi[pi][1] = 0u; qf.hi[pi][2] = qh[2 * pi + 1]; qf.hi[pi][3] = 0u;
+        qf.lo[pi][0] = ql[2 * pi]; qf.lo[pi][1] = 0u; qf.lo[pi][2] = ql[2 * pi + 1]; qf.lo[pi][3] = 0u;
       }
+      qf.hi_last = qh[NK - 1];
+      qf.lo_last = ql[NK - 1];
     }
     if constexpr (RESID) {
       const __nv_bfloat16* q = p.q + (((size_t)un.b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (p.H * p.G) + (size_t)h * p.G + g) * D;
 #pragma unroll
       for (int grp = 0; grp < NG; ++grp) {
         qf.qa[grp][0] = (g < p.G) ? *reinterpret_cast<const uint32_t*>(q + 16 * grp + 2 * t) : 0u;
-        qf.qa[grp][1] = (g < p.G) ? *reinterpret_cast<const uint32_t*>(q + 16 * grp + 8 + 2 * t) : 0u;
-        const float2 x = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qf.qa[grp][0]));
-        const float2 y = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&qf.qa[grp][1]));
-        float sum = (x.x + x.y) + (y.x + y.y);
-        sum += __shfl_xor_sync(kFull, sum, 1);
-        sum += __shfl_xor_sync(kFull, sum, 2);
-        qf.qbias[grp] = -136.f * sum;
+        qf.qa[grp][1] = 0u;
+        qf.qa[grp][2] = (g < p.G) ? *reinterpret_cast<const uint32_t*>(q + 16 * grp + 8 + 2 * t) : 0u;
+        qf.qa[grp][3] = 0u;
       }
     } else {
-      qf.qa[0][0] = qf.qa[0][1] = 0u;
-      qf.qbias[0] = 0.f;
+      qf.qa[0][0] = qf.qa[0][1] = qf.qa[0][2] = qf.qa[0][3] = 0u;
     }
     State<NK, RESID, D> st;
     st.m = 0.f;
@@ -348,16 +365,25 @@ __device__ __forceinline__ int run_class(const Scan2Params& p, WarpCtx& cx, int&
 #pragma unroll
     for (int i = 0; i < NK; ++i) st.acc[i][0] = st.acc[i][1] = st.acc[i][2] = st.acc[i][3] = 0.f;
 #pragma unroll
-    for (int c = 0; c < G::NE; ++c) st.eacc[c][0] = st.eacc[c][1] = 0.f;
+    for (int c = 0; c < (RESID ? NG : 1); ++c) st.eacc[c][0] = st.eacc[c][1] = st.eacc[c][2] = st.eacc[c][3] = 0.f;
 
-    const int nst = nstages(un);
+    int sub_left = nsubs(un);
     int nv_left = un.ntok;
+    bool first = true;
 #pragma unroll 1
-    for (int sidx = 0; sidx < nst; ++sidx) {
+    while (sub_left > 0) {
       mbar_wait(cx.bar0 + 8 * k_c, (cx.phase >> k_c) & 1u);
       cx.phase ^= 1u << k_c;
-      process_stage<NK, RESID, D>(st, cx.ring_s + k_c * SB, nv_left, lane, sidx == 0, qf, p.cscale);
-      nv_left -= G::SUBTOK;
+      const uint32_t sp = cx.ring_s + k_c * G::SB;
+#pragma unroll
+      for (int b = 0; b < BPS; ++b) {
+        if (b == 0 || sub_left > b) {
+          process_sub<NK, RESID, D>(st, sp + b * SB1, nv_left - b * G::SUBTOK, lane, first && b == 0, qf, p.cscale);
+        }
+      }
+      first = false;
+      nv_left -= BPS * G::SUBTOK;
+      sub_left -= BPS;
       k_c = (k_c + 1 == NS) ? 0 : k_c + 1;
       __syncwarp();
       fetch_one();     // refill the slot that was just consumed
@@ -371,10 +397,19 @@ __device__ __forceinline__ int run_class(const Scan2Params& p, WarpCtx& cx, int&
       if (t == 0) *reinterpret_cast<float2*>(prec) = make_float2(st.m, st.l);
 #pragma unroll
       for (int i = 0; i < NK; ++i) *reinterpret_cast<float2*>(prec + 2 + 8 * i + 2 * t) = make_float2(st.acc[i][0], st.acc[i][1]);
-      if constexpr (RESID) {
-        float* erec = p.epart + ((size_t)lh * p.n_eunits_total + un.epart) * (size_t)(p.G * D) + g * D;
+    }
+    if constexpr (RESID) {
+      float* erec = p.epart + ((size_t)lh * p.n_eunits_total + un.epart) * (size_t)(p.G * D);
 #pragma unroll
-        for (int c = 0; c < G::NE; ++c) *reinterpret_cast<float2*>(erec + 8 * c + 2 * t) = make_float2(st.eacc[c][0], st.eacc[c][1]);
+      for (int x = 0; x < 2; ++x) {
+        const int head = 2 * t + x;
+        if (head < p.G) {
+#pragma unroll
+          for (int grp = 0; grp < NG; ++grp) {
+            erec[head * D + 16 * grp + g] = st.eacc[grp][x];
+            erec[head * D + 16 * grp + 8 + g] = st.eacc[grp][2 + x];
+          }
+        }
       }
     }
     ++done;
@@ -388,11 +423,12 @@ __device__ __forceinline__ int run_class(const Scan2Params& p, WarpCtx& cx, int&
   return done;
 }
 
-template <int D>
-__global__ void __launch_bounds__(kWarps * 32, 1) scan2_kernel(const __grid_constant__ Scan2Params p) {
+template <int D, bool RESID>
+__global__ void __launch_bounds__((RESID ? kWarpsResid : kWarpsPlain) * 32, 1) scan2_kernel(const __grid_constant__ Scan2Params p) {
+  constexpr int WARPS = RESID ? kWarpsResid : kWarpsPlain;
   extern __shared__ __align__(128) uint8_t smem[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t bars = smem_u32(smem + kWarps * kRing) + warp * kMaxStages * 8;
+  const uint32_t bars = smem_u32(smem + WARPS * kRing) + warp * kMaxStages * 8;
   if (lane == 0) {
     for (int s = 0; s < kMaxStages; ++s) mbar_init(bars + 8 * s, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -407,40 +443,43 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan2_kernel(const __grid_cons
   Unit un = load_unit(p.units + u);
   WarpCtx cx{smem_u32(smem) + warp * kRing, bars, 0u, lane};
   while (left > 0) {
-    const int key = (un.rk >> 3) * 2 + (un.cls & 1);
+    const int nk = un.rk >> 3;
     int n = left;
-    switch (key) {
-      case 2: n = run_class<1, false, D>(p, cx, u, lh, un, left); break;
-      case 4: n = run_class<2, false, D>(p, cx, u, lh, un, left); break;
-      case 6: n = run_class<3, false, D>(p, cx, u, lh, un, left); break;
-      case 8: n = run_class<4, false, D>(p, cx, u, lh, un, left); break;
-      case 12: n = run_class<6, false, D>(p, cx, u, lh, un, left); break;
-      case 16: n = run_class<8, false, D>(p, cx, u, lh, un, left); break;
-      case 3: n = run_class<1, true, D>(p, cx, u, lh, un, left); break;
-      case 5: n = run_class<2, true, D>(p, cx, u, lh, un, left); break;
-      case 7: n = run_class<3, true, D>(p, cx, u, lh, un, left); break;
-      case 9: n = run_class<4, true, D>(p, cx, u, lh, un, left); break;
-      case 13: n = run_class<6, true, D>(p, cx, u, lh, un, left); break;
-      case 17: n = run_class<8, true, D>(p, cx, u, lh, un, left); break;
+    switch (nk) {
+      case 1: n = run_class<1, RESID, D>(p, cx, u, lh, un, left); break;
+      case 2: n = run_class<2, RESID, D>(p, cx, u, lh, un, left); break;
+      case 3: n = run_class<3, RESID, D>(p, cx, u, lh, un, left); break;
+      case 4: n = run_class<4, RESID, D>(p, cx, u, lh, un, left); break;
+      case 6: n = run_class<6, RESID, D>(p, cx, u, lh, un, left); break;
+      case 8: n = run_class<8, RESID, D>(p, cx, u, lh, un, left); break;
       default: break;   // unsupported rank (the host refuses these configurations)
     }
     left -= n;
   }
 }
 
+template <int D, bool RESID>
+void launch_one(const Scan2Params& p, int n_sms, cudaStream_t s) {
+  constexpr int WARPS = RESID ? kWarpsResid : kWarpsPlain;
+  const int smem = WARPS * kRing + WARPS * kMaxStages * 8;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(scan2_kernel<D, RESID>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    attr_set = true;
+  }
+  scan2_kernel<D, RESID><<<n_sms, WARPS * 32, smem, s>>>(p);
+}
+
 }  // namespace
 
-int scan2_num_warps(int n_sms) { return n_sms * kWarps; }
+int scan2_num_warps(int n_sms, int resid) { return n_sms * (resid ? kWarpsResid : kWarpsPlain); }
 
-int launch_scan2(const Scan2Params& p, int n_sms, cudaStream_t s) {
-  const int smem = kWarps * kRing + kWarps * kMaxStages * 8;
-  static bool attr_set[2] = {false, false};
-  if (p.d == 128) {
-    if (!attr_set[0]) { cudaFuncSetAttribute(scan2_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set[0] = true; }
-    scan2_kernel<128><<<n_sms, kWarps * 32, smem, s>>>(p);
+// `p.wstart` must be the slice table of the flagged (resid = 1) or unflagged (resid = 0) item range.
+int launch_scan2(const Scan2Params& p, int resid, int n_sms, cudaStream_t s) {
+  if (resid) {
+    if (p.d == 128) launch_one<128, true>(p, n_sms, s); else launch_one<64, true>(p, n_sms, s);
   } else {
-    if (!attr_set[1]) { cudaFuncSetAttribute(scan2_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set[1] = true; }
-    scan2_kernel<64><<<n_sms, kWarps * 32, smem, s>>>(p);
+    launch_one<128, false>(p, n_sms, s);      // D is irrelevant for unflagged classes
   }
   return 1;
 }
