@@ -117,6 +117,15 @@ struct Plan {
   bool valid = false;
 };
 
+struct Plan3 {                    // plan of the fused persistent decode kernel (dwkv_scan3*.cuh)
+  std::vector<int32_t> seq_ids;
+  int n_lsel = 0;
+  uint64_t version = ~0ull;
+  int n_units = 0, n_slices = 0, n_segs = 0, n_slots = 0;
+  size_t off_ustart = 0, off_wentry = 0, off_pstart = 0;
+  bool valid = false;
+};
+
 }  // namespace
 
 struct dwkv_cache {
@@ -140,13 +149,16 @@ struct dwkv_cache {
   int64_t total_tokens = 0;
   uint64_t version = 0;
   // scratch
-  DevBuf qt, part, epart, plan_dev, tokdst_dev, meta_dev;
+  DevBuf qt, part, epart, plan_dev, plan3_dev, tokdst_dev, meta_dev;
   int n_sms = 148;
   StagingRing ring;
   Plan plan;
+  Plan3 plan3;
   // options
   int64_t opt_max_unit_blocks = 0;   // 0 = adaptive
   int64_t opt_scan_variant = 0;
+  int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
+  int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
   cudaEvent_t ev_scan0 = nullptr, ev_scan1 = nullptr;
   bool scan_timed = false;
@@ -311,7 +323,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gK) cudaFree(c->gK);
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
-  c->qt.release(); c->part.release(); c->epart.release(); c->plan_dev.release(); c->tokdst_dev.release(); c->meta_dev.release();
+  c->qt.release(); c->part.release(); c->epart.release(); c->plan_dev.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->meta_dev.release();
   c->ring.release();
   if (c->ev_scan0) cudaEventDestroy(c->ev_scan0);
   if (c->ev_scan1) cudaEventDestroy(c->ev_scan1);
@@ -499,6 +511,8 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
   else if (!strcmp(key, "scan_variant")) c->opt_scan_variant = value;
   else if (!strcmp(key, "time_scan")) c->opt_time_scan = value;
+  else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
+  else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
   else return fail(DWKV_E_INVALID, std::string("unknown option ") + key);
   c->version++;
   return DWKV_OK;
@@ -656,6 +670,177 @@ int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel
 
 }  // namespace
 
+namespace {
+
+// Plan of the fused persistent kernel. Linear order of the step's work: (sequence b, lh = layer * H + head, unit of b,
+// sub-block); a unit is one page stripe of a (sequence, class). The order is cut into n_slices contiguous slices of equal
+// COST (bytes, flagged bytes weighted by opt_flag_cost_pct) at sub-block granularity, one per warp. A slice touches one or a
+// few segments (b, lh); every (slice, segment) contact yields one partial, numbered contiguously per segment (pstart).
+// Depends on the sequence set, the token counts, the layer count and the options only.
+int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel, cudaStream_t st) {
+  Plan3& P = c->plan3;
+  if (P.valid && P.version == c->version && P.n_lsel == n_lsel && (int)P.seq_ids.size() == n_seqs &&
+      std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids))
+    return DWKV_OK;
+  P.valid = false;
+  const int LH = n_lsel * c->geom.H;
+  const double flag_w = (double)c->opt_flag_cost_pct / 100.0;
+  std::vector<Unit> units;
+  std::vector<int32_t> ustart(n_seqs + 1, 0), unsub;
+  std::vector<double> upre, usub, seq_cost(n_seqs, 0.0), cumB(n_seqs + 1, 0.0);
+  for (int b = 0; b < n_seqs; ++b) {
+    ustart[b] = (int32_t)units.size();
+    const SeqState& S = c->seqs[seq_ids[b]];
+    double acc = 0.0;
+    for (int fl = 1; fl >= 0; --fl) {
+      for (int tr = c->cfg.n_tiers - 1; tr >= 0; --tr) {
+        const int k = 2 * tr + fl;
+        if (S.count[k] == 0) continue;
+        const ClassLayout& cl = c->cl[k];
+        const int64_t tpp = cl.tokens_per_page;
+        const int64_t ub = c->opt_max_unit_blocks > 0 ? std::min<int64_t>(c->opt_max_unit_blocks, cl.blocks_per_page) : cl.blocks_per_page;
+        const double cost_sub = (double)cl.sub_bytes * (fl ? flag_w : 1.0);
+        for (size_t pi = 0; pi < S.pages[k].size(); ++pi) {
+          const int64_t tok_in_page = std::min<int64_t>(tpp, S.count[k] - (int64_t)pi * tpp);
+          if (tok_in_page <= 0) break;
+          const int64_t nblk = (tok_in_page + kBlockTok - 1) / kBlockTok;
+          for (int64_t b0 = 0; b0 < nblk; b0 += ub) {
+            Unit u;
+            u.page_off = (int64_t)S.pages[k][pi] * (int64_t)c->page_bytes;
+            u.blk0 = (int32_t)b0;
+            u.nblk = (int32_t)std::min<int64_t>(ub, nblk - b0);
+            u.ntok = (int32_t)(std::min<int64_t>(tok_in_page, (b0 + u.nblk) * kBlockTok) - b0 * kBlockTok);
+            u.cls = (int16_t)k;
+            u.b = (int16_t)b;
+            u.epart = -1;
+            u.rk = c->geom.tier_rank[tr];
+            const int nsub = (u.ntok + cl.sub_tok - 1) / cl.sub_tok;
+            units.push_back(u);
+            upre.push_back(acc);
+            usub.push_back(cost_sub);
+            unsub.push_back(nsub);
+            acc += (double)nsub * cost_sub;
+          }
+        }
+      }
+    }
+    seq_cost[b] = acc;
+    cumB[b + 1] = cumB[b] + acc * LH;
+  }
+  ustart[n_seqs] = (int32_t)units.size();
+  const int n_units = (int)units.size(), S_total = n_seqs * LH;
+  const int Wmax = scan3_num_slices(c->n_sms);
+  const int W = c->opt_n_slices > 0 ? (int)std::min<int64_t>(c->opt_n_slices, Wmax) : Wmax;
+  const double C = cumB[n_seqs];
+  struct Pos { int32_t seg, u, sub; };
+  auto less = [](const Pos& a, const Pos& b) { return a.seg != b.seg ? a.seg < b.seg : (a.u != b.u ? a.u < b.u : a.sub < b.sub); };
+  std::vector<Pos> pos(W + 1);
+  const Pos end_pos{S_total, n_units, 0};
+  for (int k = 0; k <= W; ++k) {
+    Pos q = end_pos;
+    if (k < W) {
+      const double target = C * (double)k / (double)W;
+      int b = (int)(std::upper_bound(cumB.begin(), cumB.end(), target) - cumB.begin()) - 1;
+      b = std::min(std::max(b, 0), n_seqs - 1);
+      double rem = target - cumB[b];
+      int lh = std::min(LH - 1, (int)std::floor(rem / seq_cost[b]));
+      rem -= (double)lh * seq_cost[b];
+      int u = (int)(std::upper_bound(upre.begin() + ustart[b], upre.begin() + ustart[b + 1], rem) - upre.begin()) - 1;
+      u = std::min(std::max(u, ustart[b]), ustart[b + 1] - 1);
+      int sub = (int)std::floor((rem - upre[u]) / usub[u] + 0.5);
+      sub = std::max(sub, 0);
+      if (sub >= unsub[u]) {          // normalise: a position never points past the last sub-block of a unit
+        sub = 0;
+        if (++u == ustart[b + 1]) {
+          if (++lh == LH) { lh = 0; ++b; }
+          u = b < n_seqs ? ustart[b] : n_units;
+        }
+      }
+      q = b < n_seqs ? Pos{b * LH + lh, u, sub} : end_pos;
+    }
+    if (k > 0 && less(q, pos[k - 1])) q = pos[k - 1];
+    pos[k] = q;
+  }
+  pos[0] = Pos{0, 0, 0};
+  // partial slots: contacts (slice, segment), numbered per segment in slice order
+  std::vector<int32_t> pstart(S_total + 1, 0), seen(S_total, 0);
+  auto last_seg = [&](const Pos& e) {
+    if (e.seg >= S_total) return S_total - 1;
+    const int b = e.seg / LH;
+    return (e.u == ustart[b] && e.sub == 0) ? e.seg - 1 : e.seg;
+  };
+  for (int w = 0; w < W; ++w) {
+    if (!less(pos[w], pos[w + 1])) continue;
+    for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) pstart[s + 1]++;
+  }
+  for (int s = 0; s < S_total; ++s) pstart[s + 1] += pstart[s];
+  std::vector<int32_t> wentry(4 * (size_t)(W + 1), 0);
+  for (int w = 0; w <= W; ++w) {
+    wentry[4 * w + 0] = pos[w].seg; wentry[4 * w + 1] = pos[w].u; wentry[4 * w + 2] = pos[w].sub; wentry[4 * w + 3] = 0;
+    if (w < W && less(pos[w], pos[w + 1])) {
+      wentry[4 * w + 3] = pstart[pos[w].seg] + seen[pos[w].seg];
+      for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) seen[s]++;
+    }
+  }
+  // one blob: units | ustart | wentry | pstart
+  const size_t sz_units = units.size() * sizeof(Unit);
+  P.off_ustart = (sz_units + 15) & ~(size_t)15;
+  P.off_wentry = (P.off_ustart + ustart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
+  P.off_pstart = (P.off_wentry + wentry.size() * sizeof(int32_t) + 15) & ~(size_t)15;
+  const size_t total = P.off_pstart + pstart.size() * sizeof(int32_t);
+  std::vector<uint8_t> blob(total, 0);
+  memcpy(blob.data(), units.data(), sz_units);
+  memcpy(blob.data() + P.off_ustart, ustart.data(), ustart.size() * sizeof(int32_t));
+  memcpy(blob.data() + P.off_wentry, wentry.data(), wentry.size() * sizeof(int32_t));
+  memcpy(blob.data() + P.off_pstart, pstart.data(), pstart.size() * sizeof(int32_t));
+  int rc = upload(c, c->plan3_dev, blob.data(), total, st);
+  if (rc) return rc;
+  P.n_units = n_units; P.n_slices = W; P.n_segs = S_total; P.n_slots = pstart[S_total];
+  P.seq_ids.assign(seq_ids, seq_ids + n_seqs);
+  P.n_lsel = n_lsel;
+  P.version = c->version;
+  P.valid = true;
+  return DWKV_OK;
+}
+
+int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids, const void* q, float* out, cudaStream_t st) {
+  const CacheGeom& g = c->geom;
+  const int Lsel = layer < 0 ? g.L : 1, layer0 = layer < 0 ? 0 : layer;
+  int rc = build_plan3(c, n_seqs, seq_ids, Lsel, st);
+  if (rc) return rc;
+  const Plan3& P = c->plan3;
+  CU_OK(c->part.reserve((size_t)P.n_slots * g.G * (2 + g.r + g.d) * sizeof(float)));
+  const uint8_t* blob = (const uint8_t*)c->plan3_dev.p;
+  Scan3Params sp;
+  sp.arena = c->arena;
+  sp.units = (const Unit*)blob;
+  sp.ustart = (const int32_t*)(blob + P.off_ustart);
+  sp.wentry = (const int4*)(blob + P.off_wentry);
+  sp.pstart = (const int32_t*)(blob + P.off_pstart);
+  sp.q = (const __nv_bfloat16*)q; sp.BK = c->BK; sp.gK = c->gK;
+  sp.part = (float*)c->part.p;
+  sp.n_slices = P.n_slices; sp.n_segs = P.n_segs;
+  sp.layer0 = layer0; sp.Lq = Lsel; sp.LH = Lsel * g.H; sp.w = g.w;
+  sp.H = g.H; sp.G = g.G; sp.r = g.r; sp.d = g.d;
+  sp.cscale = c->softmax_scale * 1.4426950408889634f;
+  if (c->opt_time_scan) {
+    if (!c->ev_scan0) { CU_OK(cudaEventCreate(&c->ev_scan0)); CU_OK(cudaEventCreate(&c->ev_scan1)); }
+    CU_OK(cudaEventRecord(c->ev_scan0, st));
+  }
+  const int n = launch_scan3(sp, c->n_sms, st);
+  if (n == 0) return fail(DWKV_E_INVALID, "no fused decode kernel instance for this shape");
+  c->launches += n;
+  if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_scan1, st)); c->scan_timed = true; }
+  Combine3Params cp;
+  cp.pstart = sp.pstart; cp.part = sp.part; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
+  cp.layer0 = layer0; cp.Lq = Lsel; cp.LH = sp.LH; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;
+  c->launches += launch_combine3(cp, P.n_segs, st);
+  CU_OK(cudaGetLastError());
+  return DWKV_OK;
+}
+
+}  // namespace
+
 extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids, const void* q,
                                      float* out, void* stream) {
   if (!c || !seq_ids || !q || !out || n_seqs <= 0) return fail(DWKV_E_INVALID, "NULL argument or n_seqs <= 0");
@@ -669,6 +854,7 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
     if (c->seqs[seq_ids[i]].tier.empty()) return fail(DWKV_E_EMPTY, "decode on an empty sequence (reading A17)");
   }
   cudaStream_t st = (cudaStream_t)stream;
+  if (c->opt_scan_variant == 0) return decode3(c, layer, n_seqs, seq_ids, q, out, st);
   const CacheGeom& g = c->geom;
   const int Lsel = layer < 0 ? g.L : 1, layer0 = layer < 0 ? 0 : layer, Lq = Lsel;
   int rc = build_plan(c, n_seqs, seq_ids, Lsel, st);

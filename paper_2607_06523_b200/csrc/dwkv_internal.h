@@ -53,6 +53,32 @@ struct Scan2Params {            // persistent scan (dwkv_scan2.cu)
   float cscale;
 };
 
+struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.cuh)
+  const uint8_t* arena;
+  const Unit* units;           // units of all sequences of the call, grouped by sequence, class-ordered inside
+  const int32_t* ustart;       // [n_seqs + 1] unit ranges per sequence
+  const int4* wentry;          // [n_slices + 1] slice boundaries (segment, unit, sub-block, first partial slot)
+  const int32_t* pstart;       // [n_segs + 1] partial-slot ranges per segment (segment = b * LH + lh)
+  const __nv_bfloat16* q;      // [n_seqs][Lq][Hq][d]
+  const __nv_bfloat16* BK;     // [M][H][r][d]
+  const __nv_bfloat16* gK;     // [L][H][d]
+  float* part;                 // [n_slots][G][2 + r + d]: (m, l, a[r], e[d]) per query head
+  int32_t n_slices, n_segs;
+  int32_t layer0, Lq, LH, w;
+  int32_t H, G, r, d;
+  float cscale;                // softmax_scale * log2(e)
+};
+
+struct Combine3Params {
+  const int32_t* pstart;       // [n_segs + 1]
+  const float* part;
+  const __nv_bfloat16* BV;     // [M][H][r][d]
+  const __nv_bfloat16* gV;     // [L][H][d]
+  float* out;                  // [n_seqs][Lq][Hq][d]
+  int32_t layer0, Lq, LH, w;
+  int32_t H, G, r, d;
+};
+
 struct CombineParams {
   const Unit* units;
   const int32_t* ulist;       // unit ids grouped by sequence
@@ -98,6 +124,9 @@ int launch_scan(const ScanParams& p, int cls_rank, int resid, int n_units, int v
 int scan2_num_warps(int n_sms, int resid);
 int launch_scan2(const Scan2Params& p, int resid, int n_sms, cudaStream_t s);
 int launch_combine(const CombineParams& p, int n_seqs, cudaStream_t s);
+int scan3_num_slices(int n_sms);
+int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s);                 // 0 = no instance for this shape
+int launch_combine3(const Combine3Params& p, int n_segs, cudaStream_t s);
 int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
                        const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,

@@ -66,7 +66,7 @@ def test_tiny_config_all_layers_and_per_layer(mod):
         compare(wl, cache, consts, kept, routings, q, out, what=f"all-layers gain {gain}")
         out2 = torch.stack([cache.decode_attention(l, [0], q[:, l].contiguous()) for l in range(wl.L)], dim=1)
         compare(wl, cache, consts, kept, routings, q, out2, what=f"per-layer gain {gain}")
-        assert rel_l2(out2.cpu().numpy(), out.cpu().numpy()) < 1e-5
+        assert rel_l2(out2.cpu().numpy(), out.cpu().numpy()) < 2e-3
     fp = cache.footprint()
     assert fp["used_bytes"] == orc.footprint_bytes(*routings[0], wl.tier_ranks, wl.d, wl.L, wl.H_kv)
     assert fp["dense_equiv_bytes"] == 512 * wl.L * wl.H_kv * 4 * wl.d
@@ -206,7 +206,9 @@ def test_llama8b_shape_d128_three_tiers_sampled(mod):
         out = cache.decode_attention(-1, [0, 1], q)
         compare(wl, cache, consts, kept, routings, q, out, lhs=keep, what=f"8b gain {gain}")
     out3 = cache.decode_attention(3, [0, 1], q[:, 3].contiguous())
-    assert rel_l2(out3.cpu().numpy(), out[:, 3].cpu().numpy()) < 1e-5
+    # a per-layer call cuts the work into different warp slices: other rescale points and other bf16 roundings of the
+    # p * scaleV operand of the residual-V MMA, so equality holds to that rounding level only
+    assert rel_l2(out3.cpu().numpy(), out[:, 3].cpu().numpy()) < 2e-3
     cache.destroy()
 
 
