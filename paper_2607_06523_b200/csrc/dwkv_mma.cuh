@@ -46,7 +46,9 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 // offset-binary nibble pair s of word w -> bf16x2 (code_lo, code_hi), exact small integers.
 // (w >> 4s) & 0x000F000F | 0x43004300 is the bf16 pair (128 + u_lo, 128 + u_hi) = (136 + code).
 __device__ __forceinline__ uint32_t nib_to_bf16x2_biased(uint32_t w, int s) {
-  return ((w >> (4 * s)) & 0x000F000Fu) | 0x43004300u;
+  uint32_t r;   // one LOP3: (x & 0x000F000F) | 0x43004300, both constants in registers (0xEA = (a & b) | c)
+  asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(r) : "r"(w >> (4 * s)), "r"(0x000F000Fu), "r"(0x43004300u));
+  return r;
 }
 __device__ __forceinline__ uint32_t nib_to_bf16x2(uint32_t w, int s) {
   uint32_t x = nib_to_bf16x2_biased(w, s);

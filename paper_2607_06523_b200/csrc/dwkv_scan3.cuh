@@ -99,8 +99,9 @@ __device__ __forceinline__ Unit load_unit(const Unit* u) {
 template <int NKB, int D>
 struct Ring {
   static constexpr int SLOT_RAW = (NKB * 1024 > NKB * 512 + 20 * D) ? NKB * 1024 : NKB * 512 + 20 * D;
-  static constexpr int SLOT = (SLOT_RAW + 127) & ~127;
-  static constexpr int NS = (kRingBytes / SLOT) < kMaxSlots ? (kRingBytes / SLOT) : kMaxSlots;
+  static constexpr int SLOT1 = (SLOT_RAW + 127) & ~127;                 // bytes of the fattest sub-block
+  static constexpr int NS = 3;                                          // few, large stages: per-stage overhead is amortised
+  static constexpr int SLOT = (kRingBytes / NS) / SLOT1 * SLOT1;        // a whole number of fattest sub-blocks
   static_assert(NS >= 2, "ring too small for this rank");
 };
 

@@ -130,8 +130,18 @@ __device__ __forceinline__ void process_stage(State<NKB, D>& st, const uint32_t 
                                               const QRegs<NKB, D, PAIR>& q, const float cscale) {
   constexpr int SUBTOK = RESID ? 16 : 32;
   constexpr int SB1 = RESID ? NK * 512 + 20 * D : NK * 1024;
+  if constexpr (RESID || NK > 2) {
 #pragma unroll 1
-  for (int sb = 0; sb < n; ++sb) process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+    for (int sb = 0; sb < n; ++sb) process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+  } else {   // two independent sub-blocks per iteration: more instruction-level parallelism for the 2 warps per scheduler
+    int sb = 0;
+#pragma unroll 1
+    for (; sb + 2 <= n; sb += 2) {
+      process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+      process_sub<NK, RESID, NKB, D, PAIR>(st, sp + (sb + 1) * SB1, ntok - (sb + 1) * SUBTOK, lane, q, cscale);
+    }
+    if (sb < n) process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+  }
 }
 
 template <int NKB, int D, bool PAIR>
@@ -169,6 +179,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     f_ntok = un.ntok;
     f_nsub = (un.ntok + f_subtok - 1) / f_subtok;
     f_per = SLOT / f_sb1;
+    if (f_per > 2) f_per &= ~1;       // even stages: the unflagged low-rank classes are processed two sub-blocks at a time
     f_base = p.arena + un.page_off + (size_t)(p.layer0 * p.H + f_lh) * kPageLhBytes + (size_t)un.blk0 * (size_t)(f_sb1 * (kBlockTok / f_subtok));
   };
   unit_setup();
