@@ -178,7 +178,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llama8b_64k_b8")
-    ap.add_argument("--variant", type=int, default=0, help="scan_variant option of the library (A/B experiments)")
+    ap.add_argument("--opt", action="append", default=[], help="library option key=value (experiments), repeatable")
     ap.add_argument("--no-dense", action="store_true", help="skip the dense-bf16 comparison kernel")
     ap.add_argument("--no-extra", action="store_true", help="skip batch 1/4, per-layer mode and the CPU baseline")
     args = ap.parse_args()
@@ -200,8 +200,9 @@ def main():
     # ---- build the cache (every rank: its own replica of the batch, different seeds would not change the timing) ----
     routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
     cache, consts = harness.make_cache(wl, arena_bytes=harness.arena_bytes_for(wl, routings, 1), device=local)
-    if args.variant:
-        cache.set_option("scan_variant", args.variant)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        cache.set_option(k, int(v))
     sample_layers = [0]
     keep = [(l, h) for l in sample_layers for h in range(wl.H_kv)] if (rank == 0 and not args.no_extra) else []
     kept0 = None
@@ -276,7 +277,7 @@ def main():
     alg_bytes = fp["used_bytes"]                      # compressed records: 4 r_t + f_t*2*(d/2+d/8) per (l, h, token)
     achieved = alg_bytes / (scan_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "scan_kernel<NK,RESID,D,PF> (all class launches of one step)",
+                "traffic": None, "kernel": "scan3_kernel<NKB,D,PAIR> (fused q pre-projection + split-T scan, one persistent launch per step)",
                 "scan_ms": scan_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "frac_of_8TBps_nominal": achieved / 8000.0, "step_frac_of_peak": alg_bytes / (ms * 1e-3) / 1e9 / peak}
 

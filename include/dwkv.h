@@ -145,10 +145,18 @@ int64_t dwkv_seq_len(const dwkv_cache* c, int32_t seq_id);
  * reserved = bytes of arena pages currently allocated to sequences; dense_equiv = tokens * L * H_kv * 2*d*2. */
 int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved_bytes, uint64_t* dense_equiv_bytes);
 
-/* Tuning knobs for experiments (bench / tests): key in {"max_unit_blocks", "scan_variant", "time_scan"}; see DESIGN.md section 6. */
+/* Tuning knobs for experiments (bench / tests); see DESIGN.md section 6. Keys:
+ *   "time_scan"       1 = bracket the fused decode kernel with CUDA events (dwkv_get_stat "scan_ms")
+ *   "max_unit_blocks" planner: blocks (of 32 token slots) per work unit, 0 = by "unit_kb"
+ *   "unit_kb"         planner: target size of a work unit per (layer, head), KB (default 64 = one page stripe)
+ *   "n_slices"        planner: number of warp slices the step is cut into, 0 = one per warp of the persistent grid
+ *   "interleave"      planner: 1 = interleave the classes of a sequence in the work order, 0 = class after class
+ *   "cost_coef_pct", "cost_tok", "cost_resid_pct", "flag_cost_pct"   planner cost model (byte-equivalents per coefficient
+ *                     byte in %, per token, per residual byte in %, extra weight of flagged classes in %)
+ * Any change invalidates the cached plan. Errors: INVALID (unknown key). */
 int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);
 
-/* Measurement aid: with option "time_scan" = 1 every dwkv_decode_attention brackets its split-T scan launches (step a2)
+/* Measurement aid: with option "time_scan" = 1 every dwkv_decode_attention brackets its fused decode kernel (steps a1 + a2)
  * with CUDA events on `stream`; dwkv_get_stat(c, "scan_ms") waits for the last bracket and returns its duration in
  * milliseconds (negative = none recorded / error). */
 double dwkv_get_stat(dwkv_cache* c, const char* key);

@@ -106,17 +106,6 @@ struct SeqState {
   std::vector<int32_t> pages[kMaxClasses];
 };
 
-struct Plan {
-  std::vector<int32_t> seq_ids;
-  int layer_mode = -2;          // -1 = all layers, 0 = single layer
-  uint64_t version = ~0ull;
-  int n_units = 0, n_eunits = 0;
-  int cls_unit0[kMaxClasses], cls_units[kMaxClasses];
-  int n_flag_units = 0;           // flagged-class units come first in the unit list
-  size_t off_ulist = 0, off_ustart = 0, off_wstart[2] = {0, 0};   // wstart[0]: unflagged items, [1]: flagged items
-  bool valid = false;
-};
-
 struct Plan3 {                    // plan of the fused persistent decode kernel (dwkv_scan3*.cuh)
   std::vector<int32_t> seq_ids;
   int n_lsel = 0;
@@ -149,14 +138,15 @@ struct dwkv_cache {
   int64_t total_tokens = 0;
   uint64_t version = 0;
   // scratch
-  DevBuf qt, part, epart, plan_dev, plan3_dev, tokdst_dev, meta_dev;
+  DevBuf part, plan3_dev, tokdst_dev;
   int n_sms = 148;
   StagingRing ring;
-  Plan plan;
   Plan3 plan3;
   // options
   int64_t opt_max_unit_blocks = 0;   // 0 = adaptive
-  int64_t opt_scan_variant = 0;
+  int64_t opt_cost_coef_pct = 80, opt_cost_tok = 16, opt_cost_resid_pct = 200;   // planner cost model
+  int64_t opt_interleave = 0;        // planner: interleave the classes of a sequence (0 = class after class)
+  int64_t opt_unit_kb = 64;          // planner: target bytes of a work unit (per layer-head), KB
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
@@ -323,7 +313,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gK) cudaFree(c->gK);
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
-  c->qt.release(); c->part.release(); c->epart.release(); c->plan_dev.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->meta_dev.release();
+  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release();
   c->ring.release();
   if (c->ev_scan0) cudaEventDestroy(c->ev_scan0);
   if (c->ev_scan1) cudaEventDestroy(c->ev_scan1);
@@ -509,10 +499,14 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
 int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!c || !key) return fail(DWKV_E_INVALID, "NULL argument");
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
-  else if (!strcmp(key, "scan_variant")) c->opt_scan_variant = value;
   else if (!strcmp(key, "time_scan")) c->opt_time_scan = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
   else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
+  else if (!strcmp(key, "interleave")) c->opt_interleave = value;
+  else if (!strcmp(key, "cost_coef_pct")) c->opt_cost_coef_pct = value;
+  else if (!strcmp(key, "cost_tok")) c->opt_cost_tok = value;
+  else if (!strcmp(key, "cost_resid_pct")) c->opt_cost_resid_pct = value;
+  else if (!strcmp(key, "unit_kb")) c->opt_unit_kb = std::max<int64_t>(1, value);
   else return fail(DWKV_E_INVALID, std::string("unknown option ") + key);
   c->version++;
   return DWKV_OK;
@@ -539,139 +533,6 @@ double dwkv_get_stat(dwkv_cache* c, const char* key) {
 // =================================================================================================================
 namespace {
 
-// Cut every (sequence, class) page stripe into units of roughly equal BYTES. Units are ordered by class (one scan
-// launch per class); `ulist` groups unit ids by sequence for the combine. The plan depends only on the sequence set,
-// the token counts and the options, not on the layer, so per-layer calls of one step reuse it.
-int build_plan(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel, cudaStream_t st) {
-  Plan& P = c->plan;
-  const int mode = n_lsel == 1 ? 0 : -1;
-  if (P.valid && P.version == c->version && P.layer_mode == mode && (int)P.seq_ids.size() == n_seqs &&
-      std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids))
-    return DWKV_OK;
-  P.valid = false;
-  // bytes per (layer, head) over the whole call -> target unit size: about 16 items per warp of the persistent scan
-  double total_bytes = 0;
-  for (int b = 0; b < n_seqs; ++b)
-    for (int k = 0; k < c->n_classes; ++k)
-      total_bytes += (double)((c->seqs[seq_ids[b]].count[k] + kBlockTok - 1) / kBlockTok) * c->cl[k].block_bytes;
-  const int W = scan2_num_warps(c->n_sms, 0);
-  const int LHsel = n_lsel * c->geom.H;
-  double unit_bytes = total_bytes * LHsel / ((double)W * 16.0);
-  unit_bytes = std::min(std::max(unit_bytes, 8192.0), (double)kPageLhBytes);
-
-  std::vector<Unit> units_by_cls[kMaxClasses];
-  for (int b = 0; b < n_seqs; ++b) {
-    const SeqState& S = c->seqs[seq_ids[b]];
-    for (int k = 0; k < c->n_classes; ++k) {
-      if (S.count[k] == 0) continue;
-      const ClassLayout& cl = c->cl[k];
-      int64_t ub = c->opt_max_unit_blocks > 0 ? c->opt_max_unit_blocks
-                                              : std::max<int64_t>(1, (int64_t)(unit_bytes / cl.block_bytes));
-      ub = std::min<int64_t>(ub, cl.blocks_per_page);
-      const int64_t tpp = cl.tokens_per_page;
-      for (size_t pi = 0; pi < S.pages[k].size(); ++pi) {
-        const int64_t tok_in_page = std::min<int64_t>(tpp, S.count[k] - (int64_t)pi * tpp);
-        if (tok_in_page <= 0) break;
-        const int64_t nblk = (tok_in_page + kBlockTok - 1) / kBlockTok;
-        // equal-sized units inside the page
-        const int64_t nu = (nblk + ub - 1) / ub;
-        const int64_t per = (nblk + nu - 1) / nu;
-        for (int64_t b0 = 0; b0 < nblk; b0 += per) {
-          Unit u;
-          u.page_off = (int64_t)S.pages[k][pi] * (int64_t)c->page_bytes;
-          u.blk0 = (int32_t)b0;
-          u.nblk = (int32_t)std::min<int64_t>(per, nblk - b0);
-          u.ntok = (int32_t)(std::min<int64_t>(tok_in_page, (b0 + u.nblk) * kBlockTok) - b0 * kBlockTok);
-          u.cls = (int16_t)k;
-          u.b = (int16_t)b;
-          u.epart = -1;
-          u.rk = c->geom.tier_rank[k >> 1];
-          units_by_cls[k].push_back(u);
-        }
-      }
-    }
-  }
-  // unit order: flagged classes first (highest rank first), then unflagged (highest rank first)
-  std::vector<Unit> units;
-  int n_e = 0;
-  for (int k = 0; k < kMaxClasses; ++k) { P.cls_unit0[k] = 0; P.cls_units[k] = 0; }
-  for (int fl = 1; fl >= 0; --fl) {
-    for (int tr = c->cfg.n_tiers - 1; tr >= 0; --tr) {
-      const int k = 2 * tr + fl;
-      P.cls_unit0[k] = (int)units.size();
-      P.cls_units[k] = (int)units_by_cls[k].size();
-      for (Unit& u : units_by_cls[k]) {
-        if (fl) u.epart = n_e++;
-        units.push_back(u);
-      }
-    }
-    if (fl) P.n_flag_units = (int)units.size();
-  }
-  P.n_units = (int)units.size();
-  P.n_eunits = n_e;
-  std::vector<int32_t> ustart(n_seqs + 1, 0), ulist(units.size());
-  for (const Unit& u : units) ustart[u.b + 1]++;
-  for (int b = 0; b < n_seqs; ++b) ustart[b + 1] += ustart[b];
-  {
-    std::vector<int32_t> fill(ustart.begin(), ustart.end() - 1);
-    for (int i = 0; i < (int)units.size(); ++i) ulist[fill[units[i].b]++] = i;
-  }
-  // byte-balanced slices of the item list (item = unit * LHsel + lh) for the warps of the persistent scan kernels:
-  // one table over the flagged units [0, n_flag_units), one over the unflagged units [n_flag_units, n_units).
-  std::vector<int32_t> wtab[2];
-  for (int fl = 0; fl < 2; ++fl) {
-    const int u_lo = fl ? 0 : P.n_flag_units, u_hi = fl ? P.n_flag_units : (int)units.size();
-    const int Wk = scan2_num_warps(c->n_sms, fl);
-    std::vector<int32_t>& wstart = wtab[fl];
-    wstart.assign(Wk + 1, u_lo * LHsel);
-    const int n = u_hi - u_lo;
-    const double kItemOverhead = 1024.0;     // prologue / epilogue of an item, in byte-equivalents
-    std::vector<double> cum(n + 1, 0.0);
-    for (int i = 0; i < n; ++i)
-      cum[i + 1] = cum[i] + ((double)units[u_lo + i].nblk * c->cl[units[u_lo + i].cls].block_bytes + kItemOverhead) * LHsel;
-    const double C = cum[n];
-    int u = 0;
-    for (int k = 0; k <= Wk; ++k) {
-      const double target = C * (double)k / (double)Wk;
-      while (u < n && cum[u + 1] <= target) ++u;
-      int64_t pos;
-      if (u >= n) pos = (int64_t)n * LHsel;
-      else {
-        const double per = (cum[u + 1] - cum[u]) / LHsel;
-        pos = (int64_t)u * LHsel + std::min<int64_t>(LHsel, (int64_t)std::floor((target - cum[u]) / per + 0.5));
-      }
-      wstart[k] = (int32_t)((int64_t)u_lo * LHsel + pos);
-    }
-    wstart[0] = u_lo * LHsel;
-    wstart[Wk] = u_hi * LHsel;
-    for (int k = 1; k <= Wk; ++k) wstart[k] = std::max(wstart[k], wstart[k - 1]);
-  }
-  // one blob: units | ulist | ustart | wstart
-  const size_t sz_units = units.size() * sizeof(Unit);
-  P.off_ulist = (sz_units + 15) & ~(size_t)15;
-  P.off_ustart = (P.off_ulist + ulist.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  P.off_wstart[0] = (P.off_ustart + ustart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  P.off_wstart[1] = (P.off_wstart[0] + wtab[0].size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  const size_t total = P.off_wstart[1] + wtab[1].size() * sizeof(int32_t);
-  std::vector<uint8_t> blob(total, 0);
-  memcpy(blob.data() + P.off_wstart[0], wtab[0].data(), wtab[0].size() * sizeof(int32_t));
-  memcpy(blob.data() + P.off_wstart[1], wtab[1].data(), wtab[1].size() * sizeof(int32_t));
-  memcpy(blob.data(), units.data(), sz_units);
-  memcpy(blob.data() + P.off_ulist, ulist.data(), ulist.size() * sizeof(int32_t));
-  memcpy(blob.data() + P.off_ustart, ustart.data(), ustart.size() * sizeof(int32_t));
-  int rc = upload(c, c->plan_dev, blob.data(), total, st);
-  if (rc) return rc;
-  P.seq_ids.assign(seq_ids, seq_ids + n_seqs);
-  P.layer_mode = mode;
-  P.version = c->version;
-  P.valid = true;
-  return DWKV_OK;
-}
-
-}  // namespace
-
-namespace {
-
 // Plan of the fused persistent kernel. Linear order of the step's work: (sequence b, lh = layer * H + head, unit of b,
 // sub-block); a unit is one page stripe of a (sequence, class). The order is cut into n_slices contiguous slices of equal
 // COST (bytes, flagged bytes weighted by opt_flag_cost_pct) at sub-block granularity, one per warp. A slice touches one or a
@@ -692,20 +553,31 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
     ustart[b] = (int32_t)units.size();
     const SeqState& S = c->seqs[seq_ids[b]];
     double acc = 0.0;
+    // units of ~opt_unit_kb per class, then the classes are interleaved in proportion (largest remainder) so that every
+    // slice of the order sees the sequence's class mix: classes differ in instructions per byte, equal-cost slices of one
+    // class each would finish at different times
+    struct CU { Unit u; double cost_sub; int nsub; };
+    std::vector<CU> byc[kMaxClasses];
     for (int fl = 1; fl >= 0; --fl) {
       for (int tr = c->cfg.n_tiers - 1; tr >= 0; --tr) {
         const int k = 2 * tr + fl;
         if (S.count[k] == 0) continue;
         const ClassLayout& cl = c->cl[k];
         const int64_t tpp = cl.tokens_per_page;
-        const int64_t ub = c->opt_max_unit_blocks > 0 ? std::min<int64_t>(c->opt_max_unit_blocks, cl.blocks_per_page) : cl.blocks_per_page;
-        const double cost_sub = (double)cl.sub_bytes * (fl ? flag_w : 1.0);
+        int64_t ub = c->opt_max_unit_blocks > 0 ? c->opt_max_unit_blocks
+                                                : std::max<int64_t>(1, (c->opt_unit_kb * 1024 + cl.block_bytes / 2) / cl.block_bytes);
+        ub = std::min<int64_t>(ub, cl.blocks_per_page);
+        // cost of a sub-block in byte-equivalents: the warp is partly issue bound, so tokens (softmax work) and residual
+        // bytes (int4 unpack, group scales) weigh more than coefficient bytes (fit to per-warp finish times)
+        const double cost_sub = 0.01 * (double)c->opt_cost_coef_pct * 2.0 * cl.coef_bytes + (double)c->opt_cost_tok * cl.sub_tok +
+                                0.01 * (double)c->opt_cost_resid_pct * flag_w * 2.0 * (cl.code_bytes + cl.scale_bytes);
         for (size_t pi = 0; pi < S.pages[k].size(); ++pi) {
           const int64_t tok_in_page = std::min<int64_t>(tpp, S.count[k] - (int64_t)pi * tpp);
           if (tok_in_page <= 0) break;
           const int64_t nblk = (tok_in_page + kBlockTok - 1) / kBlockTok;
           for (int64_t b0 = 0; b0 < nblk; b0 += ub) {
-            Unit u;
+            CU x;
+            Unit& u = x.u;
             u.page_off = (int64_t)S.pages[k][pi] * (int64_t)c->page_bytes;
             u.blk0 = (int32_t)b0;
             u.nblk = (int32_t)std::min<int64_t>(ub, nblk - b0);
@@ -714,15 +586,30 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
             u.b = (int16_t)b;
             u.epart = -1;
             u.rk = c->geom.tier_rank[tr];
-            const int nsub = (u.ntok + cl.sub_tok - 1) / cl.sub_tok;
-            units.push_back(u);
-            upre.push_back(acc);
-            usub.push_back(cost_sub);
-            unsub.push_back(nsub);
-            acc += (double)nsub * cost_sub;
+            x.cost_sub = cost_sub;
+            x.nsub = (u.ntok + cl.sub_tok - 1) / cl.sub_tok;
+            byc[k].push_back(x);
           }
         }
       }
+    }
+    size_t taken[kMaxClasses] = {0, 0, 0, 0, 0, 0, 0, 0}, left = 0;
+    for (int k = 0; k < kMaxClasses; ++k) left += byc[k].size();
+    while (left > 0) {
+      int best = -1;
+      double best_key = 0.0;
+      for (int k = 0; k < kMaxClasses; ++k) {
+        if (taken[k] == byc[k].size()) continue;
+        const double key = c->opt_interleave ? ((double)taken[k] + 0.5) / (double)byc[k].size() : (double)((k & 1) ? 0 : 8) + (7 - k);
+        if (best < 0 || key < best_key) { best = k; best_key = key; }
+      }
+      const CU& x = byc[best][taken[best]++];
+      units.push_back(x.u);
+      upre.push_back(acc);
+      usub.push_back(x.cost_sub);
+      unsub.push_back(x.nsub);
+      acc += (double)x.nsub * x.cost_sub;
+      --left;
     }
     seq_cost[b] = acc;
     cumB[b + 1] = cumB[b] + acc * LH;
@@ -732,13 +619,14 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   const int Wmax = scan3_num_slices(c->n_sms);
   const int W = c->opt_n_slices > 0 ? (int)std::min<int64_t>(c->opt_n_slices, Wmax) : Wmax;
   const double C = cumB[n_seqs];
+  const int NSL = W;
   struct Pos { int32_t seg, u, sub; };
   auto less = [](const Pos& a, const Pos& b) { return a.seg != b.seg ? a.seg < b.seg : (a.u != b.u ? a.u < b.u : a.sub < b.sub); };
-  std::vector<Pos> pos(W + 1);
+  std::vector<Pos> pos(NSL + 1);
   const Pos end_pos{S_total, n_units, 0};
-  for (int k = 0; k <= W; ++k) {
+  for (int k = 0; k <= NSL; ++k) {
     Pos q = end_pos;
-    if (k < W) {
+    if (k < NSL) {
       const double target = C * (double)k / (double)W;
       int b = (int)(std::upper_bound(cumB.begin(), cumB.end(), target) - cumB.begin()) - 1;
       b = std::min(std::max(b, 0), n_seqs - 1);
@@ -769,15 +657,15 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
     const int b = e.seg / LH;
     return (e.u == ustart[b] && e.sub == 0) ? e.seg - 1 : e.seg;
   };
-  for (int w = 0; w < W; ++w) {
+  for (int w = 0; w < NSL; ++w) {
     if (!less(pos[w], pos[w + 1])) continue;
     for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) pstart[s + 1]++;
   }
   for (int s = 0; s < S_total; ++s) pstart[s + 1] += pstart[s];
-  std::vector<int32_t> wentry(4 * (size_t)(W + 1), 0);
-  for (int w = 0; w <= W; ++w) {
+  std::vector<int32_t> wentry(4 * (size_t)(NSL + 1), 0);
+  for (int w = 0; w <= NSL; ++w) {
     wentry[4 * w + 0] = pos[w].seg; wentry[4 * w + 1] = pos[w].u; wentry[4 * w + 2] = pos[w].sub; wentry[4 * w + 3] = 0;
-    if (w < W && less(pos[w], pos[w + 1])) {
+    if (w < NSL && less(pos[w], pos[w + 1])) {
       wentry[4 * w + 3] = pstart[pos[w].seg] + seen[pos[w].seg];
       for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) seen[s]++;
     }
@@ -795,7 +683,7 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   memcpy(blob.data() + P.off_pstart, pstart.data(), pstart.size() * sizeof(int32_t));
   int rc = upload(c, c->plan3_dev, blob.data(), total, st);
   if (rc) return rc;
-  P.n_units = n_units; P.n_slices = W; P.n_segs = S_total; P.n_slots = pstart[S_total];
+  P.n_units = n_units; P.n_slices = NSL; P.n_segs = S_total; P.n_slots = pstart[S_total];
   P.seq_ids.assign(seq_ids, seq_ids + n_seqs);
   P.n_lsel = n_lsel;
   P.version = c->version;
@@ -854,71 +742,5 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
     if (c->seqs[seq_ids[i]].tier.empty()) return fail(DWKV_E_EMPTY, "decode on an empty sequence (reading A17)");
   }
   cudaStream_t st = (cudaStream_t)stream;
-  if (c->opt_scan_variant == 0) return decode3(c, layer, n_seqs, seq_ids, q, out, st);
-  const CacheGeom& g = c->geom;
-  const int Lsel = layer < 0 ? g.L : 1, layer0 = layer < 0 ? 0 : layer, Lq = Lsel;
-  int rc = build_plan(c, n_seqs, seq_ids, Lsel, st);
-  if (rc) return rc;
-  const Plan& P = c->plan;
-  const size_t LH = (size_t)Lsel * g.H;
-  const size_t qt_elems = (size_t)n_seqs * LH * 8 * g.r;
-  CU_OK(c->qt.reserve(2 * qt_elems * sizeof(__nv_bfloat16)));
-  CU_OK(c->part.reserve(LH * (size_t)P.n_units * g.G * (2 + g.r) * sizeof(float)));
-  CU_OK(c->epart.reserve(std::max<size_t>(16, LH * (size_t)P.n_eunits * g.G * g.d * sizeof(float))));
-  const float cscale = c->softmax_scale * 1.4426950408889634f;
-
-  QPrepParams qp;
-  qp.q = (const __nv_bfloat16*)q; qp.BK = c->BK; qp.gK = c->gK;
-  qp.qt_hi = (__nv_bfloat16*)c->qt.p; qp.qt_lo = qp.qt_hi + qt_elems;
-  qp.n_seqs = n_seqs; qp.Lsel = Lsel; qp.layer0 = layer0; qp.Lq = Lq; qp.w = g.w;
-  qp.H = g.H; qp.G = g.G; qp.r = g.r; qp.d = g.d; qp.cscale = cscale;
-  c->launches += launch_qprep(qp, st);
-
-  ScanParams sp;
-  sp.arena = c->arena;
-  sp.units = (const Unit*)c->plan_dev.p;
-  sp.n_units_total = P.n_units; sp.n_eunits_total = P.n_eunits;
-  sp.qt_hi = qp.qt_hi; sp.qt_lo = qp.qt_lo; sp.q = qp.q;
-  sp.part = (float*)c->part.p; sp.epart = (float*)c->epart.p;
-  sp.Lsel = Lsel; sp.layer0 = layer0; sp.Lq = Lq; sp.H = g.H; sp.G = g.G; sp.r = g.r; sp.d = g.d; sp.cscale = cscale;
-  if (c->opt_time_scan) {
-    if (!c->ev_scan0) { CU_OK(cudaEventCreate(&c->ev_scan0)); CU_OK(cudaEventCreate(&c->ev_scan1)); }
-    CU_OK(cudaEventRecord(c->ev_scan0, st));
-  }
-  {
-    Scan2Params s2;
-    s2.arena = c->arena; s2.units = sp.units;
-    s2.n_units_total = P.n_units; s2.n_eunits_total = P.n_eunits;
-    s2.qt_hi = sp.qt_hi; s2.qt_lo = sp.qt_lo; s2.q = sp.q; s2.part = sp.part; s2.epart = sp.epart;
-    s2.Lsel = Lsel; s2.layer0 = layer0; s2.Lq = Lq; s2.LH = Lsel * g.H; s2.H = g.H; s2.G = g.G; s2.r = g.r; s2.d = g.d;
-    s2.cscale = cscale;
-    if (P.n_flag_units > 0) {                       // flagged classes: the register-hungry kernel, 8 warps per SM
-      s2.wstart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_wstart[1]);
-      c->launches += launch_scan2(s2, 1, c->n_sms, st);
-    }
-    if (c->opt_scan_variant != 1 && P.n_units > P.n_flag_units) {
-      s2.wstart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_wstart[0]);
-      c->launches += launch_scan2(s2, 0, c->n_sms, st);
-    }
-  }
-  if (c->opt_scan_variant == 1) {   // A/B: unflagged classes through the one-CTA-per-unit kernels, one launch per class
-    for (int k = c->n_classes - 2; k >= 0; k -= 2) {
-      if (P.cls_units[k] == 0) continue;
-      sp.unit0 = P.cls_unit0[k];
-      const int n = launch_scan(sp, g.tier_rank[k >> 1], 0, P.cls_units[k], 0, st);
-      if (n == 0) return fail(DWKV_E_INVALID, "no scan kernel for this class");
-      c->launches += n;
-    }
-  }
-  if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_scan1, st)); c->scan_timed = true; }
-  CombineParams cp;
-  cp.units = sp.units;
-  cp.ulist = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_ulist);
-  cp.ustart = (const int32_t*)((const uint8_t*)c->plan_dev.p + P.off_ustart);
-  cp.part = sp.part; cp.epart = sp.epart; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
-  cp.n_units_total = P.n_units; cp.n_eunits_total = P.n_eunits;
-  cp.Lsel = Lsel; cp.layer0 = layer0; cp.Lq = Lq; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;
-  c->launches += launch_combine(cp, n_seqs, st);
-  CU_OK(cudaGetLastError());
-  return DWKV_OK;
+  return decode3(c, layer, n_seqs, seq_ids, q, out, st);
 }

@@ -14,92 +14,90 @@ bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
 namespace {
 using namespace dwkv::dev;
 
-constexpr int kChunk = 64;
-
-__global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
-  __shared__ float red[16][8];
-  __shared__ float mstar[8], lstar[8];
-  __shared__ float wbuf[kChunk][8];
-  __shared__ float astar[8][64];
-  const int seg = blockIdx.x, tid = threadIdx.x;
+// One warp merges the partials of one (segment, query head) and writes o[head, :]. Lanes run over partials for the
+// (m, l) pass, over rank columns for a*, over channels (D / 32 each) for e* and the back-projection.
+template <int D>
+__device__ __forceinline__ void combine_head(const Combine3Params& p, const int seg, const int gq, const int lane) {
+  constexpr int CPL = D / 32;                       // channels per lane
   const int b = seg / p.LH, lh = seg - b * p.LH;
   const int layer = p.layer0 + lh / p.H, h = lh % p.H;
-  const int G = p.G, r = p.r, d = p.d, PR = 2 + p.r + p.d;
-  const int P0 = p.pstart[seg], n = p.pstart[seg + 1] - P0;
-  const float* part = p.part + (size_t)P0 * (size_t)(G * PR);
-  {
-    const int gq = tid & 7, sl = tid >> 3;
-    float mx = -INFINITY;
-    if (gq < G)
-      for (int k = sl; k < n; k += 16) mx = fmaxf(mx, part[(size_t)k * (G * PR) + gq * PR]);
-    red[sl][gq] = mx;
-    __syncthreads();
-    if (tid < 8) {
-      float v = red[0][tid];
-      for (int s2 = 1; s2 < 16; ++s2) v = fmaxf(v, red[s2][tid]);
-      mstar[tid] = v;
-    }
-    __syncthreads();
-  }
-  float lacc = 0.f;
-  float areg[4] = {0.f, 0.f, 0.f, 0.f};   // elements idx = tid + 128*x of the G x r matrix a*
-  float ereg[8];                          // thread i < d: e*[gq][i]
+  const int G = p.G, r = p.r, PR = 2 + p.r + D;
+  const int P0 = __ldg(p.pstart + seg), n = __ldg(p.pstart + seg + 1) - P0;
+  const float* part = p.part + ((size_t)P0 * G + gq) * PR;       // partial k of this head: part + k * G * PR
+  const size_t stride = (size_t)G * PR;
+  // basis rows and gate of this lane's channels: independent of the partials, issued first
+  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
+  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
+  float mstar = -INFINITY;
+  for (int k = lane; k < n; k += 32) mstar = fmaxf(mstar, part[k * stride]);
 #pragma unroll
-  for (int gq = 0; gq < 8; ++gq) ereg[gq] = 0.f;
-  for (int c0 = 0; c0 < n; c0 += kChunk) {
-    const int nc = min(kChunk, n - c0);
-    const float* pc = part + (size_t)c0 * (G * PR);
-    for (int idx = tid; idx < nc * G; idx += 128) {
-      const int k = idx / G, gq = idx - k * G;
-      const float m = pc[(size_t)k * (G * PR) + gq * PR];
-      wbuf[k][gq] = (m == -INFINITY) ? 0.f : ex2(m - mstar[gq]);
-    }
-    __syncthreads();
-    if (tid < G)
-      for (int k = 0; k < nc; ++k) lacc = fmaf(wbuf[k][tid], pc[(size_t)k * (G * PR) + tid * PR + 1], lacc);
+  for (int o = 16; o > 0; o >>= 1) mstar = fmaxf(mstar, __shfl_xor_sync(kFull, mstar, o));
+  float lstar = 0.f, a0 = 0.f, a1 = 0.f, e[CPL];
 #pragma unroll
-    for (int x = 0; x < 4; ++x) {
-      const int idx = tid + 128 * x;
-      if (idx < G * r) {
-        const int gq = idx / r, j = idx - gq * r;
-        float a = areg[x];
-        for (int k = 0; k < nc; ++k) a = fmaf(wbuf[k][gq], pc[(size_t)k * (G * PR) + gq * PR + 2 + j], a);
-        areg[x] = a;
+  for (int c = 0; c < CPL; ++c) e[c] = 0.f;
+  for (int k0 = 0; k0 < n; k0 += 32) {
+    const int kk = k0 + lane;
+    float wk = 0.f;
+    if (kk < n) {
+      const float2 ml = *reinterpret_cast<const float2*>(part + kk * stride);
+      wk = (ml.x == -INFINITY) ? 0.f : ex2(ml.x - mstar);
+      lstar = fmaf(wk, ml.y, lstar);
+    }
+    const int nc = min(32, n - k0);
+#pragma unroll 4
+    for (int k = 0; k < nc; ++k) {
+      const float w = __shfl_sync(kFull, wk, k);
+      const float* rec = part + (size_t)(k0 + k) * stride + 2;
+      if (lane < r) a0 = fmaf(w, rec[lane], a0);
+      if (lane + 32 < r) a1 = fmaf(w, rec[lane + 32], a1);
+      if constexpr (CPL == 4) {
+        const float2 v = *reinterpret_cast<const float2*>(rec + r + lane * 4);       // records are 8-byte aligned only
+        const float2 u = *reinterpret_cast<const float2*>(rec + r + lane * 4 + 2);
+        e[0] = fmaf(w, v.x, e[0]); e[1] = fmaf(w, v.y, e[1]); e[2] = fmaf(w, u.x, e[2]); e[3] = fmaf(w, u.y, e[3]);
+      } else {
+        const float2 v = *reinterpret_cast<const float2*>(rec + r + lane * 2);
+        e[0] = fmaf(w, v.x, e[0]); e[1] = fmaf(w, v.y, e[1]);
       }
     }
-    if (tid < d) {
-      for (int k = 0; k < nc; ++k) {
-        const float* e = pc + (size_t)k * (G * PR) + 2 + r + tid;
+  }
 #pragma unroll
-        for (int gq = 0; gq < 8; ++gq)
-          if (gq < G) ereg[gq] = fmaf(wbuf[k][gq], e[gq * PR], ereg[gq]);
-      }
+  for (int o = 16; o > 0; o >>= 1) lstar += __shfl_xor_sync(kFull, lstar, o);
+  float acc[CPL];
+#pragma unroll
+  for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
+#pragma unroll 8
+  for (int j = 0; j < r; ++j) {
+    const float aj = __shfl_sync(kFull, j < 32 ? a0 : a1, j & 31);
+    if constexpr (CPL == 4) {
+      const uint2 bw = __ldg(reinterpret_cast<const uint2*>(BV + (size_t)j * D));
+      acc[0] = fmaf(aj, __uint_as_float(bw.x << 16), acc[0]); acc[1] = fmaf(aj, __uint_as_float(bw.x & 0xffff0000u), acc[1]);
+      acc[2] = fmaf(aj, __uint_as_float(bw.y << 16), acc[2]); acc[3] = fmaf(aj, __uint_as_float(bw.y & 0xffff0000u), acc[3]);
+    } else {
+      const uint32_t bw = __ldg(reinterpret_cast<const uint32_t*>(BV + (size_t)j * D));
+      acc[0] = fmaf(aj, __uint_as_float(bw << 16), acc[0]); acc[1] = fmaf(aj, __uint_as_float(bw & 0xffff0000u), acc[1]);
     }
-    __syncthreads();
   }
-  if (tid < G) lstar[tid] = lacc;
-#pragma unroll
-  for (int x = 0; x < 4; ++x) {
-    const int idx = tid + 128 * x;
-    if (idx < G * r) astar[idx / r][idx % r] = areg[x];
+  const float inv = 1.f / lstar;
+  float* out = p.out + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * G) + (size_t)h * G + gq) * D + lane * CPL;
+  if constexpr (CPL == 4) {
+    const uint2 gw = __ldg(reinterpret_cast<const uint2*>(gVp));
+    float4 o;
+    o.x = (__uint_as_float(gw.x << 16) * acc[0] + e[0]) * inv; o.y = (__uint_as_float(gw.x & 0xffff0000u) * acc[1] + e[1]) * inv;
+    o.z = (__uint_as_float(gw.y << 16) * acc[2] + e[2]) * inv; o.w = (__uint_as_float(gw.y & 0xffff0000u) * acc[3] + e[3]) * inv;
+    *reinterpret_cast<float4*>(out) = o;
+  } else {
+    const uint32_t gw = __ldg(reinterpret_cast<const uint32_t*>(gVp));
+    float2 o;
+    o.x = (__uint_as_float(gw << 16) * acc[0] + e[0]) * inv; o.y = (__uint_as_float(gw & 0xffff0000u) * acc[1] + e[1]) * inv;
+    *reinterpret_cast<float2*>(out) = o;
   }
-  __syncthreads();
-  if (tid < d) {
-    const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * d + tid;
-    const float gv = __bfloat162float(p.gV[((size_t)layer * p.H + h) * d + tid]);
-    float acc[8];
-#pragma unroll
-    for (int gq = 0; gq < 8; ++gq) acc[gq] = 0.f;
-    for (int j = 0; j < r; ++j) {
-      const float bv = __bfloat162float(BV[(size_t)j * d]);
-#pragma unroll
-      for (int gq = 0; gq < 8; ++gq) acc[gq] = fmaf(astar[gq][j], bv, acc[gq]);
-    }
-    float* out = p.out + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * G) + (size_t)h * G) * d + tid;
-#pragma unroll
-    for (int gq = 0; gq < 8; ++gq)
-      if (gq < G) out[(size_t)gq * d] = (gv * acc[gq] + ereg[gq]) / lstar[gq];
-  }
+}
+
+// grid = segments, 4 warps per CTA: warp w merges heads w, w + 4
+template <int D>
+__global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
+  const int seg = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int gq = warp; gq < p.G; gq += 4) combine_head<D>(p, seg, gq, lane);
 }
 
 }  // namespace
@@ -115,7 +113,8 @@ int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s) {
 }
 
 int launch_combine3(const Combine3Params& p, int n_segs, cudaStream_t s) {
-  combine3_kernel<<<n_segs, 128, 0, s>>>(p);
+  if (p.d == 128) combine3_kernel<128><<<n_segs, 128, 0, s>>>(p);
+  else combine3_kernel<64><<<n_segs, 128, 0, s>>>(p);
   return 1;
 }
 

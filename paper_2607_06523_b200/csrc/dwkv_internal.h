@@ -9,8 +9,8 @@
 
 namespace dwkv {
 
-// One work unit of the split-T scan: a run of blocks of one (sequence, class) inside one page; the same unit is
-// processed for every (layer, kv head) by grid dimension y.
+// One work unit of the split-T scan: a run of blocks of one (sequence, class) inside one page stripe; the same unit
+// exists for every (layer, kv head) (the stripe of (l, h) lies (l*H + h) * kPageLhBytes into the page).
 struct __align__(16) Unit {
   int64_t page_off;   // byte offset of the page in the arena
   int32_t blk0;       // first block inside the page's (l,h) stripe
@@ -18,39 +18,8 @@ struct __align__(16) Unit {
   int32_t ntok;       // valid tokens in the unit (last block may be partial)
   int16_t cls;        // class id = 2*tier + flag
   int16_t b;          // index of the sequence in this call's seq_ids
-  int32_t epart;      // index into the residual-V partial buffer, -1 for unflagged classes
+  int32_t epart;      // unused (-1)
   int32_t rk;         // rank of the class
-};
-
-struct ScanParams {
-  const uint8_t* arena;
-  const Unit* units;          // all units of the plan
-  int32_t unit0;              // first unit of the class handled by this launch
-  int32_t n_units_total;      // number of units in the plan (stride of the partial buffers)
-  int32_t n_eunits_total;     // number of flagged-class units in the plan
-  const __nv_bfloat16* qt_hi; // [n_seqs][Lsel][H][8][r]  q~ high part (bf16), rows >= G are zero
-  const __nv_bfloat16* qt_lo; // same shape, low part: q~ = hi + lo to 16 significant bits
-  const __nv_bfloat16* q;     // [n_seqs][Lq][Hq][d] raw queries (residual-K term)
-  float* part;                // [Lsel*H][n_units_total][G][2 + r]  (m, l, a[r]) per query head
-  float* epart;               // [Lsel*H][n_eunits_total][G][d]
-  int32_t Lsel, layer0, Lq;   // layers in this call, first absolute layer, layer stride of q (1 or L)
-  int32_t H, G, r, d;
-  float cscale;               // softmax_scale * log2(e)
-};
-
-struct Scan2Params {            // persistent scan (dwkv_scan2.cu)
-  const uint8_t* arena;
-  const Unit* units;
-  const int32_t* wstart;       // [n_warps + 1] item positions; item = unit * LH + (lsel * H + h)
-  int32_t n_units_total, n_eunits_total;
-  const __nv_bfloat16* qt_hi;
-  const __nv_bfloat16* qt_lo;
-  const __nv_bfloat16* q;
-  float* part;
-  float* epart;
-  int32_t Lsel, layer0, Lq, LH;
-  int32_t H, G, r, d;
-  float cscale;
 };
 
 struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.cuh)
@@ -79,31 +48,6 @@ struct Combine3Params {
   int32_t H, G, r, d;
 };
 
-struct CombineParams {
-  const Unit* units;
-  const int32_t* ulist;       // unit ids grouped by sequence
-  const int32_t* ustart;      // [n_seqs+1] ranges into ulist
-  const float* part;
-  const float* epart;
-  const __nv_bfloat16* BV;    // [M][H][r][d]
-  const __nv_bfloat16* gV;    // [L][H][d]
-  float* out;                 // [n_seqs][Lq][Hq][d]
-  int32_t n_units_total, n_eunits_total;
-  int32_t Lsel, layer0, Lq, w;
-  int32_t H, G, r, d;
-};
-
-struct QPrepParams {
-  const __nv_bfloat16* q;     // [n_seqs][Lq][Hq][d]
-  const __nv_bfloat16* BK;    // [M][H][r][d]
-  const __nv_bfloat16* gK;    // [L][H][d]
-  __nv_bfloat16* qt_hi;
-  __nv_bfloat16* qt_lo;
-  int32_t n_seqs, Lsel, layer0, Lq, w;
-  int32_t H, G, r, d;
-  float cscale;
-};
-
 // per-token destination for the scatter / gather kernels
 struct TokDst {
   int64_t page_off;   // page of the token's class
@@ -118,12 +62,7 @@ struct CacheGeom {
   int32_t tier_rank[4];
 };
 
-// kernel launchers (dwkv_scan.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
-int launch_qprep(const QPrepParams& p, cudaStream_t s);
-int launch_scan(const ScanParams& p, int cls_rank, int resid, int n_units, int variant, cudaStream_t s);
-int scan2_num_warps(int n_sms, int resid);
-int launch_scan2(const Scan2Params& p, int resid, int n_sms, cudaStream_t s);
-int launch_combine(const CombineParams& p, int n_seqs, cudaStream_t s);
+// kernel launchers (dwkv_combine3.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
 int scan3_num_slices(int n_sms);
 int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s);                 // 0 = no instance for this shape
 int launch_combine3(const Combine3Params& p, int n_segs, cudaStream_t s);

@@ -159,17 +159,18 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
   }
   __syncwarp();
   const int gw = warp * gridDim.x + blockIdx.x;      // consecutive slices of the linear order go to different SMs
+
   if (gw >= p.n_slices) return;
   const int4 ws = __ldg(p.wentry + gw), we = __ldg(p.wentry + gw + 1);
   if (ws.x == we.x && ws.y == we.y && ws.z == we.z) return;
 
-  // ---- fetch cursor (warp-uniform) ------------------------------------------------------------------------------------
+  // ---- fetch cursor (warp-uniform) over the slice [ws, we) of the linear order ----------------------------------------------
   int f_seg = ws.x, f_u = ws.y, f_sub = ws.z;
   int f_b = f_seg / p.LH, f_lh = f_seg - f_b * p.LH;
   int f_ubeg = __ldg(p.ustart + f_b), f_uend = __ldg(p.ustart + f_b + 1);
   bool f_on = true;
-  int f_code, f_nsub, f_per, f_sb1, f_subtok, f_ntok;
-  const uint8_t* f_base;
+  int f_code = 0, f_nsub = 0, f_per = 0, f_sb1 = 0, f_subtok = 0, f_ntok = 0;
+  const uint8_t* f_base = nullptr;
   auto unit_setup = [&]() {
     const Unit un = load_unit(p.units + f_u);
     const int nk = un.rk >> 3, fl = un.cls & 1;
@@ -192,7 +193,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     const int n = min(f_per, limit - f_sub);
     if (lane == 0) {
       const int ntok = min(f_ntok - f_sub * f_subtok, n * f_subtok);
-      sts128(descs + 16 * k, f_code, n, ntok, f_seg);
+      sts128(descs + 16 * k, f_code | (n << 16), ntok, f_seg, 0);
       mbar_expect_tx(bars + 8 * k, (uint32_t)(n * f_sb1));
       bulk_g2s(ring + k * SLOT, f_base + (size_t)f_sub * f_sb1, (uint32_t)(n * f_sb1), bars + 8 * k);
     }
@@ -228,22 +229,23 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
   uint32_t phase = 0u;
   while (true) {
     const uint4 dsc = lds128(descs + 16 * k_c);
-    const int n = (int)dsc.y;
+    const int n = (int)(dsc.x >> 16);
     if (n == 0) break;
-    if ((int)dsc.w != cur_seg) {
+    const int seg = (int)dsc.z;
+    if (seg != cur_seg) {
       if (cur_seg >= 0) {
         flush_partial<NKB, D, PAIR>(st, p, slot_next, lane);
-        slot_next = __ldg(p.pstart + (int)dsc.w);     // later segments are entered at their start: first partial slot
+        slot_next = __ldg(p.pstart + seg);     // a segment entered inside a slice is entered at its start: its first slot
       }
-      cur_seg = (int)dsc.w;
       state_reset<NKB, D>(st);
-      segment_prologue<NKB, D, PAIR>(q, p, cur_seg, lane);
+      segment_prologue<NKB, D, PAIR>(q, p, seg, lane);
+      cur_seg = seg;
     }
     mbar_wait(bars + 8 * k_c, (phase >> k_c) & 1u);
     phase ^= 1u << k_c;
     const uint32_t sp = ring + k_c * SLOT;
-    const int ntok = (int)dsc.z;
-    switch (dsc.x) {
+    const int ntok = (int)dsc.y;
+    switch (dsc.x & 0xffffu) {
       case 0x001: process_stage<1, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
       case 0x101: process_stage<1, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
       case 0x002: process_stage<2, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;

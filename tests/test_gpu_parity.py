@@ -137,20 +137,23 @@ def test_raw_mode_b_codes_and_minus_eight(mod):
 
 
 def test_split_invariance_p11(mod):
-    """Result independent of the work-list shape: one block per unit vs whole pages (pin P11). The split changes each
-    unit's running max, hence the bf16 rounding of the unnormalised p fed to the value MMA (error
-    budget ~1-2e-3 rel-L2), so the bar is that rounding level, and every variant must also meet the oracle tolerance."""
+    """Result independent of the work split (pin P11): one block per unit, a single warp slice for the whole step, a few
+    slices, class-interleaved order with tiny units, and the default plan. Different cuts move the rescale points and the
+    bf16 roundings of the p * scaleV operand of the residual-V MMA, so the bar between variants is
+    that rounding level (1e-3 rel-L2); every variant must also meet the oracle tolerance."""
     binding, harness = mod
     wl = gen.WORKLOADS["tiny"]
     routings = [gen.make_routing(wl, 0)]
     cache, consts, kept = load(harness, wl, routings)
     q = gen.make_q(wl, device="cuda", gain=4.0)
     outs = []
-    for ub in (1, 2, 1 << 20, 0):
-        cache.set_option("max_unit_blocks", ub)
+    base = {"max_unit_blocks": 0, "n_slices": 0, "interleave": 0, "unit_kb": 64}
+    for change in ({"max_unit_blocks": 1}, {"n_slices": 1}, {"n_slices": 7}, {"interleave": 1, "unit_kb": 1}, {}):
+        for k, v in {**base, **change}.items():
+            cache.set_option(k, v)
         outs.append(cache.decode_attention(-1, [0], q).double().cpu().numpy())
     for o in outs[1:]:
-        assert rel_l2(o, outs[0]) < 4e-3
+        assert rel_l2(o, outs[0]) < 1e-3
     for o in outs:
         compare(wl, cache, consts, kept, routings, q, torch.as_tensor(o), what="split variant")
     cache.destroy()
