@@ -186,16 +186,11 @@ def main():
     if args.impl == "reference":
         return run_reference(args, wl)
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2607_06523_b200 import harness, binding, replicas
+    rank, world, local = replicas.env_rank()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
-
-    from paper_2607_06523_b200 import harness, binding
+    replicas.init("nccl", dev)          # replicas only: the group serves the barrier and the max over ranks of the time
 
     # ---- build the cache (every rank: its own replica of the batch, different seeds would not change the timing) ----
     routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
@@ -228,17 +223,13 @@ def main():
 
     # ---- timed region: K steps, inputs resident in HBM ------------------------------------------------------------
     step(); torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
+    replicas.barrier()
     l0 = cache.launch_count()
     with ClockSampler(local) as cs:
         ms = time_steps(step, args.steps, args.warmup)
     launches = (cache.launch_count() - l0) * args.steps // (args.steps + args.warmup)
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = tokens_per_step * world / (ms * 1e-3)
+    ms = replicas.max_over_ranks(ms, dev)
+    value = replicas.aggregate_throughput(tokens_per_step, ms, world)
 
     # ---- e2e: host q -> device, decode, result -> host, every step ------------------------------------------------
     q_host = [q.cpu().pin_memory() for q in qs]
@@ -258,11 +249,8 @@ def main():
     for _ in range(args.steps):
         step_e2e()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / args.steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e = {"value": tokens_per_step * world / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+    e2e_ms = replicas.max_over_ranks(e2e_ms, dev)
+    e2e = {"value": replicas.aggregate_throughput(tokens_per_step, e2e_ms, world), "unit": UNIT, "ms_per_step": e2e_ms,
            "h2d_bytes_per_step": q_dev.numel() * 2, "d2h_bytes_per_step": out.numel() * 4}
 
     # ---- roofline of the dominant kernel group (split-T scan), CUDA events inside the library on the launch stream --
@@ -301,6 +289,21 @@ def main():
             for l in range(L):
                 cache.decode_attention(l, seq_ids, ql[l], ol[l])
         extra["per_layer_mode_us_per_step"] = time_steps(per_layer, max(3, args.steps // 2), args.warmup) * 1e3
+        try:        # the same L per-layer calls captured once in a CUDA graph (no host work between the layers)
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                per_layer()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=side):
+                    per_layer()
+            torch.cuda.current_stream().wait_stream(side)
+            extra["per_layer_graph_us_per_step"] = time_steps(graph.replay, max(3, args.steps // 2), args.warmup) * 1e3
+            got = torch.stack(ol, dim=1)
+            cache.decode_attention(-1, seq_ids, qs[0], out)
+            extra["per_layer_graph_vs_all_layers_rel_l2"] = float((got - out).norm() / out.norm())
+        except Exception as ex:  # pragma: no cover
+            extra["per_layer_graph_error"] = repr(ex)[:200]
         # CPU oracle on the host cores: bounded sample, and parity of the sampled slices at full size
         tier, flag = routings[0]
         o_gpu = out.clone()
@@ -359,7 +362,7 @@ def main():
         print(json.dumps(line))
     cache.destroy()
     if world > 1:
-        dist.destroy_process_group()
+        torch.distributed.destroy_process_group()
 
 
 if __name__ == "__main__":

@@ -1,5 +1,5 @@
 // dwkv_combine3.cu -- a3: split-combine + back-projection, and the dispatcher of the fused
-// decode kernel instances. One CTA per segment (sequence b, layer, kv head): log-sum-exp merge of the few warp partials
+// decode kernel instances. One CTA per (segment = (sequence b, layer, kv head), query head): log-sum-exp merge of the warp partials
 // (m, l, a[r], e[d]) the scan left for the segment, then  o = ( gV * (BV^T a) + e ) / l  for the G query heads.
 #include "dwkv_internal.h"
 #include "dwkv_mma.cuh"
@@ -14,54 +14,86 @@ bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
 namespace {
 using namespace dwkv::dev;
 
-// One warp merges the partials of one (segment, query head) and writes o[head, :]. Lanes run over partials for the
-// (m, l) pass, over rank columns for a*, over channels (D / 32 each) for e* and the back-projection.
+// One CTA of 4 warps merges the partials of one (segment, query head) and writes o[head, :]. The warps split the partial
+// list (warp w takes partials w, w+4, ...: matters in per-layer calls, where a segment has ~150 partials; all-layer steps
+// have ~2-6), lanes run over rank columns for a*, over channels (D / 32 each) for e* and the back-projection.
 template <int D>
-__device__ __forceinline__ void combine_head(const Combine3Params& p, const int seg, const int gq, const int lane) {
+__global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
   constexpr int CPL = D / 32;                       // channels per lane
+  __shared__ float sh_l[4];
+  __shared__ float sh_a[4][64];
+  __shared__ float sh_e[4][D];
+  const int seg = blockIdx.x, gq = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int b = seg / p.LH, lh = seg - b * p.LH;
   const int layer = p.layer0 + lh / p.H, h = lh % p.H;
   const int G = p.G, r = p.r, PR = 2 + p.r + D;
   const int P0 = __ldg(p.pstart + seg), n = __ldg(p.pstart + seg + 1) - P0;
-  const float* part = p.part + ((size_t)P0 * G + gq) * PR;       // partial k of this head: part + k * G * PR
+  const float* part = p.part + ((size_t)P0 * G + gq) * PR;       // partial k of this head: part + k * stride
   const size_t stride = (size_t)G * PR;
-  // basis rows and gate of this lane's channels: independent of the partials, issued first
-  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
-  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
+  // pass 1: m* over all partials (every warp computes it: n is small, the loads hit L2)
   float mstar = -INFINITY;
-  for (int k = lane; k < n; k += 32) mstar = fmaxf(mstar, part[k * stride]);
+  for (int k0 = lane; k0 < n; k0 += 32 * 8) {       // 8 independent loads in flight per lane
+    float v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = (k0 + 32 * u < n) ? part[(size_t)(k0 + 32 * u) * stride] : -INFINITY;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) mstar = fmaxf(mstar, v[u]);
+  }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) mstar = fmaxf(mstar, __shfl_xor_sync(kFull, mstar, o));
-  float lstar = 0.f, a0 = 0.f, a1 = 0.f, e[CPL];
+  // pass 2: this warp's partials w, w+4, ...; lane j of a 32-batch owns the weight of the batch's j-th partial
+  float lsum = 0.f, a0 = 0.f, a1 = 0.f, e[CPL];
 #pragma unroll
   for (int c = 0; c < CPL; ++c) e[c] = 0.f;
-  for (int k0 = 0; k0 < n; k0 += 32) {
-    const int kk = k0 + lane;
+  const int nw = (n > warp) ? (n - warp + 3) / 4 : 0;            // partials of this warp
+  for (int i0 = 0; i0 < nw; i0 += 32) {
+    const int i = i0 + lane;
     float wk = 0.f;
-    if (kk < n) {
-      const float2 ml = *reinterpret_cast<const float2*>(part + kk * stride);
+    if (i < nw) {
+      const float2 ml = *reinterpret_cast<const float2*>(part + (size_t)(warp + 4 * i) * stride);
       wk = (ml.x == -INFINITY) ? 0.f : ex2(ml.x - mstar);
-      lstar = fmaf(wk, ml.y, lstar);
+      lsum = fmaf(wk, ml.y, lsum);
     }
-    const int nc = min(32, n - k0);
-#pragma unroll 4
-    for (int k = 0; k < nc; ++k) {
-      const float w = __shfl_sync(kFull, wk, k);
-      const float* rec = part + (size_t)(k0 + k) * stride + 2;
-      if (lane < r) a0 = fmaf(w, rec[lane], a0);
-      if (lane + 32 < r) a1 = fmaf(w, rec[lane + 32], a1);
-      if constexpr (CPL == 4) {
-        const float2 v = *reinterpret_cast<const float2*>(rec + r + lane * 4);       // records are 8-byte aligned only
-        const float2 u = *reinterpret_cast<const float2*>(rec + r + lane * 4 + 2);
-        e[0] = fmaf(w, v.x, e[0]); e[1] = fmaf(w, v.y, e[1]); e[2] = fmaf(w, u.x, e[2]); e[3] = fmaf(w, u.y, e[3]);
-      } else {
-        const float2 v = *reinterpret_cast<const float2*>(rec + r + lane * 2);
-        e[0] = fmaf(w, v.x, e[0]); e[1] = fmaf(w, v.y, e[1]);
+    const int nc = min(32, nw - i0);
+    for (int k0 = 0; k0 < nc; k0 += 8) {              // explicit batches of 8 partials: all loads issued before any use
+      float w[8], va0[8], va1[8];
+      float2 ve[8][CPL / 2];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int k = k0 + u;
+        w[u] = __shfl_sync(kFull, wk, k & 31);          // lanes >= nc hold weight 0
+        const float* rec = part + (size_t)(warp + 4 * (i0 + min(k, nc - 1))) * stride + 2;
+        va0[u] = (lane < r) ? rec[lane] : 0.f;
+        va1[u] = (lane + 32 < r) ? rec[lane + 32] : 0.f;
+#pragma unroll
+        for (int c = 0; c < CPL / 2; ++c) ve[u][c] = *reinterpret_cast<const float2*>(rec + r + lane * CPL + 2 * c);   // 8-byte aligned
+      }
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const float wu = (k0 + u < nc) ? w[u] : 0.f;
+        a0 = fmaf(wu, va0[u], a0);
+        a1 = fmaf(wu, va1[u], a1);
+#pragma unroll
+        for (int c = 0; c < CPL / 2; ++c) { e[2 * c] = fmaf(wu, ve[u][c].x, e[2 * c]); e[2 * c + 1] = fmaf(wu, ve[u][c].y, e[2 * c + 1]); }
       }
     }
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) lstar += __shfl_xor_sync(kFull, lstar, o);
+  for (int o = 16; o > 0; o >>= 1) lsum += __shfl_xor_sync(kFull, lsum, o);
+  if (lane == 0) sh_l[warp] = lsum;
+  sh_a[warp][lane] = a0; sh_a[warp][lane + 32] = a1;
+#pragma unroll
+  for (int c = 0; c < CPL; ++c) sh_e[warp][lane * CPL + c] = e[c];
+  __syncthreads();
+  if (warp != 0) return;
+  const float lstar = sh_l[0] + sh_l[1] + sh_l[2] + sh_l[3];
+  a0 = sh_a[0][lane] + sh_a[1][lane] + sh_a[2][lane] + sh_a[3][lane];
+  a1 = sh_a[0][lane + 32] + sh_a[1][lane + 32] + sh_a[2][lane + 32] + sh_a[3][lane + 32];
+#pragma unroll
+  for (int c = 0; c < CPL; ++c) e[c] = sh_e[0][lane * CPL + c] + sh_e[1][lane * CPL + c] + sh_e[2][lane * CPL + c] + sh_e[3][lane * CPL + c];
+  // back-projection o = (gV * (BV^T a*) + e*) / l*: basis rows as coalesced loads, a*_j broadcast by shuffle
+  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
+  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
   float acc[CPL];
 #pragma unroll
   for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
@@ -93,13 +125,6 @@ __device__ __forceinline__ void combine_head(const Combine3Params& p, const int 
   }
 }
 
-// grid = segments, 4 warps per CTA: warp w merges heads w, w + 4
-template <int D>
-__global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
-  const int seg = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int gq = warp; gq < p.G; gq += 4) combine_head<D>(p, seg, gq, lane);
-}
-
 }  // namespace
 
 int scan3_num_slices(int n_sms) { return n_sms * 8; }
@@ -113,8 +138,9 @@ int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s) {
 }
 
 int launch_combine3(const Combine3Params& p, int n_segs, cudaStream_t s) {
-  if (p.d == 128) combine3_kernel<128><<<n_segs, 128, 0, s>>>(p);
-  else combine3_kernel<64><<<n_segs, 128, 0, s>>>(p);
+  const dim3 grid(n_segs, p.G);
+  if (p.d == 128) combine3_kernel<128><<<grid, 128, 0, s>>>(p);
+  else combine3_kernel<64><<<grid, 128, 0, s>>>(p);
   return 1;
 }
 
