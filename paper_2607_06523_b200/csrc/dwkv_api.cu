@@ -144,8 +144,9 @@ struct dwkv_cache {
   Plan3 plan3;
   // options
   int64_t opt_max_unit_blocks = 0;   // 0 = adaptive
-  int64_t opt_cost_coef_pct = 80, opt_cost_tok = 16, opt_cost_resid_pct = 200;   // planner cost model
+  int64_t opt_cost_coef_pct = 80, opt_cost_tok = 24, opt_cost_resid_pct = 235, opt_cost_seg = 24576;   // planner cost model
   int64_t opt_interleave = 0;        // planner: interleave the classes of a sequence (0 = class after class)
+  int64_t opt_stamps_ptr = 0;        // device pointer [n_slices] u64 for per-warp end stamps (measurement aid), 0 = off
   int64_t opt_unit_kb = 64;          // planner: target bytes of a work unit (per layer-head), KB
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
@@ -503,8 +504,10 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
   else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
   else if (!strcmp(key, "interleave")) c->opt_interleave = value;
+  else if (!strcmp(key, "stamps_ptr")) c->opt_stamps_ptr = value;
   else if (!strcmp(key, "cost_coef_pct")) c->opt_cost_coef_pct = value;
   else if (!strcmp(key, "cost_tok")) c->opt_cost_tok = value;
+  else if (!strcmp(key, "cost_seg")) c->opt_cost_seg = std::max<int64_t>(0, value);
   else if (!strcmp(key, "cost_resid_pct")) c->opt_cost_resid_pct = value;
   else if (!strcmp(key, "unit_kb")) c->opt_unit_kb = std::max<int64_t>(1, value);
   else return fail(DWKV_E_INVALID, std::string("unknown option ") + key);
@@ -546,6 +549,7 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   P.valid = false;
   const int LH = n_lsel * c->geom.H;
   const double flag_w = (double)c->opt_flag_cost_pct / 100.0;
+  const double seg_ovh = (double)c->opt_cost_seg;
   std::vector<Unit> units;
   std::vector<int32_t> ustart(n_seqs + 1, 0), unsub;
   std::vector<double> upre, usub, seq_cost(n_seqs, 0.0), cumB(n_seqs + 1, 0.0);
@@ -611,8 +615,8 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
       acc += (double)x.nsub * x.cost_sub;
       --left;
     }
-    seq_cost[b] = acc;
-    cumB[b + 1] = cumB[b] + acc * LH;
+    seq_cost[b] = acc + seg_ovh;       // entering a segment costs a prologue (q pre-projection) and a partial flush
+    cumB[b + 1] = cumB[b] + seq_cost[b] * LH;
   }
   ustart[n_seqs] = (int32_t)units.size();
   const int n_units = (int)units.size(), S_total = n_seqs * LH;
@@ -633,6 +637,7 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
       double rem = target - cumB[b];
       int lh = std::min(LH - 1, (int)std::floor(rem / seq_cost[b]));
       rem -= (double)lh * seq_cost[b];
+      rem = std::max(0.0, rem - seg_ovh);   // the overhead sits at the start of the segment
       int u = (int)(std::upper_bound(upre.begin() + ustart[b], upre.begin() + ustart[b + 1], rem) - upre.begin()) - 1;
       u = std::min(std::max(u, ustart[b]), ustart[b + 1] - 1);
       int sub = (int)std::floor((rem - upre[u]) / usub[u] + 0.5);
@@ -707,6 +712,7 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   sp.pstart = (const int32_t*)(blob + P.off_pstart);
   sp.q = (const __nv_bfloat16*)q; sp.BK = c->BK; sp.gK = c->gK;
   sp.part = (float*)c->part.p;
+  sp.stamps = (unsigned long long*)c->opt_stamps_ptr;
   sp.n_slices = P.n_slices; sp.n_segs = P.n_segs;
   sp.layer0 = layer0; sp.Lq = Lsel; sp.LH = Lsel * g.H; sp.w = g.w;
   sp.H = g.H; sp.G = g.G; sp.r = g.r; sp.d = g.d;

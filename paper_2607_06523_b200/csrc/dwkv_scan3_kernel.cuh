@@ -11,45 +11,117 @@ __device__ __forceinline__ float2 bf2(uint32_t w) { return make_float2(__uint_as
 // a1: q~ = cscale * BK[m,h] . (gK[l,h] * q) for the rows of this lane, straight into A-fragment registers; also the raw-q
 // fragments and code-offset biases of the residual-K term. gK*q is exact in fp32 and split into hi + lo bf16 (exact);
 // BK is bf16, so the tensor-core products are exact and only the fp32 accumulation rounds.
-template <int NKB, int D, bool PAIR>
-__device__ __forceinline__ void segment_prologue(QRegs<NKB, D, PAIR>& q, const Scan3Params& p, const int seg, const int lane) {
-  const int g = lane >> 2, t = lane & 3;
+// Split in two: the loads (one batch, issued as early as possible: under load a DRAM round trip costs several microseconds
+// because it queues behind the chip's outstanding bulk copies) and the arithmetic.
+template <int NKB, int D>
+struct ProLoads {
+  static constexpr int NKK = D / 16;
+  static constexpr int JB = NKB < 4 ? NKB : 4;       // basis row chunks of the first load batch
+  uint32_t qv[NKK][2], gv[NKK][2];
+  uint32_t bw[JB][NKK][2];
+};
+
+struct SegPtrs {
+  const __nv_bfloat16 *qhead, *gk, *Bk;               // first query head of the kv head, gate row, basis block
+};
+__device__ __forceinline__ SegPtrs seg_ptrs(const Scan3Params& p, const int seg, const int D) {
   const int b = seg / p.LH, lh = seg - b * p.LH;
   const int layer = p.layer0 + lh / p.H, h = lh % p.H;
+  SegPtrs s;
+  s.qhead = p.q + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * p.G) + (size_t)h * p.G) * D;
+  s.gk = p.gK + ((size_t)layer * p.H + h) * D;
+  s.Bk = p.BK + ((size_t)(layer / p.w) * p.H + h) * (size_t)p.r * D;
+  return s;
+}
+
+// L2 prefetch of everything the prologue of `seg` will read (q rows, gate row, basis block); called by the fetch cursor
+// when it crosses into the segment, a few stages ahead of the compute side.
+__device__ __forceinline__ void prefetch_segment(const Scan3Params& p, const int seg, const int D, const int lane) {
+  const SegPtrs sp = seg_ptrs(p, seg, D);
+  const int nq = (p.G * D * 2 + 127) / 128, ng = (D * 2 + 127) / 128, nb = (p.r * D * 2 + 127) / 128;
+  for (int i = lane; i < nq + ng + nb; i += 32) {
+    const char* a = i < nq ? (const char*)sp.qhead + 128 * i : i < nq + ng ? (const char*)sp.gk + 128 * (i - nq) : (const char*)sp.Bk + 128 * (i - nq - ng);
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+  }
+}
+
+template <int NKB, int D, bool PAIR>
+__device__ __forceinline__ void prologue_load(ProLoads<NKB, D>& pl, const Scan3Params& p, const int seg, const int lane) {
+  constexpr int NKK = D / 16, JB = ProLoads<NKB, D>::JB;
+  const int g = lane >> 2, t = lane & 3;
   const int hd = PAIR ? (g & 3) : g;
   const bool valid = hd < p.G;
+  const SegPtrs sp = seg_ptrs(p, seg, D);
+  const __nv_bfloat16* qrow = sp.qhead + (size_t)(valid ? hd : 0) * D;
+#pragma unroll
+  for (int kk = 0; kk < NKK; ++kk) {
+    pl.qv[kk][0] = valid ? ldg32(qrow + 16 * kk + 2 * t) : 0u;
+    pl.qv[kk][1] = valid ? ldg32(qrow + 16 * kk + 8 + 2 * t) : 0u;
+    pl.gv[kk][0] = ldg32(sp.gk + 16 * kk + 2 * t);
+    pl.gv[kk][1] = ldg32(sp.gk + 16 * kk + 8 + 2 * t);
+  }
+#pragma unroll
+  for (int jb = 0; jb < JB; ++jb) {
+    const int row = 8 * jb + g;
+    const bool ok = row < p.r;
+    const __nv_bfloat16* br = sp.Bk + (size_t)(ok ? row : 0) * D + 2 * t;
+#pragma unroll
+    for (int kk = 0; kk < NKK; ++kk) {
+      pl.bw[jb][kk][0] = ok ? ldg32(br + 16 * kk) : 0u;
+      pl.bw[jb][kk][1] = ok ? ldg32(br + 16 * kk + 8) : 0u;
+    }
+  }
+}
+
+template <int NKB, int D, bool PAIR>
+__device__ __forceinline__ void prologue_compute(QRegs<NKB, D, PAIR>& q, const ProLoads<NKB, D>& pl, const Scan3Params& p, const int seg,
+                                                 const int lane) {
+  constexpr int NKK = D / 16, JB = ProLoads<NKB, D>::JB;
+  const int g = lane >> 2, t = lane & 3;
   const uint32_t mA = (g < 4) ? 0xffffffffu : 0u;
-  const __nv_bfloat16* qrow = p.q + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * p.G) + (size_t)h * p.G + (valid ? hd : 0)) * D;
-  const __nv_bfloat16* gk = p.gK + ((size_t)layer * p.H + h) * D;
-  const __nv_bfloat16* Bk = p.BK + ((size_t)(layer / p.w) * p.H + h) * (size_t)p.r * D;
+  uint32_t af[NKK][4];
   float c[NKB][4];
 #pragma unroll
   for (int jj = 0; jj < NKB; ++jj) c[jj][0] = c[jj][1] = c[jj][2] = c[jj][3] = 0.f;
 #pragma unroll
-  for (int kk = 0; kk < D / 16; ++kk) {
-    const uint32_t q0 = valid ? ldg32(qrow + 16 * kk + 2 * t) : 0u, q2 = valid ? ldg32(qrow + 16 * kk + 8 + 2 * t) : 0u;
-    const float2 g0 = bf2(ldg32(gk + 16 * kk + 2 * t)), g2 = bf2(ldg32(gk + 16 * kk + 8 + 2 * t));
-    const float2 x0 = bf2(q0), x2 = bf2(q2);
-    uint32_t a0, a1, a2, a3;
-    split_bf16x2(x0.x * g0.x, x0.y * g0.y, a0, a1);
-    split_bf16x2(x2.x * g2.x, x2.y * g2.y, a2, a3);
-#pragma unroll
-    for (int jj = 0; jj < NKB; ++jj) {
-      const int row = 8 * jj + g;
-      const bool ok = row < p.r;
-      const __nv_bfloat16* br = Bk + (size_t)(ok ? row : 0) * D + 16 * kk + 2 * t;
-      const uint32_t b0 = ok ? ldg32(br) : 0u, b1 = ok ? ldg32(br + 8) : 0u;
-      mma16(c[jj], a0, a1, a2, a3, b0, b1);
-    }
+  for (int kk = 0; kk < NKK; ++kk) {
+    const float2 x0 = bf2(pl.qv[kk][0]), x2 = bf2(pl.qv[kk][1]), g0 = bf2(pl.gv[kk][0]), g2 = bf2(pl.gv[kk][1]);
+    split_bf16x2(x0.x * g0.x, x0.y * g0.y, af[kk][0], af[kk][1]);
+    split_bf16x2(x2.x * g2.x, x2.y * g2.y, af[kk][2], af[kk][3]);
     if constexpr (PAIR) {
-      q.qr[kk][0] = q0 & mA; q.qr[kk][1] = q2 & mA; q.qr[kk][2] = q0 & ~mA; q.qr[kk][3] = q2 & ~mA;
+      q.qr[kk][0] = pl.qv[kk][0] & mA; q.qr[kk][1] = pl.qv[kk][1] & mA; q.qr[kk][2] = pl.qv[kk][0] & ~mA; q.qr[kk][3] = pl.qv[kk][1] & ~mA;
     } else {
-      q.qr[kk][0] = q0; q.qr[kk][1] = q2;
+      q.qr[kk][0] = pl.qv[kk][0]; q.qr[kk][1] = pl.qv[kk][1];
     }
     float sum = (x0.x + x0.y) + (x2.x + x2.y);
     sum += __shfl_xor_sync(kFull, sum, 1);
     sum += __shfl_xor_sync(kFull, sum, 2);
     q.qbias[kk] = -136.f * sum;
+  }
+#pragma unroll
+  for (int jb = 0; jb < JB; ++jb) {
+#pragma unroll
+    for (int kk = 0; kk < NKK; ++kk) mma16(c[jb], af[kk][0], af[kk][1], af[kk][2], af[kk][3], pl.bw[jb][kk][0], pl.bw[jb][kk][1]);
+  }
+  if constexpr (NKB > JB) {      // remaining basis row chunks (basis rank > 32): a second load batch
+    const SegPtrs sp = seg_ptrs(p, seg, D);
+    uint32_t bw2[NKB - JB][NKK][2];
+#pragma unroll
+    for (int jb = 0; jb < NKB - JB; ++jb) {
+      const int row = 8 * (JB + jb) + g;
+      const bool ok = row < p.r;
+      const __nv_bfloat16* br = sp.Bk + (size_t)(ok ? row : 0) * D + 2 * t;
+#pragma unroll
+      for (int kk = 0; kk < NKK; ++kk) {
+        bw2[jb][kk][0] = ok ? ldg32(br + 16 * kk) : 0u;
+        bw2[jb][kk][1] = ok ? ldg32(br + 16 * kk + 8) : 0u;
+      }
+    }
+#pragma unroll
+    for (int jb = 0; jb < NKB - JB; ++jb) {
+#pragma unroll
+      for (int kk = 0; kk < NKK; ++kk) mma16(c[JB + jb], af[kk][0], af[kk][1], af[kk][2], af[kk][3], bw2[jb][kk][0], bw2[jb][kk][1]);
+    }
   }
 #pragma unroll
   for (int jj = 0; jj < NKB; ++jj) {
@@ -205,6 +277,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
       moved = true;
       if (f_u == f_uend) {
         ++f_seg;
+        if (f_seg < p.n_segs) prefetch_segment(p, f_seg, D, lane);
         if (++f_lh == p.LH) {
           f_lh = 0;
           ++f_b;
@@ -218,14 +291,20 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     if (f_seg == we.x && f_u == we.y && f_sub == we.z) f_on = false;
     else if (moved) unit_setup();
   };
-#pragma unroll 1
-  for (int k = 0; k < NS; ++k) fetch_one(k);
-  __syncwarp();
-
-  // ---- compute stream ----------------------------------------------------------------------------------------------------
   State<NKB, D> st;
   QRegs<NKB, D, PAIR> q;
-  int cur_seg = -1, k_c = 0, slot_next = ws.w;
+  {   // first segment: loads ahead of the ring fills in the memory queues, arithmetic while the ring fills land
+    ProLoads<NKB, D> pl;
+    prologue_load<NKB, D, PAIR>(pl, p, ws.x, lane);
+#pragma unroll 1
+    for (int k = 0; k < NS; ++k) fetch_one(k);
+    __syncwarp();
+    prologue_compute<NKB, D, PAIR>(q, pl, p, ws.x, lane);
+    state_reset<NKB, D>(st);
+  }
+
+  // ---- compute stream ----------------------------------------------------------------------------------------------------
+  int cur_seg = ws.x, k_c = 0, slot_next = ws.w;
   uint32_t phase = 0u;
   while (true) {
     const uint4 dsc = lds128(descs + 16 * k_c);
@@ -233,12 +312,12 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     if (n == 0) break;
     const int seg = (int)dsc.z;
     if (seg != cur_seg) {
-      if (cur_seg >= 0) {
-        flush_partial<NKB, D, PAIR>(st, p, slot_next, lane);
-        slot_next = __ldg(p.pstart + seg);     // a segment entered inside a slice is entered at its start: its first slot
-      }
+      ProLoads<NKB, D> pl;
+      prologue_load<NKB, D, PAIR>(pl, p, seg, lane);       // L2 hits: the fetch cursor prefetched them when it crossed over
+      flush_partial<NKB, D, PAIR>(st, p, slot_next, lane);
+      slot_next = __ldg(p.pstart + seg);       // a segment entered inside a slice is entered at its start: its first slot
+      prologue_compute<NKB, D, PAIR>(q, pl, p, seg, lane);
       state_reset<NKB, D>(st);
-      segment_prologue<NKB, D, PAIR>(q, p, seg, lane);
       cur_seg = seg;
     }
     mbar_wait(bars + 8 * k_c, (phase >> k_c) & 1u);
@@ -265,7 +344,12 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     __syncwarp();
     k_c = (k_c + 1 == NS) ? 0 : k_c + 1;
   }
-  if (cur_seg >= 0) flush_partial<NKB, D, PAIR>(st, p, slot_next, lane);
+  flush_partial<NKB, D, PAIR>(st, p, slot_next, lane);
+  if (p.stamps && lane == 0) {       // measurement aid: when did this warp finish (planner cost-model fits)
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    p.stamps[gw] = t;
+  }
 }
 
 template <int NKB, int D, bool PAIR>
