@@ -14,22 +14,28 @@ bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
 namespace {
 using namespace dwkv::dev;
 
-// One CTA of 4 warps merges the partials of one (segment, query head) and writes o[head, :]. The warps split the partial
-// list (warp w takes partials w, w+4, ...: matters in per-layer calls, where a segment has ~150 partials; all-layer steps
-// have ~2-6), lanes run over rank columns for a*, over channels (D / 32 each) for e* and the back-projection.
-template <int D>
+// SPLIT: one CTA of 4 warps merges the partials of one (segment, query head); the warps split the partial list (warp w takes
+// partials w, w+4, ...) -- for per-layer calls, where a segment has ~150 partials. !SPLIT: one CTA per segment, warp w merges
+// heads w, w+4 on its own -- for all-layer steps (1-6 partials per segment, thousands of segments). Lanes run over rank
+// columns for a*, over channels (D / 32 each) for e* and the back-projection.
+template <int D, bool SPLIT>
 __global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
   constexpr int CPL = D / 32;                       // channels per lane
   __shared__ float sh_l[4];
   __shared__ float sh_a[4][64];
   __shared__ float sh_e[4][D];
-  const int seg = blockIdx.x, gq = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int seg = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int S = SPLIT ? 4 : 1;                  // warps sharing one head's partial list
+  const int ws = SPLIT ? warp : 0;                  // this warp's offset in the split
+  // programmatic dependent launch: this grid may start while the decode kernel drains; wait for its completion and flush
+  cudaGridDependencySynchronize();
   const int b = seg / p.LH, lh = seg - b * p.LH;
   const int layer = p.layer0 + lh / p.H, h = lh % p.H;
   const int G = p.G, r = p.r, PR = 2 + p.r + D;
   const int P0 = __ldg(p.pstart + seg), n = __ldg(p.pstart + seg + 1) - P0;
-  const float* part = p.part + ((size_t)P0 * G + gq) * PR;       // partial k of this head: part + k * stride
   const size_t stride = (size_t)G * PR;
+  for (int gq = SPLIT ? (int)blockIdx.y : warp; gq < G; gq += SPLIT ? G : 4) {
+  const float* part = p.part + ((size_t)P0 * G + gq) * PR;       // partial k of this head: part + k * stride
   // pass 1: m* over all partials (every warp computes it: n is small, the loads hit L2)
   float mstar = -INFINITY;
   for (int k0 = lane; k0 < n; k0 += 32 * 8) {       // 8 independent loads in flight per lane
@@ -45,12 +51,12 @@ __global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
   float lsum = 0.f, a0 = 0.f, a1 = 0.f, e[CPL];
 #pragma unroll
   for (int c = 0; c < CPL; ++c) e[c] = 0.f;
-  const int nw = (n > warp) ? (n - warp + 3) / 4 : 0;            // partials of this warp
+  const int nw = (n > ws) ? (n - ws + S - 1) / S : 0;            // partials of this warp
   for (int i0 = 0; i0 < nw; i0 += 32) {
     const int i = i0 + lane;
     float wk = 0.f;
     if (i < nw) {
-      const float2 ml = *reinterpret_cast<const float2*>(part + (size_t)(warp + 4 * i) * stride);
+      const float2 ml = *reinterpret_cast<const float2*>(part + (size_t)(ws + S * i) * stride);
       wk = (ml.x == -INFINITY) ? 0.f : ex2(ml.x - mstar);
       lsum = fmaf(wk, ml.y, lsum);
     }
@@ -62,7 +68,7 @@ __global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
       for (int u = 0; u < 8; ++u) {
         const int k = k0 + u;
         w[u] = __shfl_sync(kFull, wk, k & 31);          // lanes >= nc hold weight 0
-        const float* rec = part + (size_t)(warp + 4 * (i0 + min(k, nc - 1))) * stride + 2;
+        const float* rec = part + (size_t)(ws + S * (i0 + min(k, nc - 1))) * stride + 2;
         va0[u] = (lane < r) ? rec[lane] : 0.f;
         va1[u] = (lane + 32 < r) ? rec[lane + 32] : 0.f;
 #pragma unroll
@@ -80,17 +86,20 @@ __global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) lsum += __shfl_xor_sync(kFull, lsum, o);
-  if (lane == 0) sh_l[warp] = lsum;
-  sh_a[warp][lane] = a0; sh_a[warp][lane + 32] = a1;
+  float lstar = lsum;
+  if constexpr (SPLIT) {
+    if (lane == 0) sh_l[warp] = lsum;
+    sh_a[warp][lane] = a0; sh_a[warp][lane + 32] = a1;
 #pragma unroll
-  for (int c = 0; c < CPL; ++c) sh_e[warp][lane * CPL + c] = e[c];
-  __syncthreads();
-  if (warp != 0) return;
-  const float lstar = sh_l[0] + sh_l[1] + sh_l[2] + sh_l[3];
-  a0 = sh_a[0][lane] + sh_a[1][lane] + sh_a[2][lane] + sh_a[3][lane];
-  a1 = sh_a[0][lane + 32] + sh_a[1][lane + 32] + sh_a[2][lane + 32] + sh_a[3][lane + 32];
+    for (int c = 0; c < CPL; ++c) sh_e[warp][lane * CPL + c] = e[c];
+    __syncthreads();
+    if (warp != 0) return;
+    lstar = sh_l[0] + sh_l[1] + sh_l[2] + sh_l[3];
+    a0 = sh_a[0][lane] + sh_a[1][lane] + sh_a[2][lane] + sh_a[3][lane];
+    a1 = sh_a[0][lane + 32] + sh_a[1][lane + 32] + sh_a[2][lane + 32] + sh_a[3][lane + 32];
 #pragma unroll
-  for (int c = 0; c < CPL; ++c) e[c] = sh_e[0][lane * CPL + c] + sh_e[1][lane * CPL + c] + sh_e[2][lane * CPL + c] + sh_e[3][lane * CPL + c];
+    for (int c = 0; c < CPL; ++c) e[c] = sh_e[0][lane * CPL + c] + sh_e[1][lane * CPL + c] + sh_e[2][lane * CPL + c] + sh_e[3][lane * CPL + c];
+  }
   // back-projection o = (gV * (BV^T a*) + e*) / l*: basis rows as coalesced loads, a*_j broadcast by shuffle
   const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
   const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
@@ -123,6 +132,7 @@ __global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
     o.x = (__uint_as_float(gw << 16) * acc[0] + e[0]) * inv; o.y = (__uint_as_float(gw & 0xffff0000u) * acc[1] + e[1]) * inv;
     *reinterpret_cast<float2*>(out) = o;
   }
+  }   // heads of this warp
 }
 
 }  // namespace
@@ -137,10 +147,19 @@ int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s) {
   return ok ? 1 : 0;
 }
 
-int launch_combine3(const Combine3Params& p, int n_segs, cudaStream_t s) {
-  const dim3 grid(n_segs, p.G);
-  if (p.d == 128) combine3_kernel<128><<<grid, 128, 0, s>>>(p);
-  else combine3_kernel<64><<<grid, 128, 0, s>>>(p);
+int launch_combine3(const Combine3Params& p, int n_segs, bool split, cudaStream_t s) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = split ? dim3(n_segs, p.G) : dim3(n_segs);       // split: 4 warps share the partial list of one head
+  cfg.blockDim = dim3(128);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;     // overlap this launch with the tail of the scan
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (p.d == 128) { if (split) cudaLaunchKernelEx(&cfg, combine3_kernel<128, true>, p); else cudaLaunchKernelEx(&cfg, combine3_kernel<128, false>, p); }
+  else { if (split) cudaLaunchKernelEx(&cfg, combine3_kernel<64, true>, p); else cudaLaunchKernelEx(&cfg, combine3_kernel<64, false>, p); }
   return 1;
 }
 
