@@ -144,7 +144,7 @@ struct dwkv_cache {
   Plan3 plan3;
   // options
   int64_t opt_max_unit_blocks = 0;   // 0 = adaptive
-  int64_t opt_cost_coef_pct = 80, opt_cost_tok = 24, opt_cost_resid_pct = 235, opt_cost_seg = 24576;   // planner cost model
+  int64_t opt_cost_coef_pct = 80, opt_cost_tok = -1, opt_cost_resid_pct = -1, opt_cost_seg = 24576;   // planner cost model (-1 = by G)
   int64_t opt_interleave = 0;        // planner: interleave the classes of a sequence (0 = class after class)
   int64_t opt_stamps_ptr = 0;        // device pointer [n_slices] u64 for per-warp end stamps (measurement aid), 0 = off
   int64_t opt_unit_kb = 64;          // planner: target bytes of a work unit (per layer-head), KB
@@ -550,6 +550,9 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   const int LH = n_lsel * c->geom.H;
   const double flag_w = (double)c->opt_flag_cost_pct / 100.0;
   const double seg_ovh = (double)c->opt_cost_seg;
+  // per-token and per-residual-byte work grows with the query heads per kv head (fits at G = 4: 24 / 235 %, G = 8: 40 / 265 %)
+  const double cost_tok = c->opt_cost_tok >= 0 ? (double)c->opt_cost_tok : 8.0 + 4.0 * c->geom.G;
+  const double cost_resid_pct = c->opt_cost_resid_pct >= 0 ? (double)c->opt_cost_resid_pct : 205.0 + 7.5 * c->geom.G;
   std::vector<Unit> units;
   std::vector<int32_t> ustart(n_seqs + 1, 0), unsub;
   std::vector<double> upre, usub, seq_cost(n_seqs, 0.0), cumB(n_seqs + 1, 0.0);
@@ -573,8 +576,8 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
         ub = std::min<int64_t>(ub, cl.blocks_per_page);
         // cost of a sub-block in byte-equivalents: the warp is partly issue bound, so tokens (softmax work) and residual
         // bytes (int4 unpack, group scales) weigh more than coefficient bytes (fit to per-warp finish times)
-        const double cost_sub = 0.01 * (double)c->opt_cost_coef_pct * 2.0 * cl.coef_bytes + (double)c->opt_cost_tok * cl.sub_tok +
-                                0.01 * (double)c->opt_cost_resid_pct * flag_w * 2.0 * (cl.code_bytes + cl.scale_bytes);
+        const double cost_sub = 0.01 * (double)c->opt_cost_coef_pct * 2.0 * cl.coef_bytes + cost_tok * cl.sub_tok +
+                                0.01 * cost_resid_pct * flag_w * 2.0 * (cl.code_bytes + cl.scale_bytes);
         for (size_t pi = 0; pi < S.pages[k].size(); ++pi) {
           const int64_t tok_in_page = std::min<int64_t>(tpp, S.count[k] - (int64_t)pi * tpp);
           if (tok_in_page <= 0) break;

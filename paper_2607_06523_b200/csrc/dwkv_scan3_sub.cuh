@@ -80,14 +80,14 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
 #pragma unroll
       for (int grp = 0; grp < NG; ++grp) {
         const int qq = 2 * grp;
-        float c[4] = {q.qbias[grp], q.qbias[grp], 0.f, 0.f};
-        mma16(c, q.qr[grp][0], 0u, q.qr[grp][1], 0u, nib_to_bf16x2_biased(wA[qq >> 2], qq & 3),
-              nib_to_bf16x2_biased(wA[qq >> 2], (qq & 3) + 1));
+        float c[4];
+        mma16z(c, q.qr[grp][0], 0u, q.qr[grp][1], 0u, nib_to_bf16x2_biased(wA[qq >> 2], qq & 3),
+               nib_to_bf16x2_biased(wA[qq >> 2], (qq & 3) + 1));
         mma16(c, q.qr[grp][2], 0u, q.qr[grp][3], 0u, nib_to_bf16x2_biased(wB[qq >> 2], qq & 3),
               nib_to_bf16x2_biased(wB[qq >> 2], (qq & 3) + 1));
         const float2 f = h2f2(sc[grp]);
-        sr0 = fmaf(c[0], f.x, sr0);
-        sr1 = fmaf(c[1], f.y, sr1);
+        sr0 = fmaf(c[0] + q.qbias[grp], f.x, sr0);      // the -136 * sum(q) offset of the biased codes
+        sr1 = fmaf(c[1] + q.qbias[grp], f.y, sr1);
       }
       s[0][0] = fmaf(cscale, sr0, s[0][0]);
       s[0][1] = fmaf(cscale, sr1, s[0][1]);
@@ -101,19 +101,20 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
 #pragma unroll
         for (int grp = 0; grp < NG; ++grp) {
           const int qq = 2 * grp;
-          float c[4] = {q.qbias[grp], q.qbias[grp], 0.f, 0.f};
-          mma16(c, q.qr[grp][0], 0u, q.qr[grp][1], 0u, nib_to_bf16x2_biased(w[qq >> 2], qq & 3),
-                nib_to_bf16x2_biased(w[qq >> 2], (qq & 3) + 1));
+          float c[4];
+          mma16z(c, q.qr[grp][0], 0u, q.qr[grp][1], 0u, nib_to_bf16x2_biased(w[qq >> 2], qq & 3),
+                 nib_to_bf16x2_biased(w[qq >> 2], (qq & 3) + 1));
           const float2 f = h2f2(sc[grp]);
-          sr0 = fmaf(c[0], f.x, sr0);
-          sr1 = fmaf(c[1], f.y, sr1);
+          sr0 = fmaf(c[0] + q.qbias[grp], f.x, sr0);
+          sr1 = fmaf(c[1] + q.qbias[grp], f.y, sr1);
         }
         s[j][0] = fmaf(cscale, sr0, s[j][0]);
         s[j][1] = fmaf(cscale, sr1, s[j][1]);
       }
     }
   }
-  if (nv < 8 * TB) {   // ragged tail: slots >= nv do not exist
+  if (nv < 8 * TB) {   // ragged tail: slots >= nv do not exist (rare: a real branch, not predication of every score)
+    asm volatile("");
 #pragma unroll
     for (int x = 0; x < NSC; ++x) {
       const int slot = PAIR ? (16 * x + 8 * jt + 2 * t) : (8 * x + 2 * t);
