@@ -179,6 +179,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="llama8b_64k_b8")
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (experiments), repeatable")
+    ap.add_argument("--append", action="store_true",
+                    help="BASELINE.json configs[4]: dwkv_append_compress of wl.n_append new tokens per sequence before every decode step")
     ap.add_argument("--no-dense", action="store_true", help="skip the dense-bf16 comparison kernel")
     ap.add_argument("--no-extra", action="store_true", help="skip batch 1/4, per-layer mode and the CPU baseline")
     args = ap.parse_args()
@@ -194,7 +196,11 @@ def main():
 
     # ---- build the cache (every rank: its own replica of the batch, different seeds would not change the timing) ----
     routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
-    cache, consts = harness.make_cache(wl, arena_bytes=harness.arena_bytes_for(wl, routings, 1), device=local)
+    n_app = wl.n_append if args.append else 0
+    app_steps = 2 * (args.steps + args.warmup) + 4
+    slack = 1 + (n_app * app_steps + 127) // 128        # pages per (sequence, class) for the appended tokens (>= 227 tokens per page)
+    cache, consts = harness.make_cache(wl, max_tokens=max(wl.T) + 4096 + n_app * app_steps,
+                                       arena_bytes=harness.arena_bytes_for(wl, routings, slack), device=local)
     for kv in args.opt:
         k, v = kv.split("=")
         cache.set_option(k, int(v))
@@ -220,6 +226,29 @@ def main():
     def step():
         cache.decode_attention(-1, seq_ids, qs[it[0] % nq], out)
         it[0] += 1
+
+    append_ms = []
+    if n_app:
+        # dense K/V of the new tokens (x = gate * (c . B) + e, gen.make_dense_kv_chunk) and their tiers / flags, generated once
+        BK, BV, gK, gV = consts
+        rng = np.random.Generator(np.random.PCG64([gen.BASE_SEED, wl.index, 99]))
+        n_new = [n_app] * n_seq
+        kd, vd = [], []
+        for s_ in range(n_seq):
+            k_, v_ = gen.make_dense_kv_chunk(wl, s_, 10 ** 6, n_app, BK, BV, gK, gV, device=dev)
+            kd.append(k_); vd.append(v_)
+        k_new, v_new = torch.cat(kd), torch.cat(vd)
+        a_tier = rng.choice(len(wl.tier_ranks), size=n_app * n_seq, p=list(wl.tier_frac)).astype(np.uint8)
+        a_flag = ((a_tier == len(wl.tier_ranks) - 1) & (rng.random(n_app * n_seq) < 0.8)).astype(np.uint8)
+        decode_only = step
+
+        def step():
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            cache.append_compress(seq_ids, n_new, k_new, v_new, a_tier, a_flag)
+            e1.record()
+            decode_only()
+            append_ms.append((e0, e1))
 
     # ---- timed region: K steps, inputs resident in HBM ------------------------------------------------------------
     step(); torch.cuda.synchronize()
@@ -269,7 +298,15 @@ def main():
                 "scan_ms": scan_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "frac_of_8TBps_nominal": achieved / 8000.0, "step_frac_of_peak": alg_bytes / (ms * 1e-3) / 1e9 / peak}
 
-    extra = {"fill_s": t_fill, "footprint": fp, "compression_ratio": fp["dense_equiv_bytes"] / fp["used_bytes"],
+    extra_append = None
+    if n_app:
+        torch.cuda.synchronize()
+        am = [a.elapsed_time(b) for a, b in append_ms[-args.steps:]]
+        extra_append = {"tokens_per_seq_per_step": n_app, "append_us_per_step": float(np.mean(am)) * 1e3,
+                        "decode_us_per_step": (ms - float(np.mean(am))) * 1e3, "new_vectors_per_step": 2 * n_app * n_seq * L * wl.H_kv,
+                        "dense_bytes_read_per_step": 2 * n_app * n_seq * L * wl.H_kv * wl.d * 2,
+                        "note": "ms_per_step = append + plan rebuild + decode; the cache grows by n_append tokens per sequence every step"}
+    extra = {"fill_s": t_fill, "append": extra_append, "footprint": fp, "compression_ratio": fp["dense_equiv_bytes"] / fp["used_bytes"],
              "us_per_step": ms * 1e3}
     cpu_baseline = None
     if rank == 0 and not args.no_extra:

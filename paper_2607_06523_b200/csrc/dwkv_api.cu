@@ -206,6 +206,8 @@ void route_commit(dwkv_cache* c, int32_t seq, int32_t n, const uint8_t* tier, co
     td.slot = (int32_t)(in_page % kBlockTok);
     td.cls = k;
     td.ridx = flag[i] ? (*ridx_base)++ : -1;
+    td.src = (int32_t)out->size();
+    td.pad_ = 0;
     out->push_back(td);
     S.tier.push_back(tier[i]);
     S.flag.push_back(flag[i]);
@@ -379,11 +381,14 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
     route_commit(c, seq_ids[i], n_new[i], tier + off, flag + off, &ridx, &dst, &new_pages);
     off += n_new[i];
   }
+  // flagged tokens first: only their 16-token tiles run the reconstruction + int4 quantiser part of the kernel
+  for (size_t i = 0; i < dst.size(); ++i) { dst[i].src = (int32_t)i; dst[i].pad_ = 0; }
+  std::stable_partition(dst.begin(), dst.end(), [](const TokDst& t) { return t.ridx >= 0; });
   int rc = zero_new_pages(c, new_pages, st);
   if (rc) return rc;
   rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
   if (rc) return rc;
-  c->launches += launch_compress(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, (const __nv_bfloat16*)k_new,
+  c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, (const __nv_bfloat16*)k_new,
                                  (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, st);
   CU_OK(cudaGetLastError());
   return DWKV_OK;
@@ -443,6 +448,8 @@ int dwkv_export_tokens(dwkv_cache* c, int32_t seq_id, int64_t t0, int64_t n, con
     td.slot = (int32_t)((sl % tpp) % kBlockTok);
     td.cls = k;
     td.ridx = -1;
+    td.src = (int32_t)i;
+    td.pad_ = 0;
     dst[i] = td;
   }
   int rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);

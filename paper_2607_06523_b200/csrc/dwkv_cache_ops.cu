@@ -1,6 +1,4 @@
-// dwkv_cache_ops.cu -- cache construction side (SURVEY.md section 8a step a4 and the load / dump auxiliaries):
-//   compress_kernel     append/compress: project new K/V on the shared basis, quantise the residual, write tier pages
-//                       (readings A13, A14)
+// dwkv_cache_ops.cu -- load / dump auxiliaries of the cache (the append/compress kernel, step a4, is dwkv_compress.cu):
 //   scatter_raw_kernel  load pre-compressed token-ordered entries into the fragment-native pages
 //   gather_kernel       token-ordered dump of stored entries (bit-exact checks of routing and int4 dequantisation)
 #include "dwkv_internal.h"
@@ -103,61 +101,6 @@ __global__ void __launch_bounds__(128) scatter_raw_kernel(const uint8_t* arena, 
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// a4: append / compress. One CTA per (new token, layer, kv head); both K and V.
-//   c = bf16( B[:r_t] . (x / g) )      e = x - g * (c . B[:r_t])      (readings A13, A14)
-__global__ void __launch_bounds__(128) compress_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst,
-                                                       const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
-                                                       const __nv_bfloat16* BK, const __nv_bfloat16* BV,
-                                                       const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
-  __shared__ float xn[128];
-  __shared__ float cf[64];
-  const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int l = lh / g.H, h = lh % g.H, d = g.d;
-  const TokDst td = dst[tok];
-  const BlockPtr bp = block_ptr(arena, g, td, lh);
-  const size_t row = (size_t)tok * LH + lh;
-  for (int z = 0; z < 2; ++z) {
-    const __nv_bfloat16* xs = (z ? v_new : k_new) + row * d;
-    const __nv_bfloat16* B = (z ? BV : BK) + ((size_t)(l / g.w) * g.H + h) * (size_t)g.r * d;
-    const __nv_bfloat16* gt = (z ? gV : gK) + (size_t)lh * d;
-    float x = 0.f, gate = 1.f;
-    if (tid < d) {
-      x = __bfloat162float(xs[tid]);
-      gate = __bfloat162float(gt[tid]);
-      xn[tid] = __fdiv_rn(x, gate);
-    }
-    __syncthreads();
-    for (int j = warp; j < bp.rk; j += 4) {
-      float acc = 0.f;
-      for (int i = lane; i < d; i += 32) acc = fmaf(__bfloat162float(B[(size_t)j * d + i]), xn[i], acc);
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
-      if (lane == 0) {
-        const __nv_bfloat16 c = __float2bfloat16_rn(acc);
-        cf[j] = __bfloat162float(c);
-        const int off = z ? off_coefV(bp.cl) + vcoef_elem_off(bp.slot, j, bp.cl.tb) : off_coefK(bp.cl) + kcoef_elem_off(bp.slot, j, bp.cl.tb);
-        *reinterpret_cast<__nv_bfloat16*>(bp.blk + off) = c;
-      }
-    }
-    __syncthreads();
-    if (td.ridx >= 0 && tid < d) {
-      float rec = 0.f;
-      for (int j = 0; j < bp.rk; ++j) rec = fmaf(cf[j], __bfloat162float(B[(size_t)j * d + tid]), rec);
-      const float e = fmaf(-gate, rec, x);
-      const float amax = group16_amax(fabsf(e));
-      __half s;
-      const int code = quant_code(e, amax, &s);
-      int wo, bit;
-      if (z == 0) kcode_nibble(bp.slot, tid, d, &wo, &bit); else vcode_nibble(bp.slot, tid, d, &wo, &bit);
-      store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
-      if ((tid & 15) == 0)
-        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(bp.slot, tid >> 4, d)) = s;
-    }
-    __syncthreads();
-  }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst, DumpPtrs o) {
   const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x;
   const TokDst td = dst[tok];
@@ -211,15 +154,6 @@ int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* d
   if (n <= 0) return 0;
   dim3 grid(n, g.L * g.H);
   scatter_raw_kernel<<<grid, 128, 0, s>>>(arena, g, dst, coefK, coefV, residK, residV, codeK, codeV, scaleK, scaleV);
-  return 1;
-}
-
-int launch_compress(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const __nv_bfloat16* k_new,
-                    const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
-                    const __nv_bfloat16* gK, const __nv_bfloat16* gV, cudaStream_t s) {
-  if (n <= 0) return 0;
-  dim3 grid(n, g.L * g.H);
-  compress_kernel<<<grid, 128, 0, s>>>(arena, g, dst, k_new, v_new, BK, BV, gK, gV);
   return 1;
 }
 

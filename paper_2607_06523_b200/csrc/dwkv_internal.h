@@ -56,6 +56,8 @@ struct TokDst {
   int32_t slot;       // slot inside the block (0..31)
   int32_t cls;        // class id
   int32_t ridx;       // index among the flagged tokens of this call (-1 if unflagged)
+  int32_t src;        // append/compress: row of the token in k_new / v_new (the table is sorted flagged-first)
+  int32_t pad_;
 };
 
 struct CacheGeom {
@@ -71,7 +73,7 @@ int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* d
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
                        const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,
                        const __half* scaleK, const __half* scaleV, cudaStream_t s);
-int launch_compress(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
+int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
                     const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK, const __nv_bfloat16* gV,
                     cudaStream_t s);
