@@ -285,6 +285,74 @@ def test_append_compress_against_oracle(mod):
     cache.destroy()
 
 
+@pytest.mark.parametrize("shape", ["8b", "70b", "odd"])
+def test_append_compress_tensor_core_tiles(mod, shape):
+    """dwkv_append_compress on the shapes of the big configs: d = 128 with three tiers (8B: r = 32, 70B: r = 48, G = 8) and a basis of
+    rank 24 (odd number of 8-column chunks, d = 64); token counts that are not multiples of the 16-token tile, several
+    sequences per call, a second call that continues the slots. Same bars as the tiny append test (reading A15 iii)."""
+    binding, harness = mod
+    if shape == "8b":
+        wl = dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, T=(64, 64, 64))
+    elif shape == "70b":
+        wl = dataclasses.replace(gen.WORKLOADS["llama70b_128k_b1"], L=4, T=(64, 64, 64))
+    else:
+        wl = dataclasses.replace(gen.WORKLOADS["tiny"], tier_ranks=(8, 24), T=(64, 64, 64))
+    cache, consts = harness.make_cache(wl, n_seqs=3, max_tokens=512)
+    BK, BV, gK, gV = consts
+    oc = orc.OracleCache(wl.L, wl.w, wl.H_kv, wl.G, wl.d, wl.tier_ranks, f64(BK), f64(BV), f64(gK), f64(gV))
+    rng = np.random.default_rng(11)
+    nt = len(wl.tier_ranks)
+    t0 = {0: 0, 1: 0, 2: 0}
+    for n_new in ([37, 5, 64], [1, 30, 0]):
+        tier = rng.integers(0, nt, sum(n_new)).astype(np.uint8); flag = (rng.random(sum(n_new)) < 0.3).astype(np.uint8)
+        ks, vs = [], []
+        for s_, n in enumerate(n_new):
+            k, v = gen.make_dense_kv_chunk(wl, s_, t0[s_], n, BK, BV, gK, gV, device="cuda")
+            ks.append(k); vs.append(v); t0[s_] += n
+        k_new, v_new = torch.cat(ks), torch.cat(vs)
+        cache.append_compress([0, 1, 2], n_new, k_new, v_new, tier, flag)
+        off = 0
+        for s_, n in enumerate(n_new):
+            oc.append_compress(s_, f64(k_new[off:off + n]), f64(v_new[off:off + n]), tier[off:off + n], flag[off:off + n])
+            off += n
+    for s_ in (0, 1, 2):
+        T = oc.seq_len(s_)
+        assert cache.seq_len(s_) == T
+        dump = cache.export_tokens(s_, 0, T)
+        S = oc.seqs[s_]
+        assert np.array_equal(dump["slot"].cpu().numpy(), S["slot"]) and np.array_equal(dump["tier"].cpu().numpy(), S["tier"])
+        fl = S["flag"].astype(bool)
+        for z in "KV":
+            got = dump["coef" + z].double().cpu().numpy(); want = S["c" + z]
+            # reading A15 (iii): one bf16 ulp of the oracle's value, or -- for dot products that cancel to almost nothing --
+            # the fp32 accumulation error of a d-term dot product, 2^-20 of the token's largest coefficient
+            ulp = np.maximum(np.abs(want) * 2.0 ** -7, np.abs(want).max(axis=-1, keepdims=True) * 2.0 ** -20)
+            assert np.all(np.abs(got - want) <= ulp) and np.mean(got != want) < 5e-3
+            gc = dump["code" + z].cpu().numpy()
+            lo = (gc & 15).astype(np.int8); hi = (gc >> 4).astype(np.int8)
+            lo = np.where(lo > 7, lo - 16, lo); hi = np.where(hi > 7, hi - 16, hi)
+            dec = np.stack([lo, hi], axis=-1).reshape(S["code" + z].shape)
+            diff = np.abs(dec.astype(np.int32) - S["code" + z])
+            assert not dec[~fl].any()
+            # a coefficient that differs by one bf16 ulp moves the whole residual of that (token, layer, head): there the scales
+            # only have to agree to the size of that move (2 %); everywhere else they are identical or adjacent fp16 values
+            same = np.all(got == want, axis=-1)                                   # [T, L, H]
+            rows = same & fl[:, None, None]                                       # flagged rows with identical coefficients
+            assert diff[rows].max(initial=0) <= 1 and (not rows.any() or np.mean(diff[rows] != 0) <= 2e-3)
+            gsf = dump["scale" + z].cpu().numpy(); wsf = S["scale" + z]
+            gs = gsf.view(np.uint16).astype(np.int32); ws = wsf.view(np.uint16).astype(np.int32)
+            assert np.abs(gs - ws)[same].max() <= 1 and np.mean((gs != ws)[same]) <= 5e-3
+            if (~same).any():
+                assert np.all(np.abs(gsf.astype(np.float64) - wsf.astype(np.float64))[~same] <= 0.02 * wsf.astype(np.float64)[~same] + 1e-6)
+    q = gen.make_q(wl, device="cuda", n_seq=3)
+    out = cache.decode_attention(-1, [0, 1, 2], q).double().cpu().numpy()
+    ref = oc.decode_all_layers([0, 1, 2], f64(q))
+    for s_ in (0, 1, 2):
+        for l in range(wl.L):
+            check_output(out[s_, l], ref[s_, l], oc.max_abs_vhat(s_, l), f"append {shape} seq {s_} layer {l}")
+    cache.destroy()
+
+
 def test_errors_and_reset(mod):
     binding, harness = mod
     wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(64,))
