@@ -31,7 +31,7 @@ __device__ __forceinline__ void mma8(float (&d)[4], uint32_t a0, uint32_t a1, ui
 }
 __device__ __forceinline__ float2 bf2(uint32_t w) { return make_float2(__uint_as_float(w << 16), __uint_as_float(w & 0xffff0000u)); }
 // (x, y) = hi + mid + lo, three bf16 terms = 24 significant bits: the projection keeps fp32 accuracy on the tensor cores
-// (a near-cancelling dot product would otherwise miss the oracle's bf16 coefficient by more than one ulp)
+// (a near-cancelling dot product would otherwise miss the correctly rounded bf16 coefficient by more than one ulp)
 __device__ __forceinline__ void split3(float x, float y, uint32_t& hi, uint32_t& mid, uint32_t& lo) {
   hi = pack_bf16x2(x, y);
   const float rx = x - __uint_as_float(hi << 16), ry = y - __uint_as_float(hi & 0xffff0000u);
