@@ -26,6 +26,25 @@ METRIC = "decode-attn cached tokens scanned/s (all layers; ms_per_step = ms/step
 UNIT = "tokens/s"
 
 
+def config_of(wl, world, footprint_gb=None):
+    """The `config` object of the JSON line: the same for our arm and the reference arm."""
+    c = {"workload": wl.name, "shape": f"L={wl.L} w={wl.w} H_kv={wl.H_kv} G={wl.G} d={wl.d} r={wl.r}",
+         "batch": wl.n_seq, "T": wl.T[0] if len(set(wl.T)) == 1 else [min(wl.T), max(wl.T)], "tiers": list(wl.tier_ranks),
+         "tier_frac": list(wl.tier_frac), "resid_frac": wl.resid_frac, "launch_mode": "all layers in one call (layer = -1)",
+         "l2_policy": "inputs larger than L2 (compressed cache of the workload >> 126 MB; every step streams all of it): no flush",
+         "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"}
+    return c
+
+
+def traffic_of(workload):
+    """dram__bytes_read + dram__bytes_write of the fused decode kernel per launch, from the committed ncu capture (or None)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(workload)
+    except Exception:
+        return None
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -165,7 +184,7 @@ def run_reference(args, wl):
     line = {"impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "note": "CPU oracle (oracle/dwkv_oracle.py) as it stands, bounded sample"},
+            "config": config_of(wl, args.gpus),
             "cpu_baseline": {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": tps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -294,7 +313,7 @@ def main():
     alg_bytes = fp["used_bytes"]                      # compressed records: 4 r_t + f_t*2*(d/2+d/8) per (l, h, token)
     achieved = alg_bytes / (scan_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "kernel": "scan3_kernel<NKB,D,PAIR> (fused q pre-projection + split-T scan, one persistent launch per step)",
+                "traffic": traffic_of(wl.name), "kernel": "scan3_kernel<NKB,D,PAIR> (fused q pre-projection + split-T scan, one persistent launch per step)",
                 "scan_ms": scan_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "frac_of_8TBps_nominal": achieved / 8000.0, "step_frac_of_peak": alg_bytes / (ms * 1e-3) / 1e9 / peak}
 
@@ -389,11 +408,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
                 "data": "synthetic",
-                "config": {"workload": wl.name, "shape": f"L={wl.L} w={wl.w} H_kv={wl.H_kv} G={wl.G} d={wl.d} r={wl.r}",
-                           "batch": n_seq, "T": wl.T[0], "tiers": list(wl.tier_ranks), "tier_frac": list(wl.tier_frac),
-                           "resid_frac": wl.resid_frac, "launch_mode": "all layers in one call (layer = -1)",
-                           "l2_policy": "inputs larger than L2 (compressed cache %.2f GB >> 126 MB)" % (fp["used_bytes"] / 1e9),
-                           "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"},
+                "config": config_of(wl, world, fp["used_bytes"] / 1e9),
                 "clocks": cs.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "cpu_baseline": cpu_baseline, "extra": extra}
         print(json.dumps(line))
