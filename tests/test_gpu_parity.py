@@ -285,6 +285,32 @@ def test_append_compress_against_oracle(mod):
     cache.destroy()
 
 
+@pytest.mark.parametrize("d,G,ranks", [(64, 1, (8,)), (64, 3, (16, 24)), (64, 8, (8, 16)), (64, 5, (24, 48, 64)), (128, 2, (8, 64)),
+                                        (128, 6, (16, 32)), (128, 7, (8, 24, 48)), (128, 8, (32, 64)), (128, 4, (8, 16, 24, 32))])
+def test_kernel_instances_small_shapes(mod, d, G, ranks):
+    """Every instance family of the fused decode kernel (PAIR for G <= 4, FULL for G <= 8; head dim 64 / 128; basis ranks 8 .. 64,
+    odd and even numbers of 8-column chunks; 1 .. 4 tiers) against the oracle on a small ragged two-sequence cache, all-layer
+    and per-layer calls, with a peaked-softmax variant."""
+    binding, harness = mod
+    nt = len(ranks)
+    frac = tuple([1.0 / nt] * nt)
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], d=d, G=G, tier_ranks=ranks, tier_frac=frac, resid_frac=0.2, L=2, w=1, H_kv=2,
+                             T=(333, 70), S0=8)
+    rng = np.random.default_rng(d + 7 * G + len(ranks))
+    routings = []
+    for T in wl.T:
+        tier = rng.integers(0, nt, T).astype(np.uint8); flag = (rng.random(T) < 0.3).astype(np.uint8)
+        routings.append((tier, flag))
+    cache, consts, kept = load(harness, wl, routings, chunk=100)
+    for gain in (1.0, 16.0):
+        q = gen.make_q(wl, device="cuda", gain=gain)
+        out = cache.decode_attention(-1, [0, 1], q)
+        compare(wl, cache, consts, kept, routings, q, out, what=f"d={d} G={G} ranks={ranks} gain={gain}")
+    out1 = cache.decode_attention(1, [0, 1], q[:, 1].contiguous())
+    assert rel_l2(out1.cpu().numpy(), out[:, 1].cpu().numpy()) < 2e-3
+    cache.destroy()
+
+
 @pytest.mark.parametrize("shape", ["8b", "70b", "odd"])
 def test_append_compress_tensor_core_tiles(mod, shape):
     """dwkv_append_compress on the shapes of the big configs: d = 128 with three tiers (8B: r = 32, 70B: r = 48, G = 8) and a basis of
