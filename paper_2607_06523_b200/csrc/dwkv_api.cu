@@ -144,9 +144,9 @@ struct dwkv_cache {
   Plan3 plan3;
   // options
   int64_t opt_max_unit_blocks = 0;   // 0 = adaptive
-  int64_t opt_cost_coef_pct = 80, opt_cost_tok = -1, opt_cost_resid_pct = -1, opt_cost_seg = 24576;   // planner cost model (-1 = by G)
+  int64_t opt_cost_coef_pct = 80, opt_cost_tok = -1, opt_cost_resid_pct = -1, opt_cost_seg = 40000;   // planner cost model (-1 = by G)
   int64_t opt_interleave = 0;        // planner: interleave the classes of a sequence (0 = class after class)
-  int64_t opt_stamps_ptr = 0;        // device pointer [n_slices] u64 for per-warp end stamps (measurement aid), 0 = off
+  int64_t opt_stamps_ptr = 0;        // device pointer [2 * n_slices] u64 for per-warp end stamps + segment counts (measurement aid), 0 = off
   int64_t opt_unit_kb = 64;          // planner: target bytes of a work unit (per layer-head), KB
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
@@ -557,8 +557,8 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   const int LH = n_lsel * c->geom.H;
   const double flag_w = (double)c->opt_flag_cost_pct / 100.0;
   const double seg_ovh = (double)c->opt_cost_seg;
-  // per-token and per-residual-byte work grows with the query heads per kv head (fits at G = 4: 24 / 235 %, G = 8: 40 / 265 %)
-  const double cost_tok = c->opt_cost_tok >= 0 ? (double)c->opt_cost_tok : 8.0 + 4.0 * c->geom.G;
+  // per-token and per-residual-byte work grows with the query heads per kv head (fits at G = 4: 24 / 235 %, G = 8: 48 / 265 %)
+  const double cost_tok = c->opt_cost_tok >= 0 ? (double)c->opt_cost_tok : 6.0 * c->geom.G;
   const double cost_resid_pct = c->opt_cost_resid_pct >= 0 ? (double)c->opt_cost_resid_pct : 205.0 + 7.5 * c->geom.G;
   std::vector<Unit> units;
   std::vector<int32_t> ustart(n_seqs + 1, 0), unsub;

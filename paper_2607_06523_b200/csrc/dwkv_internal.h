@@ -32,7 +32,7 @@ struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.c
   const __nv_bfloat16* BK;     // [M][H][r][d]
   const __nv_bfloat16* gK;     // [L][H][d]
   float* part;                 // [n_slots][G][2 + r + d]: (m, l, a[r], e[d]) per query head
-  unsigned long long* stamps;  // optional [n_slices]: globaltimer at the end of every warp slice (NULL = off)
+  unsigned long long* stamps;  // optional [2 * n_slices]: globaltimer at the end of every warp slice, segments it touched (NULL = off)
   int32_t n_slices, n_segs;
   int32_t layer0, Lq, LH, w;
   int32_t H, G, r, d;

@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
   }
 
   // ---- compute stream ----------------------------------------------------------------------------------------------------
-  int cur_seg = ws.x, k_c = 0, slot_next = ws.w;
+  int cur_seg = ws.x, k_c = 0, slot_next = ws.w, n_entered = 1;
   uint32_t phase = 0u;
   while (true) {
     const uint4 dsc = lds128(descs + 16 * k_c);
@@ -319,6 +319,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
       prologue_compute<NKB, D, PAIR>(q, pl, p, seg, lane);
       state_reset<NKB, D>(st);
       cur_seg = seg;
+      ++n_entered;
     }
     mbar_wait(bars + 8 * k_c, (phase >> k_c) & 1u);
     phase ^= 1u << k_c;
@@ -349,6 +350,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     p.stamps[gw] = t;
+    p.stamps[p.n_slices + gw] = (unsigned long long)n_entered;     // segments this slice touched
   }
 }
 
