@@ -377,7 +377,9 @@ def main():
                         "sampled_parity_rel_l2_max": max(rels)}
 
     # ---- dense bf16 comparison kernel on the same shapes ------------------------------------------------------------
-    if rank == 0 and not args.no_dense:
+    if rank == 0 and not args.no_dense and len(set(wl.T)) > 1:
+        extra["dense"] = {"skipped": "the dense comparison kernel takes one length for all sequences; this workload is ragged"}
+    elif rank == 0 and not args.no_dense:
         try:
             T = wl.T[0]
             free, _ = torch.cuda.mem_get_info()
