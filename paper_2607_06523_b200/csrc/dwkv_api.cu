@@ -388,8 +388,8 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
   if (rc) return rc;
   rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
   if (rc) return rc;
-  c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, (const __nv_bfloat16*)k_new,
-                                 (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, st);
+  c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, ridx, (const __nv_bfloat16*)k_new,
+                                     (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, c->n_sms, st);
   CU_OK(cudaGetLastError());
   return DWKV_OK;
 }

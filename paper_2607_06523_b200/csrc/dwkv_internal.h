@@ -73,10 +73,10 @@ int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* d
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
                        const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,
                        const __half* scaleK, const __half* scaleV, cudaStream_t s);
-int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
+int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, int n_flagged /* sorted first in dst */,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
                     const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK, const __nv_bfloat16* gV,
-                    cudaStream_t s);
+                    int n_sms, cudaStream_t s);
 struct DumpPtrs {
   __nv_bfloat16 *coefK, *coefV;
   uint8_t *codeK, *codeV;
