@@ -738,7 +738,7 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   Combine3Params cp;
   cp.pstart = sp.pstart; cp.part = sp.part; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
   cp.layer0 = layer0; cp.Lq = Lsel; cp.LH = sp.LH; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;
-  c->launches += launch_combine3(cp, P.n_segs, (double)P.n_slots > 8.0 * (double)P.n_segs, st);
+  c->launches += launch_combine3(cp, P.n_segs, P.n_slots > 64LL * P.n_segs ? 16 : (P.n_slots > 8LL * P.n_segs ? 4 : 1), st);
   CU_OK(cudaGetLastError());
   return DWKV_OK;
 }

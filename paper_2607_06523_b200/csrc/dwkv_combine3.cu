@@ -14,18 +14,19 @@ bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
 namespace {
 using namespace dwkv::dev;
 
-// SPLIT: one CTA of 4 warps merges the partials of one (segment, query head); the warps split the partial list (warp w takes
-// partials w, w+4, ...) -- for per-layer calls, where a segment has ~150 partials. !SPLIT: one CTA per segment, warp w merges
+// SPLIT (S = 4 or 16): one CTA of S warps merges the partials of one (segment, query head); the warps split the partial list
+// (warp w takes partials w, w+S, ...) -- for per-layer calls, where a segment has 20-150 partials and there are only a few
+// dozen (segment, head) pairs: the merge is a chain of dependent L2 round trips, so its time is set by the partials per warp. !SPLIT: one CTA per segment, warp w merges
 // heads w, w+4 on its own -- for all-layer steps (1-6 partials per segment, thousands of segments). Lanes run over rank
 // columns for a*, over channels (D / 32 each) for e* and the back-projection.
-template <int D, bool SPLIT>
-__global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
+template <int D, int S>      // S = warps sharing one head's partial list: 1 (no split), 4 or 16
+__global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Combine3Params p) {
+  constexpr bool SPLIT = S > 1;
   constexpr int CPL = D / 32;                       // channels per lane
-  __shared__ float sh_l[4];
-  __shared__ float sh_a[4][64];
-  __shared__ float sh_e[4][D];
+  __shared__ float sh_l[S];
+  __shared__ float sh_a[S][64];
+  __shared__ float sh_e[S][D];
   const int seg = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  constexpr int S = SPLIT ? 4 : 1;                  // warps sharing one head's partial list
   const int ws = SPLIT ? warp : 0;                  // this warp's offset in the split
   // programmatic dependent launch: this grid may start while the decode kernel drains; wait for its completion and flush
   cudaGridDependencySynchronize();
@@ -94,11 +95,15 @@ __global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
     for (int c = 0; c < CPL; ++c) sh_e[warp][lane * CPL + c] = e[c];
     __syncthreads();
     if (warp != 0) return;
-    lstar = sh_l[0] + sh_l[1] + sh_l[2] + sh_l[3];
-    a0 = sh_a[0][lane] + sh_a[1][lane] + sh_a[2][lane] + sh_a[3][lane];
-    a1 = sh_a[0][lane + 32] + sh_a[1][lane + 32] + sh_a[2][lane + 32] + sh_a[3][lane + 32];
+    lstar = 0.f; a0 = 0.f; a1 = 0.f;
 #pragma unroll
-    for (int c = 0; c < CPL; ++c) e[c] = sh_e[0][lane * CPL + c] + sh_e[1][lane * CPL + c] + sh_e[2][lane * CPL + c] + sh_e[3][lane * CPL + c];
+    for (int c = 0; c < CPL; ++c) e[c] = 0.f;
+#pragma unroll
+    for (int w = 0; w < S; ++w) {
+      lstar += sh_l[w]; a0 += sh_a[w][lane]; a1 += sh_a[w][lane + 32];
+#pragma unroll
+      for (int c = 0; c < CPL; ++c) e[c] += sh_e[w][lane * CPL + c];
+    }
   }
   // back-projection o = (gV * (BV^T a*) + e*) / l*: basis rows as coalesced loads, a*_j broadcast by shuffle
   const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
@@ -147,10 +152,10 @@ int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s) {
   return ok ? 1 : 0;
 }
 
-int launch_combine3(const Combine3Params& p, int n_segs, bool split, cudaStream_t s) {
+int launch_combine3(const Combine3Params& p, int n_segs, int split, cudaStream_t s) {
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = split ? dim3(n_segs, p.G) : dim3(n_segs);       // split: 4 warps share the partial list of one head
-  cfg.blockDim = dim3(128);
+  cfg.gridDim = split > 1 ? dim3(n_segs, p.G) : dim3(n_segs);       // split: 16 warps share the partial list of one head
+  cfg.blockDim = dim3(split > 4 ? 32 * split : 128);
   cfg.dynamicSmemBytes = 0;
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
@@ -158,8 +163,15 @@ int launch_combine3(const Combine3Params& p, int n_segs, bool split, cudaStream_
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  if (p.d == 128) { if (split) cudaLaunchKernelEx(&cfg, combine3_kernel<128, true>, p); else cudaLaunchKernelEx(&cfg, combine3_kernel<128, false>, p); }
-  else { if (split) cudaLaunchKernelEx(&cfg, combine3_kernel<64, true>, p); else cudaLaunchKernelEx(&cfg, combine3_kernel<64, false>, p); }
+  if (p.d == 128) {
+    if (split == 16) cudaLaunchKernelEx(&cfg, combine3_kernel<128, 16>, p);
+    else if (split == 4) cudaLaunchKernelEx(&cfg, combine3_kernel<128, 4>, p);
+    else cudaLaunchKernelEx(&cfg, combine3_kernel<128, 1>, p);
+  } else {
+    if (split == 16) cudaLaunchKernelEx(&cfg, combine3_kernel<64, 16>, p);
+    else if (split == 4) cudaLaunchKernelEx(&cfg, combine3_kernel<64, 4>, p);
+    else cudaLaunchKernelEx(&cfg, combine3_kernel<64, 1>, p);
+  }
   return 1;
 }
 

@@ -68,7 +68,7 @@ struct CacheGeom {
 // kernel launchers (dwkv_combine3.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
 int scan3_num_slices(int n_sms);
 int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s);                 // 0 = no instance for this shape
-int launch_combine3(const Combine3Params& p, int n_segs, bool split, cudaStream_t s);
+int launch_combine3(const Combine3Params& p, int n_segs, int split /* 1, 4 or 16 warps per (segment, head) */, cudaStream_t s);
 int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
                        const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,
