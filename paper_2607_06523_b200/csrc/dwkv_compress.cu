@@ -9,9 +9,9 @@
 //   e   = x - g * rec  ->  int4 / group 16 / fp16 scale  (quantiser A14, fp32 IEEE, no reciprocal)
 // Persistent grid: the (layer-head, tile) items are cut into equal-cost contiguous ranges, one per CTA (a flagged tile counts
 // kCostFlag, an unflagged one kCostPlain); a CTA stages B' of its current (layer, head) in shared memory in the register
-// order of the MMA B fragments (one 16-byte + one 8-byte ld.shared per MMA triple) and its 8 warps take tiles round-robin.
-// The contraction index of the projection is permuted so that a lane's A fragments are plain 16-byte global loads of its
-// token rows; the loads of the next Z / next tile are in flight while the current one is multiplied. Results go straight
+// order of the MMA B fragments (one 16-byte + one 8-byte ld.shared per MMA triple) and its 8 or 12 warps take tiles round-robin.
+// Every warp streams its token rows through a private shared-memory ring filled by cp.async 2-4 stages ahead (a stage = the 16
+// rows of one tile and one Z) and reads the A fragments back with ldmatrix. Results go straight
 // to their fragment-native positions in the class pages (dwkv_layout.cuh): every 32-bit coefficient word, 16-byte K-code row,
 // V-code byte and scale is owned by exactly one (token, lane), so no atomics are needed (pages are zeroed when allocated).
 #include <algorithm>
@@ -24,7 +24,7 @@ namespace {
 using namespace dwkv::dev;
 
 constexpr int kCostFlag = 4, kCostPlain = 1;   // relative cost of a tile with / without the reconstruction + quantiser part
-constexpr int kCompressWarps = 12;
+constexpr int kCompressMaxWarps = 16;
 
 __device__ __forceinline__ void mma16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
   asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
@@ -96,32 +96,67 @@ __device__ __forceinline__ void cost_to_item(long long pos, int per_lh, int nf, 
   *tile = rem < nf * kCostFlag ? rem / kCostFlag : min(nt_lh, nf + (rem - nf * kCostFlag) / kCostPlain);
 }
 
+// ---- per-warp shared-memory ring of token-row stages -------------------------------------------------------------------------
+// A stage holds the 16 token rows of one tile for one Z, row-major with a row pitch of 2 * D + 16 bytes (ldmatrix and 4-byte
+// reads of 8 consecutive rows are then bank-conflict free). Lane (g, t) copies channels 32u + 8t .. +7 of rows g and g + 8 with
+// 16-byte cp.async (zero-filled for rows beyond n_tok); one ldmatrix.x4 per k step returns the A fragment of the projection as
+// an aligned register quad. A stage is complete for the warp after cp.async.wait_group + __syncwarp.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait(int pending) {     // pending = stages - 1 (2..4 stages)
+  if (pending >= 3) asm volatile("cp.async.wait_group 3;" ::: "memory");
+  else if (pending == 2) asm volatile("cp.async.wait_group 2;" ::: "memory");
+  else asm volatile("cp.async.wait_group 1;" ::: "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 r;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(a));
+  return r;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t r;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(a));
+  return r;
+}
+
+__device__ __forceinline__ void ldmatrix_x4(uint32_t a, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(a));
+}
+
 template <int D>
-__device__ __forceinline__ void load_x(const __nv_bfloat16* X, const RowDst& ra, const RowDst& rb, int LH, int lh, int t,
-                                       uint4 (&xa)[D / 32], uint4 (&xb)[D / 32]) {
-  // lane (g, t) takes channels 32u + 8t .. +7 of rows g and g+8: with the permuted contraction index these are the A registers
-  const uint4* pa = reinterpret_cast<const uint4*>(X + ((size_t)ra.src * LH + lh) * D + 8 * t);
-  const uint4* pb = reinterpret_cast<const uint4*>(X + ((size_t)rb.src * LH + lh) * D + 8 * t);
+__device__ __forceinline__ void issue_rows(uint32_t stage, const __nv_bfloat16* X, int2 src, int LH, int lh, int lane) {
+  constexpr int PITCH = 2 * D + 16;
+  const int g = lane >> 2, t = lane & 3;
+  const char* pa = reinterpret_cast<const char*>(X + ((size_t)max(src.x, 0) * LH + lh) * D + 8 * t);
+  const char* pb = reinterpret_cast<const char*>(X + ((size_t)max(src.y, 0) * LH + lh) * D + 8 * t);
+  const int sa = src.x >= 0 ? 16 : 0, sb = src.y >= 0 ? 16 : 0;
+  const uint32_t da = stage + g * PITCH + 16 * t, db = da + 8 * PITCH;
 #pragma unroll
   for (int u = 0; u < D / 32; ++u) {
-    xa[u] = ra.valid() ? __ldg(pa + 4 * u) : make_uint4(0u, 0u, 0u, 0u);
-    xb[u] = rb.valid() ? __ldg(pb + 4 * u) : make_uint4(0u, 0u, 0u, 0u);
+    cp_async16(da + 64 * u, pa + 64 * u, sa);
+    cp_async16(db + 64 * u, pb + 64 * u, sb);
   }
 }
 
-// C = X . B'^T for one Z: 3 MMAs (lo, mid, hi term of B') per (k step, rank chunk); returns the rounded coefficients of rows g
-// (ca) and g+8 (cb), columns 8nt + 2t, +1, zero beyond the token's rank
+// bf16 pair (channels ch, ch+1; ch even) of row `row` of a stage
+template <int D>
+__device__ __forceinline__ uint32_t stage_x(uint32_t stage, int row, int ch) { return lds32(stage + row * (2 * D + 16) + ch * 2); }
+
+// C = X . B'^T for one Z: 3 MMAs (lo, mid, hi term of B') per (k step, rank chunk); returns the rounded coefficients of rows g (ca) and g+8 (cb), columns 8nt + 2t, +1, zero beyond the rank
 template <int D, int NT>
-__device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int lane, const uint4 (&xa)[D / 32], const uint4 (&xb)[D / 32],
-                                        const RowDst& ra, const RowDst& rb, uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
+__device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int lane, uint32_t stage, const RowDst& ra, const RowDst& rb,
+                                        uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
   float c[NT][4];
 #pragma unroll
   for (int nt = 0; nt < NT; ++nt) c[nt][0] = c[nt][1] = c[nt][2] = c[nt][3] = 0.f;
+  // ldmatrix: lanes 8i .. 8i+7 address the rows of matrix i = (rows 0-7 | 8-15) x (channels +0 | +8) of the k step
+  const uint32_t am = stage + ((lane & 7) + 8 * ((lane >> 3) & 1)) * (2 * D + 16) + 16 * (lane >> 4);
 #pragma unroll
   for (int kk = 0; kk < D / 16; ++kk) {
-    const int u = kk >> 1;
-    const uint32_t a0 = (kk & 1) ? xa[u].z : xa[u].x, a2 = (kk & 1) ? xa[u].w : xa[u].y;
-    const uint32_t a1 = (kk & 1) ? xb[u].z : xb[u].x, a3 = (kk & 1) ? xb[u].w : xb[u].y;
+    uint32_t a0, a1, a2, a3;
+    ldmatrix_x4(am + 32 * kk, a0, a1, a2, a3);
 #pragma unroll
     for (int nt = 0; nt < NT; ++nt) {
       const uint4 hm = P4[(kk * NT + nt) * 32 + lane];
@@ -156,11 +191,11 @@ __device__ __forceinline__ void store_coef(const RowDst& rd, const uint32_t (&cw
 }
 
 // rec = c . B, e = x - g * rec, int4 quantiser (A14), fragment-native code / scale stores: tiles with a flagged token only.
-// x is re-read from global (L1 / L2 hits) in the unpermuted channel order of the reconstruction's n dimension; the loop is
-// kept rolled so the kernel stays inside the instruction cache.
+// x is read from the shared-memory stage in the unpermuted channel order of the reconstruction's n dimension; the loop is kept
+// rolled so the kernel stays inside the instruction cache.
 template <int D, int NT>
 __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfloat16* BTz, const int ldT, const __nv_bfloat16* gt,
-                                                     const __nv_bfloat16* xa, const __nv_bfloat16* xb, const RowDst& ra, const RowDst& rb,
+                                                     const uint32_t stage, const RowDst& ra, const RowDst& rb,
                                                      const uint32_t (&ca)[NT], const uint32_t (&cb)[NT], const int gr, const int t) {
 #pragma unroll 1
   for (int wx = 0; wx < D / 32; ++wx) {     // K code word wx of a row = groups 2wx, 2wx+1 (registers q = 4wx .. 4wx+3)
@@ -188,9 +223,8 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
 #pragma unroll
       for (int row = 0; row < 2; ++row) {
         const RowDst& rd = row ? rb : ra;
-        const __nv_bfloat16* xp = row ? xb : xa;
-        const float2 x0 = bf2(rd.valid() ? __ldg(reinterpret_cast<const uint32_t*>(xp + 16 * grp)) : 0u);
-        const float2 x2 = bf2(rd.valid() ? __ldg(reinterpret_cast<const uint32_t*>(xp + 16 * grp + 8)) : 0u);
+        const float2 x0 = bf2(stage_x<D>(stage, gr + 8 * row, 16 * grp + 2 * t));          // rows beyond n_tok were zero-filled
+        const float2 x2 = bf2(stage_x<D>(stage, gr + 8 * row, 16 * grp + 8 + 2 * t));
         float e[4];
         e[0] = fmaf(-g0.x, rec[0][2 * row], x0.x); e[1] = fmaf(-g0.y, rec[0][2 * row + 1], x0.y);
         e[2] = fmaf(-g2.x, rec[1][2 * row], x2.x); e[3] = fmaf(-g2.y, rec[1][2 * row + 1], x2.y);
@@ -229,11 +263,11 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
 }
 
 template <int D, int NT>      // NT = basis rank / 8
-__global__ void __launch_bounds__(kCompressWarps * 32, 1)
-compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, const int n_tok, const int n_flag_tiles,
+__global__ void __launch_bounds__(kCompressMaxWarps * 32, 1)
+compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, const int n_tok, const int n_flag_tiles, const int n_stages,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
                     const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
-  constexpr int NKK = D / 16, r = 8 * NT, ldT = r + 8, NFRAG = NKK * NT * 32, NTHR = kCompressWarps * 32;
+  constexpr int NKK = D / 16, r = 8 * NT, ldT = r + 8, NFRAG = NKK * NT * 32, STAGE = 16 * (2 * D + 16);
   extern __shared__ __align__(16) uint8_t smem_raw[];
   uint4* P4 = reinterpret_cast<uint4*>(smem_raw);                        // [2][NFRAG]  (hi.b0, hi.b1, mid.b0, mid.b1) of B'
   uint2* P2 = reinterpret_cast<uint2*>(P4 + 2 * NFRAG);                  // [2][NFRAG]  (lo.b0, lo.b1)
@@ -241,6 +275,8 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
   const int LH = g.L * g.H;
   const uint32_t ranks4 = (uint32_t)g.tier_rank[0] | ((uint32_t)g.tier_rank[1] << 8) | ((uint32_t)g.tier_rank[2] << 16) | ((uint32_t)g.tier_rank[3] << 24);
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gr = lane >> 2, t = lane & 3;
+  const int NTHR = blockDim.x, W = NTHR >> 5;
+  const uint32_t ring = (uint32_t)__cvta_generic_to_shared(BT + 2 * D * ldT) + (uint32_t)(warp * n_stages) * STAGE;   // this warp's stages
   const int nt_lh = (n_tok + 15) >> 4, nf = n_flag_tiles;
   const int per_lh = nf * kCostFlag + (nt_lh - nf) * kCostPlain;
   const long long total = (long long)LH * per_lh;
@@ -252,7 +288,32 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
     const int tb = lh == lh0 ? t0 : 0, te = lh == lh1 ? t1 : nt_lh;
     if (tb >= te) continue;
     const int l = lh / g.H, h = lh - l * g.H;
-    __syncthreads();                                                     // the previous segment's readers are done
+    // ---- this warp's tiles of the segment: tb + warp, + W, ...; their row copies start before the basis is staged ----------
+    const int n = (te - tb - warp + W - 1) / W;                          // tiles of this warp (may be <= 0)
+    const int nst = 2 * n;                                               // stages: (tile 0, K), (tile 0, V), (tile 1, K), ...
+    int issued = 0, slot_i = 0;
+    int2 src_cur = make_int2(-1, -1), src_nxt = make_int2(-1, -1);       // source rows (-1: beyond n_tok) of the tile being issued / the next
+    auto fetch_src = [&](int i) {
+      const int tok = 16 * (tb + warp + W * i) + gr;
+      return make_int2(tok < n_tok ? __ldg(&dst[tok].src) : -1, tok + 8 < n_tok ? __ldg(&dst[tok + 8].src) : -1);
+    };
+    auto issue_one = [&]() {
+      if (issued < nst) {
+        issue_rows<D>(ring + slot_i * STAGE, (issued & 1) ? v_new : k_new, src_cur, LH, lh, lane);
+        if (issued & 1) {
+          src_cur = src_nxt;
+          const int ni = (issued >> 1) + 2;
+          if (ni < n) src_nxt = fetch_src(ni);
+        }
+        ++issued;
+        slot_i = slot_i + 1 == n_stages ? 0 : slot_i + 1;
+      }
+      cp_async_commit();                                                 // always: uniform group counting
+    };
+    if (n > 0) src_cur = fetch_src(0);
+    if (n > 1) src_nxt = fetch_src(1);
+    for (int k = 0; k + 1 < n_stages; ++k) issue_one();
+    __syncthreads();                                                     // the previous segment's readers of B' are done
     // ---- stage B' = B / g (hi + mid + lo) in B-fragment order and the transposed basis --------------------------------------
 #pragma unroll 1
     for (int z = 0; z < 2; ++z) {
@@ -261,10 +322,10 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
       for (int idx = tid; idx < NFRAG; idx += NTHR) {
         const int fl = idx & 31, fnt = (idx >> 5) % NT, fkk = (idx >> 5) / NT;
         const int fg = fl >> 2, ft = fl & 3;
-        const int ch = 32 * (fkk >> 1) + 8 * ft + 4 * (fkk & 1);           // k slots 2t, 2t+1, 8+2t, 8+2t+1 <-> channels ch .. ch+3
-        const uint2 bw = __ldg(reinterpret_cast<const uint2*>(B + (size_t)(8 * fnt + fg) * D + ch));
-        const uint2 gw = __ldg(reinterpret_cast<const uint2*>(gz + ch));
-        const float2 b01 = bf2(bw.x), b23 = bf2(bw.y), g01 = bf2(gw.x), g23 = bf2(gw.y);
+        const int ch = 16 * fkk + 2 * ft;                                  // k slots 2t, 2t+1 | 8+2t, 8+2t+1 <-> channels ch, ch+1 | ch+8, ch+9
+        const __nv_bfloat16* bp = B + (size_t)(8 * fnt + fg) * D + ch;
+        const float2 b01 = bf2(__ldg(reinterpret_cast<const uint32_t*>(bp))), b23 = bf2(__ldg(reinterpret_cast<const uint32_t*>(bp + 8)));
+        const float2 g01 = bf2(__ldg(reinterpret_cast<const uint32_t*>(gz + ch))), g23 = bf2(__ldg(reinterpret_cast<const uint32_t*>(gz + ch + 8)));
         uint32_t h0, m0, l0, h1, m1, l1;
         split3(__fdiv_rn(b01.x, g01.x), __fdiv_rn(b01.y, g01.y), h0, m0, l0);
         split3(__fdiv_rn(b23.x, g23.x), __fdiv_rn(b23.y, g23.y), h1, m1, l1);
@@ -279,39 +340,39 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
       }
     }
     __syncthreads();
-    // ---- this warp's tiles of the segment: tb + warp, + 8, ... ; loads run one Z ahead of the multiplications ---------------
-    int tile = tb + warp;
-    if (tile >= te) continue;
-    RowDst ra = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr, n_tok, lh), rb = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr + 8, n_tok, lh);
-    uint4 xka[D / 32], xkb[D / 32], xva[D / 32], xvb[D / 32];
-    load_x<D>(k_new, ra, rb, LH, lh, t, xka, xkb);
-#pragma unroll 1
-    while (true) {
-      const bool any_flag = __any_sync(kFull, ra.flagged() || rb.flagged());
-      const int next = tile + kCompressWarps;
-      RowDst na = ra, nb = rb;
-      if (next < te) {                       // destination table rows of the next tile: needed (src) before its K rows can be fetched
-        na = row_dst(arena, ranks4, g.d, dst, 16 * next + gr, n_tok, lh);
-        nb = row_dst(arena, ranks4, g.d, dst, 16 * next + gr + 8, n_tok, lh);
-      }
-      load_x<D>(v_new, ra, rb, LH, lh, t, xva, xvb);
-      uint32_t ca[NT], cb[NT];
-      project<D, NT>(P4, P2, lane, xka, xkb, ra, rb, ca, cb);
-      store_coef<NT>(ra, ca, 0, t);
-      store_coef<NT>(rb, cb, 0, t);
-      if (any_flag)
-        reconstruct_quantise<D, NT>(0, BT, ldT, gK + (size_t)lh * D + 2 * t, k_new + ((size_t)ra.src * LH + lh) * D + 2 * t,
-                                    k_new + ((size_t)rb.src * LH + lh) * D + 2 * t, ra, rb, ca, cb, gr, t);
-      if (next < te) load_x<D>(k_new, na, nb, LH, lh, t, xka, xkb);
-      project<D, NT>(P4 + NFRAG, P2 + NFRAG, lane, xva, xvb, ra, rb, ca, cb);
-      store_coef<NT>(ra, ca, 1, t);
-      store_coef<NT>(rb, cb, 1, t);
-      if (any_flag)
-        reconstruct_quantise<D, NT>(1, BT + D * ldT, ldT, gV + (size_t)lh * D + 2 * t, v_new + ((size_t)ra.src * LH + lh) * D + 2 * t,
-                                    v_new + ((size_t)rb.src * LH + lh) * D + 2 * t, ra, rb, ca, cb, gr, t);
-      if (next >= te) break;
-      ra = na; rb = nb; tile = next;
+    // destination rows of the current tile and (loaded one stage early, so the table read is off the critical path) of the next
+    RowDst ra, rb, na, nb;
+    if (n > 0) {
+      na = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr, n_tok, lh);
+      nb = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr + 8, n_tok, lh);
     }
+    bool any_flag = false;
+    int slot_c = 0;
+#pragma unroll 1
+    for (int s = 0; s < nst; ++s) {
+      __syncwarp();                                                      // every lane is done with the stage that is refilled now
+      issue_one();
+      cp_async_wait(n_stages - 1);                                       // this lane's copies of stage s have landed ...
+      __syncwarp();                                                      // ... and so have the other lanes' (the reconstruction reads across lanes)
+      const uint32_t stage = ring + slot_c * STAGE;
+      const int z = s & 1;
+      if (z == 0) {
+        ra = na; rb = nb;
+        any_flag = __any_sync(kFull, ra.flagged() || rb.flagged());
+      } else if (s + 1 < nst) {
+        const int tile = tb + warp + W * ((s + 1) >> 1);
+        na = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr, n_tok, lh);
+        nb = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr + 8, n_tok, lh);
+      }
+      uint32_t ca[NT], cb[NT];
+      project<D, NT>(P4 + z * NFRAG, P2 + z * NFRAG, lane, stage, ra, rb, ca, cb);
+      store_coef<NT>(ra, ca, z, t);
+      store_coef<NT>(rb, cb, z, t);
+      if (any_flag)
+        reconstruct_quantise<D, NT>(z, BT + z * D * ldT, ldT, (z ? gV : gK) + (size_t)lh * D + 2 * t, stage, ra, rb, ca, cb, gr, t);
+      slot_c = slot_c + 1 == n_stages ? 0 : slot_c + 1;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");                 // only empty groups are left
   }
 }
 
@@ -322,16 +383,22 @@ int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* 
                         const __nv_bfloat16* gV, int n_sms, cudaStream_t s) {
   if (n <= 0) return 0;
   const int nfrag = (g.d / 16) * (g.r / 8) * 32;
-  const size_t smem = (size_t)2 * nfrag * 24 + (size_t)2 * g.d * (g.r + 8) * 2;
+  const size_t fixed = (size_t)2 * nfrag * 24 + (size_t)2 * g.d * (g.r + 8) * 2, stage = (size_t)16 * (2 * g.d + 16);
+  const size_t cap = 227 * 1024;
+  // warps per CTA and ring stages per warp: 16 warps (the kernel is latency-bound: 4 warps per scheduler) if they can have 2
+  // stages each, else 8 warps
+  int warps = kCompressMaxWarps, stages = (int)std::min<size_t>(4, (cap - fixed) / (warps * stage));
+  if (stages < 2) { warps = 8; stages = (int)std::min<size_t>(4, (cap - fixed) / (warps * stage)); }
+  if (stages < 2) return 0;
+  const size_t smem = fixed + (size_t)warps * stages * stage;
   const long long tiles = (long long)g.L * g.H * ((n + 15) / 16);
-  const int per_sm = 1;
-  const int grid = (int)std::max<long long>(1, std::min<long long>((long long)per_sm * n_sms, tiles));
+  const int grid = (int)std::max<long long>(1, std::min<long long>((long long)n_sms, tiles));
   const int nft = (n_flagged + 15) / 16;
   bool ok = true;
 #define DWKV_COMPRESS_CASE(DD, NN)                                                                                              \
   case NN:                                                                                                                      \
     cudaFuncSetAttribute(compress_mma_kernel<DD, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                  \
-    compress_mma_kernel<DD, NN><<<grid, kCompressWarps * 32, smem, s>>>(arena, g, dst, n, nft, k_new, v_new, BK, BV, gK, gV);    \
+    compress_mma_kernel<DD, NN><<<grid, warps * 32, smem, s>>>(arena, g, dst, n, nft, stages, k_new, v_new, BK, BV, gK, gV);     \
     break;
   if (g.d == 128) {
     switch (g.r / 8) { DWKV_COMPRESS_CASE(128, 1) DWKV_COMPRESS_CASE(128, 2) DWKV_COMPRESS_CASE(128, 3) DWKV_COMPRESS_CASE(128, 4)
