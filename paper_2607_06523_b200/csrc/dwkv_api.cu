@@ -188,27 +188,32 @@ int route_check(const dwkv_cache* c, int32_t seq, int32_t n, const uint8_t* tier
 void route_commit(dwkv_cache* c, int32_t seq, int32_t n, const uint8_t* tier, const uint8_t* flag, int* ridx_base,
                   std::vector<TokDst>* out, std::vector<int32_t>* new_pages) {
   SeqState& S = c->seqs[seq];
+  S.tier.reserve(S.tier.size() + n); S.flag.reserve(S.flag.size() + n); S.slot.reserve(S.slot.size() + n);
+  // per class: page index and position inside the page of the next slot, advanced without divisions in the token loop
+  int64_t pi[kMaxClasses], in_page[kMaxClasses];
+  for (int k = 0; k < c->n_classes; ++k) {
+    const int64_t tpp = c->cl[k].tokens_per_page;
+    pi[k] = S.count[k] / tpp; in_page[k] = S.count[k] % tpp;
+  }
   for (int i = 0; i < n; ++i) {
     const int k = 2 * tier[i] + flag[i];
     const int64_t sl = S.count[k]++;
-    const int64_t tpp = c->cl[k].tokens_per_page;
-    const int64_t pi = sl / tpp;
-    if (pi >= (int64_t)S.pages[k].size()) {
+    if (pi[k] >= (int64_t)S.pages[k].size()) {
       const int32_t pg = c->free_pages.back();
       c->free_pages.pop_back();
       S.pages[k].push_back(pg);
       new_pages->push_back(pg);
     }
-    const int64_t in_page = sl % tpp;
     TokDst td;
-    td.page_off = (int64_t)S.pages[k][pi] * (int64_t)c->page_bytes;
-    td.blk = (int32_t)(in_page / kBlockTok);
-    td.slot = (int32_t)(in_page % kBlockTok);
+    td.page_off = (int64_t)S.pages[k][pi[k]] * (int64_t)c->page_bytes;
+    td.blk = (int32_t)(in_page[k] / kBlockTok);
+    td.slot = (int32_t)(in_page[k] % kBlockTok);
     td.cls = k;
     td.ridx = flag[i] ? (*ridx_base)++ : -1;
     td.src = (int32_t)out->size();
     td.pad_ = 0;
     out->push_back(td);
+    if (++in_page[k] == c->cl[k].tokens_per_page) { in_page[k] = 0; pi[k]++; }
     S.tier.push_back(tier[i]);
     S.flag.push_back(flag[i]);
     S.slot.push_back((int32_t)sl);
@@ -381,14 +386,31 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
     route_commit(c, seq_ids[i], n_new[i], tier + off, flag + off, &ridx, &dst, &new_pages);
     off += n_new[i];
   }
-  // flagged tokens first: only their 16-token tiles run the reconstruction + int4 quantiser part of the kernel
+  // flagged tokens first, then by descending rank: only the flagged 16-token tiles run the reconstruction + int4 quantiser part
+  // of the kernel, and a tile multiplies only the rank chunks its tokens keep
   for (size_t i = 0; i < dst.size(); ++i) { dst[i].src = (int32_t)i; dst[i].pad_ = 0; }
-  std::stable_partition(dst.begin(), dst.end(), [](const TokDst& t) { return t.ridx >= 0; });
+  {   // counting sort by key = (flag, tier), descending, stable
+    size_t start[8] = {0}, cnt[8] = {0};
+    auto key = [](const TokDst& t) { return ((t.cls & 1) << 2) | (t.cls >> 1); };
+    for (const TokDst& t : dst) cnt[key(t)]++;
+    size_t acc = 0;
+    for (int k = 7; k >= 0; --k) { start[k] = acc; acc += cnt[k]; }
+    std::vector<TokDst> sorted(dst.size());
+    for (const TokDst& t : dst) sorted[start[key(t)]++] = t;
+    dst.swap(sorted);
+  }
+  CompressRuns runs = {};
+  for (size_t t0 = 0; t0 < dst.size(); t0 += 16) {            // the first token of a tile has its largest key
+    const int cost = compress_tile_cost(dst[t0].cls & 1, c->geom.tier_rank[dst[t0].cls >> 1] / 8);
+    if (runs.n == 0 || runs.cost[runs.n - 1] != cost) { runs.n++; runs.cost[runs.n - 1] = cost; runs.count[runs.n - 1] = 0; }
+    runs.count[runs.n - 1]++;
+    runs.per_lh += cost;
+  }
   int rc = zero_new_pages(c, new_pages, st);
   if (rc) return rc;
   rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
   if (rc) return rc;
-  c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, ridx, (const __nv_bfloat16*)k_new,
+  c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, runs, (const __nv_bfloat16*)k_new,
                                      (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, c->n_sms, st);
   CU_OK(cudaGetLastError());
   return DWKV_OK;

@@ -7,8 +7,9 @@
 //   c   = bf16(C), columns >= r_t of a token dropped (leading-r_t coefficients of its tier)
 //   rec = c . B                [16 x d]   exact bf16 products, fp32 accumulate     (only if a token of the tile is flagged)
 //   e   = x - g * rec  ->  int4 / group 16 / fp16 scale  (quantiser A14, fp32 IEEE, no reciprocal)
-// Persistent grid: the (layer-head, tile) items are cut into equal-cost contiguous ranges, one per CTA (a flagged tile counts
-// kCostFlag, an unflagged one kCostPlain); a CTA stages B' of its current (layer, head) in shared memory in the register
+// Persistent grid: the (layer-head, tile) items are cut into equal-cost contiguous ranges, one per CTA (the host sorts the call's tokens
+// flagged-first and by descending rank, so a tile's tokens share a rank; a tile costs compress_tile_cost(flagged, rank / 8) and
+// only the rank chunks its tokens keep are multiplied); a CTA stages B' of its current (layer, head) in shared memory in the register
 // order of the MMA B fragments (one 16-byte + one 8-byte ld.shared per MMA triple) and its 8 or 12 warps take tiles round-robin.
 // Every warp streams its token rows through a private shared-memory ring filled by cp.async 2-4 stages ahead (a stage = the 16
 // rows of one tile and one Z) and reads the A fragments back with ldmatrix. Results go straight
@@ -23,7 +24,6 @@ namespace dwkv {
 namespace {
 using namespace dwkv::dev;
 
-constexpr int kCostFlag = 4, kCostPlain = 1;   // relative cost of a tile with / without the reconstruction + quantiser part
 constexpr int kCompressMaxWarps = 16;
 
 __device__ __forceinline__ void mma16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
@@ -89,11 +89,17 @@ __device__ __forceinline__ RowDst row_dst(const uint8_t* arena, const uint32_t r
   return r;
 }
 
-// item position in cost space -> (layer-head, tile). Per layer-head: nf flagged tiles first (cost kCostFlag each), then plain ones.
-__device__ __forceinline__ void cost_to_item(long long pos, int per_lh, int nf, int nt_lh, int* lh, int* tile) {
-  *lh = (int)(pos / per_lh);
-  const int rem = (int)(pos - (long long)*lh * per_lh);
-  *tile = rem < nf * kCostFlag ? rem / kCostFlag : min(nt_lh, nf + (rem - nf * kCostFlag) / kCostPlain);
+// item position in cost space -> (layer-head, tile). Per layer-head the tiles come in runs of equal cost (CompressRuns).
+__device__ __forceinline__ void cost_to_item(long long pos, const CompressRuns& R, int* lh, int* tile) {
+  *lh = (int)(pos / R.per_lh);
+  int rem = (int)(pos - (long long)*lh * R.per_lh), t0 = 0;
+#pragma unroll 1
+  for (int i = 0; i < R.n; ++i) {
+    const int c = R.count[i] * R.cost[i];
+    if (rem < c) { *tile = t0 + rem / R.cost[i]; return; }
+    rem -= c; t0 += R.count[i];
+  }
+  *tile = t0;
 }
 
 // ---- per-warp shared-memory ring of token-row stages -------------------------------------------------------------------------
@@ -145,12 +151,16 @@ template <int D>
 __device__ __forceinline__ uint32_t stage_x(uint32_t stage, int row, int ch) { return lds32(stage + row * (2 * D + 16) + ch * 2); }
 
 // C = X . B'^T for one Z: 3 MMAs (lo, mid, hi term of B') per (k step, rank chunk); returns the rounded coefficients of rows g (ca) and g+8 (cb), columns 8nt + 2t, +1, zero beyond the rank
-template <int D, int NT>
-__device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int lane, uint32_t stage, const RowDst& ra, const RowDst& rb,
-                                        uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
-  float c[NT][4];
+template <int D, int NT, int NTM>      // NTM = rank chunks any token of the tile keeps: only those are multiplied
+__device__ __forceinline__ void project_n(const uint4* P4, const uint2* P2, int lane, uint32_t stage, const RowDst& ra, const RowDst& rb,
+                                          uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
+  // few chunks: one accumulator chain per term of B' (lo, mid, hi) so that the MMAs of a k step are independent
+  constexpr int NA = NTM <= 2 ? 3 : 1;
+  float c[NA][NTM][4];
 #pragma unroll
-  for (int nt = 0; nt < NT; ++nt) c[nt][0] = c[nt][1] = c[nt][2] = c[nt][3] = 0.f;
+  for (int a = 0; a < NA; ++a)
+#pragma unroll
+    for (int nt = 0; nt < NTM; ++nt) c[a][nt][0] = c[a][nt][1] = c[a][nt][2] = c[a][nt][3] = 0.f;
   // ldmatrix: lanes 8i .. 8i+7 address the rows of matrix i = (rows 0-7 | 8-15) x (channels +0 | +8) of the k step
   const uint32_t am = stage + ((lane & 7) + 8 * ((lane >> 3) & 1)) * (2 * D + 16) + 16 * (lane >> 4);
 #pragma unroll
@@ -158,19 +168,34 @@ __device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int la
     uint32_t a0, a1, a2, a3;
     ldmatrix_x4(am + 32 * kk, a0, a1, a2, a3);
 #pragma unroll
-    for (int nt = 0; nt < NT; ++nt) {
+    for (int nt = 0; nt < NTM; ++nt) {
       const uint4 hm = P4[(kk * NT + nt) * 32 + lane];
       const uint2 lo = P2[(kk * NT + nt) * 32 + lane];
-      mma16(c[nt], a0, a1, a2, a3, lo.x, lo.y);      // small terms first
-      mma16(c[nt], a0, a1, a2, a3, hm.z, hm.w);
-      mma16(c[nt], a0, a1, a2, a3, hm.x, hm.y);
+      mma16(c[0][nt], a0, a1, a2, a3, lo.x, lo.y);      // small terms first
+      mma16(c[NA == 3 ? 1 : 0][nt], a0, a1, a2, a3, hm.z, hm.w);
+      mma16(c[NA == 3 ? 2 : 0][nt], a0, a1, a2, a3, hm.x, hm.y);
     }
   }
 #pragma unroll
   for (int nt = 0; nt < NT; ++nt) {
-    ca[nt] = (8 * nt < ra.rk() && ra.valid()) ? pack_bf16x2(c[nt][0], c[nt][1]) : 0u;
-    cb[nt] = (8 * nt < rb.rk() && rb.valid()) ? pack_bf16x2(c[nt][2], c[nt][3]) : 0u;
+    ca[nt] = cb[nt] = 0u;
+    if (nt < NTM) {
+      float v[4];
+#pragma unroll
+      for (int x = 0; x < 4; ++x) v[x] = NA == 3 ? (c[0][nt][x] + c[1][nt][x]) + c[NA - 1][nt][x] : c[0][nt][x];
+      if (8 * nt < ra.rk() && ra.valid()) ca[nt] = pack_bf16x2(v[0], v[1]);
+      if (8 * nt < rb.rk() && rb.valid()) cb[nt] = pack_bf16x2(v[2], v[3]);
+    }
   }
+}
+
+template <int D, int NT>
+__device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int lane, uint32_t stage, const RowDst& ra, const RowDst& rb,
+                                        const int ntmax /* warp-uniform */, uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
+  if (ntmax <= 1) project_n<D, NT, 1>(P4, P2, lane, stage, ra, rb, ca, cb);
+  else if (NT >= 2 && ntmax == 2) project_n<D, NT, (NT >= 2 ? 2 : NT)>(P4, P2, lane, stage, ra, rb, ca, cb);
+  else if (NT >= 3 && ntmax == 3) project_n<D, NT, (NT >= 3 ? 3 : NT)>(P4, P2, lane, stage, ra, rb, ca, cb);
+  else project_n<D, NT, NT>(P4, P2, lane, stage, ra, rb, ca, cb);
 }
 
 template <int NT>
@@ -264,7 +289,7 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
 
 template <int D, int NT>      // NT = basis rank / 8
 __global__ void __launch_bounds__(kCompressMaxWarps * 32, 1)
-compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, const int n_tok, const int n_flag_tiles, const int n_stages,
+compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, const int n_tok, const CompressRuns runs, const int n_stages,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
                     const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
   constexpr int NKK = D / 16, r = 8 * NT, ldT = r + 8, NFRAG = NKK * NT * 32, STAGE = 16 * (2 * D + 16);
@@ -277,12 +302,11 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, gr = lane >> 2, t = lane & 3;
   const int NTHR = blockDim.x, W = NTHR >> 5;
   const uint32_t ring = (uint32_t)__cvta_generic_to_shared(BT + 2 * D * ldT) + (uint32_t)(warp * n_stages) * STAGE;   // this warp's stages
-  const int nt_lh = (n_tok + 15) >> 4, nf = n_flag_tiles;
-  const int per_lh = nf * kCostFlag + (nt_lh - nf) * kCostPlain;
-  const long long total = (long long)LH * per_lh;
+  const int nt_lh = (n_tok + 15) >> 4;
+  const long long total = (long long)LH * runs.per_lh;
   int lh0, t0, lh1, t1;
-  cost_to_item(total * blockIdx.x / gridDim.x, per_lh, nf, nt_lh, &lh0, &t0);
-  cost_to_item(total * (blockIdx.x + 1) / gridDim.x, per_lh, nf, nt_lh, &lh1, &t1);
+  cost_to_item(total * blockIdx.x / gridDim.x, runs, &lh0, &t0);
+  cost_to_item(total * (blockIdx.x + 1) / gridDim.x, runs, &lh1, &t1);
 #pragma unroll 1
   for (int lh = lh0; lh <= lh1 && lh < LH; ++lh) {
     const int tb = lh == lh0 ? t0 : 0, te = lh == lh1 ? t1 : nt_lh;
@@ -347,6 +371,7 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
       nb = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr + 8, n_tok, lh);
     }
     bool any_flag = false;
+    int ntmax = NT;
     int slot_c = 0;
 #pragma unroll 1
     for (int s = 0; s < nst; ++s) {
@@ -359,13 +384,14 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
       if (z == 0) {
         ra = na; rb = nb;
         any_flag = __any_sync(kFull, ra.flagged() || rb.flagged());
+        ntmax = __reduce_max_sync(kFull, max(ra.valid() ? ra.rk() : 0, rb.valid() ? rb.rk() : 0)) >> 3;
       } else if (s + 1 < nst) {
         const int tile = tb + warp + W * ((s + 1) >> 1);
         na = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr, n_tok, lh);
         nb = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr + 8, n_tok, lh);
       }
       uint32_t ca[NT], cb[NT];
-      project<D, NT>(P4 + z * NFRAG, P2 + z * NFRAG, lane, stage, ra, rb, ca, cb);
+      project<D, NT>(P4 + z * NFRAG, P2 + z * NFRAG, lane, stage, ra, rb, ntmax, ca, cb);
       store_coef<NT>(ra, ca, z, t);
       store_coef<NT>(rb, cb, z, t);
       if (any_flag)
@@ -378,7 +404,7 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
 
 }  // namespace
 
-int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, int n_flagged, const __nv_bfloat16* k_new,
+int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const CompressRuns& runs, const __nv_bfloat16* k_new,
                         const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK,
                         const __nv_bfloat16* gV, int n_sms, cudaStream_t s) {
   if (n <= 0) return 0;
@@ -393,12 +419,11 @@ int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* 
   const size_t smem = fixed + (size_t)warps * stages * stage;
   const long long tiles = (long long)g.L * g.H * ((n + 15) / 16);
   const int grid = (int)std::max<long long>(1, std::min<long long>((long long)n_sms, tiles));
-  const int nft = (n_flagged + 15) / 16;
   bool ok = true;
 #define DWKV_COMPRESS_CASE(DD, NN)                                                                                              \
   case NN:                                                                                                                      \
     cudaFuncSetAttribute(compress_mma_kernel<DD, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                  \
-    compress_mma_kernel<DD, NN><<<grid, warps * 32, smem, s>>>(arena, g, dst, n, nft, stages, k_new, v_new, BK, BV, gK, gV);     \
+    compress_mma_kernel<DD, NN><<<grid, warps * 32, smem, s>>>(arena, g, dst, n, runs, stages, k_new, v_new, BK, BV, gK, gV);     \
     break;
   if (g.d == 128) {
     switch (g.r / 8) { DWKV_COMPRESS_CASE(128, 1) DWKV_COMPRESS_CASE(128, 2) DWKV_COMPRESS_CASE(128, 3) DWKV_COMPRESS_CASE(128, 4)

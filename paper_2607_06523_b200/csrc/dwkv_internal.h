@@ -73,7 +73,16 @@ int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* d
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
                        const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,
                        const __half* scaleK, const __half* scaleV, cudaStream_t s);
-int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, int n_flagged /* sorted first in dst */,
+// append/compress work description: the tiles (16 tokens of the sorted table) of one (layer, head) as runs of equal cost
+struct CompressRuns {
+  int32_t n;            // runs used
+  int32_t per_lh;       // sum of count * cost
+  int32_t count[16];    // tiles in the run
+  int32_t cost[16];     // cost of one tile of the run (compress_tile_cost)
+};
+// relative cost of one tile: fixed part (row loads, stores), per kept rank chunk, reconstruction + quantiser if a token is flagged
+inline int compress_tile_cost(bool flagged, int rank_chunks) { return 4 + 2 * rank_chunks + (flagged ? 12 : 0); }
+int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const CompressRuns& runs /* dst is sorted to match */,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
                     const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK, const __nv_bfloat16* gV,
                     int n_sms, cudaStream_t s);
