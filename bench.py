@@ -114,6 +114,38 @@ def time_steps(fn, steps, warmup):
     return e0.elapsed_time(e1) / steps
 
 
+def prefill_compress(wl, harness, local, reps=3):
+    """Batched (prefill-sized) dwkv_append_compress: all tokens of one sequence of the workload's length (capped at 64K) in ONE
+    call on a cache of its own -- the TTFT side of the method (PAPER.md:74 'during prefill ... projects keys and values into
+    shared coefficient space, stores quantized residuals'). Returns ms per call (host routing + page zeroing + kernel, the
+    GPU idle at the start) and the dense bytes read."""
+    import dataclasses
+    n = min(max(wl.T), 65536)
+    wl1 = dataclasses.replace(wl, T=(n,), patterns=())
+    tier, flag = gen.make_routing(wl1, 0)
+    cache, (BK, BV, gK, gV) = harness.make_cache(wl1, arena_bytes=harness.arena_bytes_for(wl1, [(tier, flag)], 1), device=local)
+    dev = torch.device("cuda", local)
+    ks, vs = [], []
+    for t0 in range(0, n, 8192):              # generator intermediates are fp32: build the dense input chunk-wise
+        k, v = gen.make_dense_kv_chunk(wl1, 0, t0, min(8192, n - t0), BK, BV, gK, gV, device=dev)
+        ks.append(k.contiguous()); vs.append(v.contiguous())
+    k_new, v_new = torch.cat(ks), torch.cat(vs)
+    del ks, vs
+    ms = []
+    for _ in range(reps + 1):
+        cache.reset_seq(0)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); cache.append_compress([0], [n], k_new, v_new, tier, flag); e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    cache.destroy()
+    dense_bytes = 2 * k_new.numel() * 2
+    best = min(ms[1:])
+    return {"tokens": n, "ms_per_call": best, "dense_bytes_read": dense_bytes, "dense_GBps": dense_bytes / best / 1e6,
+            "tokens_per_s": n / best * 1e3, "note": "one dwkv_append_compress call, timed from an idle GPU: host routing + page zeroing + kernel"}
+
+
 def oracle_sample(wl, consts, tier, flag, kept, q_host, layers, budget_s=25.0):
     """Time the CPU oracle as it stands on (layer, kv head) slices of sequence 0; returns (token-layers/s, sample text,
     threads, worst rel-L2 vs `gpu_out` if given)."""
@@ -223,7 +255,8 @@ def main():
     for kv in args.opt:
         k, v = kv.split("=")
         cache.set_option(k, int(v))
-    sample_layers = [0]
+    # layers of sequence 0 the CPU oracle is timed on (and the GPU output is compared with): ~1.5 s of host time per layer at T = 64K
+    sample_layers = sorted(set(int(x) for x in np.linspace(0, wl.L - 1, min(wl.L, 8 if max(wl.T) <= 65536 else 4))))
     keep = [(l, h) for l in sample_layers for h in range(wl.H_kv)] if (rank == 0 and not args.no_extra) else []
     kept0 = None
     t_fill = time.perf_counter()
@@ -360,6 +393,10 @@ def main():
             extra["per_layer_graph_vs_all_layers_rel_l2"] = float((got - out).norm() / out.norm())
         except Exception as ex:  # pragma: no cover
             extra["per_layer_graph_error"] = repr(ex)[:200]
+        try:
+            extra["prefill_compress"] = prefill_compress(wl, harness, local)
+        except Exception as ex:
+            extra["prefill_compress"] = {"error": repr(ex)[:200]}
         # CPU oracle on the host cores: bounded sample, and parity of the sampled slices at full size
         tier, flag = routings[0]
         o_gpu = out.clone()

@@ -30,6 +30,7 @@ __global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Co
   const int ws = SPLIT ? warp : 0;                  // this warp's offset in the split
   // programmatic dependent launch: this grid may start while the decode kernel drains; wait for its completion and flush
   cudaGridDependencySynchronize();
+  cudaTriggerProgrammaticLaunchCompletion();        // the next decode kernel of the stream may become resident; it waits for this grid's end
   const int b = seg / p.LH, lh = seg - b * p.LH;
   const int layer = p.layer0 + lh / p.H, h = lh % p.H;
   const int G = p.G, r = p.r, PR = 2 + p.r + D;

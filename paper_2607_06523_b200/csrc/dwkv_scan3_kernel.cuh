@@ -230,6 +230,9 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncwarp();
+  // programmatic dependent launch: the grid may be resident (barriers initialised) while the previous kernel of the stream
+  // -- the combine of the previous layer in per-layer decoding -- still runs; nothing it wrote (q, partials, cache) is read before
+  cudaGridDependencySynchronize();
   const int gw = warp * gridDim.x + blockIdx.x;      // consecutive slices of the linear order go to different SMs
 
   if (gw >= p.n_slices) return;
@@ -362,7 +365,17 @@ void launch_instance(const Scan3Params& p, int n_sms, cudaStream_t s) {
     cudaFuncSetAttribute(scan3_kernel<NKB, D, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     attr_set = true;
   }
-  scan3_kernel<NKB, D, PAIR><<<n_sms, kWarps * 32, smem, s>>>(p);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(n_sms);
+  cfg.blockDim = dim3(kWarps * 32);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, scan3_kernel<NKB, D, PAIR>, p);
 }
 
 template <int D, bool PAIR>
