@@ -146,7 +146,8 @@ int64_t dwkv_seq_len(const dwkv_cache* c, int32_t seq_id);
 int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved_bytes, uint64_t* dense_equiv_bytes);
 
 /* Tuning knobs for experiments (bench / tests); see DESIGN.md section 6. Keys:
- *   "time_scan"       1 = bracket the fused decode kernel with CUDA events (dwkv_get_stat "scan_ms")
+ *   "time_scan"       1 = bracket the fused decode kernel and the append/compress kernel with CUDA events
+ *                     (dwkv_get_stat "scan_ms" / "compress_ms")
  *   "max_unit_blocks" planner: blocks (of 32 token slots) per work unit, 0 = by "unit_kb"
  *   "unit_kb"         planner: target size of a work unit per (layer, head), KB (default 64 = one page stripe)
  *   "n_slices"        planner: number of warp slices the step is cut into, 0 = one per warp of the persistent grid
@@ -158,7 +159,8 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);
 
 /* Measurement aid: with option "time_scan" = 1 every dwkv_decode_attention brackets its fused decode kernel (steps a1 + a2)
  * with CUDA events on `stream`; dwkv_get_stat(c, "scan_ms") waits for the last bracket and returns its duration in
- * milliseconds (negative = none recorded / error). */
+ * milliseconds (negative = none recorded / error); "compress_ms" is the same for the append/compress kernel (step a4) of the
+ * last dwkv_append_compress. */
 double dwkv_get_stat(dwkv_cache* c, const char* key);
 
 /* Kernels launched by this handle since creation (bench's gpu_launches claim). */

@@ -151,8 +151,8 @@ struct dwkv_cache {
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
-  cudaEvent_t ev_scan0 = nullptr, ev_scan1 = nullptr;
-  bool scan_timed = false;
+  cudaEvent_t ev_scan0 = nullptr, ev_scan1 = nullptr, ev_app0 = nullptr, ev_app1 = nullptr;
+  bool scan_timed = false, app_timed = false;
   int64_t launches = 0;
 };
 
@@ -325,6 +325,8 @@ void dwkv_destroy(dwkv_cache* c) {
   c->ring.release();
   if (c->ev_scan0) cudaEventDestroy(c->ev_scan0);
   if (c->ev_scan1) cudaEventDestroy(c->ev_scan1);
+  if (c->ev_app0) cudaEventDestroy(c->ev_app0);
+  if (c->ev_app1) cudaEventDestroy(c->ev_app1);
   delete c;
 }
 
@@ -410,8 +412,13 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
   if (rc) return rc;
   rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
   if (rc) return rc;
+  if (c->opt_time_scan) {
+    if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
+    CU_OK(cudaEventRecord(c->ev_app0, st));
+  }
   c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, runs, (const __nv_bfloat16*)k_new,
                                      (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, c->n_sms, st);
+  if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_app1, st)); c->app_timed = true; }
   CU_OK(cudaGetLastError());
   return DWKV_OK;
 }
@@ -553,6 +560,13 @@ double dwkv_get_stat(dwkv_cache* c, const char* key) {
     if (cudaEventSynchronize(c->ev_scan1) != cudaSuccess) return -1.0;
     float ms = -1.f;
     if (cudaEventElapsedTime(&ms, c->ev_scan0, c->ev_scan1) != cudaSuccess) return -1.0;
+    return (double)ms;
+  }
+  if (!strcmp(key, "compress_ms")) {
+    if (!c->app_timed) return -1.0;
+    if (cudaEventSynchronize(c->ev_app1) != cudaSuccess) return -1.0;
+    float ms = -1.f;
+    if (cudaEventElapsedTime(&ms, c->ev_app0, c->ev_app1) != cudaSuccess) return -1.0;
     return (double)ms;
   }
   return -1.0;
