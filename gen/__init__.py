@@ -16,6 +16,7 @@ from .workloads import (  # noqa: F401
     make_coef_chunk,
     make_resid_chunk,
     make_dense_kv_chunk,
+    make_omega,
     class_of,
     expected_bytes_per_lht,
 )

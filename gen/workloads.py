@@ -22,7 +22,7 @@ import torch
 BASE_SEED = 260706523
 
 # tensor ids for seed sub-streams
-_TID_BASIS, _TID_GATES, _TID_Q, _TID_COEF, _TID_RESID, _TID_ROUTE, _TID_DENSE, _TID_LEN = range(8)
+_TID_BASIS, _TID_GATES, _TID_Q, _TID_COEF, _TID_RESID, _TID_ROUTE, _TID_DENSE, _TID_LEN, _TID_OMEGA = range(9)
 
 
 @dataclass(frozen=True)
@@ -274,3 +274,9 @@ def make_dense_kv_chunk(wl: Workload, seq: int, t0: int, n: int, BK, BV, gK, gV,
         x = torch.einsum("nlhr,lhrd->nlhd", c, Bl) * gt.to(device=device, dtype=torch.float32)[None] + e
         out.append(x.to(torch.bfloat16))
     return out[0], out[1]
+
+
+def make_omega(wl: Workload, n: int, n_sketch: int, device="cpu") -> torch.Tensor:
+    """Random test matrix of the basis sketch (an INPUT of dwkv_build_basis): bf16 [w, n_sketch, n] ~ N(0, 1)."""
+    g = _gen(device, wl.index, _TID_OMEGA, n_sketch)
+    return torch.randn(wl.w, n_sketch, n, generator=g, device=device, dtype=torch.float32).to(torch.bfloat16)

@@ -72,6 +72,23 @@ void dwkv_destroy(dwkv_cache* c);
  * orthonormal, used as stored. Copied. Errors: STATE if any sequence already holds tokens (reading A19). */
 int dwkv_set_basis(dwkv_cache* c, const void* Bk, const void* Bv, void* stream);
 
+/* Build the bases from the dense K/V of a prefill instead of setting them ("we compute a small randomized low-rank
+ * sketch of the cached keys and values after prefill"; reading A24): for every (depth window m, kv head h, Z)
+ *     S = sum_{l in window m} Omega_j^T (X_l / gate_l)      (n_sketch x d;  X_l = the n rows k_dense[:, l, h, :], j = l - m*w)
+ *     B[m,h] = the r right singular vectors of S with the largest singular values, in descending order, each signed so that its
+ *              largest-magnitude entry is positive, rounded to bf16
+ * and installs them as dwkv_set_basis would. The gates must be set first (gate-normalised space, reading A13).
+ *   k_dense, v_dense  dev bf16 [n, L, H_kv, d]     the prefill vectors (the same layout dwkv_append_compress takes)
+ *   omega             dev bf16 [w, n_sketch, n]    the random test matrix the method draws (an INPUT: e.g. N(0,1) values), shared by
+ *                                                  all windows, heads and Z; omega[j] multiplies layer j of each window
+ *   n                 positive multiple of 8;  n_sketch  multiple of 16, r <= n_sketch <= min(80, d)
+ * Enqueues on `stream`, no host sync. Errors: STATE (gates not set, or tokens exist), INVALID (sizes), CUDA. */
+int dwkv_build_basis(dwkv_cache* c, int32_t n, const void* k_dense, const void* v_dense, const void* omega, int32_t n_sketch,
+                     void* stream);
+
+/* Copy the current bases out: dev bf16 [L/w, H_kv, r, d] each. Errors: STATE (no basis yet). */
+int dwkv_export_basis(dwkv_cache* c, void* Bk_out, void* Bv_out, void* stream);
+
 /* Per-layer per-channel gates (reading A8): dev bf16 [L, H_kv, d]. Copied. Synchronises `stream` to validate that
  * every entry is finite and non-zero (STATE otherwise). STATE if any sequence already holds tokens. */
 int dwkv_set_gates(dwkv_cache* c, const void* gK, const void* gV, void* stream);

@@ -22,6 +22,7 @@ EXPORTED = [
     "dwkv_create", "dwkv_destroy", "dwkv_set_basis", "dwkv_set_gates", "dwkv_append_compress", "dwkv_decode_attention",
     "dwkv_append_raw", "dwkv_export_tokens", "dwkv_reset_seq", "dwkv_seq_len", "dwkv_footprint", "dwkv_set_option",
     "dwkv_launch_count", "dwkv_get_stat", "dwkv_last_error", "dwkv_dense_workspace_bytes", "dwkv_dense_decode_attention",
+    "dwkv_build_basis", "dwkv_export_basis",
 ]
 
 
@@ -58,6 +59,8 @@ def _load() -> C.CDLL:
     lib.dwkv_destroy.restype = None
     lib.dwkv_set_basis.argtypes = [vp, vp, vp, vp]
     lib.dwkv_set_gates.argtypes = [vp, vp, vp, vp]
+    lib.dwkv_build_basis.argtypes = [vp, i32, vp, vp, vp, i32, vp]
+    lib.dwkv_export_basis.argtypes = [vp, vp, vp, vp]
     lib.dwkv_append_compress.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.dwkv_decode_attention.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.dwkv_append_raw.argtypes = [vp, i32, i32, vp, vp, C.POINTER(dwkv_raw_tokens), vp]
@@ -143,6 +146,19 @@ class DwkvCache:
 
     def set_basis(self, BK: torch.Tensor, BV: torch.Tensor):
         _check(lib.dwkv_set_basis(self._h, _ptr(BK, torch.bfloat16), _ptr(BV, torch.bfloat16), _stream()))
+
+    def build_basis(self, k_dense: torch.Tensor, v_dense: torch.Tensor, omega: torch.Tensor):
+        """k_dense, v_dense: bf16 [n, L, H_kv, d]; omega: bf16 [w, n_sketch, n] (the random test matrix, an input)."""
+        n, n_sketch = int(k_dense.shape[0]), int(omega.shape[1])
+        assert k_dense.shape == v_dense.shape and omega.shape[2] == n
+        _check(lib.dwkv_build_basis(self._h, n, _ptr(k_dense, torch.bfloat16), _ptr(v_dense, torch.bfloat16),
+                                    _ptr(omega, torch.bfloat16), n_sketch, _stream()))
+
+    def export_basis(self, M: int, H: int, r: int, d: int):
+        BK = torch.empty(M, H, r, d, dtype=torch.bfloat16, device=torch.device("cuda", torch.cuda.current_device()))
+        BV = torch.empty_like(BK)
+        _check(lib.dwkv_export_basis(self._h, _ptr(BK, torch.bfloat16), _ptr(BV, torch.bfloat16), _stream()))
+        return BK, BV
 
     def set_gates(self, gK: torch.Tensor, gV: torch.Tensor):
         _check(lib.dwkv_set_gates(self._h, _ptr(gK, torch.bfloat16), _ptr(gV, torch.bfloat16), _stream()))

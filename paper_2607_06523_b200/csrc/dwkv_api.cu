@@ -138,7 +138,7 @@ struct dwkv_cache {
   int64_t total_tokens = 0;
   uint64_t version = 0;
   // scratch
-  DevBuf part, plan3_dev, tokdst_dev;
+  DevBuf part, plan3_dev, tokdst_dev, basis_scratch;
   int n_sms = 148;
   StagingRing ring;
   Plan3 plan3;
@@ -321,7 +321,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gK) cudaFree(c->gK);
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
-  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release();
+  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release();
   c->ring.release();
   if (c->ev_scan0) cudaEventDestroy(c->ev_scan0);
   if (c->ev_scan1) cudaEventDestroy(c->ev_scan1);
@@ -338,6 +338,37 @@ int dwkv_set_basis(dwkv_cache* c, const void* Bk, const void* Bv, void* stream) 
   CU_OK(cudaMemcpyAsync(c->BK, Bk, nb, cudaMemcpyDeviceToDevice, st));
   CU_OK(cudaMemcpyAsync(c->BV, Bv, nb, cudaMemcpyDeviceToDevice, st));
   c->basis_set = true;
+  return DWKV_OK;
+}
+
+int dwkv_build_basis(dwkv_cache* c, int32_t n, const void* k_dense, const void* v_dense, const void* omega, int32_t n_sketch,
+                     void* stream) {
+  if (!c || !k_dense || !v_dense || !omega) return fail(DWKV_E_INVALID, "NULL argument");
+  if (!c->gates_set) return fail(DWKV_E_STATE, "gates must be set before the basis is built (the sketch is taken in gate-normalised space)");
+  if (c->total_tokens > 0) return fail(DWKV_E_STATE, "basis is frozen once tokens exist (reading A19)");
+  if (n <= 0 || n % 8) return fail(DWKV_E_INVALID, "n must be a positive multiple of 8");
+  if (n_sketch % 16 || n_sketch < c->geom.r || n_sketch > 80 || n_sketch > c->geom.d)
+    return fail(DWKV_E_INVALID, "n_sketch must be a multiple of 16 with r <= n_sketch <= min(80, d_head)");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int ns = basis_num_splits(c->geom, n, c->n_sms);
+  CU_OK(c->basis_scratch.reserve(basis_scratch_bytes(c->geom, n_sketch, ns)));
+  const int launched = launch_build_basis(c->geom, n, (const __nv_bfloat16*)k_dense, (const __nv_bfloat16*)v_dense,
+                                          (const __nv_bfloat16*)omega, n_sketch, ns, (float*)c->basis_scratch.p, c->gK, c->gV, c->BK,
+                                          c->BV, st);
+  if (!launched) return fail(DWKV_E_INVALID, "no sketch kernel instance for this shape");
+  c->launches += launched;
+  CU_OK(cudaGetLastError());
+  c->basis_set = true;
+  return DWKV_OK;
+}
+
+int dwkv_export_basis(dwkv_cache* c, void* Bk_out, void* Bv_out, void* stream) {
+  if (!c || !Bk_out || !Bv_out) return fail(DWKV_E_INVALID, "NULL argument");
+  if (!c->basis_set) return fail(DWKV_E_STATE, "no basis set");
+  const size_t nb = (size_t)(c->geom.L / c->geom.w) * c->geom.H * c->geom.r * c->geom.d * sizeof(__nv_bfloat16);
+  cudaStream_t st = (cudaStream_t)stream;
+  CU_OK(cudaMemcpyAsync(Bk_out, c->BK, nb, cudaMemcpyDeviceToDevice, st));
+  CU_OK(cudaMemcpyAsync(Bv_out, c->BV, nb, cudaMemcpyDeviceToDevice, st));
   return DWKV_OK;
 }
 

@@ -1,0 +1,255 @@
+// dwkv_basis.cu -- basis construction from the prefill K/V ("a small randomized
+// low-rank sketch of the cached keys and values after prefill"; reading A24).
+//
+//   sketch_kernel<D, MT>   P[split][(l,h,Z)] = Omega_j^T X_l over a token range: bf16 x bf16 on mma.sync, fp32 accumulate.
+//                          A = Omega tile (sketch rows x tokens), B = the token rows (tokens x channels); both tiles are
+//                          staged by cp.async (double buffer) and read with ldmatrix / ldmatrix.trans. HBM-bound: the dense
+//                          K/V of the prefill is read exactly once.
+//   basis_svd_kernel<D>    per (window, head, Z): S = sum over the window's layers and the splits of P / gate, one-sided Jacobi
+//                          (Hestenes) on the rows of S until they are mutually orthogonal -- they are then sigma_i * w_i^T --,
+//                          the r rows of largest norm, normalised, signed (largest-magnitude entry positive), rounded to bf16.
+#include "dwkv_internal.h"
+#include "dwkv_mma.cuh"
+
+namespace dwkv {
+namespace {
+using namespace dwkv::dev;
+
+constexpr int kSketchTok = 64;       // tokens per staged tile
+constexpr int kSketchWarps = 8;
+
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void mma16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+
+// grid (L*H*2, n_split); 8 warps, warp w owns channels [w*D/8, (w+1)*D/8) of the k x D sketch block
+template <int D, int MT>      // MT = sketch rows / 16
+__global__ void __launch_bounds__(kSketchWarps * 32) sketch_kernel(const __nv_bfloat16* k_dense, const __nv_bfloat16* v_dense,
+                                                                  const __nv_bfloat16* omega, float* part, const int n, const int LH,
+                                                                  const int H, const int w) {
+  constexpr int K = 16 * MT, XP = 2 * D + 16, OP = 2 * kSketchTok + 16;      // row pitches (bytes) of the X and Omega tiles
+  constexpr int XT = kSketchTok * XP, OT = K * OP, NT = D / 64;                // NT = 8-channel n-tiles per warp
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  const uint32_t sm = (uint32_t)__cvta_generic_to_shared(smem_raw);           // [2][X tile | Omega tile]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int item = blockIdx.x, lh = item >> 1, z = item & 1, l = lh / H;
+  const __nv_bfloat16* X = z ? v_dense : k_dense;
+  const __nv_bfloat16* Om = omega + (size_t)(l % w) * K * n;                  // omega[j][i][t], j = layer inside its window
+  const int per = ((n + gridDim.y - 1) / gridDim.y + kSketchTok - 1) / kSketchTok * kSketchTok;
+  const int t_beg = blockIdx.y * per, t_end = min(n, t_beg + per);
+  float c[MT][NT][4];
+#pragma unroll
+  for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < NT; ++ni) c[mi][ni][0] = c[mi][ni][1] = c[mi][ni][2] = c[mi][ni][3] = 0.f;
+  auto stage = [&](int buf, int t0) {
+    const uint32_t xs = sm + buf * (XT + OT), os = xs + XT;
+    for (int i = tid; i < kSketchTok * (D / 8); i += kSketchWarps * 32) {      // 16-byte pieces of the token rows
+      const int r = i / (D / 8), p = i - r * (D / 8), t = t0 + r;
+      cp_async16(xs + r * XP + 16 * p, X + ((size_t)min(t, n - 1) * LH + lh) * D + 8 * p, t < t_end ? 16 : 0);
+    }
+    for (int i = tid; i < K * (kSketchTok / 8); i += kSketchWarps * 32) {       // 16-byte pieces of the Omega rows (8 tokens)
+      const int r = i / (kSketchTok / 8), p = i - r * (kSketchTok / 8), t = t0 + 8 * p;
+      cp_async16(os + r * OP + 16 * p, Om + (size_t)r * n + min(t, n - 8), t < t_end ? 16 : 0);   // n % 8 == 0, t_end % 8 == 0
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  if (t_beg < t_end) stage(0, t_beg);
+  int buf = 0;
+  for (int t0 = t_beg; t0 < t_end; t0 += kSketchTok) {
+    if (t0 + kSketchTok < t_end) {
+      stage(buf ^ 1, t0 + kSketchTok);
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
+    } else {
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    const uint32_t xs = sm + buf * (XT + OT), os = xs + XT;
+#pragma unroll
+    for (int ks = 0; ks < kSketchTok / 16; ++ks) {
+      // B fragments: matrices (tokens +0..7 | +8..15) x (channels c0 .. +7 | c0+8 .. +15), transposed on load
+      uint32_t b[NT][2];
+      {
+        const int mat = lane >> 3, tok = 16 * ks + (lane & 7) + 8 * (mat & 1);
+        const uint32_t a = xs + tok * XP + 2 * (warp * (D / 8) + 8 * (mat >> 1));
+        if constexpr (NT == 2) {
+          asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                       : "=r"(b[0][0]), "=r"(b[0][1]), "=r"(b[1][0]), "=r"(b[1][1]) : "r"(a));
+        } else {
+          asm volatile("ldmatrix.sync.aligned.m8n8.x2.trans.shared.b16 {%0,%1}, [%2];" : "=r"(b[0][0]), "=r"(b[0][1]) : "r"(a));
+        }
+      }
+#pragma unroll
+      for (int mi = 0; mi < MT; ++mi) {
+        uint32_t a0, a1, a2, a3;   // (sketch rows 16mi + 0..7 | +8..15) x (tokens 16ks + 0..7 | +8..15)
+        const uint32_t a = os + (16 * mi + (lane & 7) + 8 * ((lane >> 3) & 1)) * OP + 2 * (16 * ks + 8 * (lane >> 4));
+        asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];" : "=r"(a0), "=r"(a1), "=r"(a2), "=r"(a3) : "r"(a));
+#pragma unroll
+        for (int ni = 0; ni < NT; ++ni) mma16(c[mi][ni], a0, a1, a2, a3, b[ni][0], b[ni][1]);
+      }
+    }
+    __syncthreads();
+    buf ^= 1;
+  }
+  float* out = part + ((size_t)blockIdx.y * (2 * LH) + item) * (size_t)(K * D);
+  const int g = lane >> 2, t = lane & 3;
+#pragma unroll
+  for (int mi = 0; mi < MT; ++mi)
+#pragma unroll
+    for (int ni = 0; ni < NT; ++ni) {
+      const int col = warp * (D / 8) + 8 * ni + 2 * t;
+      *reinterpret_cast<float2*>(out + (size_t)(16 * mi + g) * D + col) = make_float2(c[mi][ni][0], c[mi][ni][1]);
+      *reinterpret_cast<float2*>(out + (size_t)(16 * mi + g + 8) * D + col) = make_float2(c[mi][ni][2], c[mi][ni][3]);
+    }
+}
+
+// grid (M*H*2); 256 threads. Dynamic shared memory: S[k][D + 1] fp32, norms[k], order[k].
+template <int D>
+__global__ void __launch_bounds__(256) basis_svd_kernel(const float* part, const int n_split, const __nv_bfloat16* gK,
+                                                        const __nv_bfloat16* gV, __nv_bfloat16* BK, __nv_bfloat16* BV, const int K,
+                                                        const int r, const int L, const int H, const int w) {
+  constexpr int LD = D + 1;
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  float* S = reinterpret_cast<float*>(smem_raw);
+  float* nrm = S + K * LD;
+  __shared__ int rotated;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int item = blockIdx.x, mh = item >> 1, z = item & 1, m = mh / H, h = mh - m * H, LH = L * H;
+  const __nv_bfloat16* gate = z ? gV : gK;
+  // ---- S = sum over the window's layers and the splits of P / gate (column scaling commutes with the sum over tokens) --------
+  for (int i = tid; i < K * D; i += 256) {
+    const int row = i / D, col = i - row * D;
+    float acc = 0.f;
+    for (int j = 0; j < w; ++j) {
+      const int lh = (m * w + j) * H + h;
+      float p = 0.f;
+      for (int s = 0; s < n_split; ++s) p += part[((size_t)s * (2 * LH) + 2 * lh + z) * (size_t)(K * D) + i];
+      acc += __fdiv_rn(p, __bfloat162float(gate[(size_t)lh * D + col]));
+    }
+    S[row * LD + col] = acc;
+  }
+  __syncthreads();
+  // ---- one-sided Jacobi: rotate row pairs until all rows are mutually orthogonal (round-robin pairing, disjoint pairs per step)
+  const float tol = 1e-6f;
+  for (int sweep = 0; sweep < 30; ++sweep) {
+    if (tid == 0) rotated = 0;
+    __syncthreads();
+    for (int step = 0; step < K - 1; ++step) {
+      for (int pi = warp; pi < K / 2; pi += 8) {
+        int p, q;
+        if (pi == 0) { p = K - 1; q = step; }
+        else { p = (step + pi) % (K - 1); q = (step - pi + (K - 1)) % (K - 1); }
+        float* sp = S + p * LD; float* sq = S + q * LD;
+        float a = 0.f, b = 0.f, gmm = 0.f;
+#pragma unroll
+        for (int x = 0; x < D / 32; ++x) {
+          const float u = sp[lane + 32 * x], v = sq[lane + 32 * x];
+          a = fmaf(u, u, a); b = fmaf(v, v, b); gmm = fmaf(u, v, gmm);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          a += __shfl_xor_sync(kFull, a, o); b += __shfl_xor_sync(kFull, b, o); gmm += __shfl_xor_sync(kFull, gmm, o);
+        }
+        if (fabsf(gmm) > tol * sqrtf(a * b) && gmm != 0.f) {
+          const float zeta = (b - a) / (2.f * gmm);
+          const float tt = copysignf(1.f, zeta) / (fabsf(zeta) + sqrtf(1.f + zeta * zeta));
+          const float cs = rsqrtf(1.f + tt * tt), sn = cs * tt;
+#pragma unroll
+          for (int x = 0; x < D / 32; ++x) {
+            const float u = sp[lane + 32 * x], v = sq[lane + 32 * x];
+            sp[lane + 32 * x] = cs * u - sn * v;
+            sq[lane + 32 * x] = sn * u + cs * v;
+          }
+          if (lane == 0) rotated = 1;
+        }
+      }
+      __syncthreads();
+    }
+    if (!rotated) break;
+    __syncthreads();
+  }
+  // ---- the r rows of largest norm, in descending order ---------------------------------------------------------------------
+  for (int row = warp; row < K; row += 8) {
+    float a = 0.f;
+#pragma unroll
+    for (int x = 0; x < D / 32; ++x) { const float u = S[row * LD + lane + 32 * x]; a = fmaf(u, u, a); }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(kFull, a, o);
+    if (lane == 0) nrm[row] = a;
+  }
+  __syncthreads();
+  __nv_bfloat16* B = (z ? BV : BK) + (size_t)mh * r * D;
+  for (int row = warp; row < K; row += 8) {
+    const float a = nrm[row];
+    int rank = 0;
+    for (int o = 0; o < K; ++o) rank += (nrm[o] > a) || (nrm[o] == a && o < row);
+    if (rank >= r) continue;
+    // sign: the entry of largest magnitude is positive (first one on ties)
+    float best = -1.f; int bi = 0;
+#pragma unroll
+    for (int x = 0; x < D / 32; ++x) {
+      const float u = fabsf(S[row * LD + lane + 32 * x]);
+      if (u > best) { best = u; bi = lane + 32 * x; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const float ob = __shfl_xor_sync(kFull, best, o); const int oi = __shfl_xor_sync(kFull, bi, o);
+      if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+    }
+    const float inv = a > 0.f ? (S[row * LD + bi] < 0.f ? -1.f : 1.f) / sqrtf(a) : 0.f;
+#pragma unroll
+    for (int x = 0; x < D / 32; ++x) B[(size_t)rank * D + lane + 32 * x] = __float2bfloat16_rn(S[row * LD + lane + 32 * x] * inv);
+  }
+}
+
+}  // namespace
+
+size_t basis_scratch_bytes(const CacheGeom& g, int n_sketch, int n_split) {
+  return (size_t)n_split * 2 * g.L * g.H * (size_t)n_sketch * g.d * sizeof(float);
+}
+
+int basis_num_splits(const CacheGeom& g, int n, int n_sms) {
+  const int items = 2 * g.L * g.H;
+  int s = (2 * n_sms + items - 1) / items;                       // about two CTAs per SM
+  s = std::min(s, (n + kSketchTok - 1) / kSketchTok);
+  return std::max(1, std::min(s, 16));
+}
+
+int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, const __nv_bfloat16* v_dense, const __nv_bfloat16* omega,
+                       int n_sketch, int n_split, float* part, const __nv_bfloat16* gK, const __nv_bfloat16* gV, __nv_bfloat16* BK,
+                       __nv_bfloat16* BV, cudaStream_t s) {
+  const int LH = g.L * g.H, MT = n_sketch / 16;
+  const size_t smem1 = 2 * ((size_t)kSketchTok * (2 * g.d + 16) + (size_t)n_sketch * (2 * kSketchTok + 16));
+  dim3 grid1(2 * LH, n_split);
+  bool ok = true;
+#define DWKV_SKETCH_CASE(DD, MM)                                                                                            \
+  case MM:                                                                                                                  \
+    cudaFuncSetAttribute(sketch_kernel<DD, MM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1);                   \
+    sketch_kernel<DD, MM><<<grid1, kSketchWarps * 32, smem1, s>>>(k_dense, v_dense, omega, part, n, LH, g.H, g.w);            \
+    break;
+  if (g.d == 128) {
+    switch (MT) { DWKV_SKETCH_CASE(128, 1) DWKV_SKETCH_CASE(128, 2) DWKV_SKETCH_CASE(128, 3) DWKV_SKETCH_CASE(128, 4) DWKV_SKETCH_CASE(128, 5)
+                  default: ok = false; }
+  } else {
+    switch (MT) { DWKV_SKETCH_CASE(64, 1) DWKV_SKETCH_CASE(64, 2) DWKV_SKETCH_CASE(64, 3) DWKV_SKETCH_CASE(64, 4) default: ok = false; }
+  }
+#undef DWKV_SKETCH_CASE
+  if (!ok) return 0;
+  const size_t smem2 = ((size_t)n_sketch * (g.d + 1) + n_sketch) * sizeof(float);
+  const int items2 = 2 * (g.L / g.w) * g.H;
+  if (g.d == 128) {
+    cudaFuncSetAttribute(basis_svd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+    basis_svd_kernel<128><<<items2, 256, smem2, s>>>(part, n_split, gK, gV, BK, BV, n_sketch, g.r, g.L, g.H, g.w);
+  } else {
+    cudaFuncSetAttribute(basis_svd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
+    basis_svd_kernel<64><<<items2, 256, smem2, s>>>(part, n_split, gK, gV, BK, BV, n_sketch, g.r, g.L, g.H, g.w);
+  }
+  return 2;
+}
+
+}  // namespace dwkv

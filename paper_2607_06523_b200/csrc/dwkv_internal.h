@@ -86,6 +86,12 @@ int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* 
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
                     const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK, const __nv_bfloat16* gV,
                     int n_sms, cudaStream_t s);
+// basis construction (dwkv_basis.cu): sketch GEMM + one-sided Jacobi; returns the number of kernels launched (0 = no instance)
+size_t basis_scratch_bytes(const CacheGeom& g, int n_sketch, int n_split);
+int basis_num_splits(const CacheGeom& g, int n, int n_sms);
+int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, const __nv_bfloat16* v_dense, const __nv_bfloat16* omega,
+                       int n_sketch, int n_split, float* part, const __nv_bfloat16* gK, const __nv_bfloat16* gV, __nv_bfloat16* BK,
+                       __nv_bfloat16* BV, cudaStream_t s);
 struct DumpPtrs {
   __nv_bfloat16 *coefK, *coefV;
   uint8_t *codeK, *codeV;
