@@ -281,3 +281,25 @@ def attention_slice(coefK, coefV, ranks, flag, codeK, scaleK, codeV, scaleV, BK,
     K = reconstruct(coefK, ranks, flag, dK, BK, gK)
     V = reconstruct(coefV, ranks, flag, dV, BV, gV)
     return softmax_attention(q, K, V, scale), K, V
+
+
+def probe_error(attn_ref, attn_cmp, G: int, eps: float) -> np.ndarray:
+    """Attention-output probe, Eq. (3):  e[h] = || Attn(Q,K,V) - Attn(Q,K^,V^) ||_2 / ( || Attn(Q,K,V) ||_2 + eps ).
+
+    attn_ref, attn_cmp: [n_q, H_q, d] attention outputs of the n_q probed query positions over the higher-fidelity cache and
+    over the compressed reconstruction; the norm of kv head h runs over its G query heads, all positions and all channels
+    (reading A25: "a small subset of heads and recent query positions", one number per (layer, kv head))."""
+    a = np.asarray(attn_ref, np.float64); b = np.asarray(attn_cmp, np.float64)
+    n_q, Hq, d = a.shape
+    H = Hq // G
+    e = np.zeros(H)
+    for h in range(H):
+        num = 0.0; den = 0.0
+        for i in range(n_q):
+            for g in range(G):
+                for ch in range(d):
+                    x = a[i, h * G + g, ch]; y = b[i, h * G + g, ch]
+                    num += (x - y) * (x - y)
+                    den += x * x
+        e[h] = np.sqrt(num) / (np.sqrt(den) + eps)
+    return e

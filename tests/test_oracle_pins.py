@@ -356,3 +356,21 @@ def test_generated_tiny_workload_statistics():
     q = f64(gen.make_q(wl))[0]
     o = oc.decode_all_layers([0], q[None])
     assert np.isfinite(o).all() and o.shape == (1, 2, 4, 64)
+
+
+def test_probe_error_eq3_closed_forms():
+    """Eq. (3): hand values. ref = (3, 4) on one head, cmp = 0 -> 5 / (5 + eps); identical outputs -> 0; a
+    uniformly scaled output (1 + delta) * ref -> delta * |ref| / (|ref| + eps); heads of different kv heads do not mix."""
+    ref = np.zeros((1, 2, 2)); ref[0, 0] = [3.0, 4.0]; ref[0, 1] = [0.0, 12.0]
+    cmp_ = np.zeros_like(ref); cmp_[0, 1] = [0.0, 12.0]
+    e = orc.probe_error(ref, cmp_, G=1, eps=1.0)
+    assert np.allclose(e, [5.0 / 6.0, 0.0])
+    e2 = orc.probe_error(ref, cmp_, G=2, eps=0.0)                       # one kv head over both query heads
+    assert np.allclose(e2, [5.0 / 13.0])
+    rng = np.random.default_rng(0)
+    a = rng.standard_normal((3, 4, 8))
+    assert np.allclose(orc.probe_error(a, a, 2, 1e-6), 0.0)
+    e3 = orc.probe_error(a, 1.25 * a, 2, 0.5)
+    for h in range(2):
+        nrm = np.linalg.norm(a[:, 2 * h:2 * h + 2])
+        assert np.isclose(e3[h], 0.25 * nrm / (nrm + 0.5))
