@@ -155,6 +155,20 @@ int dwkv_export_tokens(dwkv_cache* c, int32_t seq_id, int64_t t0, int64_t n, con
 /* Drop all tokens of a sequence and return its pages to the pool. */
 int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id);
 
+/* Attention-output probe, Eq. (3) (reading A25): for one sequence and
+ * layer and n_q probed query positions, the attention output over the compressed cache is compared with the output over a
+ * "temporarily materialized higher-fidelity cache" the caller provides for that layer:
+ *     e[h] = || Attn(Q, K_ref, V_ref) - Attn(Q, K-hat, V-hat) ||_2 / ( || Attn(Q, K_ref, V_ref) ||_2 + eps )
+ * with the norms over the G query heads of kv head h, the n_q positions and all channels. Both attentions use the cache's softmax
+ * scale and no mask (every probed query attends to all T = dwkv_seq_len tokens, reading A10).
+ *   q            dev bf16 [n_q, H_q, d]
+ *   K_ref, V_ref dev bf16 [H_kv, T, d]     (head-major: the layout of the dense comparison kernel)
+ *   e_out        dev fp32 [H_kv]
+ * Runs dwkv_decode_attention and the dense kernel n_q times each plus one reduction, on `stream`; scratch is owned by the
+ * handle. Errors: INVALID, STATE (no basis / gates), EMPTY (T = 0), CUDA. */
+int dwkv_probe_error(dwkv_cache* c, int32_t layer, int32_t seq_id, int32_t n_q, const void* q, const void* K_ref, const void* V_ref,
+                     float eps, float* e_out, void* stream);
+
 /* Number of cached tokens of a sequence (negative = error code). */
 int64_t dwkv_seq_len(const dwkv_cache* c, int32_t seq_id);
 

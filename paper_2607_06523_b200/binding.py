@@ -22,7 +22,7 @@ EXPORTED = [
     "dwkv_create", "dwkv_destroy", "dwkv_set_basis", "dwkv_set_gates", "dwkv_append_compress", "dwkv_decode_attention",
     "dwkv_append_raw", "dwkv_export_tokens", "dwkv_reset_seq", "dwkv_seq_len", "dwkv_footprint", "dwkv_set_option",
     "dwkv_launch_count", "dwkv_get_stat", "dwkv_last_error", "dwkv_dense_workspace_bytes", "dwkv_dense_decode_attention",
-    "dwkv_build_basis", "dwkv_export_basis",
+    "dwkv_build_basis", "dwkv_export_basis", "dwkv_probe_error",
 ]
 
 
@@ -61,6 +61,7 @@ def _load() -> C.CDLL:
     lib.dwkv_set_gates.argtypes = [vp, vp, vp, vp]
     lib.dwkv_build_basis.argtypes = [vp, i32, vp, vp, vp, i32, vp]
     lib.dwkv_export_basis.argtypes = [vp, vp, vp, vp]
+    lib.dwkv_probe_error.argtypes = [vp, i32, i32, i32, vp, vp, vp, C.c_float, vp, vp]
     lib.dwkv_append_compress.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.dwkv_decode_attention.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.dwkv_append_raw.argtypes = [vp, i32, i32, vp, vp, C.POINTER(dwkv_raw_tokens), vp]
@@ -159,6 +160,13 @@ class DwkvCache:
         BV = torch.empty_like(BK)
         _check(lib.dwkv_export_basis(self._h, _ptr(BK, torch.bfloat16), _ptr(BV, torch.bfloat16), _stream()))
         return BK, BV
+
+    def probe_error(self, layer: int, seq_id: int, q: torch.Tensor, K_ref: torch.Tensor, V_ref: torch.Tensor, eps: float = 1e-6):
+        """q: bf16 [n_q, H_q, d]; K_ref, V_ref: bf16 [H_kv, T, d]. Returns fp32 [H_kv] (Eq. 3 of the paper)."""
+        e = torch.empty(K_ref.shape[0], dtype=torch.float32, device=q.device)
+        _check(lib.dwkv_probe_error(self._h, layer, seq_id, int(q.shape[0]), _ptr(q, torch.bfloat16), _ptr(K_ref, torch.bfloat16),
+                                    _ptr(V_ref, torch.bfloat16), float(eps), _ptr(e, torch.float32), _stream()))
+        return e
 
     def set_gates(self, gK: torch.Tensor, gV: torch.Tensor):
         _check(lib.dwkv_set_gates(self._h, _ptr(gK, torch.bfloat16), _ptr(gV, torch.bfloat16), _stream()))

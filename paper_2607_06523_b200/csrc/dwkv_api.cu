@@ -138,7 +138,7 @@ struct dwkv_cache {
   int64_t total_tokens = 0;
   uint64_t version = 0;
   // scratch
-  DevBuf part, plan3_dev, tokdst_dev, basis_scratch;
+  DevBuf part, plan3_dev, tokdst_dev, basis_scratch, probe_ws;
   int n_sms = 148;
   StagingRing ring;
   Plan3 plan3;
@@ -321,7 +321,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gK) cudaFree(c->gK);
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
-  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release();
+  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release();
   c->ring.release();
   if (c->ev_scan0) cudaEventDestroy(c->ev_scan0);
   if (c->ev_scan1) cudaEventDestroy(c->ev_scan1);
@@ -826,4 +826,35 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
   }
   cudaStream_t st = (cudaStream_t)stream;
   return decode3(c, layer, n_seqs, seq_ids, q, out, st);
+}
+
+extern "C" int dwkv_probe_error(dwkv_cache* c, int32_t layer, int32_t seq_id, int32_t n_q, const void* q, const void* K_ref,
+                                const void* V_ref, float eps, float* e_out, void* stream) {
+  if (!c || !q || !K_ref || !V_ref || !e_out || n_q <= 0) return fail(DWKV_E_INVALID, "NULL argument or n_q <= 0");
+  if (layer < 0 || layer >= c->geom.L) return fail(DWKV_E_INVALID, "layer out of range");
+  if (check_seq(c, seq_id)) return fail(DWKV_E_INVALID, "bad sequence id");
+  if (!c->basis_set || !c->gates_set) return fail(DWKV_E_STATE, "basis and gates must be set before the probe");
+  const int64_t T = (int64_t)c->seqs[seq_id].tier.size();
+  if (T == 0) return fail(DWKV_E_EMPTY, "probe on an empty sequence");
+  const CacheGeom& g = c->geom;
+  const int Hq = g.H * g.G;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t out_elems = (size_t)n_q * Hq * g.d;
+  const size_t dense_ws = (size_t)dwkv_dense_workspace_bytes(1, 1, Hq, g.d, T);
+  CU_OK(c->probe_ws.reserve(2 * out_elems * sizeof(float) + dense_ws));
+  float* o_cmp = (float*)c->probe_ws.p;
+  float* o_ref = o_cmp + out_elems;
+  void* ws = (void*)(o_ref + out_elems);
+  const __nv_bfloat16* qb = (const __nv_bfloat16*)q;
+  for (int i = 0; i < n_q; ++i) {       // every probed position attends to all T cached tokens (reading A10)
+    int rc = decode3(c, layer, 1, &seq_id, qb + (size_t)i * Hq * g.d, o_cmp + (size_t)i * Hq * g.d, st);
+    if (rc) return rc;
+    rc = dwkv_dense_decode_attention(K_ref, V_ref, qb + (size_t)i * Hq * g.d, o_ref + (size_t)i * Hq * g.d, ws, 1, 1, g.H, Hq, g.d, T,
+                                     c->softmax_scale, stream);
+    if (rc) return fail(rc, "dense reference attention failed");
+    c->launches += 2;
+  }
+  c->launches += launch_probe_error(o_ref, o_cmp, e_out, n_q, g.H, g.G, g.d, eps, st);
+  CU_OK(cudaGetLastError());
+  return DWKV_OK;
 }

@@ -169,4 +169,35 @@ int launch_gate_check(const __nv_bfloat16* g, int64_t n, int* bad_flag, cudaStre
   return 1;
 }
 
+// Eq. (3) of the paper: e[h] = ||ref - cmp||_2 / (||ref||_2 + eps) over the G query heads of kv head h, the
+// n_q probed positions and all channels. One CTA per kv head; ref, cmp: fp32 [n_q, H*G, d].
+namespace {
+__global__ void __launch_bounds__(256) probe_error_kernel(const float* ref, const float* cmp, float* e, int n_q, int H, int G, int d, float eps) {
+  __shared__ float sn[8], sd[8];
+  const int h = blockIdx.x, tid = threadIdx.x, per_q = G * d;
+  float num = 0.f, den = 0.f;
+  for (int i = tid; i < n_q * per_q; i += 256) {
+    const int qi = i / per_q, r = i - qi * per_q;
+    const size_t off = ((size_t)qi * H + h) * per_q + r;
+    const float a = ref[off], b = cmp[off];
+    num = fmaf(a - b, a - b, num);
+    den = fmaf(a, a, den);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { num += __shfl_xor_sync(0xffffffffu, num, o); den += __shfl_xor_sync(0xffffffffu, den, o); }
+  if ((tid & 31) == 0) { sn[tid >> 5] = num; sd[tid >> 5] = den; }
+  __syncthreads();
+  if (tid == 0) {
+    num = 0.f; den = 0.f;
+    for (int w = 0; w < 8; ++w) { num += sn[w]; den += sd[w]; }
+    e[h] = sqrtf(num) / (sqrtf(den) + eps);
+  }
+}
+}  // namespace
+
+int launch_probe_error(const float* ref, const float* cmp, float* e, int n_q, int H, int G, int d, float eps, cudaStream_t s) {
+  probe_error_kernel<<<H, 256, 0, s>>>(ref, cmp, e, n_q, H, G, d, eps);
+  return 1;
+}
+
 }  // namespace dwkv

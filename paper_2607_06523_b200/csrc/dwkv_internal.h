@@ -99,6 +99,7 @@ struct DumpPtrs {
   float *deqK, *deqV;
 };
 int launch_gather(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const DumpPtrs& o, cudaStream_t s);
+int launch_probe_error(const float* ref, const float* cmp, float* e, int n_q, int H, int G, int d, float eps, cudaStream_t s);
 int launch_gate_check(const __nv_bfloat16* g, int64_t n, int* bad_flag, cudaStream_t s);
 
 }  // namespace dwkv

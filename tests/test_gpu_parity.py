@@ -11,7 +11,7 @@ import torch
 
 import gen
 from oracle import dwkv_oracle as orc
-from helpers import f64, oracle_slice_from_kept, check_output, rel_l2
+from helpers import f64, oracle_slice_from_kept, check_output, rel_l2, make_oracle, workload_inputs, oracle_load
 
 pytestmark = pytest.mark.gpu
 
@@ -456,3 +456,45 @@ def test_dense_bf16_kernel_against_oracle_softmax(mod):
                 ref = np.concatenate([orc.softmax_attention(qn[s, l, h * G:(h + 1) * G], Kn[s, l, h], Vn[s, l, h], 1 / np.sqrt(d))
                                       for h in range(H)])
                 check_output(out[s, l], ref, float(np.abs(Vn[s, l]).max()), f"dense {(n_seq, L, H, G, d, T)}")
+
+
+@pytest.mark.parametrize("name", ["tiny", "8b"])
+def test_probe_error_eq3(mod, name):
+    """dwkv_probe_error (Eq. 3, reading A25): the compressed cache against a higher-fidelity dense cache of the same tokens
+    (here: the oracle's reconstruction plus noise, rounded to bf16), per kv head over n_q query positions, vs the oracle's number
+    computed from fp64 attention on both caches. A reference equal to the reconstruction itself gives e at the bf16 rounding level."""
+    binding, harness = mod
+    if name == "tiny":
+        wl = gen.WORKLOADS["tiny"]
+    else:
+        wl = dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, T=(777,))
+    T = wl.T[0]
+    oc, _ = make_oracle(wl)
+    inp = workload_inputs(wl, 0, T, device="cuda")
+    oracle_load(oc, 0, inp)
+    cache, consts = harness.make_cache(wl, n_seqs=1, max_tokens=T + 64)
+    nf = int(inp["flag"].sum())
+    cache.append_raw(0, inp["tier"], inp["flag"], inp["cK"], inp["cV"], residK=inp["rK"] if nf else None, residV=inp["rV"] if nf else None)
+    n_q, layer, eps = 3, wl.L - 1, 1e-6
+    rng = np.random.default_rng(5)
+    q = torch.stack([gen.make_q(wl, step=i, device="cuda", n_seq=1)[0, layer] for i in range(n_q)]).contiguous()      # [n_q, Hq, d]
+    Kh = np.stack([oc.khat_vhat(0, layer, h)[0] for h in range(wl.H_kv)]); Vh = np.stack([oc.khat_vhat(0, layer, h)[1] for h in range(wl.H_kv)])
+    for noise in (0.0, 0.05):
+        K_ref = torch.from_numpy(Kh + noise * rng.standard_normal(Kh.shape)).to(torch.bfloat16).cuda().contiguous()      # [H, T, d]
+        V_ref = torch.from_numpy(Vh + noise * rng.standard_normal(Vh.shape)).to(torch.bfloat16).cuda().contiguous()
+        e = cache.probe_error(layer, 0, q, K_ref, V_ref, eps).double().cpu().numpy()
+        a_ref = np.zeros((n_q, wl.H_q, wl.d)); a_cmp = np.zeros_like(a_ref)
+        qn = f64(q)
+        for i in range(n_q):
+            for h in range(wl.H_kv):
+                sl = slice(h * wl.G, (h + 1) * wl.G)
+                a_ref[i, sl] = orc.softmax_attention(qn[i, sl], f64(K_ref[h]), f64(V_ref[h]), oc.scale)
+                a_cmp[i, sl] = orc.softmax_attention(qn[i, sl], Kh[h], Vh[h], oc.scale)
+        want = orc.probe_error(a_ref, a_cmp, wl.G, eps)
+        # the GPU attention outputs carry their own error (<= 5e-3 rel-L2 each, typically 3e-4), which adds to the numerator
+        assert np.all(np.abs(e - want) <= 0.02 * want + 2e-3), (name, noise, e, want)
+        if noise == 0.0:
+            assert np.all(e < 1e-2)
+        else:
+            assert np.all(e > 5e-2)
+    cache.destroy()
