@@ -438,6 +438,27 @@ def test_errors_and_reset(mod):
     c2.destroy()
     with pytest.raises(binding.DwkvError):
         binding.DwkvCache(3, 2, 2, 4, 64, [8, 16], 1, 64)
+    # basis construction and probe: argument and state errors
+    c3 = binding.DwkvCache(wl.L, wl.w, wl.H_kv, wl.H_q, wl.d, list(wl.tier_ranks), 1, 64)
+    kd = torch.zeros(16, wl.L, wl.H_kv, wl.d, dtype=torch.bfloat16, device="cuda")
+    om = torch.zeros(wl.w, 32, 16, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(binding.DwkvError) as e:      # gates first: the sketch is taken in gate-normalised space
+        c3.build_basis(kd, kd, om)
+    assert e.value.code == binding.DWKV_E_STATE
+    c3.set_gates(consts[2], consts[3])
+    with pytest.raises(binding.DwkvError) as e:      # n must be a multiple of 8
+        c3.build_basis(kd[:12].contiguous(), kd[:12].contiguous(), om[:, :, :12].contiguous())
+    assert e.value.code == binding.DWKV_E_INVALID
+    with pytest.raises(binding.DwkvError) as e:      # sketch rows: multiple of 16, >= r
+        c3.build_basis(kd, kd, om[:, :8].contiguous())
+    assert e.value.code == binding.DWKV_E_INVALID
+    c3.build_basis(kd, kd, om)                       # all-zero input: rows of norm zero are written as zeros, no NaN
+    Bk, Bv = c3.export_basis(wl.M, wl.H_kv, wl.r, wl.d)
+    assert torch.isfinite(Bk.float()).all() and torch.isfinite(Bv.float()).all()
+    with pytest.raises(binding.DwkvError) as e:      # probe on an empty sequence
+        c3.probe_error(0, 0, q[:, 0].contiguous(), kd[:, 0].permute(1, 0, 2).contiguous(), kd[:, 0].permute(1, 0, 2).contiguous())
+    assert e.value.code == binding.DWKV_E_EMPTY
+    c3.destroy()
     cache.destroy()
 
 
