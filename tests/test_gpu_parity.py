@@ -519,3 +519,36 @@ def test_probe_error_eq3(mod, name):
         else:
             assert np.all(e > 5e-2)
     cache.destroy()
+
+
+@pytest.mark.parametrize("name", ["llama8b_64k_b1", "llama8b_64k_b8", "llama8b_16k_b8", "llama70b_128k_b1", "ragged32"])
+def test_full_size_sampled_slices(mod, name):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (all layers in one call, persistent grid): sampled
+    (sequence, layer, kv head) slices against the oracle, element by element, plus the peaked variant (pin P12) and, at full
+    size too, q = 0 => the output is the mean of V-hat over the tokens (pin P5) on the sampled slices."""
+    binding, harness = mod
+    wl = gen.WORKLOADS[name]
+    routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
+    cache, consts = harness.make_cache(wl, arena_bytes=harness.arena_bytes_for(wl, routings, 1))
+    keep = [(0, 0), (wl.L // 2, 3), (wl.L - 1, wl.H_kv - 1)]
+    # ragged32: T = 1, T = 12347, all-lowest, all-top-flagged, alternating tiers, and the last of the mixed sequences
+    sampled = [0, 1, 2, 3, 4, wl.n_seq - 1] if name == "ragged32" else sorted({0, wl.n_seq - 1})
+    kept = {}
+    for s, (tier, flag) in enumerate(routings):
+        kept[s] = harness.fill_sequence(cache, wl, s, s, tier, flag, chunk=8192, keep=keep if s in sampled else [])
+    ids = list(range(wl.n_seq))
+    for gain in (1.0, 8.0, 0.0):
+        q = gen.make_q(wl, device="cuda", gain=gain)
+        o = cache.decode_attention(-1, ids, q).double().cpu().numpy()
+        qn = f64(q)
+        for s in sampled:
+            tier, flag = routings[s]
+            for (l, h) in keep:
+                sl = slice(h * wl.G, (h + 1) * wl.G)
+                o_ref, V, _ = oracle_slice_from_kept(wl, consts, tier, flag, kept[s][(l, h)], qn[s, l, sl], l, h)
+                check_output(o[s, l, sl], o_ref, float(np.abs(V).max()), f"{name} gain {gain} seq {s} (l,h)=({l},{h})")
+                if gain == 0.0:
+                    assert np.allclose(o_ref, V.mean(axis=0)[None], atol=1e-12)
+    fp = cache.footprint()
+    assert fp["used_bytes"] == sum(orc.footprint_bytes(t, f, wl.tier_ranks, wl.d, wl.L, wl.H_kv) for t, f in routings)
+    cache.destroy()
