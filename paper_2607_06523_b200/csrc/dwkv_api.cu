@@ -410,45 +410,56 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
   if (need > (int64_t)c->free_pages.size()) return fail(DWKV_E_CAPACITY, "arena pages exhausted");
   if (total > 0x7fffffff) return fail(DWKV_E_INVALID, "too many tokens in one call");
   cudaStream_t st = (cudaStream_t)stream;
-  std::vector<TokDst> dst;
-  dst.reserve(total);
-  std::vector<int32_t> new_pages;
-  int ridx = 0;
-  int64_t off = 0;
-  for (int i = 0; i < n_seqs; ++i) {
-    route_commit(c, seq_ids[i], n_new[i], tier + off, flag + off, &ridx, &dst, &new_pages);
-    off += n_new[i];
-  }
-  // flagged tokens first, then by descending rank: only the flagged 16-token tiles run the reconstruction + int4 quantiser part
-  // of the kernel, and a tile multiplies only the rank chunks its tokens keep
-  for (size_t i = 0; i < dst.size(); ++i) { dst[i].src = (int32_t)i; dst[i].pad_ = 0; }
-  {   // counting sort by key = (flag, tier), descending, stable
-    size_t start[8] = {0}, cnt[8] = {0};
-    auto key = [](const TokDst& t) { return ((t.cls & 1) << 2) | (t.cls >> 1); };
-    for (const TokDst& t : dst) cnt[key(t)]++;
-    size_t acc = 0;
-    for (int k = 7; k >= 0; --k) { start[k] = acc; acc += cnt[k]; }
-    std::vector<TokDst> sorted(dst.size());
-    for (const TokDst& t : dst) sorted[start[key(t)]++] = t;
-    dst.swap(sorted);
-  }
-  CompressRuns runs = {};
-  for (size_t t0 = 0; t0 < dst.size(); t0 += 16) {            // the first token of a tile has its largest key
-    const int cost = compress_tile_cost(dst[t0].cls & 1, c->geom.tier_rank[dst[t0].cls >> 1] / 8);
-    if (runs.n == 0 || runs.cost[runs.n - 1] != cost) { runs.n++; runs.cost[runs.n - 1] = cost; runs.count[runs.n - 1] = 0; }
-    runs.count[runs.n - 1]++;
-    runs.per_lh += cost;
-  }
-  int rc = zero_new_pages(c, new_pages, st);
-  if (rc) return rc;
-  rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
-  if (rc) return rc;
   if (c->opt_time_scan) {
     if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
     CU_OK(cudaEventRecord(c->ev_app0, st));
   }
-  c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)total, runs, (const __nv_bfloat16*)k_new,
-                                     (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, c->n_sms, st);
+  // Large (prefill-sized) calls go in chunks of kChunk tokens of the call's row order: the host routes chunk i + 1 while the GPU
+  // compresses chunk i. Rows keep their global index (TokDst::src), so every launch reads k_new / v_new in place.
+  constexpr int64_t kChunk = 16384;
+  std::vector<TokDst> dst, sorted;
+  std::vector<int32_t> new_pages;
+  int ridx = 0;
+  for (int64_t g0 = 0; g0 < total; g0 += kChunk) {
+    const int64_t g1 = std::min(total, g0 + kChunk);
+    dst.clear();
+    new_pages.clear();
+    int64_t off = 0;
+    for (int i = 0; i < n_seqs; ++i) {
+      const int64_t lo = std::max(off, g0), hi = std::min(off + n_new[i], g1);
+      if (lo < hi) {
+        const size_t first = dst.size();
+        route_commit(c, seq_ids[i], (int32_t)(hi - lo), tier + lo, flag + lo, &ridx, &dst, &new_pages);
+        for (size_t k = first; k < dst.size(); ++k) dst[k].src = (int32_t)(lo + (int64_t)(k - first));
+      }
+      off += n_new[i];
+    }
+    // flagged tokens first, then by descending rank: only the flagged 16-token tiles run the reconstruction + int4 quantiser
+    // part of the kernel, and a tile multiplies only the rank chunks its tokens keep. Counting sort, stable.
+    {
+      size_t start[8] = {0}, cnt[8] = {0};
+      auto key = [](const TokDst& t) { return ((t.cls & 1) << 2) | (t.cls >> 1); };
+      for (const TokDst& t : dst) cnt[key(t)]++;
+      size_t acc = 0;
+      for (int k = 7; k >= 0; --k) { start[k] = acc; acc += cnt[k]; }
+      sorted.resize(dst.size());
+      for (const TokDst& t : dst) sorted[start[key(t)]++] = t;
+      dst.swap(sorted);
+    }
+    CompressRuns runs = {};
+    for (size_t t0 = 0; t0 < dst.size(); t0 += 16) {            // the first token of a tile has its largest key
+      const int cost = compress_tile_cost(dst[t0].cls & 1, c->geom.tier_rank[dst[t0].cls >> 1] / 8);
+      if (runs.n == 0 || runs.cost[runs.n - 1] != cost) { runs.n++; runs.cost[runs.n - 1] = cost; runs.count[runs.n - 1] = 0; }
+      runs.count[runs.n - 1]++;
+      runs.per_lh += cost;
+    }
+    int rc = zero_new_pages(c, new_pages, st);
+    if (rc) return rc;
+    rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
+    if (rc) return rc;
+    c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)dst.size(), runs, (const __nv_bfloat16*)k_new,
+                                       (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, c->n_sms, st);
+  }
   if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_app1, st)); c->app_timed = true; }
   CU_OK(cudaGetLastError());
   return DWKV_OK;

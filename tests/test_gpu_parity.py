@@ -552,3 +552,42 @@ def test_full_size_sampled_slices(mod, name):
     fp = cache.footprint()
     assert fp["used_bytes"] == sum(orc.footprint_bytes(t, f, wl.tier_ranks, wl.d, wl.L, wl.H_kv) for t, f in routings)
     cache.destroy()
+
+
+def test_append_compress_chunked_call(mod):
+    """A call larger than the library's internal chunk (16384 rows): the chunk boundary falls inside the second sequence. Routing
+    bit-exact, coefficients within one bf16 ulp of the oracle, attention within tolerance."""
+    binding, harness = mod
+    n_new = [10000, 9000]
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(n_new[0], n_new[1]))
+    cache, consts = harness.make_cache(wl, n_seqs=2, max_tokens=max(n_new) + 64)
+    BK, BV, gK, gV = consts
+    oc = orc.OracleCache(wl.L, wl.w, wl.H_kv, wl.G, wl.d, wl.tier_ranks, f64(BK), f64(BV), f64(gK), f64(gV))
+    routings = [gen.make_routing(wl, s) for s in range(2)]
+    ks, vs = [], []
+    for s, n in enumerate(n_new):
+        k, v = gen.make_dense_kv_chunk(wl, s, 0, n, BK, BV, gK, gV, device="cuda")
+        ks.append(k.contiguous()); vs.append(v.contiguous())
+    k_new, v_new = torch.cat(ks), torch.cat(vs)
+    tier = np.concatenate([r[0] for r in routings]); flag = np.concatenate([r[1] for r in routings])
+    cache.append_compress([0, 1], n_new, k_new, v_new, tier, flag)
+    off = 0
+    for s, n in enumerate(n_new):
+        oc.append_compress(s, f64(k_new[off:off + n]), f64(v_new[off:off + n]), tier[off:off + n], flag[off:off + n])
+        off += n
+    for s in (0, 1):
+        dump = cache.export_tokens(s, 0, n_new[s])
+        S = oc.seqs[s]
+        assert np.array_equal(dump["slot"].cpu().numpy(), S["slot"]) and np.array_equal(dump["tier"].cpu().numpy(), S["tier"])
+        assert np.array_equal(dump["flag"].cpu().numpy(), S["flag"])
+        for z in "KV":
+            got = dump["coef" + z].double().cpu().numpy(); want = S["c" + z]
+            ulp = np.maximum(np.abs(want) * 2.0 ** -7, np.abs(want).max(axis=-1, keepdims=True) * 2.0 ** -20)
+            assert np.all(np.abs(got - want) <= ulp) and np.mean(got != want) < 5e-3
+    q = gen.make_q(wl, device="cuda", n_seq=2)
+    out = cache.decode_attention(-1, [0, 1], q).double().cpu().numpy()
+    ref = oc.decode_all_layers([0, 1], f64(q))
+    for s in (0, 1):
+        for l in range(wl.L):
+            check_output(out[s, l], ref[s, l], oc.max_abs_vhat(s, l), f"chunked append seq {s} layer {l}")
+    cache.destroy()
