@@ -591,3 +591,27 @@ def test_append_compress_chunked_call(mod):
         for l in range(wl.L):
             check_output(out[s, l], ref[s, l], oc.max_abs_vhat(s, l), f"chunked append seq {s} layer {l}")
     cache.destroy()
+
+
+@pytest.mark.parametrize("tier_k,flag_k", [(0, 0), (0, 1), (1, 0), (1, 1)])
+def test_page_boundaries_single_class(mod, tier_k, flag_k):
+    """Sequences of ONE class whose length sits just below, at, just above one page stripe and past two (the planner's units end at
+    page ends; a page holds 64 KB / block bytes * 32 tokens per (layer, head)), all decoded in one call and one by one."""
+    binding, harness = mod
+    base = gen.WORKLOADS["tiny"]
+    rank = base.tier_ranks[tier_k]
+    tpp = (65536 // (2 * (rank // 8) * 512 + flag_k * 40 * base.d)) * 32
+    Ts = (tpp - 1, tpp, tpp + 1, 2 * tpp + 5)
+    wl = dataclasses.replace(base, T=Ts, S0=0)
+    routings = [(np.full(T, tier_k, np.uint8), np.full(T, flag_k, np.uint8)) for T in Ts]
+    cache, consts, kept = load(harness, wl, routings, chunk=700)
+    q = gen.make_q(wl, device="cuda", gain=2.0)
+    out = cache.decode_attention(-1, [0, 1, 2, 3], q)
+    compare(wl, cache, consts, kept, routings, q, out, what=f"class ({tier_k},{flag_k}) page boundary")
+    for s in range(4):
+        o1 = cache.decode_attention(-1, [s], q[s:s + 1].contiguous())
+        assert rel_l2(o1.cpu().numpy(), out[s:s + 1].cpu().numpy()) < 2e-3
+    fp = cache.footprint()
+    page = wl.L * wl.H_kv * 65536
+    assert fp["reserved_bytes"] == page * sum((T + tpp - 1) // tpp for T in Ts)
+    cache.destroy()
