@@ -199,6 +199,23 @@ int64_t dwkv_launch_count(const dwkv_cache* c);
 
 const char* dwkv_last_error(void);
 
+/* ---- token-conditional router (Eq. (2); reading A26). Host-only, stateless:
+ * "operates only on cache metadata". All pointers are HOST memory.
+ *   phi        fp32 [n, 4]  the four online features of a token (attention mass, max spike, boundary indicator, probe error)
+ *   u          fp32 [4]     router parameter
+ *   z_t = ((u0*phi_t0 + u1*phi_t1) + u2*phi_t2) + u3*phi_t3 in fp32 (no FMA contraction); sigma(z) > tau <=> z > logit(tau), so
+ *   thresholds are passed in logit space: tau_logit [n_tiers-1] ascending ("three rank levels"), tau_flag_logit for the
+ *   residual flag.  tier_t = #{k : z_t > tau_logit[k]},  flag_t = z_t > tau_flag_logit  -- the arrays dwkv_append_compress takes.
+ * Errors: INVALID (NULL, n_tiers outside 1..DWKV_MAX_TIERS, thresholds not ascending / NaN). */
+int dwkv_route_tokens(int64_t n, const float* phi, const float* u, int32_t n_tiers, const float* tau_logit, float tau_flag_logit,
+                      uint8_t* tier, uint8_t* flag);
+/* Thresholds "chosen to satisfy the current memory budget", the budget given as the fraction of tokens per tier
+ * (tier_frac [n_tiers], low -> high) and the flagged fraction: tau_logit[k-1] = the largest z_t that is not among the
+ * ceil(n * sum_{j>=k} tier_frac[j]) highest ones (the product in double; -inf if every token is, +inf if none); tau_flag_logit the same
+ * with flag_frac. With distinct z_t the routed counts are exactly those numbers. */
+int dwkv_router_thresholds(int64_t n, const float* phi, const float* u, int32_t n_tiers, const float* tier_frac, float flag_frac,
+                           float* tau_logit, float* tau_flag_logit);
+
 /* ---- dense bf16 comparison kernel (BASELINE.json "from-scratch dense-bf16-cache decode kernel")
  * Plain softmax attention over an uncompressed cache. K, V: dev bf16 [n_seqs, L, H_kv, T, d] (all sequences length T);
  * q: dev bf16 [n_seqs, L, H_q, d]; out: dev fp32 [n_seqs, L, H_q, d]; workspace: dev, >= dwkv_dense_workspace_bytes(). */

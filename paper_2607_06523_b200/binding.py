@@ -22,7 +22,7 @@ EXPORTED = [
     "dwkv_create", "dwkv_destroy", "dwkv_set_basis", "dwkv_set_gates", "dwkv_append_compress", "dwkv_decode_attention",
     "dwkv_append_raw", "dwkv_export_tokens", "dwkv_reset_seq", "dwkv_seq_len", "dwkv_footprint", "dwkv_set_option",
     "dwkv_launch_count", "dwkv_get_stat", "dwkv_last_error", "dwkv_dense_workspace_bytes", "dwkv_dense_decode_attention",
-    "dwkv_build_basis", "dwkv_export_basis", "dwkv_probe_error",
+    "dwkv_build_basis", "dwkv_export_basis", "dwkv_probe_error", "dwkv_route_tokens", "dwkv_router_thresholds",
 ]
 
 
@@ -62,6 +62,8 @@ def _load() -> C.CDLL:
     lib.dwkv_build_basis.argtypes = [vp, i32, vp, vp, vp, i32, vp]
     lib.dwkv_export_basis.argtypes = [vp, vp, vp, vp]
     lib.dwkv_probe_error.argtypes = [vp, i32, i32, i32, vp, vp, vp, C.c_float, vp, vp]
+    lib.dwkv_route_tokens.argtypes = [i64, vp, vp, i32, vp, C.c_float, vp, vp]
+    lib.dwkv_router_thresholds.argtypes = [i64, vp, vp, i32, vp, C.c_float, vp, vp]
     lib.dwkv_append_compress.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.dwkv_decode_attention.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.dwkv_append_raw.argtypes = [vp, i32, i32, vp, vp, C.POINTER(dwkv_raw_tokens), vp]
@@ -244,3 +246,24 @@ def dense_decode_attention(K: torch.Tensor, V: torch.Tensor, q: torch.Tensor, n_
                                            _ptr(out, torch.float32), _ptr(workspace), n_seqs, L, H, Hq, d, T,
                                            softmax_scale, _stream()))
     return out
+
+
+def route_tokens(phi: np.ndarray, u: np.ndarray, tau_logit, tau_flag_logit: float, n_tiers: int):
+    """Host router (Eq. 2 of the paper): phi fp32 [n, 4], u fp32 [4]. Returns (tier u8 [n], flag u8 [n])."""
+    phi = np.ascontiguousarray(phi, np.float32); u = np.ascontiguousarray(u, np.float32)
+    tau = np.ascontiguousarray(tau_logit, np.float32)
+    n = phi.shape[0]
+    tier = np.zeros(n, np.uint8); flag = np.zeros(n, np.uint8)
+    _check(lib.dwkv_route_tokens(n, phi.ctypes.data, u.ctypes.data, n_tiers, tau.ctypes.data if tau.size else None,
+                                 float(tau_flag_logit), tier.ctypes.data, flag.ctypes.data))
+    return tier, flag
+
+
+def router_thresholds(phi: np.ndarray, u: np.ndarray, tier_frac, flag_frac: float):
+    """Thresholds (logit space) that route the given fractions of the tokens: returns (tau_logit fp32 [n_tiers-1], tau_flag_logit)."""
+    phi = np.ascontiguousarray(phi, np.float32); u = np.ascontiguousarray(u, np.float32)
+    frac = np.ascontiguousarray(tier_frac, np.float32)
+    tau = np.zeros(max(len(frac) - 1, 1), np.float32); tf = C.c_float(0.0)
+    _check(lib.dwkv_router_thresholds(phi.shape[0], phi.ctypes.data, u.ctypes.data, len(frac), frac.ctypes.data, float(flag_frac),
+                                      tau.ctypes.data, C.addressof(tf)))
+    return tau[:len(frac) - 1], float(tf.value)
