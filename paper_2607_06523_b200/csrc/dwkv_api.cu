@@ -410,10 +410,6 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
   if (need > (int64_t)c->free_pages.size()) return fail(DWKV_E_CAPACITY, "arena pages exhausted");
   if (total > 0x7fffffff) return fail(DWKV_E_INVALID, "too many tokens in one call");
   cudaStream_t st = (cudaStream_t)stream;
-  if (c->opt_time_scan) {
-    if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
-    CU_OK(cudaEventRecord(c->ev_app0, st));
-  }
   // Large (prefill-sized) calls go in chunks of kChunk tokens of the call's row order: the host routes chunk i + 1 while the GPU
   // compresses chunk i. Rows keep their global index (TokDst::src), so every launch reads k_new / v_new in place.
   constexpr int64_t kChunk = 16384;
@@ -457,6 +453,10 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
     if (rc) return rc;
     rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
     if (rc) return rc;
+    if (c->opt_time_scan && g0 == 0) {       // "compress_ms": from the first kernel of the call to the end of the last
+      if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
+      CU_OK(cudaEventRecord(c->ev_app0, st));
+    }
     c->launches += launch_compress_mma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)dst.size(), runs, (const __nv_bfloat16*)k_new,
                                        (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, c->n_sms, st);
   }
