@@ -111,9 +111,9 @@ __global__ void __launch_bounds__(kSketchWarps * 32) sketch_kernel(const __nv_bf
     }
 }
 
-// grid (M*H*2); 256 threads. Dynamic shared memory: S[k][D + 1] fp32, norms[k], order[k].
+// grid (M*H*2); one warp per row pair of a Jacobi step (k/2 warps, at most 32). Dynamic shared memory: S[k][D + 1] fp32, norms[k].
 template <int D>
-__global__ void __launch_bounds__(256) basis_svd_kernel(const float* part, const int n_split, const __nv_bfloat16* gK,
+__global__ void __launch_bounds__(1024) basis_svd_kernel(const float* part, const int n_split, const __nv_bfloat16* gK,
                                                         const __nv_bfloat16* gV, __nv_bfloat16* BK, __nv_bfloat16* BV, const int K,
                                                         const int r, const int L, const int H, const int w) {
   constexpr int LD = D + 1;
@@ -121,11 +121,11 @@ __global__ void __launch_bounds__(256) basis_svd_kernel(const float* part, const
   float* S = reinterpret_cast<float*>(smem_raw);
   float* nrm = S + K * LD;
   __shared__ int rotated;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nthr = blockDim.x, nwarp = nthr >> 5;
   const int item = blockIdx.x, mh = item >> 1, z = item & 1, m = mh / H, h = mh - m * H, LH = L * H;
   const __nv_bfloat16* gate = z ? gV : gK;
   // ---- S = sum over the window's layers and the splits of P / gate (column scaling commutes with the sum over tokens) --------
-  for (int i = tid; i < K * D; i += 256) {
+  for (int i = tid; i < K * D; i += nthr) {
     const int row = i / D, col = i - row * D;
     float acc = 0.f;
     for (int j = 0; j < w; ++j) {
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(256) basis_svd_kernel(const float* part, const
     if (tid == 0) rotated = 0;
     __syncthreads();
     for (int step = 0; step < K - 1; ++step) {
-      for (int pi = warp; pi < K / 2; pi += 8) {
+      for (int pi = warp; pi < K / 2; pi += nwarp) {
         int p, q;
         if (pi == 0) { p = K - 1; q = step; }
         else { p = (step + pi) % (K - 1); q = (step - pi + (K - 1)) % (K - 1); }
@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(256) basis_svd_kernel(const float* part, const
     __syncthreads();
   }
   // ---- the r rows of largest norm, in descending order ---------------------------------------------------------------------
-  for (int row = warp; row < K; row += 8) {
+  for (int row = warp; row < K; row += nwarp) {
     float a = 0.f;
 #pragma unroll
     for (int x = 0; x < D / 32; ++x) { const float u = S[row * LD + lane + 32 * x]; a = fmaf(u, u, a); }
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(256) basis_svd_kernel(const float* part, const
   }
   __syncthreads();
   __nv_bfloat16* B = (z ? BV : BK) + (size_t)mh * r * D;
-  for (int row = warp; row < K; row += 8) {
+  for (int row = warp; row < K; row += nwarp) {
     const float a = nrm[row];
     int rank = 0;
     for (int o = 0; o < K; ++o) rank += (nrm[o] > a) || (nrm[o] == a && o < row);
@@ -247,10 +247,10 @@ int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, 
   const int items2 = 2 * (g.L / g.w) * g.H;
   if (g.d == 128) {
     cudaFuncSetAttribute(basis_svd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
-    basis_svd_kernel<128><<<items2, 256, smem2, s>>>(part, n_split, gK, gV, BK, BV, n_sketch, g.r, g.L, g.H, g.w);
+    basis_svd_kernel<128><<<items2, 32 * std::min(n_sketch / 2, 32), smem2, s>>>(part, n_split, gK, gV, BK, BV, n_sketch, g.r, g.L, g.H, g.w);
   } else {
     cudaFuncSetAttribute(basis_svd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2);
-    basis_svd_kernel<64><<<items2, 256, smem2, s>>>(part, n_split, gK, gV, BK, BV, n_sketch, g.r, g.L, g.H, g.w);
+    basis_svd_kernel<64><<<items2, 32 * std::min(n_sketch / 2, 32), smem2, s>>>(part, n_split, gK, gV, BK, BV, n_sketch, g.r, g.L, g.H, g.w);
   }
   return 2;
 }
