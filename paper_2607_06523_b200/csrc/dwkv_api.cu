@@ -151,6 +151,7 @@ struct dwkv_cache {
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
+  int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
   cudaEvent_t ev_scan0 = nullptr, ev_scan1 = nullptr, ev_app0 = nullptr, ev_app1 = nullptr;
   bool scan_timed = false, app_timed = false;
   int64_t launches = 0;
@@ -354,7 +355,7 @@ int dwkv_build_basis(dwkv_cache* c, int32_t n, const void* k_dense, const void* 
   CU_OK(c->basis_scratch.reserve(basis_scratch_bytes(c->geom, n_sketch, ns)));
   const int launched = launch_build_basis(c->geom, n, (const __nv_bfloat16*)k_dense, (const __nv_bfloat16*)v_dense,
                                           (const __nv_bfloat16*)omega, n_sketch, ns, (float*)c->basis_scratch.p, c->gK, c->gV, c->BK,
-                                          c->BV, st);
+                                          c->BV, c->opt_sketch_umma != 0, st);
   if (!launched) return fail(DWKV_E_INVALID, "no sketch kernel instance for this shape");
   c->launches += launched;
   CU_OK(cudaGetLastError());
@@ -579,6 +580,7 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!c || !key) return fail(DWKV_E_INVALID, "NULL argument");
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
   else if (!strcmp(key, "time_scan")) c->opt_time_scan = value;
+  else if (!strcmp(key, "sketch_umma")) c->opt_sketch_umma = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
   else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
   else if (!strcmp(key, "interleave")) c->opt_interleave = value;

@@ -111,6 +111,158 @@ __global__ void __launch_bounds__(kSketchWarps * 32) sketch_kernel(const __nv_bf
     }
 }
 
+// ---- tcgen05 variant of the sketch GEMM (d = 128) --------------------------------------------------------------------------------
+// P (sketch rows, padded to M = 128) x (N = 128 channels) accumulates in TMEM over the CTA's whole token range; one elected thread
+// issues tcgen05.mma (kind::f16, bf16 inputs, fp32 accumulate) on shared-memory tiles in the canonical 128-byte-swizzled layouts:
+//   A = Omega tile, K-major:  row i (sketch row) = 64 tokens = 128 bytes; 8-row groups of 1024 bytes (SBO); 16-byte chunk c of row i
+//       is stored at chunk c ^ (i % 8)
+//   B = token rows, MN-major: k-block = 8 tokens x 64 channels = 8 rows of 128 bytes (1024 bytes, SBO between k-blocks); the two
+//       64-channel halves of d = 128 lie LBO = 8 KB apart; chunk c of token t is stored at chunk c ^ (t % 8)
+// All 128 threads fill the tiles with 16-byte cp.async (a ring of kUmmaStages stages); a stage is released for refilling by the
+// tcgen05.commit of the MMAs that read it. The legacy mma.sync kernel above reaches 48 % of its tensor-pipe peak at 75 % of the HBM
+// peak; here the tensor work is a few percent of the UMMA peak and the kernel is bound by the row loads alone.
+constexpr int kUmmaStages = 3;                   // 3 x 32 KB: two CTAs per SM
+constexpr int kUmmaTok = 64;                      // tokens per stage = one 128-byte swizzle row of Omega
+constexpr int kUmmaXBytes = kUmmaTok * 256;       // 16 KB: 64 tokens x 128 channels bf16
+constexpr int kUmmaOBytes = 128 * 128;            // 16 KB: 128 (padded) sketch rows x 64 tokens bf16
+constexpr int kUmmaStageBytes = kUmmaXBytes + kUmmaOBytes;
+
+__device__ __forceinline__ void umma_mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void umma_mbar_wait(uint32_t bar, uint32_t parity) {     // bounded: a protocol error traps instead of hanging the GPU
+  for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
+    uint32_t ok;
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+  }
+  __trap();
+}
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  // start address [0,14), leading byte offset [16,30), stride byte offset [32,46) (all >> 4), version 1 at [46,48), SWIZZLE_128B = 2 at [61,64)
+  return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo_bytes >> 4) & 0x3fff) << 16) | ((uint64_t)((sbo_bytes >> 4) & 0x3fff) << 32) |
+         (1ull << 46) | (2ull << 61);
+}
+
+__global__ void __launch_bounds__(128) sketch_umma_kernel(const __nv_bfloat16* k_dense, const __nv_bfloat16* v_dense,
+                                                          const __nv_bfloat16* omega, float* part, const int n, const int LH,
+                                                          const int H, const int w, const int K /* sketch rows, multiple of 16 */) {
+  constexpr int D = 128;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[kUmmaStages + 1];
+  __shared__ uint32_t tmem_base_sh;
+  const uint32_t sm = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int item = blockIdx.x, lh = item >> 1, z = item & 1, l = lh / H;
+  const __nv_bfloat16* X = z ? v_dense : k_dense;
+  const __nv_bfloat16* Om = omega + (size_t)(l % w) * K * n;
+  const int per = ((n + gridDim.y - 1) / gridDim.y + kUmmaTok - 1) / kUmmaTok * kUmmaTok;
+  const int t_beg = blockIdx.y * per, t_end = min(n, t_beg + per);
+  const int n_tiles = t_beg < t_end ? (t_end - t_beg + kUmmaTok - 1) / kUmmaTok : 0;
+  // ---- setup: barriers, TMEM (128 fp32 columns), zero rows of the padded Omega tiles ----------------------------------------
+  if (tid == 0) {
+    for (int s = 0; s <= kUmmaStages; ++s) umma_mbar_init(bar0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"((uint32_t)__cvta_generic_to_shared(&tmem_base_sh)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int s = 0; s < kUmmaStages; ++s)           // sketch rows K .. 127 of every stage stay zero (the copies never touch them)
+    for (int i = tid; i < (128 - K) * 8; i += 128) {
+      const int row = K + i / 8, c = i % 8;
+      asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(sm + s * kUmmaStageBytes + kUmmaXBytes + row * 128 + c * 16), "r"(0u) : "memory");
+    }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem = tmem_base_sh;
+  auto fill = [&](int s, int t0) {
+    const uint32_t xs = sm + s * kUmmaStageBytes, os = xs + kUmmaXBytes;
+    for (int i = tid; i < kUmmaTok * 16; i += 128) {            // token rows: 16 chunks of 16 bytes each
+      const int r = i >> 4, c16 = i & 15, t = t0 + r;
+      const uint32_t dst = xs + (c16 >> 3) * 8192 + (r >> 3) * 1024 + (r & 7) * 128 + (((c16 & 7) ^ (r & 7)) << 4);
+      cp_async16(dst, X + ((size_t)min(t, n - 1) * LH + lh) * D + 8 * c16, t < t_end ? 16 : 0);
+    }
+    for (int i = tid; i < K * 8; i += 128) {                    // Omega rows: 8 chunks of 8 tokens
+      const int r = i >> 3, c = i & 7, t = t0 + 8 * c;
+      const uint32_t dst = os + (r >> 3) * 1024 + (r & 7) * 128 + ((c ^ (r & 7)) << 4);
+      cp_async16(dst, Om + (size_t)r * n + min(t, n - 8), t < t_end ? 16 : 0);
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  // instruction descriptor: D fp32, A / B bf16, A K-major, B MN-major, N = 128, M = 128
+  constexpr uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 16) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+  for (int k = 0; k < kUmmaStages - 1; ++k) {
+    if (k < n_tiles) fill(k, t_beg + k * kUmmaTok);
+    else asm volatile("cp.async.commit_group;" ::: "memory");
+  }
+  for (int it = 0; it < n_tiles; ++it) {
+    const int s = it % kUmmaStages;
+    {   // refill the stage that tile it - 1 used, once the MMAs that read it have completed
+      const int nt = it + kUmmaStages - 1, sn = nt % kUmmaStages;
+      if (nt < n_tiles) {
+        if (it >= 1) umma_mbar_wait(bar0 + 8 * sn, (uint32_t)(((it - 1) / kUmmaStages) & 1));
+        fill(sn, t_beg + nt * kUmmaTok);
+      } else {
+        asm volatile("cp.async.commit_group;" ::: "memory");
+      }
+    }
+    asm volatile("cp.async.wait_group %0;" ::"n"(kUmmaStages - 1) : "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic-proxy writes -> visible to the tensor core's reads
+    __syncthreads();
+    if (tid == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const uint32_t xs = sm + s * kUmmaStageBytes, os = xs + kUmmaXBytes;
+#pragma unroll
+      for (int ks = 0; ks < kUmmaTok / 16; ++ks) {
+        const uint64_t da = umma_desc(os + 32 * ks, 16, 1024);             // K-major: 16 tokens further = 32 bytes inside the swizzled row
+        const uint64_t db = umma_desc(xs + 2048 * ks, 8192, 1024);         // MN-major: 16 tokens further = two k-blocks
+        const uint32_t acc = (it > 0 || ks > 0) ? 1u : 0u;
+        asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p; }"
+                     ::"r"(tmem), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+      }
+      asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"r"(bar0 + 8 * s) : "memory");
+      if (it == n_tiles - 1)
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"r"(bar0 + 8 * kUmmaStages) : "memory");
+    }
+  }
+  // ---- epilogue: TMEM lanes = sketch rows, columns = channels -> global partial block --------------------------------------
+  float* out = part + ((size_t)blockIdx.y * (2 * LH) + item) * (size_t)(K * D);
+  if (n_tiles > 0) {
+    umma_mbar_wait(bar0 + 8 * kUmmaStages, 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  }
+  const int row = 32 * warp + lane;
+  if (32 * warp < K) {                           // warp-uniform: this warp's 32 lanes hold sketch rows 32 warp .. + 31
+#pragma unroll
+    for (int c0 = 0; c0 < D; c0 += 16) {
+      uint32_t v[16];
+      if (n_tiles > 0) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+                       "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                     : "r"(tmem + ((uint32_t)(32 * warp) << 16) + (uint32_t)c0));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      } else {
+#pragma unroll
+        for (int x = 0; x < 16; ++x) v[x] = 0u;
+      }
+      if (row < K) {
+#pragma unroll
+        for (int x = 0; x < 16; x += 4)
+          *reinterpret_cast<uint4*>(out + (size_t)row * D + c0 + x) = make_uint4(v[x], v[x + 1], v[x + 2], v[x + 3]);
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem) : "memory");
+}
+
 // grid (M*H*2); one warp per row pair of a Jacobi step (k/2 warps, at most 32). Dynamic shared memory: S[k][D + 1] fp32, norms[k].
 template <int D>
 __global__ void __launch_bounds__(1024) basis_svd_kernel(const float* part, const int n_split, const __nv_bfloat16* gK,
@@ -225,7 +377,7 @@ int basis_num_splits(const CacheGeom& g, int n, int n_sms) {
 
 int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, const __nv_bfloat16* v_dense, const __nv_bfloat16* omega,
                        int n_sketch, int n_split, float* part, const __nv_bfloat16* gK, const __nv_bfloat16* gV, __nv_bfloat16* BK,
-                       __nv_bfloat16* BV, cudaStream_t s) {
+                       __nv_bfloat16* BV, bool use_umma, cudaStream_t s) {
   const int LH = g.L * g.H, MT = n_sketch / 16;
   const size_t smem1 = kSketchStages * ((size_t)kSketchTok * (2 * g.d + 16) + (size_t)n_sketch * (2 * kSketchTok + 16));
   dim3 grid1(2 * LH, n_split);
@@ -235,7 +387,11 @@ int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, 
     cudaFuncSetAttribute(sketch_kernel<DD, MM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1);                   \
     sketch_kernel<DD, MM><<<grid1, kSketchWarps * 32, smem1, s>>>(k_dense, v_dense, omega, part, n, LH, g.H, g.w);            \
     break;
-  if (g.d == 128) {
+  if (g.d == 128 && use_umma) {
+    const size_t smem_u = (size_t)kUmmaStages * kUmmaStageBytes + 1024;
+    cudaFuncSetAttribute(sketch_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_u);
+    sketch_umma_kernel<<<grid1, 128, smem_u, s>>>(k_dense, v_dense, omega, part, n, LH, g.H, g.w, n_sketch);
+  } else if (g.d == 128) {
     switch (MT) { DWKV_SKETCH_CASE(128, 1) DWKV_SKETCH_CASE(128, 2) DWKV_SKETCH_CASE(128, 3) DWKV_SKETCH_CASE(128, 4) DWKV_SKETCH_CASE(128, 5)
                   default: ok = false; }
   } else {

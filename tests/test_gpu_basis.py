@@ -40,12 +40,15 @@ SHAPES = {
 }
 
 
+@pytest.mark.parametrize("umma", [0, 1])
 @pytest.mark.parametrize("shape", list(SHAPES))
-def test_build_basis_against_oracle(mod, shape):
+def test_build_basis_against_oracle(mod, shape, umma):
+    """umma = 1: the tcgen05 sketch kernel (d = 128 shapes; the tiny d = 64 shape stays on mma.sync either way)."""
     binding, harness = mod
     mk, n, k = SHAPES[shape]
     wl = mk()
     cache, consts = harness.make_cache(wl, n_seqs=1, max_tokens=n + 64)
+    cache.set_option("sketch_umma", umma)
     BK0, BV0, gK, gV = consts
     k_dense, v_dense = _dense(wl, n, consts)
     omega = gen.make_omega(wl, n, k, device="cuda")
