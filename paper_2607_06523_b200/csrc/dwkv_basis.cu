@@ -8,6 +8,8 @@
 //   basis_svd_kernel<D>    per (window, head, Z): S = sum over the window's layers and the splits of P / gate, one-sided Jacobi
 //                          (Hestenes) on the rows of S until they are mutually orthogonal -- they are then sigma_i * w_i^T --,
 //                          the r rows of largest norm, normalised, signed (largest-magnitude entry positive), rounded to bf16.
+#include <cuda.h>
+
 #include "dwkv_internal.h"
 #include "dwkv_mma.cuh"
 
@@ -263,6 +265,140 @@ __global__ void __launch_bounds__(128) sketch_umma_kernel(const __nv_bfloat16* k
   if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem) : "memory");
 }
 
+// ---- TMA-fed variant: the same tcgen05 pipeline, tiles brought in by cp.async.bulk.tensor with hardware 128-byte swizzle -----------
+// Warp 0 lane 0 produces (waits for a stage's release, arms its mbarrier with the byte count, issues three tensor copies: the two
+// 64-channel halves of 64 token rows and the 64-token slab of the Omega rows), warp 1 lane 0 issues the MMAs; everybody else only
+// joins for the epilogue. Tokens beyond n are zero-filled by the tensor map.
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+               ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+__global__ void __launch_bounds__(128) sketch_tma_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+                                                         const __grid_constant__ CUtensorMap mapO, float* part, const int n, const int LH,
+                                                         const int H, const int w, const int K) {
+  constexpr int D = 128, S = kUmmaStages;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[2 * S + 1];              // full[S], empty[S], done
+  __shared__ uint32_t tmem_base_sh;
+  const uint32_t sm = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
+  const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int item = blockIdx.x, lh = item >> 1, z = item & 1, l = lh / H;
+  const CUtensorMap* mapX = z ? &mapV : &mapK;
+  const int per = ((n + gridDim.y - 1) / gridDim.y + kUmmaTok - 1) / kUmmaTok * kUmmaTok;
+  const int t_beg = blockIdx.y * per, t_end = min(n, t_beg + per);
+  const int n_tiles = t_beg < t_end ? (t_end - t_beg + kUmmaTok - 1) / kUmmaTok : 0;
+  if (tid == 0) {
+    for (int s = 0; s <= 2 * S; ++s) umma_mbar_init(bar0 + 8 * s, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(mapX) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&mapO) : "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 128;" ::"r"((uint32_t)__cvta_generic_to_shared(&tmem_base_sh)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int s = 0; s < S; ++s)                     // sketch rows K .. 127 of every stage stay zero (the copies never touch them)
+    for (int i = tid; i < (128 - K) * 8; i += 128) {
+      const int row = K + i / 8, c = i % 8;
+      asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(sm + s * kUmmaStageBytes + kUmmaXBytes + row * 128 + c * 16), "r"(0u) : "memory");
+    }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem = tmem_base_sh;
+  constexpr uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 16) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+  if (warp == 0 && lane == 0) {
+    // ===== producer =====
+    const uint32_t bytes = 2 * 8192 + (uint32_t)K * 128;
+    for (int it = 0; it < n_tiles; ++it) {
+      const int s = it % S;
+      if (it >= S) umma_mbar_wait(bar0 + 8 * (S + s), (uint32_t)(((it / S) - 1) & 1));
+      const uint32_t xs = sm + s * kUmmaStageBytes, os = xs + kUmmaXBytes, full = bar0 + 8 * s;
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(full), "r"(bytes) : "memory");
+      const int t0 = t_beg + it * kUmmaTok;
+      tma_load_3d(xs, mapX, full, 0, lh, t0);
+      tma_load_3d(xs + 8192, mapX, full, 64, lh, t0);
+      tma_load_3d(os, &mapO, full, t0, 0, l % w);
+    }
+  } else if (warp == 1 && lane == 0) {
+    // ===== MMA issuer =====
+    for (int it = 0; it < n_tiles; ++it) {
+      const int s = it % S;
+      umma_mbar_wait(bar0 + 8 * s, (uint32_t)((it / S) & 1));
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const uint32_t xs = sm + s * kUmmaStageBytes, os = xs + kUmmaXBytes;
+#pragma unroll
+      for (int ks = 0; ks < kUmmaTok / 16; ++ks) {
+        const uint64_t da = umma_desc(os + 32 * ks, 16, 1024);
+        const uint64_t db = umma_desc(xs + 2048 * ks, 8192, 1024);
+        const uint32_t acc = (it > 0 || ks > 0) ? 1u : 0u;
+        asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p; }"
+                     ::"r"(tmem), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+      }
+      asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"r"(bar0 + 8 * (S + s)) : "memory");
+      if (it == n_tiles - 1)
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"r"(bar0 + 8 * (2 * S)) : "memory");
+    }
+  }
+  __syncwarp();
+  // ---- epilogue: TMEM lanes = sketch rows, columns = channels -> global partial block --------------------------------------
+  float* out = part + ((size_t)blockIdx.y * (2 * LH) + item) * (size_t)(K * D);
+  if (n_tiles > 0) {
+    umma_mbar_wait(bar0 + 8 * (2 * S), 0);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  }
+  const int row = 32 * warp + lane;
+  if (32 * warp < K) {
+#pragma unroll
+    for (int c0 = 0; c0 < D; c0 += 16) {
+      uint32_t v[16];
+      if (n_tiles > 0) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]), "=r"(v[9]),
+                       "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                     : "r"(tmem + ((uint32_t)(32 * warp) << 16) + (uint32_t)c0));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+      } else {
+#pragma unroll
+        for (int x = 0; x < 16; ++x) v[x] = 0u;
+      }
+      if (row < K) {
+#pragma unroll
+        for (int x = 0; x < 16; x += 4)
+          *reinterpret_cast<uint4*>(out + (size_t)row * D + c0 + x) = make_uint4(v[x], v[x + 1], v[x + 2], v[x + 3]);
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 128;" ::"r"(tmem) : "memory");
+}
+
+// host: tensor maps through the driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) p = nullptr;
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+bool make_map_3d(CUtensorMap* m, const void* base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t s1_bytes, uint64_t s2_bytes, uint32_t b0,
+                 uint32_t b1, uint32_t b2) {
+  EncodeTiledFn fn = encode_tiled_fn();
+  if (!fn) return false;
+  const cuuint64_t dims[3] = {d0, d1, d2}, strides[2] = {s1_bytes, s2_bytes};
+  const cuuint32_t box[3] = {b0, b1, b2}, es[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // grid (M*H*2); one warp per row pair of a Jacobi step (k/2 warps, at most 32). Dynamic shared memory: S[k][D + 1] fp32, norms[k].
 template <int D>
 __global__ void __launch_bounds__(1024) basis_svd_kernel(const float* part, const int n_split, const __nv_bfloat16* gK,
@@ -387,7 +523,17 @@ int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, 
     cudaFuncSetAttribute(sketch_kernel<DD, MM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1);                   \
     sketch_kernel<DD, MM><<<grid1, kSketchWarps * 32, smem1, s>>>(k_dense, v_dense, omega, part, n, LH, g.H, g.w);            \
     break;
-  if (g.d == 128 && use_umma) {
+  CUtensorMap mapK, mapV, mapO;
+  const bool aligned = (((uintptr_t)k_dense | (uintptr_t)v_dense | (uintptr_t)omega) & 15) == 0;
+  if (g.d == 128 && use_umma && aligned &&
+      make_map_3d(&mapK, k_dense, 128, (uint64_t)LH, (uint64_t)n, 256, (uint64_t)LH * 256, 64, 1, kUmmaTok) &&
+      make_map_3d(&mapV, v_dense, 128, (uint64_t)LH, (uint64_t)n, 256, (uint64_t)LH * 256, 64, 1, kUmmaTok) &&
+      make_map_3d(&mapO, omega, (uint64_t)n, (uint64_t)n_sketch, (uint64_t)g.w, (uint64_t)n * 2, (uint64_t)n_sketch * n * 2, kUmmaTok,
+                  (uint32_t)n_sketch, 1)) {
+    const size_t smem_u = (size_t)kUmmaStages * kUmmaStageBytes + 1024;
+    cudaFuncSetAttribute(sketch_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_u);
+    sketch_tma_kernel<<<grid1, 128, smem_u, s>>>(mapK, mapV, mapO, part, n, LH, g.H, g.w, n_sketch);
+  } else if (g.d == 128 && use_umma) {      // no driver entry point for tensor maps / unaligned inputs: cp.async-fed tcgen05 kernel
     const size_t smem_u = (size_t)kUmmaStages * kUmmaStageBytes + 1024;
     cudaFuncSetAttribute(sketch_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_u);
     sketch_umma_kernel<<<grid1, 128, smem_u, s>>>(k_dense, v_dense, omega, part, n, LH, g.H, g.w, n_sketch);
