@@ -151,6 +151,7 @@ struct dwkv_cache {
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
+  int64_t opt_compress_umma = 0;     // append/compress: 1 = tcgen05 kernel (d = 128, r <= 64), 0 = mma.sync kernel
   int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
   cudaEvent_t ev_scan0 = nullptr, ev_scan1 = nullptr, ev_app0 = nullptr, ev_app1 = nullptr;
   bool scan_timed = false, app_timed = false;
@@ -431,6 +432,23 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
       }
       off += n_new[i];
     }
+    if (c->opt_compress_umma && compress_umma_supported(c->geom, k_new, v_new)) {
+      // tcgen05 path: rows in call order (TMA tile loads), destinations in the same order
+      int rc = zero_new_pages(c, new_pages, st);
+      if (rc) return rc;
+      rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
+      if (rc) return rc;
+      if (c->opt_time_scan && g0 == 0) {
+        if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
+        CU_OK(cudaEventRecord(c->ev_app0, st));
+      }
+      const int launched = launch_compress_umma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)dst.size(), (int)g0, total,
+                                                (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV,
+                                                c->n_sms, st);
+      if (launched) { c->launches += launched; continue; }
+      // no tensor-map entry point: fall through to the mma.sync kernel (pages are zeroed and the table is re-uploaded sorted)
+      new_pages.clear();
+    }
     // flagged tokens first, then by descending rank: only the flagged 16-token tiles run the reconstruction + int4 quantiser
     // part of the kernel, and a tile multiplies only the rank chunks its tokens keep. Counting sort, stable.
     {
@@ -581,6 +599,7 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
   else if (!strcmp(key, "time_scan")) c->opt_time_scan = value;
   else if (!strcmp(key, "sketch_umma")) c->opt_sketch_umma = value;
+  else if (!strcmp(key, "compress_umma")) c->opt_compress_umma = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
   else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
   else if (!strcmp(key, "interleave")) c->opt_interleave = value;

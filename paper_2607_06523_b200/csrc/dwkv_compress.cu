@@ -17,6 +17,8 @@
 // V-code byte and scale is owned by exactly one (token, lane), so no atomics are needed (pages are zeroed when allocated).
 #include <algorithm>
 
+#include <cuda.h>
+
 #include "dwkv_internal.h"
 #include "dwkv_mma.cuh"
 
@@ -397,7 +399,416 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
   }
 }
 
+// =====================================================================================================================================
+// tcgen05 variant (d = 128): the projection and the reconstruction as UMMA tiles of 128 tokens, accumulators in TMEM.
+//   tile   = 128 consecutive rows of the call (no sorting: a thread of the epilogue owns one token row = one TMEM lane)
+//   MMA 1  : acc[128 x N1] = X[128 x 128] . B1^T, B1 = the three bf16 terms of B' = B / g as separate output columns, ordered
+//            [chunk b][term][8 columns] so that one chunk's lo / mid / hi partial sums are three 8-column TMEM loads; N1 = 3r (to 16)
+//   epi 1  : c = bf16((lo + mid) + hi), tier mask, fragment-native coefficient stores; the rows of FLAGGED tokens are written,
+//            compacted to the front, into the A operand of MMA 2
+//   MMA 2  : rec[p x 128] = c[p x 64] . B2^T, B2 = the transposed basis padded to 64 ranks
+//   epi 2  : thread p < n_flagged: e = x - g * rec (x from the token tile in shared memory), int4 quantiser A14, code / scale stores
+// Warps 0-3: epilogue (and the per-(layer, head) staging of B1 / B2); warp 4 lane 0: TMA producer (two 64-channel halves of 128
+// token rows per (tile, Z), hardware 128-byte swizzle); warp 5 lane 0: MMA issuer. mbarrier rings: x_full / x_empty (token
+// stages), acc_full / acc_empty (two accumulators), a2_ready / rec_full (second product), basis_ready (operands of a new (l, h)).
+constexpr int kCuS = 2;                               // token stages of 32 KB
+constexpr int kCuXBytes = 32768;
+constexpr int kCuAccCols = 192;                       // columns reserved per projection accumulator (N1 <= 192)
+
+__device__ __forceinline__ void cu_mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void cu_mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void cu_mbar_wait(uint32_t bar, uint32_t parity) {     // bounded: a protocol error traps instead of hanging
+  for (uint32_t spin = 0; spin < (1u << 27); ++spin) {
+    uint32_t ok;
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return;
+  }
+  __trap();
+}
+__device__ __forceinline__ uint64_t cu_desc(uint32_t saddr) {     // K-major, SWIZZLE_128B, 8-row groups 1024 bytes apart, version 1
+  return (uint64_t)((saddr >> 4) & 0x3fff) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+__device__ __forceinline__ void cu_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc) {
+  asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p; }"
+               ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void cu_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void cu_tma_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+               ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void cu_tmem_ld8(uint32_t taddr, float (&v)[8]) {
+  uint32_t r[8];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr));
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void cu_bar_epi() { asm volatile("bar.sync 1, 128;" ::: "memory"); }      // the 128 epilogue threads
+
+struct CuParams {
+  const uint8_t* arena;
+  const TokDst* dst;            // row order of the call's chunk (unsorted): row i of the chunk = global row row0 + i
+  const __nv_bfloat16 *BK, *BV, *gK, *gV;
+  int n_rows;                   // rows of this chunk
+  int row0;                     // first global row of the chunk in k_new / v_new
+  int N1;                       // 3 r rounded up to 16
+  uint32_t ranks4;
+  CacheGeom g;
+};
+
+__global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+                                                               const CuParams p) {
+  constexpr int D = 128;
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[2 * kCuS + 7];
+  __shared__ uint32_t tmem_base_sh;
+  __shared__ int nflag_sh[2], wcount_sh[4];
+  const CacheGeom& g = p.g;
+  const int r = g.r, N1 = p.N1, LH = g.L * g.H, NC = r / 8;
+  const uint32_t sm = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
+  // shared-memory map (all 1024-aligned): token stages | B1[z][atom] | B2[z] | A2 | gate[z][128] floats | flagged-row list
+  const uint32_t xs0 = sm, b1_0 = xs0 + kCuS * kCuXBytes, b1_atom = (uint32_t)N1 * 128, b2_0 = b1_0 + 4 * b1_atom, a2 = b2_0 + 2 * 16384,
+                 gam = a2 + 16384, flist = gam + 1024;
+  const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
+  const uint32_t x_full = bar0, x_empty = bar0 + 8 * kCuS, acc_full = bar0 + 16 * kCuS, acc_empty = acc_full + 16, a2_ready = acc_empty + 16,
+                 rec_full = a2_ready + 8, basis_ready = rec_full + 8;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int n_tiles = (p.n_rows + 127) >> 7;
+  const long long items = (long long)LH * n_tiles;
+  const int item0 = (int)(items * blockIdx.x / gridDim.x), item1 = (int)(items * (blockIdx.x + 1) / gridDim.x);
+  const int n_idx = 2 * (item1 - item0);                     // (item, Z) steps of this CTA
+  if (tid == 0) {
+    for (int i = 0; i < 2 * kCuS + 7; ++i) cu_mbar_init(bar0 + 8 * i, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&mapK) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&mapV) : "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((uint32_t)__cvta_generic_to_shared(&tmem_base_sh)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  for (int i = tid; i < 3 * 16384 / 16; i += 192)            // B2 (both Z) and A2: the ranks >= r stay zero for the whole kernel
+    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(b2_0 + 16 * i), "r"(0u) : "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem = tmem_base_sh;
+  const uint32_t idesc1 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N1 >> 3) << 17) | ((128u >> 4) << 24);      // both operands K-major
+  const uint32_t idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+  if (warp == 4) {
+    // ===== TMA producer =========================================================================================================
+    if (lane == 0) {
+      for (int idx = 0; idx < n_idx; ++idx) {
+        const int item = item0 + (idx >> 1), z = idx & 1, s = idx % kCuS;
+        const int lh = item / n_tiles, tile = item - lh * n_tiles;
+        if (idx >= kCuS) cu_mbar_wait(x_empty + 8 * s, (uint32_t)(((idx / kCuS) - 1) & 1));
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(x_full + 8 * s), "r"((uint32_t)kCuXBytes) : "memory");
+        const CUtensorMap* map = z ? &mapV : &mapK;
+        cu_tma_3d(xs0 + s * kCuXBytes, map, x_full + 8 * s, 0, lh, p.row0 + 128 * tile);
+        cu_tma_3d(xs0 + s * kCuXBytes + 16384, map, x_full + 8 * s, 64, lh, p.row0 + 128 * tile);
+      }
+    }
+  } else if (warp == 5) {
+    // ===== MMA issuer ===========================================================================================================
+    if (lane == 0) {
+      int n_seg = 0, n_rec = 0, cur_lh = -1;
+      auto mma1 = [&](int idx) {
+        const int item = item0 + (idx >> 1), z = idx & 1, s = idx % kCuS, buf = idx & 1;
+        const int lh = item / n_tiles;
+        if (lh != cur_lh) { cu_mbar_wait(basis_ready, (uint32_t)(n_seg & 1)); ++n_seg; cur_lh = lh; }
+        cu_mbar_wait(x_full + 8 * s, (uint32_t)((idx / kCuS) & 1));
+        if (idx >= 2) cu_mbar_wait(acc_empty + 8 * buf, (uint32_t)(((idx >> 1) - 1) & 1));
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t xs = xs0 + s * kCuXBytes, b1 = b1_0 + (uint32_t)(2 * z) * b1_atom;
+#pragma unroll
+        for (int k = 0; k < 8; ++k)       // channels 16k .. 16k+15: atom k / 4, 32 bytes per step inside the swizzled 128-byte rows
+          cu_mma(tmem + buf * kCuAccCols, cu_desc(xs + (k >> 2) * 16384 + 32 * (k & 3)), cu_desc(b1 + (k >> 2) * b1_atom + 32 * (k & 3)), idesc1, k > 0);
+        cu_commit(acc_full + 8 * buf);
+      };
+      if (n_idx > 0) mma1(0);
+      for (int idx = 0; idx < n_idx; ++idx) {
+        const int z = idx & 1;
+        const bool same_lh = idx + 1 < n_idx && ((item0 + ((idx + 1) >> 1)) / n_tiles) == cur_lh;
+        if (same_lh) mma1(idx + 1);                  // run ahead into the other accumulator while the epilogue of idx works
+        cu_mbar_wait(a2_ready, (uint32_t)(idx & 1));
+        if (nflag_sh[idx & 1] > 0) {
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint32_t b2 = b2_0 + (uint32_t)z * 16384;
+#pragma unroll
+          for (int k = 0; k < 4; ++k) cu_mma(tmem + 2 * kCuAccCols, cu_desc(a2 + 32 * k), cu_desc(b2 + 32 * k), idesc2, k > 0);
+          cu_commit(rec_full);
+          ++n_rec;
+        }
+        if (!same_lh && idx + 1 < n_idx) mma1(idx + 1);     // a new (layer, head): its operands are staged only after idx is finished
+      }
+      (void)n_rec;
+    }
+  } else {
+    // ===== epilogue warps (128 threads = TMEM lanes) ============================================================================
+    const uint32_t rows_sh = flist + 256;                       // RowDst of the tile's 128 rows (16 bytes each)
+    int cur_lh = -1, n_rec = 0, n_flag = 0, my_p = 0;
+    RowDst rd;
+    rd.blk = nullptr; rd.meta = 0; rd.src = 0;
+    const uint32_t lane_taddr = (uint32_t)(32 * warp) << 16;
+    for (int idx = 0; idx < n_idx; ++idx) {
+      const int item = item0 + (idx >> 1), z = idx & 1, s = idx % kCuS, buf = idx & 1;
+      const int lh = item / n_tiles, tile = item - lh * n_tiles;
+      if (lh != cur_lh) {
+        // ---- operands of this (layer, head): B1 = three-term split of B / g in [chunk][term][8] row order, B2 = B^T, gates ------
+        const int l = lh / g.H, h = lh - l * g.H;
+        for (int zz = 0; zz < 2; ++zz) {
+          const __nv_bfloat16* B = (zz ? p.BV : p.BK) + ((size_t)(l / g.w) * g.H + h) * (size_t)r * D;
+          const __nv_bfloat16* gz = (zz ? p.gV : p.gK) + (size_t)lh * D;
+          const uint32_t b1 = b1_0 + (uint32_t)(2 * zz) * b1_atom, b2 = b2_0 + (uint32_t)zz * 16384;
+          for (int i0 = tid; i0 < r * 64; i0 += 128 * 8) {       // 8 (rank, channel pair) items per thread with all loads issued first
+            uint32_t bwv[8], gwv[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const int i = i0 + 128 * u, j = i >> 6, ch = (i & 63) * 2;
+              const bool ok = i < r * 64;
+              bwv[u] = ok ? __ldg(reinterpret_cast<const uint32_t*>(B + (size_t)j * D + ch)) : 0u;
+              gwv[u] = ok ? __ldg(reinterpret_cast<const uint32_t*>(gz + ch)) : 0x3f803f80u;
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const int i = i0 + 128 * u, j = i >> 6, ch = (i & 63) * 2;
+              if (i >= r * 64) break;
+              const uint32_t bw = bwv[u];
+              const float2 bb = bf2(bw), gg = bf2(gwv[u]);
+              uint32_t t3[3];
+              split3(__fdiv_rn(bb.x, gg.x), __fdiv_rn(bb.y, gg.y), t3[0], t3[1], t3[2]);
+              const uint32_t col = (uint32_t)(ch >> 6) * b1_atom + (uint32_t)(ch & 7) * 2, chunk = (uint32_t)(ch & 63) >> 3;
+#pragma unroll
+              for (int term = 0; term < 3; ++term) {
+                const uint32_t nrow = (uint32_t)(j >> 3) * 24 + 8 * term + (j & 7);
+                asm volatile("st.shared.u32 [%0], %1;" ::"r"(b1 + col + nrow * 128 + ((chunk ^ (nrow & 7)) << 4)), "r"(t3[term]) : "memory");
+              }
+              // B2[ch][j] = B[j][ch]
+              asm volatile("st.shared.u16 [%0], %1;" ::"r"(b2 + (uint32_t)ch * 128 + ((((uint32_t)j >> 3) ^ (ch & 7)) << 4) + (j & 7) * 2), "h"((uint16_t)(bw & 0xffff)) : "memory");
+              asm volatile("st.shared.u16 [%0], %1;" ::"r"(b2 + (uint32_t)(ch + 1) * 128 + ((((uint32_t)j >> 3) ^ ((ch + 1) & 7)) << 4) + (j & 7) * 2), "h"((uint16_t)(bw >> 16)) : "memory");
+            }
+          }
+          for (int i = tid; i < (N1 - 3 * r) * 16; i += 128) {     // padding rows 3r .. N1-1 of both atoms
+            const uint32_t nrow = 3 * r + (i >> 4) % (N1 - 3 * r), c16 = i & 15;
+            asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(b1 + (c16 >> 3) * b1_atom + nrow * 128 + ((c16 & 7) << 4)), "r"(0u) : "memory");
+          }
+          for (int i = tid; i < D; i += 128) {
+            const float gv = __bfloat162float(gz[i]);
+            asm volatile("st.shared.f32 [%0], %1;" ::"r"(gam + (uint32_t)(zz * 128 + i) * 4), "f"(gv) : "memory");
+          }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        cu_bar_epi();
+        if (tid == 0) cu_mbar_arrive(basis_ready);
+        cur_lh = lh;
+      }
+      if (z == 0) {
+        // ---- destination of my row and compaction of the tile's flagged rows ---------------------------------------------------
+        rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * tile + tid, p.n_rows, lh);
+        const unsigned bal = __ballot_sync(kFull, rd.flagged());
+        if (lane == 0) wcount_sh[warp] = __popc(bal);
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rows_sh + 16 * tid), "r"((uint32_t)(uintptr_t)rd.blk),
+                     "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)rd.src) : "memory");
+        cu_bar_epi();
+        int pre = 0;
+        n_flag = 0;
+#pragma unroll
+        for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < warp ? cnt : 0; n_flag += cnt; }
+        my_p = pre + __popc(bal & ((1u << lane) - 1u));
+        if (rd.flagged()) asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist + 2 * my_p), "h"((uint16_t)tid) : "memory");
+      }
+      // ---- epilogue 1: coefficients ---------------------------------------------------------------------------------------------
+      cu_mbar_wait(acc_full + 8 * buf, (uint32_t)((idx >> 1) & 1));
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      {
+        const uint32_t taddr = tmem + buf * kCuAccCols + lane_taddr;
+        const bool valid = rd.valid(), fl = rd.flagged();
+        const int rk = rd.rk(), slot = rd.slot(), tb = rd.tb();
+        uint8_t* base = rd.blk + (z ? rd.coef_bytes() : 0);
+#pragma unroll 1
+        for (int b = 0; b < NC; ++b) {
+          float hi[8], mid[8], lo[8];
+          cu_tmem_ld8(taddr + 24 * b, hi);
+          cu_tmem_ld8(taddr + 24 * b + 8, mid);
+          cu_tmem_ld8(taddr + 24 * b + 16, lo);
+          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+          const bool keep = valid && 8 * b < rk;
+          uint32_t wv[4];
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            wv[k] = keep ? pack_bf16x2((lo[2 * k] + mid[2 * k]) + hi[2 * k], (lo[2 * k + 1] + mid[2 * k + 1]) + hi[2 * k + 1]) : 0u;
+          if (keep) {
+            if (z == 0) {
+#pragma unroll
+              for (int k = 0; k < 4; ++k) *reinterpret_cast<uint32_t*>(base + kcoef_elem_off(slot, 8 * b + 2 * k, tb)) = wv[k];
+            } else {
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                *reinterpret_cast<uint16_t*>(base + vcoef_elem_off(slot, 8 * b + 2 * k, tb)) = (uint16_t)(wv[k] & 0xffff);
+                *reinterpret_cast<uint16_t*>(base + vcoef_elem_off(slot, 8 * b + 2 * k + 1, tb)) = (uint16_t)(wv[k] >> 16);
+              }
+            }
+          }
+          if (fl)
+            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a2 + (uint32_t)my_p * 128 + (((uint32_t)b ^ (my_p & 7)) << 4)),
+                         "r"(wv[0]), "r"(wv[1]), "r"(wv[2]), "r"(wv[3]) : "memory");
+        }
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      cu_bar_epi();
+      if (tid == 0) {
+        cu_mbar_arrive(acc_empty + 8 * buf);
+        nflag_sh[idx & 1] = n_flag;
+        cu_mbar_arrive(a2_ready);
+      }
+      // ---- epilogue 2: residual of the flagged rows (compacted: thread p owns flagged row flist[p], rec in TMEM lane p) -----------
+      if (n_flag > 0) {
+        cu_mbar_wait(rec_full, (uint32_t)(n_rec & 1));
+        ++n_rec;
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (32 * warp < n_flag) {                                  // warp-uniform: this warp's lanes hold flagged rows
+          const bool act = tid < n_flag;
+          int q = 0;
+          RowDst rq = rd;
+          if (act) {
+            uint32_t qq, b0, b1w, mt, sr;
+            asm volatile("ld.shared.u16 %0, [%1];" : "=r"(qq) : "r"(flist + 2 * tid));
+            q = (int)qq;
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1w), "=r"(mt), "=r"(sr) : "r"(rows_sh + 16 * q));
+            rq.blk = reinterpret_cast<uint8_t*>((uintptr_t)b0 | ((uintptr_t)b1w << 32)); rq.meta = (int)mt; rq.src = (int)sr;
+          }
+          const uint32_t xrow = xs0 + s * kCuXBytes + (uint32_t)q * 128, taddr = tmem + 2 * kCuAccCols + lane_taddr;
+          const int slot = rq.slot(), sj = slot >> 3, sg = slot & 7;
+          uint8_t* res = rq.blk + 2 * rq.coef_bytes();            // [K code | K scale | V code | V scale], sub-block of 16 slots
+#pragma unroll 1
+          for (int gp = 0; gp < D / 32; ++gp) {                    // pairs of 16-channel groups: channels 32 gp .. + 31
+            float rec[32];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) cu_tmem_ld8(taddr + 32 * gp + 8 * c, *reinterpret_cast<float(*)[8]>(rec + 8 * c));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            if (act) {
+              int code[32];
+              __half sc[2];
+#pragma unroll
+              for (int gg = 0; gg < 2; ++gg) {
+                float e[16];
+                float amax = 0.f;
+#pragma unroll
+                for (int c = 0; c < 2; ++c) {                      // two 8-channel chunks of the group
+                  const int ch0 = 32 * gp + 16 * gg + 8 * c;
+                  uint4 xv, g0, g1;
+                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(xv.x), "=r"(xv.y), "=r"(xv.z), "=r"(xv.w)
+                               : "r"(xrow + (uint32_t)(ch0 >> 6) * 16384 + ((((uint32_t)(ch0 & 63) >> 3) ^ (q & 7)) << 4)));
+                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g0.x), "=r"(g0.y), "=r"(g0.z), "=r"(g0.w) : "r"(gam + (uint32_t)(z * 128 + ch0) * 4));
+                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g1.x), "=r"(g1.y), "=r"(g1.z), "=r"(g1.w) : "r"(gam + (uint32_t)(z * 128 + ch0 + 4) * 4));
+                  const uint32_t xw[4] = {xv.x, xv.y, xv.z, xv.w};
+                  const float gm[8] = {__uint_as_float(g0.x), __uint_as_float(g0.y), __uint_as_float(g0.z), __uint_as_float(g0.w),
+                                       __uint_as_float(g1.x), __uint_as_float(g1.y), __uint_as_float(g1.z), __uint_as_float(g1.w)};
+#pragma unroll
+                  for (int k = 0; k < 4; ++k) {
+                    const float2 xx = bf2(xw[k]);
+                    e[8 * c + 2 * k] = fmaf(-gm[2 * k], rec[16 * gg + 8 * c + 2 * k], xx.x);
+                    e[8 * c + 2 * k + 1] = fmaf(-gm[2 * k + 1], rec[16 * gg + 8 * c + 2 * k + 1], xx.y);
+                    amax = fmaxf(amax, fmaxf(fabsf(e[8 * c + 2 * k]), fabsf(e[8 * c + 2 * k + 1])));
+                  }
+                }
+                sc[gg] = quant_scale(amax);
+                const float sf = __half2float(sc[gg]);
+#pragma unroll
+                for (int i = 0; i < 16; ++i) code[16 * gg + i] = (quant_code(e[i], sf) + 8) & 15;     // offset binary
+              }
+              if (z == 0) {
+                // K codes: word (slot, t) of group pair gp holds, for gg, b, hi: channel 32gp + 16gg + 8b + 2t + hi at bit 4(2gg + b) + 16hi
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                  uint32_t wd = 0u;
+#pragma unroll
+                  for (int gg = 0; gg < 2; ++gg)
+#pragma unroll
+                    for (int b = 0; b < 2; ++b)
+#pragma unroll
+                      for (int hi = 0; hi < 2; ++hi) wd |= (uint32_t)code[16 * gg + 8 * b + 2 * t + hi] << (4 * (2 * gg + b) + 16 * hi);
+                  *reinterpret_cast<uint32_t*>(res + sj * 4 * D + (4 * sg + t) * (D / 8) + 4 * gp) = wd;
+                }
+#pragma unroll
+                for (int gg = 0; gg < 2; ++gg) *reinterpret_cast<__half*>(res + 8 * D + scale_elem_off(slot, 2 * gp + gg, D)) = sc[gg];
+              } else {
+                // V codes: byte (2 * hi + tile) of word (4 * gch + ts) * (D / 4) + 4 * grp holds channels gch (low nibble) and gch + 8
+                const int ts = sg >> 1, hs = sg & 1;
+#pragma unroll
+                for (int gg = 0; gg < 2; ++gg) {
+                  uint8_t* cv = res + 10 * D + 4 * (2 * gp + gg) + 2 * hs + sj;
+#pragma unroll
+                  for (int gch = 0; gch < 8; ++gch) cv[(4 * gch + ts) * (D / 4)] = (uint8_t)(code[16 * gg + gch] | (code[16 * gg + 8 + gch] << 4));
+                  *reinterpret_cast<__half*>(res + 18 * D + scale_elem_off(slot, 2 * gp + gg, D)) = sc[gg];
+                }
+              }
+            }
+          }
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      }
+      cu_bar_epi();
+      if (tid == 0) cu_mbar_arrive(x_empty + 8 * s);              // the token stage (read by MMA 1 and by epilogue 2) is free
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
+}
+
+typedef CUresult (*CuEncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool cu_make_row_map(CUtensorMap* m, const void* base, uint64_t LH, uint64_t rows) {     // dims (128 channels, LH, rows), box (64, 1, 128)
+  static CuEncodeTiledFn fn = [] {
+    void* q = nullptr;
+    cudaDriverEntryPointQueryResult st;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &q, cudaEnableDefault, &st) != cudaSuccess || st != cudaDriverEntryPointSuccess) q = nullptr;
+    return (CuEncodeTiledFn)q;
+  }();
+  if (!fn) return false;
+  const cuuint64_t dims[3] = {128, LH, rows}, strides[2] = {256, LH * 256};
+  const cuuint32_t box[3] = {64, 1, 128}, es[3] = {1, 1, 1};
+  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 }  // namespace
+
+bool compress_umma_supported(const CacheGeom& g, const void* k_new, const void* v_new) {
+  return g.d == 128 && g.r <= 64 && ((((uintptr_t)k_new | (uintptr_t)v_new) & 15) == 0);
+}
+
+// rows [row0, row0 + n_rows) of k_new / v_new (total_rows rows in all), dst = their destinations in row order (not sorted)
+int launch_compress_umma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n_rows, int row0, long long total_rows,
+                         const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
+                         const __nv_bfloat16* gK, const __nv_bfloat16* gV, int n_sms, cudaStream_t s) {
+  if (n_rows <= 0) return 0;
+  CUtensorMap mapK, mapV;
+  const uint64_t LH = (uint64_t)g.L * g.H;
+  if (!cu_make_row_map(&mapK, k_new, LH, (uint64_t)total_rows) || !cu_make_row_map(&mapV, v_new, LH, (uint64_t)total_rows)) return 0;
+  CuParams p;
+  p.arena = arena; p.dst = dst; p.BK = BK; p.BV = BV; p.gK = gK; p.gV = gV; p.n_rows = n_rows; p.row0 = row0;
+  p.N1 = (3 * g.r + 15) / 16 * 16;
+  p.ranks4 = (uint32_t)g.tier_rank[0] | ((uint32_t)g.tier_rank[1] << 8) | ((uint32_t)g.tier_rank[2] << 16) | ((uint32_t)g.tier_rank[3] << 24);
+  p.g = g;
+  const size_t smem = 1024 + (size_t)kCuS * kCuXBytes + (size_t)4 * p.N1 * 128 + 2 * 16384 + 16384 + 1024 + 256 + 2048;
+  const long long items = (long long)LH * ((n_rows + 127) / 128);
+  const int grid = (int)std::max<long long>(1, std::min<long long>(n_sms, items));
+  cudaFuncSetAttribute(compress_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  compress_umma_kernel<<<grid, 192, smem, s>>>(mapK, mapV, p);
+  return 1;
+}
 
 int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const CompressRuns& runs, const __nv_bfloat16* k_new,
                         const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK,
