@@ -404,10 +404,12 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
 //   tile   = 128 consecutive rows of the call (no sorting: a thread of the epilogue owns one token row = one TMEM lane)
 //   MMA 1  : acc[128 x N1] = X[128 x 128] . B1^T, B1 = the three bf16 terms of B' = B / g as separate output columns, ordered
 //            [chunk b][term][8 columns] so that one chunk's lo / mid / hi partial sums are three 8-column TMEM loads; N1 = 3r (to 16)
-//   epi 1  : c = bf16((lo + mid) + hi), tier mask, fragment-native coefficient stores; the rows of FLAGGED tokens are written,
-//            compacted to the front, into the A operand of MMA 2
+//   epi 1  : c = bf16((lo + mid) + hi), tier mask, fragment-native coefficient stores; the rows of FLAGGED tokens join a batch:
+//            coefficients into the A operand of MMA 2, token row and destination into side buffers. The batch (<= 128 rows, gathered
+//            over the tiles of one (layer, head, Z) run) is flushed when the run ends or the next tile's flagged rows would not fit
 //   MMA 2  : rec[p x 128] = c[p x 64] . B2^T, B2 = the transposed basis padded to 64 ranks
-//   epi 2  : thread p < n_flagged: e = x - g * rec (x from the token tile in shared memory), int4 quantiser A14, code / scale stores
+//   epi 2  : thread p < batch rows: e = x - g * rec, int4 quantiser A14, code / scale stores (one thread per row: batching over
+//            tiles is what keeps all 128 threads busy -- a single tile has only a handful of flagged rows)
 // Warps 0-3: epilogue (and the per-(layer, head) staging of B1 / B2); warp 4 lane 0: TMA producer (two 64-channel halves of 128
 // token rows per (tile, Z), hardware 128-byte swizzle); warp 5 lane 0: MMA issuer. mbarrier rings: x_full / x_empty (token
 // stages), acc_full / acc_empty (two accumulators), a2_ready / rec_full (second product), basis_ready (operands of a new (l, h)).
@@ -453,6 +455,20 @@ __device__ __forceinline__ void cu_tmem_ld8(uint32_t taddr, float (&v)[8]) {
 }
 __device__ __forceinline__ void cu_bar_epi() { asm volatile("bar.sync 1, 128;" ::: "memory"); }      // the 128 epilogue threads
 
+// the steps of a CTA: its (layer-head, tile) items [item0, item1), per layer-head first all tiles for K, then all for V
+struct CuIter {
+  int n_tiles, left, lh, z, tile, ta, tb;
+  __device__ CuIter(int item0, int item1, int nt) : n_tiles(nt), left(item1 - item0), lh(item0 / nt), z(0) {
+    ta = item0 - lh * nt; tb = min(nt, ta + left); tile = ta;
+  }
+  __device__ bool last_of_run() const { return tile == tb - 1; }
+  __device__ void next() {
+    if (++tile < tb) return;
+    if (z == 0) { z = 1; tile = ta; return; }
+    left -= tb - ta; ++lh; z = 0; ta = 0; tb = min(n_tiles, left); tile = 0;
+  }
+};
+
 struct CuParams {
   const uint8_t* arena;
   const TokDst* dst;            // row order of the call's chunk (unsorted): row i of the chunk = global row row0 + i
@@ -470,7 +486,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t bars[2 * kCuS + 7];
   __shared__ uint32_t tmem_base_sh;
-  __shared__ int nflag_sh[2], wcount_sh[4];
+  __shared__ int nflag_sh[2], wcount_sh[8];
   const CacheGeom& g = p.g;
   const int r = g.r, N1 = p.N1, LH = g.L * g.H, NC = r / 8;
   const uint32_t sm = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
@@ -507,61 +523,65 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
   if (warp == 4) {
     // ===== TMA producer =========================================================================================================
     if (lane == 0) {
-      for (int idx = 0; idx < n_idx; ++idx) {
-        const int item = item0 + (idx >> 1), z = idx & 1, s = idx % kCuS;
-        const int lh = item / n_tiles, tile = item - lh * n_tiles;
+      CuIter it(item0, item1, n_tiles);
+      for (int idx = 0; idx < n_idx; ++idx, it.next()) {
+        const int s = idx % kCuS;
         if (idx >= kCuS) cu_mbar_wait(x_empty + 8 * s, (uint32_t)(((idx / kCuS) - 1) & 1));
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(x_full + 8 * s), "r"((uint32_t)kCuXBytes) : "memory");
-        const CUtensorMap* map = z ? &mapV : &mapK;
-        cu_tma_3d(xs0 + s * kCuXBytes, map, x_full + 8 * s, 0, lh, p.row0 + 128 * tile);
-        cu_tma_3d(xs0 + s * kCuXBytes + 16384, map, x_full + 8 * s, 64, lh, p.row0 + 128 * tile);
+        const CUtensorMap* map = it.z ? &mapV : &mapK;
+        cu_tma_3d(xs0 + s * kCuXBytes, map, x_full + 8 * s, 0, it.lh, p.row0 + 128 * it.tile);
+        cu_tma_3d(xs0 + s * kCuXBytes + 16384, map, x_full + 8 * s, 64, it.lh, p.row0 + 128 * it.tile);
       }
     }
   } else if (warp == 5) {
     // ===== MMA issuer ===========================================================================================================
     if (lane == 0) {
-      int n_seg = 0, n_rec = 0, cur_lh = -1;
+      int n_seg = 0, cur_lh = -1;
+      CuIter it(item0, item1, n_tiles);          // the step MMA 1 is issued for next
       auto mma1 = [&](int idx) {
-        const int item = item0 + (idx >> 1), z = idx & 1, s = idx % kCuS, buf = idx & 1;
-        const int lh = item / n_tiles;
-        if (lh != cur_lh) { cu_mbar_wait(basis_ready, (uint32_t)(n_seg & 1)); ++n_seg; cur_lh = lh; }
+        const int s = idx % kCuS, buf = idx & 1;
+        if (it.lh != cur_lh) { cu_mbar_wait(basis_ready, (uint32_t)(n_seg & 1)); ++n_seg; cur_lh = it.lh; }
         cu_mbar_wait(x_full + 8 * s, (uint32_t)((idx / kCuS) & 1));
         if (idx >= 2) cu_mbar_wait(acc_empty + 8 * buf, (uint32_t)(((idx >> 1) - 1) & 1));
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t xs = xs0 + s * kCuXBytes, b1 = b1_0 + (uint32_t)(2 * z) * b1_atom;
+        const uint32_t xs = xs0 + s * kCuXBytes, b1 = b1_0 + (uint32_t)(2 * it.z) * b1_atom;
 #pragma unroll
         for (int k = 0; k < 8; ++k)       // channels 16k .. 16k+15: atom k / 4, 32 bytes per step inside the swizzled 128-byte rows
           cu_mma(tmem + buf * kCuAccCols, cu_desc(xs + (k >> 2) * 16384 + 32 * (k & 3)), cu_desc(b1 + (k >> 2) * b1_atom + 32 * (k & 3)), idesc1, k > 0);
         cu_commit(acc_full + 8 * buf);
+        it.next();
       };
-      if (n_idx > 0) mma1(0);
+      int z_cur = 0;
+      if (n_idx > 0) { z_cur = it.z; mma1(0); }
       for (int idx = 0; idx < n_idx; ++idx) {
-        const int z = idx & 1;
-        const bool same_lh = idx + 1 < n_idx && ((item0 + ((idx + 1) >> 1)) / n_tiles) == cur_lh;
-        if (same_lh) mma1(idx + 1);                  // run ahead into the other accumulator while the epilogue of idx works
+        const int z_this = z_cur;
+        const bool more = idx + 1 < n_idx, same_lh = more && it.lh == cur_lh;
+        if (same_lh) { z_cur = it.z; mma1(idx + 1); }      // run ahead into the other accumulator while the epilogue of idx works
         cu_mbar_wait(a2_ready, (uint32_t)(idx & 1));
-        if (nflag_sh[idx & 1] > 0) {
+        if (nflag_sh[idx & 1] > 0) {                       // the epilogue flushes its batch of flagged rows: rec = c . B2^T
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-          const uint32_t b2 = b2_0 + (uint32_t)z * 16384;
+          const uint32_t b2 = b2_0 + (uint32_t)z_this * 16384;
 #pragma unroll
           for (int k = 0; k < 4; ++k) cu_mma(tmem + 2 * kCuAccCols, cu_desc(a2 + 32 * k), cu_desc(b2 + 32 * k), idesc2, k > 0);
           cu_commit(rec_full);
-          ++n_rec;
         }
-        if (!same_lh && idx + 1 < n_idx) mma1(idx + 1);     // a new (layer, head): its operands are staged only after idx is finished
+        if (!same_lh && more) { z_cur = it.z; mma1(idx + 1); }     // a new (layer, head): staged only after idx is finished
       }
-      (void)n_rec;
     }
   } else {
     // ===== epilogue warps (128 threads = TMEM lanes) ============================================================================
-    const uint32_t rows_sh = flist + 256;                       // RowDst of the tile's 128 rows (16 bytes each)
-    int cur_lh = -1, n_rec = 0, n_flag = 0, my_p = 0;
-    RowDst rd;
-    rd.blk = nullptr; rd.meta = 0; rd.src = 0;
+    const uint32_t xbuf = flist + 256 + 2048;                   // token rows (256 bytes, unswizzled) of the batch of flagged rows
+    const uint32_t rows_sh = flist + 256;                       // RowDst (16 bytes) of the batch of flagged rows
+    int cur_lh = -1, n_rec = 0, nb = 0;                         // nb = flagged rows waiting in the batch (CTA-uniform)
     const uint32_t lane_taddr = (uint32_t)(32 * warp) << 16;
+    CuIter it(item0, item1, n_tiles);
+    // destination of my row in the current and in the next step (the table read of the next step is off the critical path)
+    RowDst rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh), rn = rd;
     for (int idx = 0; idx < n_idx; ++idx) {
-      const int item = item0 + (idx >> 1), z = idx & 1, s = idx % kCuS, buf = idx & 1;
-      const int lh = item / n_tiles, tile = item - lh * n_tiles;
+      const int z = it.z, lh = it.lh, s = idx % kCuS, buf = idx & 1;
+      const bool last_of_run = it.last_of_run();
+      it.next();
+      if (idx + 1 < n_idx) rn = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh);
       if (lh != cur_lh) {
         // ---- operands of this (layer, head): B1 = three-term split of B / g in [chunk][term][8] row order, B2 = B^T, gates ------
         const int l = lh / g.H, h = lh - l * g.H;
@@ -611,21 +631,14 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         if (tid == 0) cu_mbar_arrive(basis_ready);
         cur_lh = lh;
       }
-      if (z == 0) {
-        // ---- destination of my row and compaction of the tile's flagged rows ---------------------------------------------------
-        rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * tile + tid, p.n_rows, lh);
-        const unsigned bal = __ballot_sync(kFull, rd.flagged());
-        if (lane == 0) wcount_sh[warp] = __popc(bal);
-        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rows_sh + 16 * tid), "r"((uint32_t)(uintptr_t)rd.blk),
-                     "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)rd.src) : "memory");
-        cu_bar_epi();
-        int pre = 0;
-        n_flag = 0;
+      // ---- positions of this tile's flagged rows in the batch, and the flagged count of the next tile ---------------------------
+      const unsigned bal = __ballot_sync(kFull, rd.flagged()), baln = __ballot_sync(kFull, idx + 1 < n_idx && rn.flagged());
+      if (lane == 0) { wcount_sh[warp] = __popc(bal); wcount_sh[4 + warp] = __popc(baln); }
+      cu_bar_epi();
+      int pre = 0, n_flag = 0, n_flag_next = 0;
 #pragma unroll
-        for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < warp ? cnt : 0; n_flag += cnt; }
-        my_p = pre + __popc(bal & ((1u << lane) - 1u));
-        if (rd.flagged()) asm volatile("st.shared.u16 [%0], %1;" ::"r"(flist + 2 * my_p), "h"((uint16_t)tid) : "memory");
-      }
+      for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < warp ? cnt : 0; n_flag += cnt; n_flag_next += wcount_sh[4 + ww]; }
+      const int my_p = nb + pre + __popc(bal & ((1u << lane) - 1u));      // nb + n_flag <= 128 by the flush rule below
       // ---- epilogue 1: coefficients ---------------------------------------------------------------------------------------------
       cu_mbar_wait(acc_full + 8 * buf, (uint32_t)((idx >> 1) & 1));
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -662,32 +675,45 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
             asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a2 + (uint32_t)my_p * 128 + (((uint32_t)b ^ (my_p & 7)) << 4)),
                          "r"(wv[0]), "r"(wv[1]), "r"(wv[2]), "r"(wv[3]) : "memory");
         }
+        if (fl) {      // a flagged row joins the batch: its token row (un-swizzled) and its destination
+          const uint32_t xrow = xs0 + s * kCuXBytes + (uint32_t)tid * 128;
+#pragma unroll
+          for (int c16 = 0; c16 < 16; ++c16) {
+            uint4 v;
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                         : "r"(xrow + (uint32_t)(c16 >> 3) * 16384 + ((((uint32_t)c16 & 7) ^ (tid & 7)) << 4)));
+            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(xbuf + (uint32_t)my_p * 256 + 16 * c16), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+          }
+          asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rows_sh + 16 * my_p), "r"((uint32_t)(uintptr_t)rd.blk),
+                       "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)rd.src) : "memory");
+        }
       }
+      nb += n_flag;
+      // flush the batch through MMA 2 when the (layer, head, Z) run ends or the next tile's flagged rows would not fit
+      const int flush = (nb > 0 && (last_of_run || nb + n_flag_next > 128)) ? nb : 0;
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       cu_bar_epi();
       if (tid == 0) {
         cu_mbar_arrive(acc_empty + 8 * buf);
-        nflag_sh[idx & 1] = n_flag;
+        cu_mbar_arrive(x_empty + 8 * s);                          // the token stage was read by MMA 1 and copied from: free
+        nflag_sh[idx & 1] = flush;
         cu_mbar_arrive(a2_ready);
       }
-      // ---- epilogue 2: residual of the flagged rows (compacted: thread p owns flagged row flist[p], rec in TMEM lane p) -----------
-      if (n_flag > 0) {
+      // ---- epilogue 2: residuals of the batch (thread p owns batch row p; its rec is in TMEM lane p) ------------------------------
+      if (flush > 0) {
         cu_mbar_wait(rec_full, (uint32_t)(n_rec & 1));
         ++n_rec;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        if (32 * warp < n_flag) {                                  // warp-uniform: this warp's lanes hold flagged rows
-          const bool act = tid < n_flag;
-          int q = 0;
+        if (32 * warp < flush) {                                   // warp-uniform: this warp's lanes hold batch rows
+          const bool act = tid < flush;
           RowDst rq = rd;
           if (act) {
-            uint32_t qq, b0, b1w, mt, sr;
-            asm volatile("ld.shared.u16 %0, [%1];" : "=r"(qq) : "r"(flist + 2 * tid));
-            q = (int)qq;
-            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1w), "=r"(mt), "=r"(sr) : "r"(rows_sh + 16 * q));
+            uint32_t b0, b1w, mt, sr;
+            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1w), "=r"(mt), "=r"(sr) : "r"(rows_sh + 16 * tid));
             rq.blk = reinterpret_cast<uint8_t*>((uintptr_t)b0 | ((uintptr_t)b1w << 32)); rq.meta = (int)mt; rq.src = (int)sr;
           }
-          const uint32_t xrow = xs0 + s * kCuXBytes + (uint32_t)q * 128, taddr = tmem + 2 * kCuAccCols + lane_taddr;
+          const uint32_t xrow = xbuf + (uint32_t)tid * 256, taddr = tmem + 2 * kCuAccCols + lane_taddr;
           const int slot = rq.slot(), sj = slot >> 3, sg = slot & 7;
           uint8_t* res = rq.blk + 2 * rq.coef_bytes();            // [K code | K scale | V code | V scale], sub-block of 16 slots
 #pragma unroll 1
@@ -707,8 +733,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
                 for (int c = 0; c < 2; ++c) {                      // two 8-channel chunks of the group
                   const int ch0 = 32 * gp + 16 * gg + 8 * c;
                   uint4 xv, g0, g1;
-                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(xv.x), "=r"(xv.y), "=r"(xv.z), "=r"(xv.w)
-                               : "r"(xrow + (uint32_t)(ch0 >> 6) * 16384 + ((((uint32_t)(ch0 & 63) >> 3) ^ (q & 7)) << 4)));
+                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(xv.x), "=r"(xv.y), "=r"(xv.z), "=r"(xv.w) : "r"(xrow + 2 * ch0));
                   asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g0.x), "=r"(g0.y), "=r"(g0.z), "=r"(g0.w) : "r"(gam + (uint32_t)(z * 128 + ch0) * 4));
                   asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g1.x), "=r"(g1.y), "=r"(g1.z), "=r"(g1.w) : "r"(gam + (uint32_t)(z * 128 + ch0 + 4) * 4));
                   const uint32_t xw[4] = {xv.x, xv.y, xv.z, xv.w};
@@ -757,9 +782,10 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
           }
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        cu_bar_epi();                                               // the batch buffers and the rec columns are free again
+        nb = 0;
       }
-      cu_bar_epi();
-      if (tid == 0) cu_mbar_arrive(x_empty + 8 * s);              // the token stage (read by MMA 1 and by epilogue 2) is free
+      rd = rn;
     }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -786,7 +812,7 @@ bool cu_make_row_map(CUtensorMap* m, const void* base, uint64_t LH, uint64_t row
 }  // namespace
 
 bool compress_umma_supported(const CacheGeom& g, const void* k_new, const void* v_new) {
-  return g.d == 128 && g.r <= 64 && ((((uintptr_t)k_new | (uintptr_t)v_new) & 15) == 0);
+  return g.d == 128 && g.r <= 48 && ((((uintptr_t)k_new | (uintptr_t)v_new) & 15) == 0);
 }
 
 // rows [row0, row0 + n_rows) of k_new / v_new (total_rows rows in all), dst = their destinations in row order (not sorted)
@@ -802,7 +828,7 @@ int launch_compress_umma(const uint8_t* arena, const CacheGeom& g, const TokDst*
   p.N1 = (3 * g.r + 15) / 16 * 16;
   p.ranks4 = (uint32_t)g.tier_rank[0] | ((uint32_t)g.tier_rank[1] << 8) | ((uint32_t)g.tier_rank[2] << 16) | ((uint32_t)g.tier_rank[3] << 24);
   p.g = g;
-  const size_t smem = 1024 + (size_t)kCuS * kCuXBytes + (size_t)4 * p.N1 * 128 + 2 * 16384 + 16384 + 1024 + 256 + 2048;
+  const size_t smem = 1024 + (size_t)kCuS * kCuXBytes + (size_t)4 * p.N1 * 128 + 2 * 16384 + 16384 + 1024 + 256 + 2048 + 32768;
   const long long items = (long long)LH * ((n_rows + 127) / 128);
   const int grid = (int)std::max<long long>(1, std::min<long long>(n_sms, items));
   cudaFuncSetAttribute(compress_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
