@@ -132,12 +132,14 @@ constexpr int kUmmaStageBytes = kUmmaXBytes + kUmmaOBytes;
 __device__ __forceinline__ void umma_mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void umma_mbar_wait(uint32_t bar, uint32_t parity) {     // bounded: a protocol error traps instead of hanging the GPU
+__device__ __forceinline__ void umma_mbar_wait(uint32_t bar, uint32_t parity) {
+  // bounded (about 10 s with the back-off): a protocol error traps instead of hanging the GPU
   for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
     uint32_t ok;
     asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     if (ok) return;
+    if (spin > 4096) __nanosleep(128);
   }
   __trap();
 }

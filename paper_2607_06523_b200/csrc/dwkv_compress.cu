@@ -74,10 +74,8 @@ struct RowDst {          // destination of one token row of the tile for this (l
 };
 
 // the ClassLayout arithmetic of dwkv_layout.cuh with shifts only (tb is 2 or 4); tier ranks come as 4 bytes of one word
-__device__ __forceinline__ RowDst row_dst(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst* dst, int tok, int n_tok, int lh) {
+__device__ __forceinline__ RowDst row_dst_from(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst& td, const bool valid, int lh) {
   RowDst r;
-  const bool valid = tok < n_tok;
-  const TokDst td = dst[valid ? tok : 0];
   const int resid = td.cls & 1;
   const int rk = (ranks4 >> (8 * (td.cls >> 1))) & 0xff;
   const int tb = resid ? 2 : 4;
@@ -89,6 +87,11 @@ __device__ __forceinline__ RowDst row_dst(const uint8_t* arena, const uint32_t r
           ((resid && td.slot >= 16) ? sub_bytes : 0);
   r.meta = (resid ? (td.slot & 15) : td.slot) | (rk << 8) | ((int)valid << 16) | ((int)(valid && resid) << 17);
   return r;
+}
+__device__ __forceinline__ RowDst row_dst(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst* dst, int tok, int n_tok, int lh) {
+  const bool valid = tok < n_tok;
+  const TokDst td = dst[valid ? tok : 0];
+  return row_dst_from(arena, ranks4, d, td, valid, lh);
 }
 
 // item position in cost space -> (layer-head, tile). Per layer-head the tiles come in runs of equal cost (CompressRuns).
@@ -413,7 +416,7 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
 // Warps 0-3: epilogue (and the per-(layer, head) staging of B1 / B2); warp 4 lane 0: TMA producer (two 64-channel halves of 128
 // token rows per (tile, Z), hardware 128-byte swizzle); warp 5 lane 0: MMA issuer. mbarrier rings: x_full / x_empty (token
 // stages), acc_full / acc_empty (two accumulators), a2_ready / rec_full (second product), basis_ready (operands of a new (l, h)).
-constexpr int kCuS = 2;                               // token stages of 32 KB
+constexpr int kCuS = 3;                               // token stages of 32 KB
 constexpr int kCuXBytes = 32768;
 constexpr int kCuAccCols = 192;                       // columns reserved per projection accumulator (N1 <= 192)
 
@@ -423,12 +426,14 @@ __device__ __forceinline__ void cu_mbar_init(uint32_t bar, uint32_t count) {
 __device__ __forceinline__ void cu_mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void cu_mbar_wait(uint32_t bar, uint32_t parity) {     // bounded: a protocol error traps instead of hanging
-  for (uint32_t spin = 0; spin < (1u << 27); ++spin) {
+__device__ __forceinline__ void cu_mbar_wait(uint32_t bar, uint32_t parity) {
+  // bounded (about 10 s with the back-off): a protocol error traps instead of hanging the GPU
+  for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
     uint32_t ok;
     asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     if (ok) return;
+    if (spin > 4096) __nanosleep(128);
   }
   __trap();
 }
@@ -472,7 +477,7 @@ struct CuIter {
 struct CuParams {
   const uint8_t* arena;
   const TokDst* dst;            // row order of the call's chunk (unsorted): row i of the chunk = global row row0 + i
-  const __nv_bfloat16 *BK, *BV, *gK, *gV;
+  const __nv_bfloat16 *BK, *BV, *gK, *gV, *k_new, *v_new;
   int n_rows;                   // rows of this chunk
   int row0;                     // first global row of the chunk in k_new / v_new
   int N1;                       // 3 r rounded up to 16
@@ -549,6 +554,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         for (int k = 0; k < 8; ++k)       // channels 16k .. 16k+15: atom k / 4, 32 bytes per step inside the swizzled 128-byte rows
           cu_mma(tmem + buf * kCuAccCols, cu_desc(xs + (k >> 2) * 16384 + 32 * (k & 3)), cu_desc(b1 + (k >> 2) * b1_atom + 32 * (k & 3)), idesc1, k > 0);
         cu_commit(acc_full + 8 * buf);
+        cu_commit(x_empty + 8 * s);           // the token stage is free as soon as these products have read it
         it.next();
       };
       int z_cur = 0;
@@ -570,18 +576,20 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
     }
   } else {
     // ===== epilogue warps (128 threads = TMEM lanes) ============================================================================
-    const uint32_t xbuf = flist + 256 + 2048;                   // token rows (256 bytes, unswizzled) of the batch of flagged rows
     const uint32_t rows_sh = flist + 256;                       // RowDst (16 bytes) of the batch of flagged rows
     int cur_lh = -1, n_rec = 0, nb = 0;                         // nb = flagged rows waiting in the batch (CTA-uniform)
     const uint32_t lane_taddr = (uint32_t)(32 * warp) << 16;
     CuIter it(item0, item1, n_tiles);
     // destination of my row in the current and in the next step (the table read of the next step is off the critical path)
-    RowDst rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh), rn = rd;
+    RowDst rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh);
     for (int idx = 0; idx < n_idx; ++idx) {
-      const int z = it.z, lh = it.lh, s = idx % kCuS, buf = idx & 1;
+      const int z = it.z, lh = it.lh, tile_cur = it.tile, buf = idx & 1;
       const bool last_of_run = it.last_of_run();
       it.next();
-      if (idx + 1 < n_idx) rn = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh);
+      // the table row of the next step: the load is issued here, its first use is at the end of this step
+      const bool more = idx + 1 < n_idx, vn = more && 128 * it.tile + tid < p.n_rows;
+      const TokDst tdn = p.dst[vn ? 128 * it.tile + tid : 0];
+      const int lh_next = it.lh;
       if (lh != cur_lh) {
         // ---- operands of this (layer, head): B1 = three-term split of B / g in [chunk][term][8] row order, B2 = B^T, gates ------
         const int l = lh / g.H, h = lh - l * g.H;
@@ -632,12 +640,12 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         cur_lh = lh;
       }
       // ---- positions of this tile's flagged rows in the batch, and the flagged count of the next tile ---------------------------
-      const unsigned bal = __ballot_sync(kFull, rd.flagged()), baln = __ballot_sync(kFull, idx + 1 < n_idx && rn.flagged());
-      if (lane == 0) { wcount_sh[warp] = __popc(bal); wcount_sh[4 + warp] = __popc(baln); }
+      const unsigned bal = __ballot_sync(kFull, rd.flagged());
+      if (lane == 0) wcount_sh[warp] = __popc(bal);
       cu_bar_epi();
-      int pre = 0, n_flag = 0, n_flag_next = 0;
+      int pre = 0, n_flag = 0;
 #pragma unroll
-      for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < warp ? cnt : 0; n_flag += cnt; n_flag_next += wcount_sh[4 + ww]; }
+      for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < warp ? cnt : 0; n_flag += cnt; }
       const int my_p = nb + pre + __popc(bal & ((1u << lane) - 1u));      // nb + n_flag <= 128 by the flush rule below
       // ---- epilogue 1: coefficients ---------------------------------------------------------------------------------------------
       cu_mbar_wait(acc_full + 8 * buf, (uint32_t)((idx >> 1) & 1));
@@ -675,28 +683,23 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
             asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a2 + (uint32_t)my_p * 128 + (((uint32_t)b ^ (my_p & 7)) << 4)),
                          "r"(wv[0]), "r"(wv[1]), "r"(wv[2]), "r"(wv[3]) : "memory");
         }
-        if (fl) {      // a flagged row joins the batch: its token row (un-swizzled) and its destination
-          const uint32_t xrow = xs0 + s * kCuXBytes + (uint32_t)tid * 128;
-#pragma unroll
-          for (int c16 = 0; c16 < 16; ++c16) {
-            uint4 v;
-            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
-                         : "r"(xrow + (uint32_t)(c16 >> 3) * 16384 + ((((uint32_t)c16 & 7) ^ (tid & 7)) << 4)));
-            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(xbuf + (uint32_t)my_p * 256 + 16 * c16), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-          }
+        if (fl)        // a flagged row joins the batch: its destination and its row index in k_new / v_new (re-read from L2 at the flush)
           asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rows_sh + 16 * my_p), "r"((uint32_t)(uintptr_t)rd.blk),
-                       "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)rd.src) : "memory");
-        }
+                       "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)(p.row0 + 128 * tile_cur + tid)) : "memory");
       }
       nb += n_flag;
-      // flush the batch through MMA 2 when the (layer, head, Z) run ends or the next tile's flagged rows would not fit
-      const int flush = (nb > 0 && (last_of_run || nb + n_flag_next > 128)) ? nb : 0;
+      {   // flagged rows of the next tile (first use of the table row loaded at the top of the step)
+        const unsigned baln = __ballot_sync(kFull, vn && tdn.ridx >= 0);
+        if (lane == 0) wcount_sh[4 + warp] = __popc(baln);
+      }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       cu_bar_epi();
+      // flush the batch through MMA 2 when the (layer, head, Z) run ends or the next tile's flagged rows would not fit
+      const int n_flag_next = wcount_sh[4] + wcount_sh[5] + wcount_sh[6] + wcount_sh[7];
+      const int flush = (nb > 0 && (last_of_run || nb + n_flag_next > 128)) ? nb : 0;
       if (tid == 0) {
         cu_mbar_arrive(acc_empty + 8 * buf);
-        cu_mbar_arrive(x_empty + 8 * s);                          // the token stage was read by MMA 1 and copied from: free
         nflag_sh[idx & 1] = flush;
         cu_mbar_arrive(a2_ready);
       }
@@ -713,11 +716,18 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
             asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1w), "=r"(mt), "=r"(sr) : "r"(rows_sh + 16 * tid));
             rq.blk = reinterpret_cast<uint8_t*>((uintptr_t)b0 | ((uintptr_t)b1w << 32)); rq.meta = (int)mt; rq.src = (int)sr;
           }
-          const uint32_t xrow = xbuf + (uint32_t)tid * 256, taddr = tmem + 2 * kCuAccCols + lane_taddr;
+          const uint4* xg = reinterpret_cast<const uint4*>((z ? p.v_new : p.k_new) + ((size_t)(act ? rq.src : 0) * LH + lh) * D);
+          const uint32_t taddr = tmem + 2 * kCuAccCols + lane_taddr;
           const int slot = rq.slot(), sj = slot >> 3, sg = slot & 7;
           uint8_t* res = rq.blk + 2 * rq.coef_bytes();            // [K code | K scale | V code | V scale], sub-block of 16 slots
+          uint4 xn[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c) xn[c] = __ldg(xg + c);
 #pragma unroll 1
           for (int gp = 0; gp < D / 32; ++gp) {                    // pairs of 16-channel groups: channels 32 gp .. + 31
+            uint4 xc[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { xc[c] = xn[c]; xn[c] = __ldg(xg + 4 * min(gp + 1, D / 32 - 1) + c); }     // next pair's row chunks in flight
             float rec[32];
 #pragma unroll
             for (int c = 0; c < 4; ++c) cu_tmem_ld8(taddr + 32 * gp + 8 * c, *reinterpret_cast<float(*)[8]>(rec + 8 * c));
@@ -733,7 +743,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
                 for (int c = 0; c < 2; ++c) {                      // two 8-channel chunks of the group
                   const int ch0 = 32 * gp + 16 * gg + 8 * c;
                   uint4 xv, g0, g1;
-                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(xv.x), "=r"(xv.y), "=r"(xv.z), "=r"(xv.w) : "r"(xrow + 2 * ch0));
+                  xv = xc[2 * gg + c];
                   asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g0.x), "=r"(g0.y), "=r"(g0.z), "=r"(g0.w) : "r"(gam + (uint32_t)(z * 128 + ch0) * 4));
                   asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g1.x), "=r"(g1.y), "=r"(g1.z), "=r"(g1.w) : "r"(gam + (uint32_t)(z * 128 + ch0 + 4) * 4));
                   const uint32_t xw[4] = {xv.x, xv.y, xv.z, xv.w};
@@ -785,7 +795,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         cu_bar_epi();                                               // the batch buffers and the rec columns are free again
         nb = 0;
       }
-      rd = rn;
+      if (more) rd = row_dst_from(p.arena, p.ranks4, D, tdn, vn, lh_next);
     }
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -824,11 +834,11 @@ int launch_compress_umma(const uint8_t* arena, const CacheGeom& g, const TokDst*
   const uint64_t LH = (uint64_t)g.L * g.H;
   if (!cu_make_row_map(&mapK, k_new, LH, (uint64_t)total_rows) || !cu_make_row_map(&mapV, v_new, LH, (uint64_t)total_rows)) return 0;
   CuParams p;
-  p.arena = arena; p.dst = dst; p.BK = BK; p.BV = BV; p.gK = gK; p.gV = gV; p.n_rows = n_rows; p.row0 = row0;
+  p.arena = arena; p.dst = dst; p.BK = BK; p.BV = BV; p.gK = gK; p.gV = gV; p.k_new = k_new; p.v_new = v_new; p.n_rows = n_rows; p.row0 = row0;
   p.N1 = (3 * g.r + 15) / 16 * 16;
   p.ranks4 = (uint32_t)g.tier_rank[0] | ((uint32_t)g.tier_rank[1] << 8) | ((uint32_t)g.tier_rank[2] << 16) | ((uint32_t)g.tier_rank[3] << 24);
   p.g = g;
-  const size_t smem = 1024 + (size_t)kCuS * kCuXBytes + (size_t)4 * p.N1 * 128 + 2 * 16384 + 16384 + 1024 + 256 + 2048 + 32768;
+  const size_t smem = 1024 + (size_t)kCuS * kCuXBytes + (size_t)4 * p.N1 * 128 + 2 * 16384 + 16384 + 1024 + 256 + 2048;
   const long long items = (long long)LH * ((n_rows + 127) / 128);
   const int grid = (int)std::max<long long>(1, std::min<long long>(n_sms, items));
   cudaFuncSetAttribute(compress_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
