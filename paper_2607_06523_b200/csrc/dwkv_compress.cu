@@ -458,7 +458,9 @@ __device__ __forceinline__ void cu_tmem_ld8(uint32_t taddr, float (&v)[8]) {
 #pragma unroll
   for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
 }
-__device__ __forceinline__ void cu_bar_epi() { asm volatile("bar.sync 1, 128;" ::: "memory"); }      // the 128 epilogue threads
+constexpr int kCuEpiGroups = 2;                       // epilogue warpgroups (each 4 warps = the 4 TMEM lane quadrants)
+constexpr int kCuEpi = 128 * kCuEpiGroups, kCuThreads = kCuEpi + 64;
+__device__ __forceinline__ void cu_bar_epi() { asm volatile("bar.sync 1, %0;" ::"n"(kCuEpi) : "memory"); }      // the epilogue threads
 
 // the steps of a CTA: its (layer-head, tile) items [item0, item1), per layer-head first all tiles for K, then all for V
 struct CuIter {
@@ -485,7 +487,7 @@ struct CuParams {
   CacheGeom g;
 };
 
-__global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
+__global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
                                                                const CuParams p) {
   constexpr int D = 128;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -501,12 +503,13 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
   const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
   const uint32_t x_full = bar0, x_empty = bar0 + 8 * kCuS, acc_full = bar0 + 16 * kCuS, acc_empty = acc_full + 16, a2_ready = acc_empty + 16,
                  rec_full = a2_ready + 8, basis_ready = rec_full + 8;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid_all = threadIdx.x, lane = tid_all & 31, warp = tid_all >> 5;
+  const int tid = tid_all & 127, grp_e = tid_all >> 7;       // epilogue: row / TMEM lane of the thread, and its warpgroup (splits chunks)
   const int n_tiles = (p.n_rows + 127) >> 7;
   const long long items = (long long)LH * n_tiles;
   const int item0 = (int)(items * blockIdx.x / gridDim.x), item1 = (int)(items * (blockIdx.x + 1) / gridDim.x);
   const int n_idx = 2 * (item1 - item0);                     // (item, Z) steps of this CTA
-  if (tid == 0) {
+  if (tid_all == 0) {
     for (int i = 0; i < 2 * kCuS + 7; ++i) cu_mbar_init(bar0 + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mapK) : "memory");
@@ -516,7 +519,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((uint32_t)__cvta_generic_to_shared(&tmem_base_sh)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  for (int i = tid; i < 3 * 16384 / 16; i += 192)            // B2 (both Z) and A2: the ranks >= r stay zero for the whole kernel
+  for (int i = tid_all; i < 3 * 16384 / 16; i += kCuThreads)            // B2 (both Z) and A2: the ranks >= r stay zero for the whole kernel
     asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(b2_0 + 16 * i), "r"(0u) : "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -525,7 +528,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
   const uint32_t tmem = tmem_base_sh;
   const uint32_t idesc1 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N1 >> 3) << 17) | ((128u >> 4) << 24);      // both operands K-major
   const uint32_t idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
-  if (warp == 4) {
+  if (warp == 4 * kCuEpiGroups) {
     // ===== TMA producer =========================================================================================================
     if (lane == 0) {
       CuIter it(item0, item1, n_tiles);
@@ -538,7 +541,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         cu_tma_3d(xs0 + s * kCuXBytes + 16384, map, x_full + 8 * s, 64, it.lh, p.row0 + 128 * it.tile);
       }
     }
-  } else if (warp == 5) {
+  } else if (warp == 4 * kCuEpiGroups + 1) {
     // ===== MMA issuer ===========================================================================================================
     if (lane == 0) {
       int n_seg = 0, cur_lh = -1;
@@ -578,7 +581,8 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
     // ===== epilogue warps (128 threads = TMEM lanes) ============================================================================
     const uint32_t rows_sh = flist + 256;                       // RowDst (16 bytes) of the batch of flagged rows
     int cur_lh = -1, n_rec = 0, nb = 0;                         // nb = flagged rows waiting in the batch (CTA-uniform)
-    const uint32_t lane_taddr = (uint32_t)(32 * warp) << 16;
+    const int wq = warp & 3;                                    // TMEM lane quadrant of this warp
+    const uint32_t lane_taddr = (uint32_t)(32 * wq) << 16;
     CuIter it(item0, item1, n_tiles);
     // destination of my row in the current and in the next step (the table read of the next step is off the critical path)
     RowDst rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh);
@@ -597,18 +601,18 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
           const __nv_bfloat16* B = (zz ? p.BV : p.BK) + ((size_t)(l / g.w) * g.H + h) * (size_t)r * D;
           const __nv_bfloat16* gz = (zz ? p.gV : p.gK) + (size_t)lh * D;
           const uint32_t b1 = b1_0 + (uint32_t)(2 * zz) * b1_atom, b2 = b2_0 + (uint32_t)zz * 16384;
-          for (int i0 = tid; i0 < r * 64; i0 += 128 * 8) {       // 8 (rank, channel pair) items per thread with all loads issued first
+          for (int i0 = tid_all; i0 < r * 64; i0 += kCuEpi * 8) {       // 8 (rank, channel pair) items per thread with all loads issued first
             uint32_t bwv[8], gwv[8];
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
-              const int i = i0 + 128 * u, j = i >> 6, ch = (i & 63) * 2;
+              const int i = i0 + kCuEpi * u, j = i >> 6, ch = (i & 63) * 2;
               const bool ok = i < r * 64;
               bwv[u] = ok ? __ldg(reinterpret_cast<const uint32_t*>(B + (size_t)j * D + ch)) : 0u;
               gwv[u] = ok ? __ldg(reinterpret_cast<const uint32_t*>(gz + ch)) : 0x3f803f80u;
             }
 #pragma unroll
             for (int u = 0; u < 8; ++u) {
-              const int i = i0 + 128 * u, j = i >> 6, ch = (i & 63) * 2;
+              const int i = i0 + kCuEpi * u, j = i >> 6, ch = (i & 63) * 2;
               if (i >= r * 64) break;
               const uint32_t bw = bwv[u];
               const float2 bb = bf2(bw), gg = bf2(gwv[u]);
@@ -625,27 +629,27 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
               asm volatile("st.shared.u16 [%0], %1;" ::"r"(b2 + (uint32_t)(ch + 1) * 128 + ((((uint32_t)j >> 3) ^ ((ch + 1) & 7)) << 4) + (j & 7) * 2), "h"((uint16_t)(bw >> 16)) : "memory");
             }
           }
-          for (int i = tid; i < (N1 - 3 * r) * 16; i += 128) {     // padding rows 3r .. N1-1 of both atoms
+          for (int i = tid_all; i < (N1 - 3 * r) * 16; i += kCuEpi) {     // padding rows 3r .. N1-1 of both atoms
             const uint32_t nrow = 3 * r + (i >> 4) % (N1 - 3 * r), c16 = i & 15;
             asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(b1 + (c16 >> 3) * b1_atom + nrow * 128 + ((c16 & 7) << 4)), "r"(0u) : "memory");
           }
-          for (int i = tid; i < D; i += 128) {
+          for (int i = tid_all; i < D; i += kCuEpi) {
             const float gv = __bfloat162float(gz[i]);
             asm volatile("st.shared.f32 [%0], %1;" ::"r"(gam + (uint32_t)(zz * 128 + i) * 4), "f"(gv) : "memory");
           }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         cu_bar_epi();
-        if (tid == 0) cu_mbar_arrive(basis_ready);
+        if (tid_all == 0) cu_mbar_arrive(basis_ready);
         cur_lh = lh;
       }
       // ---- positions of this tile's flagged rows in the batch, and the flagged count of the next tile ---------------------------
       const unsigned bal = __ballot_sync(kFull, rd.flagged());
-      if (lane == 0) wcount_sh[warp] = __popc(bal);
+      if (lane == 0 && grp_e == 0) wcount_sh[wq] = __popc(bal);
       cu_bar_epi();
       int pre = 0, n_flag = 0;
 #pragma unroll
-      for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < warp ? cnt : 0; n_flag += cnt; }
+      for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < wq ? cnt : 0; n_flag += cnt; }
       const int my_p = nb + pre + __popc(bal & ((1u << lane) - 1u));      // nb + n_flag <= 128 by the flush rule below
       // ---- epilogue 1: coefficients ---------------------------------------------------------------------------------------------
       cu_mbar_wait(acc_full + 8 * buf, (uint32_t)((idx >> 1) & 1));
@@ -656,7 +660,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         const int rk = rd.rk(), slot = rd.slot(), tb = rd.tb();
         uint8_t* base = rd.blk + (z ? rd.coef_bytes() : 0);
 #pragma unroll 1
-        for (int b = 0; b < NC; ++b) {
+        for (int b = grp_e; b < NC; b += kCuEpiGroups) {       // the warpgroups split the rank chunks
           float hi[8], mid[8], lo[8];
           cu_tmem_ld8(taddr + 24 * b, hi);
           cu_tmem_ld8(taddr + 24 * b + 8, mid);
@@ -683,14 +687,14 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
             asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a2 + (uint32_t)my_p * 128 + (((uint32_t)b ^ (my_p & 7)) << 4)),
                          "r"(wv[0]), "r"(wv[1]), "r"(wv[2]), "r"(wv[3]) : "memory");
         }
-        if (fl)        // a flagged row joins the batch: its destination and its row index in k_new / v_new (re-read from L2 at the flush)
+        if (fl && grp_e == 0)        // a flagged row joins the batch: its destination and its row index in k_new / v_new (re-read from L2 at the flush)
           asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rows_sh + 16 * my_p), "r"((uint32_t)(uintptr_t)rd.blk),
                        "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)(p.row0 + 128 * tile_cur + tid)) : "memory");
       }
       nb += n_flag;
       {   // flagged rows of the next tile (first use of the table row loaded at the top of the step)
         const unsigned baln = __ballot_sync(kFull, vn && tdn.ridx >= 0);
-        if (lane == 0) wcount_sh[4 + warp] = __popc(baln);
+        if (lane == 0 && grp_e == 0) wcount_sh[4 + wq] = __popc(baln);
       }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -698,7 +702,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
       // flush the batch through MMA 2 when the (layer, head, Z) run ends or the next tile's flagged rows would not fit
       const int n_flag_next = wcount_sh[4] + wcount_sh[5] + wcount_sh[6] + wcount_sh[7];
       const int flush = (nb > 0 && (last_of_run || nb + n_flag_next > 128)) ? nb : 0;
-      if (tid == 0) {
+      if (tid_all == 0) {
         cu_mbar_arrive(acc_empty + 8 * buf);
         nflag_sh[idx & 1] = flush;
         cu_mbar_arrive(a2_ready);
@@ -708,7 +712,7 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
         cu_mbar_wait(rec_full, (uint32_t)(n_rec & 1));
         ++n_rec;
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        if (32 * warp < flush) {                                   // warp-uniform: this warp's lanes hold batch rows
+        if (32 * wq < flush) {                                   // warp-uniform: this warp's lanes hold batch rows
           const bool act = tid < flush;
           RowDst rq = rd;
           if (act) {
@@ -722,12 +726,12 @@ __global__ void __launch_bounds__(192, 1) compress_umma_kernel(const __grid_cons
           uint8_t* res = rq.blk + 2 * rq.coef_bytes();            // [K code | K scale | V code | V scale], sub-block of 16 slots
           uint4 xn[4];
 #pragma unroll
-          for (int c = 0; c < 4; ++c) xn[c] = __ldg(xg + c);
+          for (int c = 0; c < 4; ++c) xn[c] = __ldg(xg + 4 * grp_e + c);
 #pragma unroll 1
-          for (int gp = 0; gp < D / 32; ++gp) {                    // pairs of 16-channel groups: channels 32 gp .. + 31
+          for (int gp = grp_e; gp < D / 32; gp += kCuEpiGroups) {  // pairs of 16-channel groups (split over the warpgroups): channels 32 gp .. + 31
             uint4 xc[4];
 #pragma unroll
-            for (int c = 0; c < 4; ++c) { xc[c] = xn[c]; xn[c] = __ldg(xg + 4 * min(gp + 1, D / 32 - 1) + c); }     // next pair's row chunks in flight
+            for (int c = 0; c < 4; ++c) { xc[c] = xn[c]; xn[c] = __ldg(xg + 4 * min(gp + kCuEpiGroups, D / 32 - 1) + c); }     // next pair's row chunks in flight
             float rec[32];
 #pragma unroll
             for (int c = 0; c < 4; ++c) cu_tmem_ld8(taddr + 32 * gp + 8 * c, *reinterpret_cast<float(*)[8]>(rec + 8 * c));
@@ -842,7 +846,7 @@ int launch_compress_umma(const uint8_t* arena, const CacheGeom& g, const TokDst*
   const long long items = (long long)LH * ((n_rows + 127) / 128);
   const int grid = (int)std::max<long long>(1, std::min<long long>(n_sms, items));
   cudaFuncSetAttribute(compress_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  compress_umma_kernel<<<grid, 192, smem, s>>>(mapK, mapV, p);
+  compress_umma_kernel<<<grid, kCuThreads, smem, s>>>(mapK, mapV, p);
   return 1;
 }
 
