@@ -491,7 +491,7 @@ __global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __gr
                                                                const CuParams p) {
   constexpr int D = 128;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t bars[2 * kCuS + 7];
+  __shared__ __align__(8) uint64_t bars[2 * kCuS + 8];
   __shared__ uint32_t tmem_base_sh;
   __shared__ int nflag_sh[2], wcount_sh[8];
   const CacheGeom& g = p.g;
@@ -501,8 +501,10 @@ __global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __gr
   const uint32_t xs0 = sm, b1_0 = xs0 + kCuS * kCuXBytes, b1_atom = (uint32_t)N1 * 128, b2_0 = b1_0 + 4 * b1_atom, a2 = b2_0 + 2 * 16384,
                  gam = a2 + 16384, flist = gam + 1024;
   const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
+  // a2_ready is a pair (step parity): the epilogue can post two steps before the MMA thread has looked at the first, and a waiter
+  // may lag an mbarrier by one phase only
   const uint32_t x_full = bar0, x_empty = bar0 + 8 * kCuS, acc_full = bar0 + 16 * kCuS, acc_empty = acc_full + 16, a2_ready = acc_empty + 16,
-                 rec_full = a2_ready + 8, basis_ready = rec_full + 8;
+                 rec_full = a2_ready + 16, basis_ready = rec_full + 8;
   const int tid_all = threadIdx.x, lane = tid_all & 31, warp = tid_all >> 5;
   const int tid = tid_all & 127, grp_e = tid_all >> 7;       // epilogue: row / TMEM lane of the thread, and its warpgroup (splits chunks)
   const int n_tiles = (p.n_rows + 127) >> 7;
@@ -510,7 +512,7 @@ __global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __gr
   const int item0 = (int)(items * blockIdx.x / gridDim.x), item1 = (int)(items * (blockIdx.x + 1) / gridDim.x);
   const int n_idx = 2 * (item1 - item0);                     // (item, Z) steps of this CTA
   if (tid_all == 0) {
-    for (int i = 0; i < 2 * kCuS + 7; ++i) cu_mbar_init(bar0 + 8 * i, 1);
+    for (int i = 0; i < 2 * kCuS + 8; ++i) cu_mbar_init(bar0 + 8 * i, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mapK) : "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&mapV) : "memory");
@@ -566,7 +568,7 @@ __global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __gr
         const int z_this = z_cur;
         const bool more = idx + 1 < n_idx, same_lh = more && it.lh == cur_lh;
         if (same_lh) { z_cur = it.z; mma1(idx + 1); }      // run ahead into the other accumulator while the epilogue of idx works
-        cu_mbar_wait(a2_ready, (uint32_t)(idx & 1));
+        cu_mbar_wait(a2_ready + 8 * (idx & 1), (uint32_t)((idx >> 1) & 1));
         if (nflag_sh[idx & 1] > 0) {                       // the epilogue flushes its batch of flagged rows: rec = c . B2^T
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
           const uint32_t b2 = b2_0 + (uint32_t)z_this * 16384;
@@ -705,7 +707,7 @@ __global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __gr
       if (tid_all == 0) {
         cu_mbar_arrive(acc_empty + 8 * buf);
         nflag_sh[idx & 1] = flush;
-        cu_mbar_arrive(a2_ready);
+        cu_mbar_arrive(a2_ready + 8 * (idx & 1));
       }
       // ---- epilogue 2: residuals of the batch (thread p owns batch row p; its rec is in TMEM lane p) ------------------------------
       if (flush > 0) {
