@@ -5,6 +5,7 @@ paper and the mathematics fix: special cases that reduce to a library routine (t
 forms, invariants, a hand-derived brute-force case, and hand-derived quantiser vectors.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -221,7 +222,12 @@ def test_p9_hand_derived_case():
     oc.append_raw(0, [1, 0, 1], [0, 0, 1], cK, cV, codeK=codeK, scaleK=scaleK, codeV=codeV, scaleV=scaleV)
     q = np.zeros((1, d)); q[0, 0] = 2 * math.log(2); q[0, 4] = 1.0; q[0, 17] = -4 * math.log(2) / 7
     o = oc.decode_attention(0, 0, q)
-    exp = np.zeros(d); exp[31] = 1.0; exp[28] = 1.5; exp[24] = 0.5; exp[3] = 0.75; exp[20] = -0.1875
+    exp = np.zeros(d)          # the hand-derived output, stored with its derivation under tests/golden/
+    for line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "p9_hand_case.txt")):
+        if line.strip() and not line.startswith("#"):
+            ch, val = line.split()
+            exp[int(ch)] = float(val)
+    assert np.count_nonzero(exp) == 5 and exp[31] == 1.0 and exp[20] == -0.1875
     np.testing.assert_allclose(o[0], exp, rtol=0, atol=1e-14)
 
 
