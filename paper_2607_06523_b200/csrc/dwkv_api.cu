@@ -190,7 +190,13 @@ int route_check(const dwkv_cache* c, int32_t seq, int32_t n, const uint8_t* tier
 void route_commit(dwkv_cache* c, int32_t seq, int32_t n, const uint8_t* tier, const uint8_t* flag, int* ridx_base,
                   std::vector<TokDst>* out, std::vector<int32_t>* new_pages) {
   SeqState& S = c->seqs[seq];
-  S.tier.reserve(S.tier.size() + n); S.flag.reserve(S.flag.size() + n); S.slot.reserve(S.slot.size() + n);
+  {   // one growth step for the whole call, geometric (an exact reserve per call would copy the vectors at every decode step)
+    const size_t want = S.tier.size() + (size_t)n;
+    if (want > S.tier.capacity()) {
+      const size_t cap = std::max(want, 2 * S.tier.capacity());
+      S.tier.reserve(cap); S.flag.reserve(cap); S.slot.reserve(cap);
+    }
+  }
   // per class: page index and position inside the page of the next slot, advanced without divisions in the token loop
   int64_t pi[kMaxClasses], in_page[kMaxClasses];
   for (int k = 0; k < c->n_classes; ++k) {
