@@ -113,6 +113,10 @@ struct Plan3 {                    // plan of the fused persistent decode kernel 
   int n_units = 0, n_slices = 0, n_segs = 0, n_slots = 0;
   size_t off_ustart = 0, off_wentry = 0, off_pstart = 0;
   bool valid = false;
+  // structure of the cached plan (units without their token counts, sub-blocks per unit): an append that opens no new sub-block
+  // leaves the slices, the partial slots and the unit list as they are -- only Unit::ntok changes
+  std::vector<Unit> units;
+  std::vector<int32_t> unsub;
 };
 
 }  // namespace
@@ -658,6 +662,7 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   if (P.valid && P.version == c->version && P.n_lsel == n_lsel && (int)P.seq_ids.size() == n_seqs &&
       std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids))
     return DWKV_OK;
+  const bool same_call = P.valid && P.n_lsel == n_lsel && (int)P.seq_ids.size() == n_seqs && std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids);
   P.valid = false;
   const int LH = n_lsel * c->geom.H;
   const double flag_w = (double)c->opt_flag_cost_pct / 100.0;
@@ -734,6 +739,22 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
     cumB[b + 1] = cumB[b] + seq_cost[b] * LH;
   }
   ustart[n_seqs] = (int32_t)units.size();
+  if (same_call && units.size() == P.units.size() && unsub == P.unsub) {
+    // fast path (the common decode step: a few tokens appended inside existing sub-blocks): same units up to their token counts
+    bool same = true;
+    for (size_t i = 0; i < units.size() && same; ++i) {
+      const Unit &a = units[i], &b = P.units[i];
+      same = a.page_off == b.page_off && a.blk0 == b.blk0 && a.nblk == b.nblk && a.cls == b.cls && a.b == b.b && a.rk == b.rk;
+    }
+    if (same) {
+      int rc = upload(c, c->plan3_dev, units.data(), units.size() * sizeof(Unit), st);     // the unit array is the head of the blob
+      if (rc) return rc;
+      P.units.swap(units);
+      P.version = c->version;
+      P.valid = true;
+      return DWKV_OK;
+    }
+  }
   const int n_units = (int)units.size(), S_total = n_seqs * LH;
   const int Wmax = scan3_num_slices(c->n_sms);
   const int W = c->opt_n_slices > 0 ? (int)std::min<int64_t>(c->opt_n_slices, Wmax) : Wmax;
@@ -804,6 +825,8 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   int rc = upload(c, c->plan3_dev, blob.data(), total, st);
   if (rc) return rc;
   P.n_units = n_units; P.n_slices = NSL; P.n_segs = S_total; P.n_slots = pstart[S_total];
+  P.units.swap(units);
+  P.unsub.swap(unsub);
   P.seq_ids.assign(seq_ids, seq_ids + n_seqs);
   P.n_lsel = n_lsel;
   P.version = c->version;

@@ -619,3 +619,41 @@ def test_page_boundaries_single_class(mod, tier_k, flag_k):
     page = wl.L * wl.H_kv * 65536
     assert fp["reserved_bytes"] == page * sum((T + tpp - 1) // tpp for T in Ts)
     cache.destroy()
+
+
+def test_decode_loop_appends_one_token_per_step(mod):
+    """The decode loop of a server: append one token per sequence, decode, repeat. Most steps open no new sub-block, so the planner
+    only patches the token counts of its cached plan (fast path); some do and rebuild it. Every step is checked against the oracle,
+    all-layer and per-layer."""
+    binding, harness = mod
+    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(200, 77))
+    oc, consts = make_oracle(wl)
+    BK, BV, gK, gV = consts
+    cache, _ = harness.make_cache(wl, n_seqs=2, max_tokens=512)
+    for s in range(2):
+        inp = workload_inputs(wl, s, wl.T[s], device="cuda")
+        oracle_load(oc, s, inp)
+        nf = int(inp["flag"].sum())
+        cache.append_raw(s, inp["tier"], inp["flag"], inp["cK"], inp["cV"], residK=inp["rK"] if nf else None, residV=inp["rV"] if nf else None)
+    rng = np.random.default_rng(9)
+    q = gen.make_q(wl, device="cuda", n_seq=2)
+    for step in range(40):
+        tier = rng.integers(0, 2, 2).astype(np.uint8); flag = (rng.random(2) < 0.3).astype(np.uint8)
+        ks, vs = [], []
+        for s in range(2):
+            k, v = gen.make_dense_kv_chunk(wl, s, 1000 + step, 1, BK.cuda(), BV.cuda(), gK.cuda(), gV.cuda(), device="cuda")
+            ks.append(k); vs.append(v)
+        k_new, v_new = torch.cat(ks).contiguous(), torch.cat(vs).contiguous()
+        cache.append_compress([0, 1], [1, 1], k_new, v_new, tier, flag)
+        for s in range(2):
+            oc.append_compress(s, f64(k_new[s:s + 1]), f64(v_new[s:s + 1]), tier[s:s + 1], flag[s:s + 1])
+        out = cache.decode_attention(-1, [0, 1], q).double().cpu().numpy()
+        if step % 4 == 3 or step < 3:
+            ref = oc.decode_all_layers([0, 1], f64(q))
+            for s in range(2):
+                for l in range(wl.L):
+                    check_output(out[s, l], ref[s, l], oc.max_abs_vhat(s, l), f"loop step {step} seq {s} layer {l}")
+            o1 = cache.decode_attention(1, [0, 1], q[:, 1].contiguous()).double().cpu().numpy()
+            assert rel_l2(o1, out[:, 1]) < 2e-3
+    assert cache.seq_len(0) == 240 and cache.seq_len(1) == 117
+    cache.destroy()
