@@ -88,6 +88,27 @@ def project_quantise(x, B_lead, gate):
     return codes, exps, c, resid
 
 
+def append_compress_i8(oc, s, k_new, v_new, tier, flag) -> None:
+    """Append/compress in this format into an `oracle.dwkv_oracle.OracleCache` `oc` (token by token, header formulas):
+    the cache receives the dequantised coefficients (exact bf16 values) and the fp32 residuals of the flagged tokens."""
+    tier = np.asarray(tier, np.uint8); flag = np.asarray(flag, np.uint8)
+    n, L, H, d, r = len(tier), oc.L, oc.H, oc.d, oc.r
+    coef = {z: np.zeros((n, L, H, r)) for z in "KV"}
+    resid = {z: np.zeros((n, L, H, d), np.float32) for z in "KV"}
+    for z, x_all, B_all, g_all in (("K", k_new, oc.BK, oc.gK), ("V", v_new, oc.BV, oc.gV)):
+        x_all = np.asarray(x_all, np.float64)
+        for t in range(n):
+            rt = oc.tier_ranks[tier[t]]
+            for l in range(L):
+                for h in range(H):
+                    _, _, c, e = project_quantise(x_all[t, l, h], B_all[l // oc.w, h, :rt, :], g_all[l, h])
+                    coef[z][t, l, h, :rt] = c
+                    resid[z][t, l, h] = e
+    fidx = np.nonzero(flag)[0]
+    oc.append_raw(s, tier, flag, coef["K"], coef["V"],
+                  residK=resid["K"][fidx] if len(fidx) else None, residV=resid["V"][fidx] if len(fidx) else None)
+
+
 def footprint_bytes_i8(tier, flag, tier_ranks, d, L, H) -> int:
     """Compressed bytes of one sequence with int8 coefficients: per (layer, kv head, token)
     2*(r_t + ceil(r_t/32)) (codes + one exponent byte per block, K and V) + f_t * 2*(d/2 + d/8)."""

@@ -284,6 +284,7 @@ int dwkv_create(const dwkv_config* cfg, dwkv_cache** out) {
   c->geom.L = f.n_layers; c->geom.w = f.group_size; c->geom.H = f.n_kv_heads; c->geom.G = f.n_q_heads / f.n_kv_heads;
   c->geom.r = f.tier_rank[f.n_tiers - 1]; c->geom.d = f.d_head; c->geom.n_tiers = f.n_tiers;
   for (int k = 0; k < 4; ++k) c->geom.tier_rank[k] = k < f.n_tiers ? f.tier_rank[k] : 0;
+  c->geom.i8 = 0;
   c->n_classes = 2 * f.n_tiers;
   for (int k = 0; k < c->n_classes; ++k) c->cl[k] = make_class_layout(f.tier_rank[k >> 1], k & 1, f.d_head);
   c->softmax_scale = f.softmax_scale > 0.f ? f.softmax_scale : 1.0f / std::sqrt((float)f.d_head);
@@ -442,6 +443,19 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
       }
       off += n_new[i];
     }
+    if (c->geom.i8) {        // 8-bit coefficient planes: plain kernel, rows and destinations in call order
+      int rc = zero_new_pages(c, new_pages, st);
+      if (rc) return rc;
+      rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
+      if (rc) return rc;
+      if (c->opt_time_scan && g0 == 0) {
+        if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
+        CU_OK(cudaEventRecord(c->ev_app0, st));
+      }
+      c->launches += launch_compress_i8(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)dst.size(), (const __nv_bfloat16*)k_new,
+                                        (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, st);
+      continue;
+    }
     if (c->opt_compress_umma && compress_umma_supported(c->geom, k_new, v_new)) {
       // tcgen05 path: rows in call order (TMA tile loads), destinations in the same order
       int rc = zero_new_pages(c, new_pages, st);
@@ -597,7 +611,8 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
   const uint64_t LH = (uint64_t)c->geom.L * c->geom.H, d = c->geom.d;
   for (const SeqState& S : c->seqs)
     for (int k = 0; k < c->n_classes; ++k)
-      used += (uint64_t)S.count[k] * (4ull * c->geom.tier_rank[k >> 1] + (k & 1) * 2ull * (d / 2 + d / 8));
+      used += (uint64_t)S.count[k] * ((c->geom.i8 ? 2ull * (c->geom.tier_rank[k >> 1] + 1) : 4ull * c->geom.tier_rank[k >> 1]) +
+                                      (k & 1) * 2ull * (d / 2 + d / 8));
   if (used_bytes) *used_bytes = used * LH;
   if (reserved_bytes) *reserved_bytes = (uint64_t)pages_in_use(c) * c->page_bytes;
   if (dense_equiv_bytes) *dense_equiv_bytes = (uint64_t)c->total_tokens * LH * 4ull * d;
@@ -619,6 +634,14 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   else if (!strcmp(key, "cost_seg")) c->opt_cost_seg = std::max<int64_t>(0, value);
   else if (!strcmp(key, "cost_resid_pct")) c->opt_cost_resid_pct = value;
   else if (!strcmp(key, "unit_kb")) c->opt_unit_kb = std::max<int64_t>(1, value);
+  else if (!strcmp(key, "coef_int8")) {
+    // storage format of the coefficient planes: fixed once tokens exist, like the basis (A19)
+    if (value != 0 && value != 1) return fail(DWKV_E_INVALID, "coef_int8 must be 0 or 1");
+    if (c->total_tokens != 0 || pages_in_use(c) != 0) return fail(DWKV_E_STATE, "coef_int8 cannot change while the cache holds tokens");
+    if (value && c->geom.r > 32) return fail(DWKV_E_INVALID, "coef_int8 needs a basis rank <= 32 (one 32-column block per token)");
+    c->geom.i8 = (int32_t)value;
+    for (int k = 0; k < c->n_classes; ++k) c->cl[k] = make_class_layout(c->cfg.tier_rank[k >> 1], k & 1, c->cfg.d_head, c->geom.i8);
+  }
   else return fail(DWKV_E_INVALID, std::string("unknown option ") + key);
   c->version++;
   return DWKV_OK;
@@ -855,6 +878,7 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   sp.layer0 = layer0; sp.Lq = Lsel; sp.LH = Lsel * g.H; sp.w = g.w;
   sp.H = g.H; sp.G = g.G; sp.r = g.r; sp.d = g.d;
   sp.cscale = c->softmax_scale * 1.4426950408889634f;
+  sp.i8 = g.i8;
   if (c->opt_time_scan) {
     if (!c->ev_scan0) { CU_OK(cudaEventCreate(&c->ev_scan0)); CU_OK(cudaEventCreate(&c->ev_scan1)); }
     CU_OK(cudaEventRecord(c->ev_scan0, st));

@@ -40,11 +40,42 @@ struct BlockPtr {
 __device__ __forceinline__ BlockPtr block_ptr(const uint8_t* arena, const CacheGeom& g, const TokDst& td, int lh) {
   BlockPtr b;
   b.rk = g.tier_rank[td.cls >> 1];
-  b.cl = make_class_layout(b.rk, td.cls & 1, g.d);
+  b.cl = make_class_layout(b.rk, td.cls & 1, g.d, g.i8);
   b.blk = const_cast<uint8_t*>(arena) + td.page_off + (size_t)lh * kPageLhBytes + (size_t)td.blk * b.cl.block_bytes +
           sub_off(b.cl, td.slot);
   b.slot = sub_slot(b.cl, td.slot);
   return b;
+}
+
+// 8-bit blockwise coefficient quantiser (reading A27), block = the token's coefficient vector (rank <= 32):
+// e = smallest integer with amax <= 127 * 2^e, clamped to >= -126 (amax == 0 and subnormal amax land on the clamp);
+// code = rint(c / 2^e) in [-127, 127]. Every step is exact in fp32. amax = m * 2^x, m in [0.5, 1): e = x - 7 if m <= 127/128 else x - 6.
+__device__ __forceinline__ int coef8_exponent(float amax) {
+  const uint32_t b = __float_as_uint(amax);
+  const int x = (int)((b >> 23) & 0xffu) - 126;
+  const int e = ((b & 0x7fffffu) <= 0x7e0000u) ? x - 7 : x - 6;
+  return max(e, -126);
+}
+__device__ __forceinline__ int coef8_code(float c, int e) {
+  const float q = rintf(c * __uint_as_float((uint32_t)(127 - e) << 23));     // c / 2^e, exact
+  return (int)fminf(fmaxf(q, -127.f), 127.f);
+}
+__device__ __forceinline__ float warp_max(float a) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(kFull, a, o));
+  return a;
+}
+// store one token's coefficient of column col (stored byte = code + 128) and, from column 0, the exponent byte (e + 127)
+__device__ __forceinline__ void store_coef8(const BlockPtr& bp, int z, int col, int code, int e) {
+  uint8_t* base = bp.blk + (z ? off_coefV(bp.cl) : off_coefK(bp.cl));
+  base[z ? vcoef8_elem_off(bp.slot, col, bp.cl.tb) : kcoef8_elem_off(bp.slot, col, bp.cl.tb)] = (uint8_t)(code + 128);
+  if (col == 0) base[coef8_exp_off(bp.slot, bp.cl.nk, bp.cl.tb)] = (uint8_t)(e + 127);
+}
+__device__ __forceinline__ float load_coef8(const BlockPtr& bp, int z, int col) {
+  const uint8_t* base = bp.blk + (z ? off_coefV(bp.cl) : off_coefK(bp.cl));
+  const int u = base[z ? vcoef8_elem_off(bp.slot, col, bp.cl.tb) : kcoef8_elem_off(bp.slot, col, bp.cl.tb)];
+  const uint32_t eb = base[coef8_exp_off(bp.slot, bp.cl.nk, bp.cl.tb)];
+  return (float)(u - 128) * __uint_as_float(eb << 23);
 }
 
 __device__ __forceinline__ void store_code(uint8_t* region, int word_off, int bit, int code) {
@@ -66,7 +97,15 @@ __global__ void __launch_bounds__(128) scatter_raw_kernel(const uint8_t* arena, 
   const TokDst td = dst[tok];
   const BlockPtr bp = block_ptr(arena, g, td, lh);
   const size_t row = (size_t)tok * LH + lh;
-  if (tid < bp.rk) {
+  if (g.i8) {                 // quantise the given coefficients (rank <= 32: the vector sits in warp 0)
+    if (tid < 32) {
+      for (int z = 0; z < 2; ++z) {
+        const float cf = tid < bp.rk ? __bfloat162float((z ? coefV : coefK)[row * g.r + tid]) : 0.f;
+        const int e = coef8_exponent(warp_max(fabsf(cf)));
+        if (tid < bp.rk) store_coef8(bp, z, tid, coef8_code(cf, e), e);
+      }
+    }
+  } else if (tid < bp.rk) {
     *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(bp.slot, tid, bp.cl.tb)) = coefK[row * g.r + tid];
     *reinterpret_cast<__nv_bfloat16*>(bp.blk + off_coefV(bp.cl) + vcoef_elem_off(bp.slot, tid, bp.cl.tb)) = coefV[row * g.r + tid];
   }
@@ -107,7 +146,11 @@ __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, Cache
   const BlockPtr bp = block_ptr(arena, g, td, lh);
   const size_t row = (size_t)tok * LH + lh;
   const int d = g.d, ng = d / 16;
-  if (tid < g.r) {
+  if (g.i8 && tid < g.r) {     // code * 2^e has <= 7 significant bits: exactly a bf16 value
+    const __nv_bfloat16 zero = __float2bfloat16_rn(0.f);
+    if (o.coefK) o.coefK[row * g.r + tid] = tid < bp.rk ? __float2bfloat16_rn(load_coef8(bp, 0, tid)) : zero;
+    if (o.coefV) o.coefV[row * g.r + tid] = tid < bp.rk ? __float2bfloat16_rn(load_coef8(bp, 1, tid)) : zero;
+  } else if (tid < g.r) {
     const __nv_bfloat16 zero = __float2bfloat16_rn(0.f);
     if (o.coefK)
       o.coefK[row * g.r + tid] = tid < bp.rk ? *reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(bp.slot, tid, bp.cl.tb)) : zero;
@@ -138,6 +181,62 @@ __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, Cache
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Append/compress in 8-bit coefficient mode (step a4 with reading A27 in place of the bf16 rounding): one CTA of 128 threads per
+// (token, layer, head); c = B[:r_t] . (x / g) in fp32, quantised; the residual of a flagged token is taken against the DEQUANTISED
+// coefficients and goes through the A14 quantiser. Plain kernel (not tuned): the tensor-core kernel of dwkv_compress.cu serves bf16 mode.
+__global__ void __launch_bounds__(128) compress_i8_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst, const __nv_bfloat16* k_new,
+                                                          const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
+                                                          const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
+  __shared__ float xn[128], cs[32];
+  const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const TokDst td = dst[tok];
+  const BlockPtr bp = block_ptr(arena, g, td, lh);
+  const int d = g.d, layer = lh / g.H, h = lh - layer * g.H;
+  const bool fl = (td.cls & 1) != 0;
+  for (int z = 0; z < 2; ++z) {
+    const __nv_bfloat16* B = (z ? BV : BK) + ((size_t)(layer / g.w) * g.H + h) * (size_t)g.r * d;
+    float x = 0.f, gate = 1.f;
+    if (tid < d) {
+      x = __bfloat162float((z ? v_new : k_new)[((size_t)td.src * LH + lh) * d + tid]);
+      gate = __bfloat162float((z ? gV : gK)[(size_t)lh * d + tid]);
+      xn[tid] = __fdiv_rn(x, gate);
+    }
+    __syncthreads();
+    for (int j = warp; j < bp.rk; j += 4) {
+      float acc = 0.f;
+      for (int ch = lane; ch < d; ch += 32) acc = fmaf(__bfloat162float(B[(size_t)j * d + ch]), xn[ch], acc);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
+      if (lane == 0) cs[j] = acc;
+    }
+    __syncthreads();
+    if (tid < 32) {
+      const float cf = tid < bp.rk ? cs[tid] : 0.f;
+      const int e = coef8_exponent(warp_max(fabsf(cf)));
+      const int code = coef8_code(cf, e);
+      if (tid < bp.rk) {
+        store_coef8(bp, z, tid, code, e);
+        cs[tid] = (float)code * __uint_as_float((uint32_t)(e + 127) << 23);
+      }
+    }
+    __syncthreads();
+    if (fl && tid < d) {
+      float rec = 0.f;
+      for (int j = 0; j < bp.rk; ++j) rec = fmaf(cs[j], __bfloat162float(B[(size_t)j * d + tid]), rec);
+      const float e = x - gate * rec;
+      __half s;
+      const int code = quant_code(e, group16_amax(fabsf(e)), &s);
+      int wo, bit;
+      if (z == 0) kcode_nibble(bp.slot, tid, d, &wo, &bit); else vcode_nibble(bp.slot, tid, d, &wo, &bit);
+      store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
+      if ((tid & 15) == 0)
+        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(bp.slot, tid >> 4, d)) = s;
+    }
+    __syncthreads();
+  }
+}
+
 __global__ void gate_check_kernel(const __nv_bfloat16* g, int64_t n, int* bad) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) {
@@ -154,6 +253,15 @@ int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* d
   if (n <= 0) return 0;
   dim3 grid(n, g.L * g.H);
   scatter_raw_kernel<<<grid, 128, 0, s>>>(arena, g, dst, coefK, coefV, residK, residV, codeK, codeV, scaleK, scaleV);
+  return 1;
+}
+
+int launch_compress_i8(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const __nv_bfloat16* k_new,
+                       const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK,
+                       const __nv_bfloat16* gV, cudaStream_t s) {
+  if (n <= 0) return 0;
+  dim3 grid(n, g.L * g.H);
+  compress_i8_kernel<<<grid, 128, 0, s>>>(arena, g, dst, k_new, v_new, BK, BV, gK, gV);
   return 1;
 }
 

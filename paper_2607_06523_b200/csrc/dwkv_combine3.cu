@@ -10,6 +10,10 @@ bool launch_scan3_d64_p0(const Scan3Params& p, int n_sms, cudaStream_t s);
 bool launch_scan3_d64_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
 bool launch_scan3_d128_p0(const Scan3Params& p, int n_sms, cudaStream_t s);
 bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
+bool launch_scan3_d64_p0_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
+bool launch_scan3_d64_p1_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
+bool launch_scan3_d128_p0_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
+bool launch_scan3_d128_p1_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
 
 namespace {
 using namespace dwkv::dev;
@@ -148,7 +152,10 @@ int scan3_num_slices(int n_sms) { return n_sms * 8; }
 int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s) {
   const bool pair = p.G <= 4;
   bool ok = false;
-  if (p.d == 128) ok = pair ? launch_scan3_d128_p1(p, n_sms, s) : launch_scan3_d128_p0(p, n_sms, s);
+  if (p.i8) {
+    if (p.d == 128) ok = pair ? launch_scan3_d128_p1_i8(p, n_sms, s) : launch_scan3_d128_p0_i8(p, n_sms, s);
+    else if (p.d == 64) ok = pair ? launch_scan3_d64_p1_i8(p, n_sms, s) : launch_scan3_d64_p0_i8(p, n_sms, s);
+  } else if (p.d == 128) ok = pair ? launch_scan3_d128_p1(p, n_sms, s) : launch_scan3_d128_p0(p, n_sms, s);
   else if (p.d == 64) ok = pair ? launch_scan3_d64_p1(p, n_sms, s) : launch_scan3_d64_p0(p, n_sms, s);
   return ok ? 1 : 0;
 }

@@ -24,6 +24,14 @@
 //             of the transposed value MMA e^T += codeV^T . (P*scaleV): offset-binary codes of slots 8*(a>>1)+2t (low
 //             half-word) and +1 (high), channel 16*grp + 8*(a&1) + g
 //   [V scale] same arrangement as [K scale]
+//
+// 8-bit coefficient mode ("8-bit blockwise quantized"; reading A27), basis
+// rank <= 32 so that a token's coefficient vector is ONE block: the same fragment order with one BYTE per coefficient
+// (offset-binary code + 128) and, behind the nk code vectors of each of K and V, one exponent byte (e + 127) per slot:
+//   [K coef8] nk vectors of 64*TB B.  vector i, lane (g,t), half-word j : ( uK[slot 8j+g][8i+2t], uK[slot 8j+g][8i+2t+1] )
+//   [K exp]   8*TB B.                 byte (t, j, hi) = exponent byte of slot 8j + 2t + hi   (the C-fragment columns of lane t)
+//   [V coef8] nk vectors of 64*TB B.  vector i, lane (g,t), half-word j : ( uV[slot 8j+2t][8i+g], uV[slot 8j+2t+1][8i+g] )
+//   [V exp]   as [K exp]
 #pragma once
 #include <stdint.h>
 
@@ -43,9 +51,10 @@ constexpr int kMaxClasses = 8;             // 2 * DWKV_MAX_TIERS
 struct ClassLayout {
   int nk;            // rank / 8
   int resid;         // 0 / 1
+  int i8;            // 8-bit coefficient mode
   int tb;            // tiles (of 8 slots) per sub-block: 4 (unflagged) or 2 (flagged)
   int sub_tok;       // slots per sub-block = 8 * tb
-  int coef_bytes;    // nk * 128 * tb  (per K or V, per sub-block)
+  int coef_bytes;    // nk * 128 * tb  (per K or V, per sub-block); 8-bit mode: nk * 64 * tb codes + 8 * tb exponent bytes
   int code_bytes;    // per K or V, per sub-block: tb * 4 * d, 0 if !resid
   int scale_bytes;   // tb * d
   int sub_bytes;     // 2*coef + resid * 2*(code + scale)
@@ -54,13 +63,14 @@ struct ClassLayout {
   int tokens_per_page;
 };
 
-DWKV_HD ClassLayout make_class_layout(int rank, int resid, int d) {
+DWKV_HD ClassLayout make_class_layout(int rank, int resid, int d, int i8 = 0) {
   ClassLayout c;
   c.nk = rank / 8;
   c.resid = resid;
+  c.i8 = i8;
   c.tb = resid ? 2 : 4;
   c.sub_tok = 8 * c.tb;
-  c.coef_bytes = c.nk * 128 * c.tb;
+  c.coef_bytes = i8 ? c.nk * 64 * c.tb + 8 * c.tb : c.nk * 128 * c.tb;
   c.code_bytes = resid ? c.tb * 4 * d : 0;
   c.scale_bytes = resid ? c.tb * d : 0;
   c.sub_bytes = 2 * c.coef_bytes + 2 * (c.code_bytes + c.scale_bytes);
@@ -89,6 +99,19 @@ DWKV_HD int kcoef_elem_off(int s, int col, int tb) {     // byte offset of the b
 DWKV_HD int vcoef_elem_off(int s, int col, int tb) {     // byte offset of the bf16 element inside [V coef]
   const int j = s >> 3, p = s & 7, t = p >> 1, hi = p & 1, i = col >> 3, g = col & 7;
   return i * 128 * tb + (4 * g + t) * 4 * tb + j * 4 + hi * 2;
+}
+// 8-bit coefficient mode: byte offsets inside [K coef8] / [V coef8] and of the exponent byte behind the nk code vectors
+DWKV_HD int kcoef8_elem_off(int s, int col, int tb) {
+  const int j = s >> 3, g = s & 7, i = col >> 3, t = (col & 7) >> 1, hi = col & 1;
+  return i * 64 * tb + (4 * g + t) * 2 * tb + j * 2 + hi;
+}
+DWKV_HD int vcoef8_elem_off(int s, int col, int tb) {
+  const int j = s >> 3, p = s & 7, t = p >> 1, hi = p & 1, i = col >> 3, g = col & 7;
+  return i * 64 * tb + (4 * g + t) * 2 * tb + j * 2 + hi;
+}
+DWKV_HD int coef8_exp_off(int s, int nk, int tb) {
+  const int j = s >> 3, p = s & 7, t = p >> 1, hi = p & 1;
+  return nk * 64 * tb + t * 2 * tb + j * 2 + hi;
 }
 DWKV_HD void kcode_nibble(int s, int ch, int d, int* word_off, int* bit) {   // inside [K code] (s in 0..15)
   const int j = s >> 3, g = s & 7, grp = ch >> 4, wi = ch & 15, b = wi >> 3, t = (wi & 7) >> 1, hi = wi & 1;

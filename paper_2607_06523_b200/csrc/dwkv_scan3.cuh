@@ -62,6 +62,21 @@ __device__ __forceinline__ uint2 lds64(uint32_t a) {
   asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(a));
   return r;
 }
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t r;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(r) : "r"(a));
+  return r;
+}
+// 8-bit coefficient mode: bytes 2k, 2k+1 of w (offset-binary codes u = code + 128) -> bf16x2 (code_lo, code_hi), exact.
+// PRMT builds the float 2^23 + u (bytes u, 0, 0, 0x4B), the subtraction of 2^23 + 128 is exact, the pack rounds nothing (|code| <= 128).
+__device__ __forceinline__ uint32_t u8pair_to_bf16x2(uint32_t w, int k) {
+  uint32_t f0, f1;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(f0) : "r"(w), "r"(0x4B000000u), "r"(0x7440u | (uint32_t)(2 * k)));
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(f1) : "r"(w), "r"(0x4B000000u), "r"(0x7440u | (uint32_t)(2 * k + 1)));
+  return pack_bf16x2(__uint_as_float(f0) - 8388736.f, __uint_as_float(f1) - 8388736.f);
+}
+// exponent byte (e + 127) at bit position sh of w -> 2^e
+__device__ __forceinline__ float exp_byte_to_scale(uint32_t w, int sh) { return __uint_as_float(((w >> sh) & 0xffu) << 23); }
 __device__ __forceinline__ void sts128(uint32_t a, int x, int y, int z, int w) {
   asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }

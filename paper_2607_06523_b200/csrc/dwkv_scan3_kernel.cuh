@@ -197,26 +197,26 @@ __device__ __forceinline__ void flush_partial(const State<NKB, D>& st, const Sca
   }
 }
 
-template <int NK, bool RESID, int NKB, int D, bool PAIR>
+template <int NK, bool RESID, int NKB, int D, bool PAIR, bool I8>
 __device__ __forceinline__ void process_stage(State<NKB, D>& st, const uint32_t sp, const int n, const int ntok, const int lane,
                                               const QRegs<NKB, D, PAIR>& q, const float cscale) {
   constexpr int SUBTOK = RESID ? 16 : 32;
-  constexpr int SB1 = RESID ? NK * 512 + 20 * D : NK * 1024;
+  constexpr int SB1 = I8 ? (RESID ? 2 * (NK * 128 + 16) + 20 * D : 2 * (NK * 256 + 32)) : (RESID ? NK * 512 + 20 * D : NK * 1024);
   if constexpr (RESID || NK > 2) {
 #pragma unroll 1
-    for (int sb = 0; sb < n; ++sb) process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+    for (int sb = 0; sb < n; ++sb) process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
   } else {   // two independent sub-blocks per iteration: more instruction-level parallelism for the 2 warps per scheduler
     int sb = 0;
 #pragma unroll 1
     for (; sb + 2 <= n; sb += 2) {
-      process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
-      process_sub<NK, RESID, NKB, D, PAIR>(st, sp + (sb + 1) * SB1, ntok - (sb + 1) * SUBTOK, lane, q, cscale);
+      process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+      process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + (sb + 1) * SB1, ntok - (sb + 1) * SUBTOK, lane, q, cscale);
     }
-    if (sb < n) process_sub<NK, RESID, NKB, D, PAIR>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+    if (sb < n) process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
   }
 }
 
-template <int NKB, int D, bool PAIR>
+template <int NKB, int D, bool PAIR, bool I8>
 __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_constant__ Scan3Params p) {
   using RG = Ring<NKB, D>;
   constexpr int SLOT = RG::SLOT, NS = RG::NS;
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     const Unit un = load_unit(p.units + f_u);
     const int nk = un.rk >> 3, fl = un.cls & 1;
     f_code = nk | (fl << 8);
-    f_sb1 = fl ? nk * 512 + 20 * D : nk * 1024;
+    f_sb1 = I8 ? (fl ? 2 * (nk * 128 + 16) + 20 * D : 2 * (nk * 256 + 32)) : (fl ? nk * 512 + 20 * D : nk * 1024);
     f_subtok = fl ? 16 : 32;
     f_ntok = un.ntok;
     f_nsub = (un.ntok + f_subtok - 1) / f_subtok;
@@ -329,18 +329,18 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     const uint32_t sp = ring + k_c * SLOT;
     const int ntok = (int)dsc.y;
     switch (dsc.x & 0xffffu) {
-      case 0x001: process_stage<1, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x101: process_stage<1, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x002: process_stage<2, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x102: process_stage<2, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x003: if constexpr (NKB >= 3) process_stage<3, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x103: if constexpr (NKB >= 3) process_stage<3, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x004: if constexpr (NKB >= 4) process_stage<4, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x104: if constexpr (NKB >= 4) process_stage<4, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x006: if constexpr (NKB >= 6) process_stage<6, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x106: if constexpr (NKB >= 6) process_stage<6, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x008: if constexpr (NKB >= 8) process_stage<8, false, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
-      case 0x108: if constexpr (NKB >= 8) process_stage<8, true, NKB, D, PAIR>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x001: process_stage<1, false, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x101: process_stage<1, true, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x002: process_stage<2, false, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x102: process_stage<2, true, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x003: if constexpr (NKB >= 3) process_stage<3, false, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x103: if constexpr (NKB >= 3) process_stage<3, true, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x004: if constexpr (NKB >= 4) process_stage<4, false, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x104: if constexpr (NKB >= 4) process_stage<4, true, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x006: if constexpr (NKB >= 6) process_stage<6, false, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x106: if constexpr (NKB >= 6) process_stage<6, true, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x008: if constexpr (NKB >= 8) process_stage<8, false, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
+      case 0x108: if constexpr (NKB >= 8) process_stage<8, true, NKB, D, PAIR, I8>(st, sp, n, ntok, lane, q, p.cscale); break;
       default: break;   // unsupported rank (the host refuses these configurations)
     }
     __syncwarp();
@@ -357,12 +357,12 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
   }
 }
 
-template <int NKB, int D, bool PAIR>
+template <int NKB, int D, bool PAIR, bool I8>
 void launch_instance(const Scan3Params& p, int n_sms, cudaStream_t s) {
   const int smem = kWarps * kWarpSmem;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(scan3_kernel<NKB, D, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(scan3_kernel<NKB, D, PAIR, I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     attr_set = true;
   }
   cudaLaunchConfig_t cfg = {};
@@ -375,17 +375,27 @@ void launch_instance(const Scan3Params& p, int n_sms, cudaStream_t s) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, scan3_kernel<NKB, D, PAIR>, p);
+  cudaLaunchKernelEx(&cfg, scan3_kernel<NKB, D, PAIR, I8>, p);
 }
 
 template <int D, bool PAIR>
 bool launch_by_rank(const Scan3Params& p, int n_sms, cudaStream_t s) {
   const int nkb = (p.r + 15) / 16 * 2;      // basis rank / 8 rounded up to even
   switch (nkb) {
-    case 2: launch_instance<2, D, PAIR>(p, n_sms, s); return true;
-    case 4: launch_instance<4, D, PAIR>(p, n_sms, s); return true;
-    case 6: launch_instance<6, D, PAIR>(p, n_sms, s); return true;
-    case 8: launch_instance<8, D, PAIR>(p, n_sms, s); return true;
+    case 2: launch_instance<2, D, PAIR, false>(p, n_sms, s); return true;
+    case 4: launch_instance<4, D, PAIR, false>(p, n_sms, s); return true;
+    case 6: launch_instance<6, D, PAIR, false>(p, n_sms, s); return true;
+    case 8: launch_instance<8, D, PAIR, false>(p, n_sms, s); return true;
+  }
+  return false;
+}
+// 8-bit coefficient planes: basis rank <= 32 (one block per token vector)
+template <int D, bool PAIR>
+bool launch_by_rank_i8(const Scan3Params& p, int n_sms, cudaStream_t s) {
+  const int nkb = (p.r + 15) / 16 * 2;
+  switch (nkb) {
+    case 2: launch_instance<2, D, PAIR, true>(p, n_sms, s); return true;
+    case 4: launch_instance<4, D, PAIR, true>(p, n_sms, s); return true;
   }
   return false;
 }

@@ -31,11 +31,13 @@ def arena_bytes_for(wl: gen.Workload, routings, slack_pages_per_class: int = 1) 
 
 
 def make_cache(wl: gen.Workload, n_seqs: Optional[int] = None, max_tokens: Optional[int] = None, arena_bytes: int = 0,
-               device: int = 0, softmax_scale: float = 0.0):
+               device: int = 0, softmax_scale: float = 0.0, coef_int8: bool = False):
     n_seqs = wl.n_seq if n_seqs is None else n_seqs
     max_tokens = (max(wl.T) + 4096) if max_tokens is None else max_tokens
     cache = binding.DwkvCache(wl.L, wl.w, wl.H_kv, wl.H_q, wl.d, list(wl.tier_ranks), n_seqs, max_tokens,
                               softmax_scale=softmax_scale, device=device, arena_bytes=arena_bytes)
+    if coef_int8:       # 8-bit coefficient planes (dwkv.h option "coef_int8"): must be chosen while the cache is empty
+        cache.set_option("coef_int8", 1)
     dev = torch.device("cuda", device)
     BK, BV = gen.make_basis(wl, device=dev)
     gK, gV = gen.make_gates(wl, device=dev)
