@@ -26,13 +26,14 @@ METRIC = "decode-attn cached tokens scanned/s (all layers; ms_per_step = ms/step
 UNIT = "tokens/s"
 
 
-def config_of(wl, world, footprint_gb=None):
+def config_of(wl, world, footprint_gb=None, coef_int8=False):
     """The `config` object of the JSON line: the same for our arm and the reference arm."""
     c = {"workload": wl.name, "shape": f"L={wl.L} w={wl.w} H_kv={wl.H_kv} G={wl.G} d={wl.d} r={wl.r}",
          "batch": wl.n_seq, "T": wl.T[0] if len(set(wl.T)) == 1 else [min(wl.T), max(wl.T)], "tiers": list(wl.tier_ranks),
          "tier_frac": list(wl.tier_frac), "resid_frac": wl.resid_frac, "launch_mode": "all layers in one call (layer = -1)",
          "l2_policy": "inputs larger than L2 (compressed cache of the workload >> 126 MB; every step streams all of it): no flush",
          "parallelism": "replicas only (no sharding, no collective)" if world > 1 else "single GPU"}
+    c["coefficients"] = "int8 codes + one power-of-two exponent byte per 32-column block (PAPER.md:56, A27)" if coef_int8 else "bf16 (BASELINE.json north_star)"
     return c
 
 
@@ -160,7 +161,7 @@ def prefill_compress(wl, harness, local, reps=3):
             "build_basis_dense_GBps": 2 * k_new[:n8].numel() * 2 / min(bms[1:]) / 1e6, "note": "one dwkv_append_compress call, timed from an idle GPU: host routing + page zeroing + kernel"}
 
 
-def oracle_sample(wl, consts, tier, flag, kept, q_host, layers, budget_s=25.0):
+def oracle_sample(wl, consts, tier, flag, kept, q_host, layers, budget_s=25.0, coef_int8=False):
     """Time the CPU oracle as it stands on (layer, kv head) slices of sequence 0; returns (token-layers/s, sample text,
     threads, worst rel-L2 vs `gpu_out` if given)."""
     from oracle import dwkv_oracle as orc
@@ -175,6 +176,18 @@ def oracle_sample(wl, consts, tier, flag, kept, q_host, layers, budget_s=25.0):
     ranks = np.asarray(wl.tier_ranks)[tier]
     idx = np.nonzero(flag)[0]
     outs = {}
+
+    def coef(c):        # the stored coefficients as float64: the generator's bf16 values, or their 8-bit quantisation (A27)
+        c = f64(c)
+        if not coef_int8:
+            return c
+        from oracle import dwkv_coef8_oracle as c8
+        q8 = np.zeros_like(c)
+        for rk in set(ranks.tolist()):
+            sel = ranks == rk
+            codes, exps = c8.quantize_coef_i8(c[sel].astype(np.float32), rank=rk)
+            q8[sel] = c8.dequant_coef_i8(codes, exps)
+        return q8
     t0 = time.perf_counter()
     done_layers = 0
     for l in layers:
@@ -185,7 +198,7 @@ def oracle_sample(wl, consts, tier, flag, kept, q_host, layers, budget_s=25.0):
             if len(idx):
                 cK_[idx], sK_[idx] = orc.quantize_int4_g16(k["rK"].numpy())
                 cV_[idx], sV_[idx] = orc.quantize_int4_g16(k["rV"].numpy())
-            o, _, V = orc.attention_slice(f64(k["cK"]), f64(k["cV"]), ranks, flag, cK_, sK_, cV_, sV_, BK[l // wl.w, h],
+            o, _, V = orc.attention_slice(coef(k["cK"]), coef(k["cV"]), ranks, flag, cK_, sK_, cV_, sV_, BK[l // wl.w, h],
                                           BV[l // wl.w, h], gK[l, h], gV[l, h], q_host[l, h * wl.G:(h + 1) * wl.G],
                                           1.0 / np.sqrt(wl.d))
             outs[(l, h)] = (o, float(np.abs(V).max()))
@@ -246,6 +259,8 @@ def main():
     ap.add_argument("--opt", action="append", default=[], help="library option key=value (experiments), repeatable")
     ap.add_argument("--append", action="store_true",
                     help="BASELINE.json configs[4]: dwkv_append_compress of wl.n_append new tokens per sequence before every decode step")
+    ap.add_argument("--coef-int8", action="store_true",
+                    help="store the coefficients in 8-bit blockwise form (PAPER.md:56; dwkv.h option coef_int8; DESIGN.md A27; rank <= 32)")
     ap.add_argument("--no-dense", action="store_true", help="skip the dense-bf16 comparison kernel")
     ap.add_argument("--no-extra", action="store_true", help="skip batch 1/4, per-layer mode and the CPU baseline")
     args = ap.parse_args()
@@ -266,6 +281,8 @@ def main():
     slack = 1 + (n_app * app_steps + 127) // 128        # pages per (sequence, class) for the appended tokens (>= 227 tokens per page)
     cache, consts = harness.make_cache(wl, max_tokens=max(wl.T) + 4096 + n_app * app_steps,
                                        arena_bytes=harness.arena_bytes_for(wl, routings, slack), device=local)
+    if args.coef_int8:
+        cache.set_option("coef_int8", 1)
     for kv in args.opt:
         k, v = kv.split("=")
         cache.set_option(k, int(v))
@@ -353,13 +370,19 @@ def main():
     cache.set_option("time_scan", 1)
     scan_ms, compress_ms = [], []
     fp_before = cache.footprint()
-    for i in range(args.steps):
-        if not n_app:     # sample a kernel that runs back to back with its predecessors, as in the timed region (a launch
-            step(); step()   # into an idle GPU right after get_stat's synchronise measures ~5 % slower)
-        step()
-        scan_ms.append(cache.get_stat("scan_ms"))
-        if n_app:
+    if not n_app:         # the kernel as it runs in the timed region: steps back to back, no synchronise between the samples
+        for i in range(args.warmup + min(args.steps, 60)):    # (the library keeps the event brackets of the last 64 calls)
+            if i == args.warmup:
+                cache.set_option("time_scan", 1)              # restarts the sample count after the warm-up steps
+            step()
+        scan_ms = [cache.get_stat("scan_ms_mean")]
+        scan_min = cache.get_stat("scan_ms_min")
+    else:
+        for i in range(args.steps):
+            step()
+            scan_ms.append(cache.get_stat("scan_ms"))
             compress_ms.append(cache.get_stat("compress_ms"))
+        scan_min = float(np.min(scan_ms))
     cache.set_option("time_scan", 0)
     scan_ms = float(np.mean(scan_ms))
     peak, peak_src = peaks()
@@ -367,8 +390,8 @@ def main():
     alg_bytes = (fp_before["used_bytes"] + cache.footprint()["used_bytes"]) // 2 if n_app else fp["used_bytes"]
     achieved = alg_bytes / (scan_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic_of(wl.name), "kernel": "scan3_kernel<NKB,D,PAIR> (fused q pre-projection + split-T scan, one persistent launch per step)",
-                "scan_ms": scan_ms, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
+                "traffic": traffic_of(wl.name + ("_i8" if args.coef_int8 else "")), "kernel": "scan3_kernel<NKB,D,PAIR> (fused q pre-projection + split-T scan, one persistent launch per step)",
+                "scan_ms": scan_ms, "scan_ms_min": scan_min, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "frac_of_8TBps_nominal": achieved / 8000.0, "step_frac_of_peak": alg_bytes / (ms * 1e-3) / 1e9 / peak}
 
     extra_append = None
@@ -428,7 +451,7 @@ def main():
         cache.decode_attention(-1, seq_ids, qs[0], o_gpu)
         torch.cuda.synchronize()
         tps, nl, dt, threads, outs = oracle_sample(wl, consts, tier, flag, kept0, qs[0][s_samp].double().cpu().numpy(),
-                                                   sample_layers, budget_s=25.0)
+                                                   sample_layers, budget_s=25.0, coef_int8=args.coef_int8)
         og = o_gpu[s_samp].double().cpu().numpy()
         rels = []
         for (l, h), (o_ref, vmax) in outs.items():
@@ -472,7 +495,7 @@ def main():
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
                 "data": "synthetic",
-                "config": config_of(wl, world, fp["used_bytes"] / 1e9),
+                "config": config_of(wl, world, fp["used_bytes"] / 1e9, args.coef_int8),
                 "clocks": cs.summary(), "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "cpu_baseline": cpu_baseline, "extra": extra}
         print(json.dumps(line))

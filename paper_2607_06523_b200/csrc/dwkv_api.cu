@@ -157,8 +157,10 @@ struct dwkv_cache {
   int64_t opt_time_scan = 0;
   int64_t opt_compress_umma = 0;     // append/compress: 1 = tcgen05 kernel (d = 128, r <= 64), 0 = mma.sync kernel
   int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
-  cudaEvent_t ev_scan0 = nullptr, ev_scan1 = nullptr, ev_app0 = nullptr, ev_app1 = nullptr;
-  bool scan_timed = false, app_timed = false;
+  static constexpr int kScanRing = 64;   // "time_scan": the last 64 decode kernels are bracketed, read back without a sync in between
+  cudaEvent_t ev_scan0[kScanRing] = {}, ev_scan1[kScanRing] = {}, ev_app0 = nullptr, ev_app1 = nullptr;
+  int64_t scan_samples = 0;              // decode kernels timed since "time_scan" was last set
+  bool app_timed = false;
   int64_t launches = 0;
 };
 
@@ -336,8 +338,10 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->d_flag) cudaFree(c->d_flag);
   c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release();
   c->ring.release();
-  if (c->ev_scan0) cudaEventDestroy(c->ev_scan0);
-  if (c->ev_scan1) cudaEventDestroy(c->ev_scan1);
+  for (int i = 0; i < dwkv_cache::kScanRing; ++i) {
+    if (c->ev_scan0[i]) cudaEventDestroy(c->ev_scan0[i]);
+    if (c->ev_scan1[i]) cudaEventDestroy(c->ev_scan1[i]);
+  }
   if (c->ev_app0) cudaEventDestroy(c->ev_app0);
   if (c->ev_app1) cudaEventDestroy(c->ev_app1);
   delete c;
@@ -622,7 +626,7 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
 int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!c || !key) return fail(DWKV_E_INVALID, "NULL argument");
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
-  else if (!strcmp(key, "time_scan")) c->opt_time_scan = value;
+  else if (!strcmp(key, "time_scan")) { c->opt_time_scan = value; c->scan_samples = 0; }
   else if (!strcmp(key, "sketch_umma")) c->opt_sketch_umma = value;
   else if (!strcmp(key, "compress_umma")) c->opt_compress_umma = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
@@ -651,12 +655,21 @@ int64_t dwkv_launch_count(const dwkv_cache* c) { return c ? c->launches : 0; }
 
 double dwkv_get_stat(dwkv_cache* c, const char* key) {
   if (!c || !key) return -1.0;
-  if (!strcmp(key, "scan_ms")) {
-    if (!c->scan_timed) return -1.0;
-    if (cudaEventSynchronize(c->ev_scan1) != cudaSuccess) return -1.0;
-    float ms = -1.f;
-    if (cudaEventElapsedTime(&ms, c->ev_scan0, c->ev_scan1) != cudaSuccess) return -1.0;
-    return (double)ms;
+  if (!strcmp(key, "scan_samples")) return (double)(c->scan_samples < dwkv_cache::kScanRing ? c->scan_samples : dwkv_cache::kScanRing);
+  const bool s_mean = !strcmp(key, "scan_ms_mean"), s_min = !strcmp(key, "scan_ms_min");
+  if (!strcmp(key, "scan_ms") || s_mean || s_min) {     // last kernel / mean / min over the (up to 64) kernels timed since "time_scan" was set
+    if (c->scan_samples == 0) return -1.0;
+    const int64_t n = c->scan_samples < dwkv_cache::kScanRing ? c->scan_samples : dwkv_cache::kScanRing;
+    const int64_t first = (s_mean || s_min) ? c->scan_samples - n : c->scan_samples - 1;
+    double sum = 0.0, mn = 1e30;
+    for (int64_t k = first; k < c->scan_samples; ++k) {
+      const int i = (int)(k % dwkv_cache::kScanRing);
+      if (cudaEventSynchronize(c->ev_scan1[i]) != cudaSuccess) return -1.0;
+      float ms = -1.f;
+      if (cudaEventElapsedTime(&ms, c->ev_scan0[i], c->ev_scan1[i]) != cudaSuccess) return -1.0;
+      sum += ms; mn = ms < mn ? ms : mn;
+    }
+    return s_min ? mn : sum / (double)(c->scan_samples - first);
   }
   if (!strcmp(key, "compress_ms")) {
     if (!c->app_timed) return -1.0;
@@ -879,14 +892,15 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   sp.H = g.H; sp.G = g.G; sp.r = g.r; sp.d = g.d;
   sp.cscale = c->softmax_scale * 1.4426950408889634f;
   sp.i8 = g.i8;
+  const int ev_i = (int)(c->scan_samples % dwkv_cache::kScanRing);
   if (c->opt_time_scan) {
-    if (!c->ev_scan0) { CU_OK(cudaEventCreate(&c->ev_scan0)); CU_OK(cudaEventCreate(&c->ev_scan1)); }
-    CU_OK(cudaEventRecord(c->ev_scan0, st));
+    if (!c->ev_scan0[ev_i]) { CU_OK(cudaEventCreate(&c->ev_scan0[ev_i])); CU_OK(cudaEventCreate(&c->ev_scan1[ev_i])); }
+    CU_OK(cudaEventRecord(c->ev_scan0[ev_i], st));
   }
   const int n = launch_scan3(sp, c->n_sms, st);
   if (n == 0) return fail(DWKV_E_INVALID, "no fused decode kernel instance for this shape");
   c->launches += n;
-  if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_scan1, st)); c->scan_timed = true; }
+  if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_scan1[ev_i], st)); ++c->scan_samples; }
   Combine3Params cp;
   cp.pstart = sp.pstart; cp.part = sp.part; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
   cp.layer0 = layer0; cp.Lq = Lsel; cp.LH = sp.LH; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;
