@@ -371,19 +371,25 @@ def main():
     scan_ms, compress_ms = [], []
     fp_before = cache.footprint()
     if not n_app:         # the kernel as it runs in the timed region: steps back to back, no synchronise between the samples
-        for i in range(args.warmup + min(args.steps, 60)):    # (the library keeps the event brackets of the last 64 calls)
-            if i == args.warmup:
+        n_samp, n_trail = min(args.steps, 56), 6              # (the library keeps the event brackets of the last 64 calls)
+        for i in range(args.warmup + n_samp + n_trail):       # trailing steps keep the queue full behind the last sample: the
+            if i == args.warmup:                              # last kernels before the stream drains measure 3-10 % slower
                 cache.set_option("time_scan", 1)              # restarts the sample count after the warm-up steps
             step()
-        scan_ms = [cache.get_stat("scan_ms_mean")]
-        scan_min = cache.get_stat("scan_ms_min")
+        torch.cuda.synchronize()
+        scan_ms = [cache.get_stat(f"scan_ms@{i}") for i in range(n_samp)]
+        scan_trail = [round(cache.get_stat(f"scan_ms@{i}"), 4) for i in range(n_samp, n_samp + n_trail)]
+        scan_min = float(np.min(scan_ms))
     else:
         for i in range(args.steps):
             step()
             scan_ms.append(cache.get_stat("scan_ms"))
             compress_ms.append(cache.get_stat("compress_ms"))
         scan_min = float(np.min(scan_ms))
+        scan_trail = []
     cache.set_option("time_scan", 0)
+    scan_samples = [round(float(x), 4) for x in scan_ms]
+    scan_median = float(np.median(scan_ms))
     scan_ms = float(np.mean(scan_ms))
     peak, peak_src = peaks()
     # compressed records: 4 r_t + f_t*2*(d/2+d/8) per (l, h, token); with --append the cache grows while the kernel is timed
@@ -391,7 +397,7 @@ def main():
     achieved = alg_bytes / (scan_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic_of(wl.name + ("_i8" if args.coef_int8 else "")), "kernel": "scan3_kernel<NKB,D,PAIR> (fused q pre-projection + split-T scan, one persistent launch per step)",
-                "scan_ms": scan_ms, "scan_ms_min": scan_min, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
+                "scan_ms": scan_ms, "scan_ms_min": scan_min, "scan_ms_median": scan_median, "scan_ms_samples": scan_samples, "scan_ms_trailing_unused": scan_trail, "algorithmic_bytes": alg_bytes, "peak_source": peak_src,
                 "frac_of_8TBps_nominal": achieved / 8000.0, "step_frac_of_peak": alg_bytes / (ms * 1e-3) / 1e9 / peak}
 
     extra_append = None
@@ -461,6 +467,27 @@ def main():
                         "sample": f"{nl} layer(s) x {wl.H_kv} kv heads x T={len(tier)} of sequence {s_samp} ({dt:.1f} s)",
                         "sampled_parity_rel_l2_max": max(rels)}
 
+    # ---- the paper's own coefficient format ("8-bit blockwise quantized"; option coef_int8, A27) on the same workload ---
+    if rank == 0 and not args.no_extra and not args.coef_int8 and not n_app and wl.r <= 32:
+        try:
+            c8, _ = harness.make_cache(wl, max_tokens=max(wl.T) + 4096, arena_bytes=harness.arena_bytes_for(wl, routings, 1),
+                                       device=local, coef_int8=True)
+            for s, (tier, flag) in enumerate(routings):
+                harness.fill_sequence(c8, wl, s, s, tier, flag, device=local, chunk=4096)
+            o8 = torch.empty_like(o_gpu)
+            ms8 = time_steps(lambda: c8.decode_attention(-1, seq_ids, qs[0], o8), args.steps, args.warmup)
+            fp8 = c8.footprint()
+            extra["coef_int8"] = {"us_per_step": ms8 * 1e3, "used_bytes": fp8["used_bytes"],
+                                  "compression_ratio": fp8["dense_equiv_bytes"] / fp8["used_bytes"],
+                                  "GBps": fp8["used_bytes"] / (ms8 * 1e-3) / 1e9, "frac_of_peak": fp8["used_bytes"] / (ms8 * 1e-3) / 1e9 / peak,
+                                  "rel_l2_vs_bf16_coefficients": float((o8 - o_gpu).norm() / o_gpu.norm()),
+                                  "note": "same generator outputs quantised on load (one power-of-two scale per token vector); the decode "
+                                          "kernel widens the codes in registers and is ALU-pipe bound in this mode (profiles/r1_v6.md): a "
+                                          "footprint option, not a speed-up"}
+            c8.destroy()
+        except Exception as ex:  # pragma: no cover
+            extra["coef_int8"] = {"error": repr(ex)[:200]}
+
     # ---- dense bf16 comparison kernel on the same shapes ------------------------------------------------------------
     if rank == 0 and not args.no_dense and len(set(wl.T)) > 1:
         extra["dense"] = {"skipped": "the dense comparison kernel takes one length for all sequences; this workload is ragged"}
@@ -490,6 +517,17 @@ def main():
             del K, V
         except Exception as ex:  # pragma: no cover
             extra["dense"] = {"error": repr(ex)}
+
+    # ---- the same step held for ~0.5 s: at ~1 kW the board reaches its power limit and lowers the SM clocks ----------------
+    if rank == 0 and not args.no_extra and not n_app:
+        n_long = max(300, args.steps)
+        with ClockSampler(local) as cl:
+            ms_long = time_steps(step, n_long, 10)
+        extra["sustained"] = {"steps": n_long, "us_per_step": ms_long * 1e3, "clocks": cl.summary(),
+                              "frac_of_peak": alg_bytes / (ms_long * 1e-3) / 1e9 / peak,
+                              "frac_of_8TBps_nominal": alg_bytes / (ms_long * 1e-3) / 1e9 / 8000.0,
+                              "note": "the timed region above (K steps, tens of ms) runs at full SM clocks; held for hundreds of steps the board "
+                                      "hits its power limit (sw_power_cap) and the partly issue-bound decode kernel slows with the clocks"}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

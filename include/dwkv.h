@@ -203,7 +203,7 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);
  * with CUDA events on `stream`; dwkv_get_stat(c, "scan_ms") waits for the last bracket and returns its duration in
  * milliseconds (negative = none recorded / error); the brackets of the last 64 calls are kept, so a caller can run steps back
  * to back and read them afterwards without a synchronise in between: "scan_ms_mean" / "scan_ms_min" = mean / minimum over the
- * calls timed since "time_scan" was last set (at most the last 64), "scan_samples" = how many those are. "compress_ms" is the
+ * calls timed since "time_scan" was last set (at most the last 64), "scan_samples" = how many those are, "scan_ms@i" = sample i of them (0 = oldest). "compress_ms" is the
  * bracket of the append/compress kernel (step a4) of the last dwkv_append_compress. */
 double dwkv_get_stat(dwkv_cache* c, const char* key);
 

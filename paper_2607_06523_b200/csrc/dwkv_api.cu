@@ -656,6 +656,16 @@ int64_t dwkv_launch_count(const dwkv_cache* c) { return c ? c->launches : 0; }
 double dwkv_get_stat(dwkv_cache* c, const char* key) {
   if (!c || !key) return -1.0;
   if (!strcmp(key, "scan_samples")) return (double)(c->scan_samples < dwkv_cache::kScanRing ? c->scan_samples : dwkv_cache::kScanRing);
+  if (!strncmp(key, "scan_ms@", 8)) {                  // "scan_ms@i": sample i (0 = oldest kept) of the calls timed since "time_scan" was set
+    const int64_t n = c->scan_samples < dwkv_cache::kScanRing ? c->scan_samples : dwkv_cache::kScanRing;
+    const int64_t k = atoll(key + 8);
+    if (k < 0 || k >= n) return -1.0;
+    const int i = (int)((c->scan_samples - n + k) % dwkv_cache::kScanRing);
+    if (cudaEventSynchronize(c->ev_scan1[i]) != cudaSuccess) return -1.0;
+    float ms = -1.f;
+    if (cudaEventElapsedTime(&ms, c->ev_scan0[i], c->ev_scan1[i]) != cudaSuccess) return -1.0;
+    return (double)ms;
+  }
   const bool s_mean = !strcmp(key, "scan_ms_mean"), s_min = !strcmp(key, "scan_ms_min");
   if (!strcmp(key, "scan_ms") || s_mean || s_min) {     // last kernel / mean / min over the (up to 64) kernels timed since "time_scan" was set
     if (c->scan_samples == 0) return -1.0;
@@ -729,7 +739,9 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
         ub = std::min<int64_t>(ub, cl.blocks_per_page);
         // cost of a sub-block in byte-equivalents: the warp is partly issue bound, so tokens (softmax work) and residual
         // bytes (int4 unpack, group scales) weigh more than coefficient bytes (fit to per-warp finish times)
-        const double cost_sub = 0.01 * (double)c->opt_cost_coef_pct * 2.0 * cl.coef_bytes + cost_tok * cl.sub_tok +
+        // (8-bit coefficient planes: half the bytes per coefficient and ~1.5x the instructions -- the codes are widened in
+        //  registers -- so a coefficient byte weighs 3x; measured optimum on the 64K batch-8 and the ragged workload)
+        const double cost_sub = 0.01 * (double)c->opt_cost_coef_pct * (c->geom.i8 ? 3.0 : 1.0) * 2.0 * cl.coef_bytes + cost_tok * cl.sub_tok +
                                 0.01 * cost_resid_pct * flag_w * 2.0 * (cl.code_bytes + cl.scale_bytes);
         for (size_t pi = 0; pi < S.pages[k].size(); ++pi) {
           const int64_t tok_in_page = std::min<int64_t>(tpp, S.count[k] - (int64_t)pi * tpp);
