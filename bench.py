@@ -371,6 +371,8 @@ def main():
     scan_ms, compress_ms = [], []
     fp_before = cache.footprint()
     if not n_app:         # the kernel as it runs in the timed region: steps back to back, no synchronise between the samples
+        torch.cuda.synchronize()
+        time.sleep(1.0)       # same start as the timed region: an idle board (power-limit averaging window empty), W warm-up steps, K steps
         n_samp, n_trail = min(args.steps, 56), 6              # (the library keeps the event brackets of the last 64 calls)
         for i in range(args.warmup + n_samp + n_trail):       # trailing steps keep the queue full behind the last sample: the
             if i == args.warmup:                              # last kernels before the stream drains measure 3-10 % slower
