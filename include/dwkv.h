@@ -185,7 +185,8 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *   "max_unit_blocks" planner: blocks (of 32 token slots) per work unit, 0 = by "unit_kb"
  *   "unit_kb"         planner: target size of a work unit per (layer, head), KB (default 64 = one page stripe)
  *   "n_slices"        planner: number of warp slices the step is cut into, 0 = one per warp of the persistent grid
- *   "interleave"      planner: 1 = interleave the classes of a sequence in the work order, 0 = class after class
+ *   "interleave"      planner: 1 = interleave the classes of a sequence in the work order, 0 = class after class,
+ *                     -1 (default) = interleave when G > 4 or the call lists one sequence
  *   "cost_coef_pct", "cost_tok", "cost_resid_pct", "flag_cost_pct"   planner cost model (byte-equivalents per coefficient
  *                     byte in %, per token, per residual byte in %, extra weight of flagged classes in %)
  *   "coef_int8"       1 = store the coefficients "in 8-bit blockwise quantized form" (

@@ -657,3 +657,36 @@ def test_decode_loop_appends_one_token_per_step(mod):
             assert rel_l2(o1, out[:, 1]) < 2e-3
     assert cache.seq_len(0) == 240 and cache.seq_len(1) == 117
     cache.destroy()
+
+
+def test_time_scan_sample_ring(mod):
+    """Measurement aid of dwkv.h (option "time_scan", dwkv_get_stat): the library brackets the decode kernel of every call and
+    keeps the last 64 brackets, so bench.py can run steps back to back and read every sample afterwards."""
+    binding, harness = mod
+    wl = gen.WORKLOADS["tiny"]
+    tier, flag = gen.make_routing(wl, 0)
+    cache, _ = harness.make_cache(wl)
+    harness.fill_sequence(cache, wl, 0, 0, tier, flag, chunk=512)
+    q = gen.make_q(wl, device="cuda")
+    ref = cache.decode_attention(-1, [0], q).clone()
+    assert cache.get_stat("scan_ms") < 0 and cache.get_stat("scan_samples") == 0      # nothing timed yet
+    cache.set_option("time_scan", 1)
+    for _ in range(5):
+        out = cache.decode_attention(-1, [0], q)
+    assert torch.equal(out, ref)                                                      # timing does not change the result
+    assert cache.get_stat("scan_samples") == 5
+    samples = [cache.get_stat(f"scan_ms@{i}") for i in range(5)]
+    assert all(0.0 < s < 50.0 for s in samples)
+    assert cache.get_stat("scan_ms") == samples[-1]
+    assert cache.get_stat("scan_ms_min") == min(samples)
+    assert abs(cache.get_stat("scan_ms_mean") - sum(samples) / 5) < 1e-6
+    assert cache.get_stat("scan_ms@5") < 0 and cache.get_stat("scan_ms@-1") < 0
+    for _ in range(70):                                                               # the ring keeps the last 64
+        cache.decode_attention(-1, [0], q)
+    assert cache.get_stat("scan_samples") == 64 and cache.get_stat("scan_ms@63") > 0 and cache.get_stat("scan_ms@64") < 0
+    cache.set_option("time_scan", 1)                                                  # setting the option restarts the count
+    assert cache.get_stat("scan_samples") == 0
+    cache.set_option("time_scan", 0)
+    cache.decode_attention(-1, [0], q)
+    assert cache.get_stat("scan_samples") == 0
+    cache.destroy()
