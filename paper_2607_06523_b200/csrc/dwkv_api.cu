@@ -155,6 +155,7 @@ struct dwkv_cache {
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
+  int64_t opt_combine_warps = 0;     // combine kernel: warps per (segment, head): 1 / 4 / 16, 0 = by partials per segment
   int64_t opt_compress_umma = 0;     // append/compress: 1 = tcgen05 kernel (d = 128, r <= 64), 0 = mma.sync kernel
   int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
   static constexpr int kScanRing = 64;   // "time_scan": the last 64 decode kernels are bracketed, read back without a sync in between
@@ -627,6 +628,7 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!c || !key) return fail(DWKV_E_INVALID, "NULL argument");
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
   else if (!strcmp(key, "time_scan")) { c->opt_time_scan = value; c->scan_samples = 0; }
+  else if (!strcmp(key, "combine_warps")) c->opt_combine_warps = value;
   else if (!strcmp(key, "sketch_umma")) c->opt_sketch_umma = value;
   else if (!strcmp(key, "compress_umma")) c->opt_compress_umma = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
@@ -927,7 +929,10 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   Combine3Params cp;
   cp.pstart = sp.pstart; cp.part = sp.part; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
   cp.layer0 = layer0; cp.Lq = Lsel; cp.LH = sp.LH; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;
-  c->launches += launch_combine3(cp, P.n_segs, P.n_slots > 64LL * P.n_segs ? 16 : (P.n_slots > 8LL * P.n_segs ? 4 : 1), st);
+  const int split = (c->opt_combine_warps == 1 || c->opt_combine_warps == 4 || c->opt_combine_warps == 16)
+                        ? (int)c->opt_combine_warps
+                        : (P.n_slots > 64LL * P.n_segs ? 16 : (P.n_slots > 8LL * P.n_segs ? 4 : 1));
+  c->launches += launch_combine3(cp, P.n_segs, split, st);
   CU_OK(cudaGetLastError());
   return DWKV_OK;
 }
