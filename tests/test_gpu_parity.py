@@ -147,8 +147,9 @@ def test_split_invariance_p11(mod):
     cache, consts, kept = load(harness, wl, routings)
     q = gen.make_q(wl, device="cuda", gain=4.0)
     outs = []
-    base = {"max_unit_blocks": 0, "n_slices": 0, "interleave": 0, "unit_kb": 64}
-    for change in ({"max_unit_blocks": 1}, {"n_slices": 1}, {"n_slices": 7}, {"interleave": 1, "unit_kb": 1}, {}):
+    base = {"max_unit_blocks": 0, "n_slices": 0, "interleave": 0, "unit_kb": 64, "combine_warps": 0}
+    for change in ({"max_unit_blocks": 1}, {"n_slices": 1}, {"n_slices": 7}, {"interleave": 1, "unit_kb": 1}, {"interleave": -1},
+                   {"n_slices": 296, "combine_warps": 16}, {"combine_warps": 4}, {"combine_warps": 1, "n_slices": 592}, {}):
         for k, v in {**base, **change}.items():
             cache.set_option(k, v)
         outs.append(cache.decode_attention(-1, [0], q).double().cpu().numpy())
