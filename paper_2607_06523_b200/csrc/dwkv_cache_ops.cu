@@ -1,6 +1,7 @@
 // dwkv_cache_ops.cu -- load / dump auxiliaries of the cache (the append/compress kernel, step a4, is dwkv_compress.cu):
 //   scatter_raw_kernel  load pre-compressed token-ordered entries into the fragment-native pages
 //   gather_kernel       token-ordered dump of stored entries (bit-exact checks of routing and int4 dequantisation)
+//   compress_i8_warp_kernel / compress_i8_kernel   append/compress in 8-bit coefficient mode (option "coef_int8", reading A27)
 #include <algorithm>
 #include "dwkv_internal.h"
 
