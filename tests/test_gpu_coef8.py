@@ -145,20 +145,27 @@ def test_kernel_instances(mod, d, G, ranks):
     cache.destroy()
 
 
-def test_append_compress_against_oracle(mod):
+@pytest.mark.parametrize("shape", ["tiny", "8b", "r24"])
+def test_append_compress_against_oracle(mod, shape):
     """dwkv_append_compress in 8-bit mode from dense K/V: the fp32 projection differs from the oracle's fp64 one in the last bits,
     which can move a code across a rounding boundary (reading A15 iii carried over): coefficients equal on >= 99.5 % of entries and
     within one quantisation step elsewhere; attention of the GPU path within tolerance of the oracle on ITS OWN compressed cache."""
     binding, harness = mod
-    wl = dataclasses.replace(gen.WORKLOADS["tiny"], T=(96,))
+    # tiny: d = 64, ranks 8 / 16; 8b: d = 128, G = 4, ranks 8 / 16 / 32 (1, 2 and 4 lane groups per vector in the warp kernel)
+    # and calls of more than 64 tokens (several token chunks per (layer, head)); r24: a rank that is not a power of two
+    wl = {"tiny": dataclasses.replace(gen.WORKLOADS["tiny"], T=(96,)),
+          "8b": dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, w=2, H_kv=2, T=(96, 96)),
+          "r24": dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, w=2, H_kv=1, tier_ranks=(8, 24),
+                                     tier_frac=(0.5, 0.5), T=(96, 96))}[shape]
+    n_t = len(wl.tier_ranks)
     cache, consts = harness.make_cache(wl, n_seqs=2, max_tokens=512, coef_int8=True)
     BK, BV, gK, gV = consts
     oc = orc.OracleCache(wl.L, wl.w, wl.H_kv, wl.G, wl.d, wl.tier_ranks, f64(BK), f64(BV), f64(gK), f64(gV))
     rng = np.random.default_rng(5)
     t0 = {0: 0, 1: 0}
     for step in range(2):
-        n_new = [40, 23] if step == 0 else [9, 64]
-        tier = rng.integers(0, 2, sum(n_new)).astype(np.uint8); flag = (rng.random(sum(n_new)) < 0.5).astype(np.uint8)
+        n_new = ([40, 23] if step == 0 else [9, 64]) if shape == "tiny" else ([140, 23] if step == 0 else [9, 75])
+        tier = rng.integers(0, n_t, sum(n_new)).astype(np.uint8); flag = (rng.random(sum(n_new)) < 0.5).astype(np.uint8)
         ks, vs = [], []
         for s, n in enumerate(n_new):
             k, v = gen.make_dense_kv_chunk(wl, s, t0[s], n, BK, BV, gK, gV, device="cuda")
