@@ -554,6 +554,20 @@ def test_full_size_sampled_slices(mod, name):
                 check_output(o[s, l, sl], o_ref, float(np.abs(V).max()), f"{name} gain {gain} seq {s} (l,h)=({l},{h})")
                 if gain == 0.0:
                     assert np.allclose(o_ref, V.mean(axis=0)[None], atol=1e-12)
+        if gain == 8.0:
+            # per-layer calls, the launch shape of a real decoder (and, for one long sequence, the planner's small-call slicing
+            # with fewer slices than warps): the sampled layers against the oracle, for all sequences and for sequence 0 alone
+            for (l, h) in keep:
+                sl = slice(h * wl.G, (h + 1) * wl.G)
+                o_l = cache.decode_attention(l, ids, q[:, l].contiguous()).double().cpu().numpy()
+                s0 = sampled[-1]
+                o_1 = cache.decode_attention(l, [s0], q[s0:s0 + 1, l].contiguous()).double().cpu().numpy()
+                for s in sampled:
+                    tier, flag = routings[s]
+                    o_ref, V, _ = oracle_slice_from_kept(wl, consts, tier, flag, kept[s][(l, h)], qn[s, l, sl], l, h)
+                    check_output(o_l[s, sl], o_ref, float(np.abs(V).max()), f"{name} per-layer seq {s} (l,h)=({l},{h})")
+                    if s == s0:
+                        check_output(o_1[0, sl], o_ref, float(np.abs(V).max()), f"{name} per-layer single seq {s} (l,h)=({l},{h})")
     fp = cache.footprint()
     assert fp["used_bytes"] == sum(orc.footprint_bytes(t, f, wl.tier_ranks, wl.d, wl.L, wl.H_kv) for t, f in routings)
     cache.destroy()
