@@ -508,12 +508,13 @@ def main():
             qd = qs[0][:nb].contiguous()
             od = torch.empty(nb, L, wl.H_q, wl.d, dtype=torch.float32, device=dev)
             ws = torch.empty(binding.lib.dwkv_dense_workspace_bytes(nb, L, wl.H_q, wl.d, T), dtype=torch.uint8, device=dev)
-            dms = time_steps(lambda: binding.dense_decode_attention(K, V, qd, wl.H_kv, workspace=ws, out=od),
-                             max(3, args.steps // 2), args.warmup)
+            with ClockSampler(local) as cd:
+                dms = time_steps(lambda: binding.dense_decode_attention(K, V, qd, wl.H_kv, workspace=ws, out=od),
+                                 max(3, args.steps // 2), args.warmup)
             dense_bytes = 2 * K.numel() * 2
             comp_ms_same_batch = ms if nb == n_seq else extra.get(f"batch{nb}_us_per_step", ms * 1e3 * nb / n_seq) / 1e3
             extra["dense"] = {"batch": nb, "us_per_step": dms * 1e3, "GBps": dense_bytes / (dms * 1e-3) / 1e9,
-                              "frac_of_peak": dense_bytes / (dms * 1e-3) / 1e9 / peak,
+                              "frac_of_peak": dense_bytes / (dms * 1e-3) / 1e9 / peak, "clocks": cd.summary(),
                               "speedup_compressed_vs_dense": dms / comp_ms_same_batch,
                               "required_speedup_0.7x_ratio": 0.7 * extra["compression_ratio"]}
             del K, V
