@@ -197,7 +197,8 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *                     bf16 value, so every call keeps its argument types: dwkv_append_raw quantises the bf16 coefficients it is
  *                     given (lossless if they already lie on the grid), dwkv_append_compress quantises the fp32 projection and
  *                     takes the residual against the dequantised coefficients, dwkv_export_tokens returns code * 2^e as bf16,
- *                     dwkv_decode_attention scans the byte planes. Needs a basis rank <= 32 (INVALID otherwise) and an empty
+ *                     dwkv_decode_attention scans the byte planes (its score contraction runs in fp16 in this mode: the projected
+ *                     query q~ = scale * log2(e) * B_K (g_K * q) is split hi + lo in fp16 and clamped to +-65504). Needs a basis rank <= 32 (INVALID otherwise) and an empty
  *                     cache (STATE otherwise). 0 (default) = bf16 coefficients.
  * Any change invalidates the cached plan. Errors: INVALID (unknown key). */
 int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);

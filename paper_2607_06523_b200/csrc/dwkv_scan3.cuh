@@ -75,6 +75,25 @@ __device__ __forceinline__ uint32_t u8pair_to_bf16x2(uint32_t w, int k) {
   asm("prmt.b32 %0, %1, %2, %3;" : "=r"(f1) : "r"(w), "r"(0x4B000000u), "r"(0x7440u | (uint32_t)(2 * k + 1)));
   return pack_bf16x2(__uint_as_float(f0) - 8388736.f, __uint_as_float(f1) - 8388736.f);
 }
+// 8-bit coefficient mode, K side: bytes 2k, 2k+1 of w -> f16x2 (code_lo, code_hi), exact: one PRMT builds (0x6400 | u) = 1024 + u
+// twice, one packed subtraction of 1152 = 1024 + 128 removes the offset (fp16 has ulp 1 in [1024, 2048)).
+__device__ __forceinline__ uint32_t u8pair_to_f16x2(uint32_t w, int k) {
+  uint32_t x, r;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(x) : "r"(w), "r"(0x64646464u), "r"(k ? 0x4342u : 0x4140u));
+  asm("sub.f16x2 %0, %1, %2;" : "=r"(r) : "r"(x), "r"(0x64806480u));
+  return r;
+}
+// score MMAs of the 8-bit mode: q~ (hi + lo in fp16) x integer codes in fp16
+__device__ __forceinline__ void mma16h(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ void mma8h(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0) {
+  asm("mma.sync.aligned.m16n8k8.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a0), "r"(a1), "r"(b0));
+}
 // exponent byte (e + 127) at bit position sh of w -> 2^e
 __device__ __forceinline__ float exp_byte_to_scale(uint32_t w, int sh) { return __uint_as_float(((w >> sh) & 0xffu) << 23); }
 __device__ __forceinline__ void sts128(uint32_t a, int x, int y, int z, int w) {
@@ -103,6 +122,17 @@ __device__ __forceinline__ void split_bf16x2(float x, float y, uint32_t& hi, uin
   hi = pack_bf16x2(x, y);
   const float hx = __uint_as_float(hi << 16), hy = __uint_as_float(hi & 0xffff0000u);
   lo = pack_bf16x2(x - hx, y - hy);
+}
+
+// the same split in fp16 (8-bit coefficient mode: q~ feeds an f16 MMA): 11 + 11 bits; clamped to the fp16 range so that an
+// absurdly large q saturates the score instead of producing inf - inf
+__device__ __forceinline__ void split_f16x2(float x, float y, uint32_t& hi, uint32_t& lo) {
+  x = fminf(fmaxf(x, -65504.f), 65504.f); y = fminf(fmaxf(y, -65504.f), 65504.f);
+  const __half2 h = __floats2half2_rn(x, y);
+  const float2 hf = __half22float2(h);
+  const __half2 l = __floats2half2_rn(x - hf.x, y - hf.y);
+  hi = *reinterpret_cast<const uint32_t*>(&h);
+  lo = *reinterpret_cast<const uint32_t*>(&l);
 }
 
 __device__ __forceinline__ Unit load_unit(const Unit* u) {

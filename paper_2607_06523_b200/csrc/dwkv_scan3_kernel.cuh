@@ -73,7 +73,7 @@ __device__ __forceinline__ void prologue_load(ProLoads<NKB, D>& pl, const Scan3P
   }
 }
 
-template <int NKB, int D, bool PAIR>
+template <int NKB, int D, bool PAIR, bool I8 = false>
 __device__ __forceinline__ void prologue_compute(QRegs<NKB, D, PAIR>& q, const ProLoads<NKB, D>& pl, const Scan3Params& p, const int seg,
                                                  const int lane) {
   constexpr int NKK = D / 16, JB = ProLoads<NKB, D>::JB;
@@ -126,7 +126,8 @@ __device__ __forceinline__ void prologue_compute(QRegs<NKB, D, PAIR>& q, const P
 #pragma unroll
   for (int jj = 0; jj < NKB; ++jj) {
     uint32_t hi, lo;
-    split_bf16x2((c[jj][0] + c[jj][2]) * p.cscale, (c[jj][1] + c[jj][3]) * p.cscale, hi, lo);
+    if constexpr (I8) split_f16x2((c[jj][0] + c[jj][2]) * p.cscale, (c[jj][1] + c[jj][3]) * p.cscale, hi, lo);   // f16 score MMAs
+    else split_bf16x2((c[jj][0] + c[jj][2]) * p.cscale, (c[jj][1] + c[jj][3]) * p.cscale, hi, lo);
     if constexpr (PAIR) {
       q.qa[jj][0] = hi & mA; q.qa[jj][1] = lo & mA; q.qa[jj][2] = hi & ~mA; q.qa[jj][3] = lo & ~mA;
     } else {
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
 #pragma unroll 1
     for (int k = 0; k < NS; ++k) fetch_one(k);
     __syncwarp();
-    prologue_compute<NKB, D, PAIR>(q, pl, p, ws.x, lane);
+    prologue_compute<NKB, D, PAIR, I8>(q, pl, p, ws.x, lane);
     state_reset<NKB, D>(st);
   }
 
@@ -319,7 +320,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
       prologue_load<NKB, D, PAIR>(pl, p, seg, lane);       // L2 hits: the fetch cursor prefetched them when it crossed over
       flush_partial<NKB, D, PAIR>(st, p, slot_next, lane);
       slot_next = __ldg(p.pstart + seg);       // a segment entered inside a slice is entered at its start: its first slot
-      prologue_compute<NKB, D, PAIR>(q, pl, p, seg, lane);
+      prologue_compute<NKB, D, PAIR, I8>(q, pl, p, seg, lane);
       state_reset<NKB, D>(st);
       cur_seg = seg;
       ++n_entered;

@@ -45,12 +45,12 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
       if constexpr (TB == 4) {
         const uint2 a = lds64(sp + i * 256 + lane * 8);
         const uint2 b = lds64(sp + COEF + i * 256 + lane * 8);
-        kw[i][0] = u8pair_to_bf16x2(a.x, 0); kw[i][1] = u8pair_to_bf16x2(a.x, 1); kw[i][2] = u8pair_to_bf16x2(a.y, 0); kw[i][3] = u8pair_to_bf16x2(a.y, 1);
+        kw[i][0] = u8pair_to_f16x2(a.x, 0); kw[i][1] = u8pair_to_f16x2(a.x, 1); kw[i][2] = u8pair_to_f16x2(a.y, 0); kw[i][3] = u8pair_to_f16x2(a.y, 1);
         vw[i][0] = u8pair_to_bf16x2(b.x, 0); vw[i][1] = u8pair_to_bf16x2(b.x, 1); vw[i][2] = u8pair_to_bf16x2(b.y, 0); vw[i][3] = u8pair_to_bf16x2(b.y, 1);
       } else {
         const uint32_t a = lds32(sp + i * 128 + lane * 4);
         const uint32_t b = lds32(sp + COEF + i * 128 + lane * 4);
-        kw[i][0] = u8pair_to_bf16x2(a, 0); kw[i][1] = u8pair_to_bf16x2(a, 1);
+        kw[i][0] = u8pair_to_f16x2(a, 0); kw[i][1] = u8pair_to_f16x2(a, 1);
         vw[i][0] = u8pair_to_bf16x2(b, 0); vw[i][1] = u8pair_to_bf16x2(b, 1);
       }
     }
@@ -93,12 +93,20 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
     float c[4] = {I8 ? 0.f : cinit, I8 ? 0.f : cinit, 0.f, 0.f};
     if constexpr (PAIR) {    // k = (tile 2x: 8 rank columns | tile 2x+1: 8 rank columns), block-diagonal A
 #pragma unroll
-      for (int i = 0; i < NK; ++i) mma16(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
+      for (int i = 0; i < NK; ++i) {
+        if constexpr (I8) mma16h(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
+        else mma16(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
+      }
     } else {                 // k = 16 rank columns of tile x
 #pragma unroll
-      for (int pi = 0; pi < NK / 2; ++pi)
-        mma16(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
-      if constexpr (NK & 1) mma8(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
+      for (int pi = 0; pi < NK / 2; ++pi) {
+        if constexpr (I8) mma16h(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
+        else mma16(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
+      }
+      if constexpr (NK & 1) {
+        if constexpr (I8) mma8h(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
+        else mma8(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
+      }
     }
     if constexpr (I8) {
       s[x][0] = fmaf(ksc[x][0], c[0] + c[2], cinit);
