@@ -27,7 +27,8 @@ __device__ __forceinline__ void lds_kcodes(uint32_t (&w)[D / 32], uint32_t base,
 }
 
 // NK = rank / 8 of the class, RESID = flagged class, NKB / D / PAIR = kernel instance (see State / QRegs), I8 = 8-bit coefficient
-// planes (dwkv_layout.cuh): codes are widened to exact bf16 integers in registers, the token's power-of-two scale multiplies its
+// planes (dwkv_layout.cuh): codes are widened to exact 16-bit floating integers in registers (K: fp16, the score MMA runs in fp16
+// with q~ split hi + lo in fp16; V: bf16, because p * 2^e needs the bf16 exponent range), the token's power-of-two scale multiplies its
 // score after the MMA and its p before the value MMA -- the contractions themselves are unchanged.
 template <int NK, bool RESID, int NKB, int D, bool PAIR, bool I8>
 __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp, const int nv, const int lane,
