@@ -95,7 +95,10 @@ __device__ __forceinline__ void mma8h(float (&d)[4], uint32_t a0, uint32_t a1, u
       : "r"(a0), "r"(a1), "r"(b0));
 }
 // exponent byte (e + 127) at bit position sh of w -> 2^e
-__device__ __forceinline__ float exp_byte_to_scale(uint32_t w, int sh) { return __uint_as_float(((w >> sh) & 0xffu) << 23); }
+// (one PRMT isolates the byte, the multiply by 2^23 can issue on the FMA pipe: the ALU pipe is the busy one in this mode)
+__device__ __forceinline__ float exp_byte_to_scale(uint32_t w, int sh) {
+  return __uint_as_float(__byte_perm(w, 0u, 0x4440u + (uint32_t)(sh >> 3)) * 0x00800000u);
+}
 __device__ __forceinline__ void sts128(uint32_t a, int x, int y, int z, int w) {
   asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
