@@ -20,7 +20,8 @@ What it computes (plain definition, fp64, token-ordered storage, no blocking / f
   Routing (reading A15): class = 2*tier + flag, slot = number of earlier tokens of the sequence in that class.
 
 Inputs are the stored numbers (bf16 / fp16 / int4 values held exactly in float64 / float16 / int8 arrays).
-Pins: tests/test_oracle_pins.py (P1-P10, P12, P13 of SURVEY.md §8c). The paper prints no worked numeric example
+Pins: tests/test_oracle_pins.py (P1-P10, P12, P13 of SURVEY.md §8c) and tests/test_oracle_pins_windows.py (P14 hand-derived
+append case with two depth windows, P15 / P16 multi-window decode and append against loop-built references). The paper prints no worked numeric example
 of this path, so Eq. (3)'s 0.027 and the 72.8 tok/s are *parity unpinned* (out of scope, need real activations).
 """
 from __future__ import annotations
