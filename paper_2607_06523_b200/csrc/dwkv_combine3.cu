@@ -6,14 +6,14 @@
 
 namespace dwkv {
 
-bool launch_scan3_d64_p0(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d64_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d128_p0(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d64_p0_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d64_p1_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d128_p0_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
-bool launch_scan3_d128_p1_i8(const Scan3Params& p, int n_sms, cudaStream_t s);
+bool launch_scan3_d64_p0(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d64_p1(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d128_p0(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d128_p1(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d64_p0_i8(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d64_p1_i8(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d128_p0_i8(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
+bool launch_scan3_d128_p1_i8(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);
 
 namespace {
 using namespace dwkv::dev;
@@ -149,18 +149,19 @@ __global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Co
 
 int scan3_num_slices(int n_sms) { return n_sms * 8; }
 
-int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s) {
+int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err) {
   const bool pair = p.G <= 4;
   bool ok = false;
+  *err = cudaSuccess;
   if (p.i8) {
-    if (p.d == 128) ok = pair ? launch_scan3_d128_p1_i8(p, n_sms, s) : launch_scan3_d128_p0_i8(p, n_sms, s);
-    else if (p.d == 64) ok = pair ? launch_scan3_d64_p1_i8(p, n_sms, s) : launch_scan3_d64_p0_i8(p, n_sms, s);
-  } else if (p.d == 128) ok = pair ? launch_scan3_d128_p1(p, n_sms, s) : launch_scan3_d128_p0(p, n_sms, s);
-  else if (p.d == 64) ok = pair ? launch_scan3_d64_p1(p, n_sms, s) : launch_scan3_d64_p0(p, n_sms, s);
+    if (p.d == 128) ok = pair ? launch_scan3_d128_p1_i8(p, n_sms, s, err) : launch_scan3_d128_p0_i8(p, n_sms, s, err);
+    else if (p.d == 64) ok = pair ? launch_scan3_d64_p1_i8(p, n_sms, s, err) : launch_scan3_d64_p0_i8(p, n_sms, s, err);
+  } else if (p.d == 128) ok = pair ? launch_scan3_d128_p1(p, n_sms, s, err) : launch_scan3_d128_p0(p, n_sms, s, err);
+  else if (p.d == 64) ok = pair ? launch_scan3_d64_p1(p, n_sms, s, err) : launch_scan3_d64_p0(p, n_sms, s, err);
   return ok ? 1 : 0;
 }
 
-int launch_combine3(const Combine3Params& p, int n_segs, int split, cudaStream_t s) {
+int launch_combine3(const Combine3Params& p, int n_segs, int split, cudaStream_t s, cudaError_t* err) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = split > 1 ? dim3(n_segs, p.G) : dim3(n_segs);       // split: 16 warps share the partial list of one head
   cfg.blockDim = dim3(split > 4 ? 32 * split : 128);
@@ -172,13 +173,13 @@ int launch_combine3(const Combine3Params& p, int n_segs, int split, cudaStream_t
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if (p.d == 128) {
-    if (split == 16) cudaLaunchKernelEx(&cfg, combine3_kernel<128, 16>, p);
-    else if (split == 4) cudaLaunchKernelEx(&cfg, combine3_kernel<128, 4>, p);
-    else cudaLaunchKernelEx(&cfg, combine3_kernel<128, 1>, p);
+    if (split == 16) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 16>, p);
+    else if (split == 4) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 4>, p);
+    else *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 1>, p);
   } else {
-    if (split == 16) cudaLaunchKernelEx(&cfg, combine3_kernel<64, 16>, p);
-    else if (split == 4) cudaLaunchKernelEx(&cfg, combine3_kernel<64, 4>, p);
-    else cudaLaunchKernelEx(&cfg, combine3_kernel<64, 1>, p);
+    if (split == 16) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 16>, p);
+    else if (split == 4) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 4>, p);
+    else *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 1>, p);
   }
   return 1;
 }

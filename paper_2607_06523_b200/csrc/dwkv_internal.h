@@ -38,6 +38,16 @@ struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.c
   int32_t H, G, r, d;
   float cscale;                // softmax_scale * log2(e)
   int32_t i8;                  // 8-bit coefficient planes (dwkv_layout.cuh)
+  // fused split-combine (step a3 inside the decode kernel; per-layer calls): the warps of a CTA take CONSECUTIVE slices, merge their
+  // end-of-slice partials per segment in shared memory and write one partial per (CTA, segment); every partial written is an arrival
+  // on the segment's counter, and the CTA of the last arrival merges the segment's partials, back-projects and writes `out`.
+  int32_t fuse;                // 1 = fused combine (no combine3 launch), 0 = partials only
+  int32_t spc;                 // fuse: slices per CTA (1..8); slice of warp w of CTA c = c * spc + w
+  const int32_t* wlast;        // fuse: [n_slices] partial slot of the slice's last segment (shared by the warps of a CTA that end in it)
+  int32_t* segcnt;             // fuse: [n_segs] arrival counters, zero between calls (the finishing CTA resets them)
+  const __nv_bfloat16* BV;     // fuse: [M][H][r][d]
+  const __nv_bfloat16* gV;     // fuse: [L][H][d]
+  float* out;                  // fuse: [n_seqs][Lq][Hq][d]
 };
 
 struct Combine3Params {
@@ -69,8 +79,8 @@ struct CacheGeom {
 
 // kernel launchers (dwkv_combine3.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
 int scan3_num_slices(int n_sms);
-int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s);                 // 0 = no instance for this shape
-int launch_combine3(const Combine3Params& p, int n_segs, int split /* 1, 4 or 16 warps per (segment, head) */, cudaStream_t s);
+int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err);   // 0 = no instance for this shape; *err = launch status
+int launch_combine3(const Combine3Params& p, int n_segs, int split /* 1, 4 or 16 warps per (segment, head) */, cudaStream_t s, cudaError_t* err);
 int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n,
                        const __nv_bfloat16* coefK, const __nv_bfloat16* coefV,
                        const float* residK, const float* residV, const uint8_t* codeK, const uint8_t* codeV,

@@ -146,13 +146,22 @@ def test_split_invariance_p11(mod):
     routings = [gen.make_routing(wl, 0)]
     cache, consts, kept = load(harness, wl, routings)
     q = gen.make_q(wl, device="cuda", gain=4.0)
-    outs = []
-    base = {"max_unit_blocks": 0, "n_slices": 0, "interleave": 0, "unit_kb": 64, "combine_warps": 0}
+    outs, shapes = [], []
+    base = {"max_unit_blocks": 0, "n_slices": 0, "interleave": 0, "unit_kb": 64, "combine_warps": 0, "fuse_combine": 0}
     for change in ({"max_unit_blocks": 1}, {"n_slices": 1}, {"n_slices": 7}, {"interleave": 1, "unit_kb": 1}, {"interleave": -1},
-                   {"n_slices": 296, "combine_warps": 16}, {"combine_warps": 4}, {"combine_warps": 1, "n_slices": 592}, {}):
+                   {"n_slices": 296, "combine_warps": 16}, {"combine_warps": 4}, {"combine_warps": 1, "n_slices": 592}, {},
+                   {"fuse_combine": 1}, {"fuse_combine": 1, "n_slices": 148}, {"fuse_combine": 1, "n_slices": 592, "max_unit_blocks": 1}):
         for k, v in {**base, **change}.items():
             cache.set_option(k, v)
         outs.append(cache.decode_attention(-1, [0], q).double().cpu().numpy())
+        # the plan really is the one asked for (a cached plan must not survive an option change)
+        shapes.append((int(cache.get_stat("plan_slices")), int(cache.get_stat("plan_slots")), int(cache.get_stat("plan_fused"))))
+        want = change.get("n_slices", 0)
+        if want:
+            assert shapes[-1][0] == want, (change, shapes[-1])
+        assert shapes[-1][2] == (1 if change.get("fuse_combine", 0) == 1 else 0)
+    assert shapes[1][1] == wl.L * wl.H_kv            # one slice: one partial per segment
+    assert len(set(shapes)) >= 5, shapes
     for o in outs[1:]:
         assert rel_l2(o, outs[0]) < 1e-3
     for o in outs:
