@@ -240,6 +240,47 @@ int dwkv_route_tokens(int64_t n, const float* phi, const float* u, int32_t n_tie
 int dwkv_router_thresholds(int64_t n, const float* phi, const float* u, int32_t n_tiers, const float* tier_frac, float flag_frac,
                            float* tau_logit, float* tau_flag_logit);
 
+/* ---- probe-driven controller (reading A28). Host-only state machine; all
+ * pointers are HOST memory. One state (delta_m, quiet_m) per depth window m; thresholds live in logit space (reading A26) and
+ * tau_m = base + delta_m. One probe interval = one dwkv_controller_step with the Eq. (3) errors dwkv_probe_error returned:
+ *     e_m = max of the errors reported for window m (windows without a probe keep their state)
+ *     e_m > tol_m  ->  delta_m = max(delta_m - step_down, delta_min), quiet_m = 0                     "the router lowers tau_m"
+ *     else quiet_m += 1, and when quiet_m == patience: delta_m = min(delta_m + step_up, delta_max), quiet_m = 0
+ *                                                        "below tolerance for several probe intervals, tau_m is increased"
+ * fp32, one rounding per operation (bit-exact against the oracle). Because a token's (tier, flag) is shared by all layers and
+ * heads (reading A4), dwkv_controller_thresholds returns base + min_m delta_m: the thresholds dwkv_route_tokens applies to NEW
+ * tokens. Stored tokens are never re-tiered (their original vectors no longer exist: promotion is impossible).
+ * Errors: INVALID (NULL, sizes, negative steps / tolerances, delta_min > 0 or delta_max < 0, window index out of range, NaN error). */
+typedef struct dwkv_controller dwkv_controller; /* opaque; owned by the library */
+typedef struct {
+  int32_t n_windows;     /* L / w                                                                                   */
+  int32_t patience;      /* probe intervals below tolerance before tau_m is raised (>= 1)                           */
+  float tol_default;     /* tolerance on e_{l,h} for every window ...                                               */
+  const float* tol;      /* ... or host fp32 [n_windows] "window-specific tolerance" (copied); NULL = tol_default    */
+  float step_down;       /* logit-space decrement of tau_m on a violation (>= 0)                                    */
+  float step_up;         /* logit-space increment after `patience` quiet intervals (>= 0)                           */
+  float delta_min;       /* bounds of delta_m: delta_min <= 0 <= delta_max                                          */
+  float delta_max;
+} dwkv_controller_config;
+int dwkv_controller_create(const dwkv_controller_config* cfg, dwkv_controller** out);
+void dwkv_controller_destroy(dwkv_controller* ctl);
+/* window, e: host [n_probes]: depth window (layer / w) and Eq. (3) error of every probed (layer, kv head) of this interval. */
+int dwkv_controller_step(dwkv_controller* ctl, int32_t n_probes, const int32_t* window, const float* e);
+/* delta: host fp32 [n_windows], quiet: host int32 [n_windows]; either may be NULL. */
+int dwkv_controller_state(const dwkv_controller* ctl, float* delta, int32_t* quiet);
+/* tau_logit[k] = base_tau_logit[k] + min_m delta_m (k < n_tiers - 1), *tau_flag_logit = base_flag_logit + min_m delta_m. */
+int dwkv_controller_thresholds(const dwkv_controller* ctl, int32_t n_tiers, const float* base_tau_logit, float base_flag_logit,
+                               float* tau_logit, float* tau_flag_logit);
+
+/* Router features from the decode path ("accumulated attention mass, maximum attention spike"; reading A28):
+ * for one sequence, layer and query vector the softmax probabilities p[hq, t] of all T cached tokens over the compressed cache are
+ * formed (the same scores the decode kernel uses; nothing is reconstructed), and
+ *     mass[t]  += sum_hq p[hq, t]                 spike[t] = max(spike[t], max_hq p[hq, t])
+ * so that calling it on every probe step accumulates phi_0 and phi_1 of Eq. (2) on the device. Token order = append order.
+ *   q     dev bf16 [H_q, d]        mass, spike   dev fp32 [T], T = dwkv_seq_len (read-modify-write; zero them before the first probe)
+ * Enqueues on `stream`; scratch is owned by the handle. Errors: INVALID, STATE (no basis / gates), EMPTY (T = 0), CUDA. */
+int dwkv_probe_token_stats(dwkv_cache* c, int32_t layer, int32_t seq_id, const void* q, float* mass, float* spike, void* stream);
+
 /* ---- dense bf16 comparison kernel (BASELINE.json "from-scratch dense-bf16-cache decode kernel")
  * Plain softmax attention over an uncompressed cache. K, V: dev bf16 [n_seqs, L, H_kv, T, d] (all sequences length T);
  * q: dev bf16 [n_seqs, L, H_q, d]; out: dev fp32 [n_seqs, L, H_q, d]; workspace: dev, >= dwkv_dense_workspace_bytes(). */

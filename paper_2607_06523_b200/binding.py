@@ -23,6 +23,8 @@ EXPORTED = [
     "dwkv_append_raw", "dwkv_export_tokens", "dwkv_reset_seq", "dwkv_seq_len", "dwkv_footprint", "dwkv_set_option",
     "dwkv_launch_count", "dwkv_get_stat", "dwkv_last_error", "dwkv_dense_workspace_bytes", "dwkv_dense_decode_attention",
     "dwkv_build_basis", "dwkv_export_basis", "dwkv_probe_error", "dwkv_route_tokens", "dwkv_router_thresholds",
+    "dwkv_probe_token_stats", "dwkv_controller_create", "dwkv_controller_destroy", "dwkv_controller_step", "dwkv_controller_state",
+    "dwkv_controller_thresholds",
 ]
 
 
@@ -37,6 +39,11 @@ class dwkv_config(C.Structure):
                 ("d_head", C.c_int32), ("n_tiers", C.c_int32), ("tier_rank", C.c_int32 * 4), ("max_seqs", C.c_int32),
                 ("max_tokens_per_seq", C.c_int64), ("softmax_scale", C.c_float), ("device", C.c_int32),
                 ("arena", C.c_void_p), ("arena_bytes", C.c_uint64)]
+
+
+class dwkv_controller_config(C.Structure):
+    _fields_ = [("n_windows", C.c_int32), ("patience", C.c_int32), ("tol_default", C.c_float), ("tol", C.c_void_p),
+                ("step_down", C.c_float), ("step_up", C.c_float), ("delta_min", C.c_float), ("delta_max", C.c_float)]
 
 
 class dwkv_raw_tokens(C.Structure):
@@ -64,6 +71,13 @@ def _load() -> C.CDLL:
     lib.dwkv_probe_error.argtypes = [vp, i32, i32, i32, vp, vp, vp, C.c_float, vp, vp]
     lib.dwkv_route_tokens.argtypes = [i64, vp, vp, i32, vp, C.c_float, vp, vp]
     lib.dwkv_router_thresholds.argtypes = [i64, vp, vp, i32, vp, C.c_float, vp, vp]
+    lib.dwkv_probe_token_stats.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+    lib.dwkv_controller_create.argtypes = [C.POINTER(dwkv_controller_config), C.POINTER(vp)]
+    lib.dwkv_controller_destroy.argtypes = [vp]
+    lib.dwkv_controller_destroy.restype = None
+    lib.dwkv_controller_step.argtypes = [vp, i32, vp, vp]
+    lib.dwkv_controller_state.argtypes = [vp, vp, vp]
+    lib.dwkv_controller_thresholds.argtypes = [vp, i32, vp, C.c_float, vp, vp]
     lib.dwkv_append_compress.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.dwkv_decode_attention.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.dwkv_append_raw.argtypes = [vp, i32, i32, vp, vp, C.POINTER(dwkv_raw_tokens), vp]
@@ -170,6 +184,11 @@ class DwkvCache:
                                     _ptr(V_ref, torch.bfloat16), float(eps), _ptr(e, torch.float32), _stream()))
         return e
 
+    def probe_token_stats(self, layer: int, seq_id: int, q: torch.Tensor, mass: torch.Tensor, spike: torch.Tensor):
+        """q: bf16 [H_q, d]; mass, spike: fp32 [T] on the device, updated in place (mass += sum_hq p, spike = max(spike, max_hq p))."""
+        _check(lib.dwkv_probe_token_stats(self._h, layer, seq_id, _ptr(q, torch.bfloat16), _ptr(mass, torch.float32),
+                                          _ptr(spike, torch.float32), _stream()))
+
     def set_gates(self, gK: torch.Tensor, gV: torch.Tensor):
         _check(lib.dwkv_set_gates(self._h, _ptr(gK, torch.bfloat16), _ptr(gV, torch.bfloat16), _stream()))
 
@@ -246,6 +265,62 @@ def dense_decode_attention(K: torch.Tensor, V: torch.Tensor, q: torch.Tensor, n_
                                            _ptr(out, torch.float32), _ptr(workspace), n_seqs, L, H, Hq, d, T,
                                            softmax_scale, _stream()))
     return out
+
+
+class Controller:
+    """Probe-driven threshold controller (dwkv_controller_* of the C ABI). Host-only."""
+
+    def __init__(self, n_windows: int, tol, step_down: float, step_up: float, patience: int, delta_min: float, delta_max: float):
+        cfg = dwkv_controller_config()
+        cfg.n_windows, cfg.patience = n_windows, patience
+        tol_arr = None
+        if np.ndim(tol) == 0:
+            cfg.tol_default, cfg.tol = float(tol), None
+        else:
+            tol_arr = np.ascontiguousarray(tol, np.float32)
+            assert tol_arr.shape == (n_windows,)
+            cfg.tol_default, cfg.tol = 0.0, tol_arr.ctypes.data
+        cfg.step_down, cfg.step_up, cfg.delta_min, cfg.delta_max = step_down, step_up, delta_min, delta_max
+        self.n_windows = n_windows
+        h = C.c_void_p()
+        rc = lib.dwkv_controller_create(C.byref(cfg), C.byref(h))
+        if rc:
+            raise DwkvError(rc, "dwkv_controller_create")
+        self._h = h
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib.dwkv_controller_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def step(self, window, e):
+        w = _i32(window); x = np.ascontiguousarray(e, np.float32)
+        assert len(w) == len(x)
+        rc = lib.dwkv_controller_step(self._h, len(w), w.ctypes.data, x.ctypes.data)
+        if rc:
+            raise DwkvError(rc, "dwkv_controller_step")
+
+    def state(self):
+        d = np.zeros(self.n_windows, np.float32); q = np.zeros(self.n_windows, np.int32)
+        rc = lib.dwkv_controller_state(self._h, d.ctypes.data, q.ctypes.data)
+        if rc:
+            raise DwkvError(rc, "dwkv_controller_state")
+        return d, q
+
+    def thresholds(self, base_tau_logit, base_flag_logit: float):
+        base = np.ascontiguousarray(base_tau_logit, np.float32)
+        tau = np.zeros(max(len(base), 1), np.float32); tf = C.c_float(0.0)
+        rc = lib.dwkv_controller_thresholds(self._h, len(base) + 1, base.ctypes.data if len(base) else None, float(base_flag_logit),
+                                            tau.ctypes.data, C.addressof(tf))
+        if rc:
+            raise DwkvError(rc, "dwkv_controller_thresholds")
+        return tau[:len(base)], float(tf.value)
 
 
 def route_tokens(phi: np.ndarray, u: np.ndarray, tau_logit, tau_flag_logit: float, n_tiers: int):

@@ -5,7 +5,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["dwkv_api.cu", "dwkv_combine3.cu", "dwkv_scan3_d128_p1.cu", "dwkv_scan3_d128_p0.cu", "dwkv_scan3_d64_p1.cu", "dwkv_scan3_d64_p0.cu", "dwkv_scan3_d128_p1_i8.cu", "dwkv_scan3_d128_p0_i8.cu", "dwkv_scan3_d64_p1_i8.cu", "dwkv_scan3_d64_p0_i8.cu", "dwkv_cache_ops.cu", "dwkv_compress.cu", "dwkv_dense.cu", "dwkv_basis.cu", "dwkv_router.cu"]
+SOURCES = ["dwkv_api.cu", "dwkv_combine3.cu", "dwkv_scan3_d128_p1.cu", "dwkv_scan3_d128_p0.cu", "dwkv_scan3_d64_p1.cu", "dwkv_scan3_d64_p0.cu", "dwkv_scan3_d128_p1_i8.cu", "dwkv_scan3_d128_p0_i8.cu", "dwkv_scan3_d64_p1_i8.cu", "dwkv_scan3_d64_p0_i8.cu", "dwkv_cache_ops.cu", "dwkv_compress.cu", "dwkv_dense.cu", "dwkv_basis.cu", "dwkv_router.cu", "dwkv_controller.cu"]
 LIB = os.path.join(HERE, "libdwkv.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",

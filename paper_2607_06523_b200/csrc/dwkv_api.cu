@@ -256,6 +256,24 @@ int upload(dwkv_cache* c, DevBuf& dst, const void* src, size_t bytes, cudaStream
   return DWKV_OK;
 }
 
+// where the stored tokens [t0, t0 + n) of a sequence live: the table the gather / token-statistics kernels walk
+void stored_token_table(const dwkv_cache* c, const SeqState& S, int64_t t0, int64_t n, std::vector<TokDst>* out) {
+  out->resize((size_t)n);
+  for (int64_t i = 0; i < n; ++i) {
+    const int k = 2 * S.tier[t0 + i] + S.flag[t0 + i];
+    const int64_t sl = S.slot[t0 + i], tpp = c->cl[k].tokens_per_page;
+    TokDst td;
+    td.page_off = (int64_t)S.pages[k][sl / tpp] * (int64_t)c->page_bytes;
+    td.blk = (int32_t)((sl % tpp) / kBlockTok);
+    td.slot = (int32_t)((sl % tpp) % kBlockTok);
+    td.cls = k;
+    td.ridx = -1;
+    td.src = (int32_t)i;
+    td.pad_ = 0;
+    (*out)[(size_t)i] = td;
+  }
+}
+
 int zero_new_pages(dwkv_cache* c, const std::vector<int32_t>& pages, cudaStream_t st) {
   for (int32_t pg : pages) CU_OK(cudaMemsetAsync(c->arena + (size_t)pg * c->page_bytes, 0, c->page_bytes, st));
   return DWKV_OK;
@@ -567,20 +585,8 @@ int dwkv_export_tokens(dwkv_cache* c, int32_t seq_id, int64_t t0, int64_t n, con
   if (t0 < 0 || n < 0 || t0 + n > (int64_t)S.tier.size() || n > 0x7fffffff) return fail(DWKV_E_INVALID, "token range out of bounds");
   if (n == 0) return DWKV_OK;
   cudaStream_t st = (cudaStream_t)stream;
-  std::vector<TokDst> dst(n);
-  for (int64_t i = 0; i < n; ++i) {
-    const int k = 2 * S.tier[t0 + i] + S.flag[t0 + i];
-    const int64_t sl = S.slot[t0 + i], tpp = c->cl[k].tokens_per_page;
-    TokDst td;
-    td.page_off = (int64_t)S.pages[k][sl / tpp] * (int64_t)c->page_bytes;
-    td.blk = (int32_t)((sl % tpp) / kBlockTok);
-    td.slot = (int32_t)((sl % tpp) % kBlockTok);
-    td.cls = k;
-    td.ridx = -1;
-    td.src = (int32_t)i;
-    td.pad_ = 0;
-    dst[i] = td;
-  }
+  std::vector<TokDst> dst;
+  stored_token_table(c, S, t0, n, &dst);
   int rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
   if (rc) return rc;
   DumpPtrs o;
@@ -1034,6 +1040,27 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
   }
   cudaStream_t st = (cudaStream_t)stream;
   return decode3(c, layer, n_seqs, seq_ids, q, out, st);
+}
+
+extern "C" int dwkv_probe_token_stats(dwkv_cache* c, int32_t layer, int32_t seq_id, const void* q, float* mass, float* spike, void* stream) {
+  if (!c || !q || !mass || !spike) return fail(DWKV_E_INVALID, "NULL argument");
+  if (layer < 0 || layer >= c->geom.L) return fail(DWKV_E_INVALID, "layer out of range");
+  if (check_seq(c, seq_id)) return fail(DWKV_E_INVALID, "bad sequence id");
+  if (!c->basis_set || !c->gates_set) return fail(DWKV_E_STATE, "basis and gates must be set before the probe");
+  const SeqState& S = c->seqs[seq_id];
+  const int64_t T = (int64_t)S.tier.size();
+  if (T == 0) return fail(DWKV_E_EMPTY, "token statistics of an empty sequence");
+  if (T > 0x7fffffff) return fail(DWKV_E_INVALID, "sequence too long");
+  cudaStream_t st = (cudaStream_t)stream;
+  std::vector<TokDst> dst;
+  stored_token_table(c, S, 0, T, &dst);
+  int rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
+  if (rc) return rc;
+  CU_OK(c->probe_ws.reserve(token_stats_scratch_bytes(c->geom, T)));
+  c->launches += launch_token_stats(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)T, layer, (const __nv_bfloat16*)q, c->BK, c->gK,
+                                    c->softmax_scale * 1.4426950408889634f, (float*)c->probe_ws.p, mass, spike, st);
+  CU_OK(cudaGetLastError());
+  return DWKV_OK;
 }
 
 extern "C" int dwkv_probe_error(dwkv_cache* c, int32_t layer, int32_t seq_id, int32_t n_q, const void* q, const void* K_ref,

@@ -404,7 +404,132 @@ __global__ void __launch_bounds__(256) probe_error_kernel(const float* ref, cons
     e[h] = sqrtf(num) / (sqrtf(den) + eps);
   }
 }
+
+// ---------------------------------------------------------------------------------------------------------------
+// Router features from the decode path (reading A28): per-token softmax probabilities of one (sequence,
+// layer, query vector) over the compressed cache, summed / maximised over the query heads. A probe-path kernel set (runs every p
+// decode steps on one layer), written plainly in fp32: scores with the decode kernel's algebra (q~ = cscale * BK (gK * q) once per
+// block; s = q~ . cK + cscale * sum_g scale_g * (q_g . code_g); nothing is reconstructed), then log-sum-exp per query head, then
+// mass[t] += sum_hq p, spike[t] = max(spike[t], max_hq p).
+constexpr int kStatsTok = 128;      // tokens (threads) per block of the score kernel
+
+__global__ void __launch_bounds__(kStatsTok) stats_scores_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst, int T, int layer,
+                                                               const __nv_bfloat16* q, const __nv_bfloat16* BK, const __nv_bfloat16* gK,
+                                                               float cscale, float* scores /* [T][Hq] log2 units */) {
+  extern __shared__ float sh[];
+  const int h = blockIdx.y, tid = threadIdx.x, d = g.d, r = g.r, G = g.G;
+  float* qt = sh;                 // [G][r]   q~ (log2 units)
+  float* qr = sh + G * r;         // [G][d]   cscale * q (residual term)
+  float* qg = qr + G * d;         // [G][d]   gK * q
+  const __nv_bfloat16* qh = q + (size_t)h * G * d;
+  const __nv_bfloat16* gk = gK + ((size_t)layer * g.H + h) * d;
+  const __nv_bfloat16* B = BK + ((size_t)(layer / g.w) * g.H + h) * (size_t)r * d;
+  for (int i = tid; i < G * d; i += kStatsTok) {
+    const float x = __bfloat162float(qh[i]);
+    qr[i] = cscale * x;
+    qg[i] = x * __bfloat162float(gk[i % d]);
+  }
+  __syncthreads();
+  for (int i = tid; i < G * r; i += kStatsTok) {
+    const int gq = i / r, j = i - gq * r;
+    float acc = 0.f;
+    for (int ch = 0; ch < d; ++ch) acc = fmaf(__bfloat162float(B[(size_t)j * d + ch]), qg[gq * d + ch], acc);
+    qt[i] = cscale * acc;
+  }
+  __syncthreads();
+  const int t = blockIdx.x * kStatsTok + tid;
+  if (t >= T) return;
+  const TokDst td = dst[t];
+  const BlockPtr bp = block_ptr(arena, g, td, layer * g.H + h);
+  float sc[8];
+#pragma unroll
+  for (int gq = 0; gq < 8; ++gq) sc[gq] = 0.f;
+  for (int j = 0; j < bp.rk; ++j) {
+    const float c = g.i8 ? load_coef8(bp, 0, j)
+                         : __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(bp.blk + off_coefK(bp.cl) + kcoef_elem_off(bp.slot, j, bp.cl.tb)));
+#pragma unroll
+    for (int gq = 0; gq < 8; ++gq)
+      if (gq < G) sc[gq] = fmaf(qt[gq * r + j], c, sc[gq]);
+  }
+  if (td.cls & 1) {
+    const uint8_t* creg = bp.blk + off_codeK(bp.cl);
+    const uint8_t* sreg = bp.blk + off_scaleK(bp.cl);
+    for (int grp = 0; grp < d / 16; ++grp) {
+      const float s = __half2float(*reinterpret_cast<const __half*>(sreg + scale_elem_off(bp.slot, grp, d)));
+      float dot[8];
+#pragma unroll
+      for (int gq = 0; gq < 8; ++gq) dot[gq] = 0.f;
+      for (int i = 0; i < 16; ++i) {
+        int wo, bit;
+        kcode_nibble(bp.slot, 16 * grp + i, d, &wo, &bit);
+        const float code = (float)load_code(creg, wo, bit);
+#pragma unroll
+        for (int gq = 0; gq < 8; ++gq)
+          if (gq < G) dot[gq] = fmaf(qr[gq * d + 16 * grp + i], code, dot[gq]);
+      }
+#pragma unroll
+      for (int gq = 0; gq < 8; ++gq)
+        if (gq < G) sc[gq] = fmaf(s, dot[gq], sc[gq]);
+    }
+  }
+#pragma unroll
+  for (int gq = 0; gq < 8; ++gq)
+    if (gq < G) scores[(size_t)t * (g.H * G) + h * G + gq] = sc[gq];
+}
+
+// one block per query head: lse[hq] = m + log2(sum_t 2^(s - m))
+__global__ void __launch_bounds__(256) stats_lse_kernel(const float* scores, int T, int Hq, float* lse) {
+  __shared__ float red[8];
+  const int hq = blockIdx.x, tid = threadIdx.x;
+  float m = -INFINITY;
+  for (int t = tid; t < T; t += 256) m = fmaxf(m, scores[(size_t)t * Hq + hq]);
+  m = warp_max(m);
+  if ((tid & 31) == 0) red[tid >> 5] = m;
+  __syncthreads();
+  m = red[0];
+  for (int w = 1; w < 8; ++w) m = fmaxf(m, red[w]);
+  __syncthreads();
+  float sum = 0.f;
+  for (int t = tid; t < T; t += 256) sum += exp2f(scores[(size_t)t * Hq + hq] - m);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(kFull, sum, o);
+  if ((tid & 31) == 0) red[tid >> 5] = sum;
+  __syncthreads();
+  if (tid == 0) {
+    sum = 0.f;
+    for (int w = 0; w < 8; ++w) sum += red[w];
+    lse[hq] = m + log2f(sum);
+  }
+}
+
+__global__ void __launch_bounds__(256) stats_emit_kernel(const float* scores, const float* lse, int T, int Hq, float* mass, float* spike) {
+  const int t = blockIdx.x * 256 + threadIdx.x;
+  if (t >= T) return;
+  float sum = 0.f, mx = 0.f;
+  for (int hq = 0; hq < Hq; ++hq) {
+    const float p = exp2f(scores[(size_t)t * Hq + hq] - lse[hq]);
+    sum += p;
+    mx = fmaxf(mx, p);
+  }
+  mass[t] += sum;
+  spike[t] = fmaxf(spike[t], mx);
+}
 }  // namespace
+
+size_t token_stats_scratch_bytes(const CacheGeom& g, int64_t T) { return ((size_t)T * g.H * g.G + (size_t)g.H * g.G) * sizeof(float); }
+
+int launch_token_stats(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int T, int layer, const __nv_bfloat16* q,
+                       const __nv_bfloat16* BK, const __nv_bfloat16* gK, float cscale, float* scratch, float* mass, float* spike,
+                       cudaStream_t s) {
+  const int Hq = g.H * g.G;
+  float* scores = scratch;
+  float* lse = scratch + (size_t)T * Hq;
+  const size_t smem = (size_t)(g.G * g.r + 2 * g.G * g.d) * sizeof(float);
+  stats_scores_kernel<<<dim3((T + kStatsTok - 1) / kStatsTok, g.H), kStatsTok, smem, s>>>(arena, g, dst, T, layer, q, BK, gK, cscale, scores);
+  stats_lse_kernel<<<Hq, 256, 0, s>>>(scores, T, Hq, lse);
+  stats_emit_kernel<<<(T + 255) / 256, 256, 0, s>>>(scores, lse, T, Hq, mass, spike);
+  return 3;
+}
 
 int launch_probe_error(const float* ref, const float* cmp, float* e, int n_q, int H, int G, int d, float eps, cudaStream_t s) {
   probe_error_kernel<<<H, 256, 0, s>>>(ref, cmp, e, n_q, H, G, d, eps);

@@ -121,6 +121,10 @@ struct DumpPtrs {
 };
 int launch_gather(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const DumpPtrs& o, cudaStream_t s);
 int launch_probe_error(const float* ref, const float* cmp, float* e, int n_q, int H, int G, int d, float eps, cudaStream_t s);
+// router features: per-token attention mass / spike of one (sequence, layer, query vector); dst = all T tokens in order
+size_t token_stats_scratch_bytes(const CacheGeom& g, int64_t T);
+int launch_token_stats(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int T, int layer, const __nv_bfloat16* q,
+                       const __nv_bfloat16* BK, const __nv_bfloat16* gK, float cscale, float* scratch, float* mass, float* spike, cudaStream_t s);
 int launch_gate_check(const __nv_bfloat16* g, int64_t n, int* bad_flag, cudaStream_t s);
 
 }  // namespace dwkv
