@@ -173,7 +173,8 @@ int dwkv_probe_error(dwkv_cache* c, int32_t layer, int32_t seq_id, int32_t n_q, 
 int64_t dwkv_seq_len(const dwkv_cache* c, int32_t seq_id);
 
 /* used = sum over tokens of 4*r_t + f_t*2*(d/2+d/8) bytes times L*H_kv (the compressed footprint, pin P13; with option
- * "coef_int8" the coefficient part is 2*(r_t + 1): one code byte per coefficient and one exponent byte per K / V vector);
+ * "coef_int8" the coefficient part is 2*(r_t + ceil(r_t/32)): one code byte per coefficient and one exponent byte per 32-column
+ * block of a K / V vector);
  * reserved = bytes of arena pages currently allocated to sequences; dense_equiv = tokens * L * H_kv * 2*d*2. */
 int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved_bytes, uint64_t* dense_equiv_bytes);
 
@@ -197,13 +198,14 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *   "cost_coef_pct", "cost_tok", "cost_resid_pct", "flag_cost_pct"   planner cost model (byte-equivalents per coefficient
  *                     byte in %, per token, per residual byte in %, extra weight of flagged classes in %)
  *   "coef_int8"       1 = store the coefficients "in 8-bit blockwise quantized form" (
- *                     DESIGN.md reading A27): per token and per K / V, int8 codes with one shared power-of-two scale 2^e,
+ *                     DESIGN.md reading A27): per token, per K / V and per block of 32 rank columns, int8 codes with one power-of-two scale 2^e,
  *                     e the smallest integer with max|c| <= 127 * 2^e (>= -126), code = rint(c / 2^e). code * 2^e is exactly a
  *                     bf16 value, so every call keeps its argument types: dwkv_append_raw quantises the bf16 coefficients it is
  *                     given (lossless if they already lie on the grid), dwkv_append_compress quantises the fp32 projection and
  *                     takes the residual against the dequantised coefficients, dwkv_export_tokens returns code * 2^e as bf16,
  *                     dwkv_decode_attention scans the byte planes (its score contraction runs in fp16 in this mode: the projected
- *                     query q~ = scale * log2(e) * B_K (g_K * q) is split hi + lo in fp16 and clamped to +-65504). Needs a basis rank <= 32 (INVALID otherwise) and an empty
+ *                     query q~ = scale * log2(e) * B_K (g_K * q) is split hi + lo in fp16 and clamped to +-65504). A block is 32
+ *                     consecutive rank columns of a token's vector (ranks 48 / 64: two blocks, two exponent bytes). Needs an empty
  *                     cache (STATE otherwise). 0 (default) = bf16 coefficients.
  * Any change invalidates the cached plan. Errors: INVALID (unknown key). */
 int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);

@@ -476,20 +476,7 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
       }
       off += n_new[i];
     }
-    if (c->geom.i8) {        // 8-bit coefficient planes: plain kernel, rows and destinations in call order
-      int rc = zero_new_pages(c, new_pages, st);
-      if (rc) return rc;
-      rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
-      if (rc) return rc;
-      if (c->opt_time_scan && g0 == 0) {
-        if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
-        CU_OK(cudaEventRecord(c->ev_app0, st));
-      }
-      c->launches += launch_compress_i8(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)dst.size(), (const __nv_bfloat16*)k_new,
-                                        (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV, st);
-      continue;
-    }
-    if (c->opt_compress_umma && compress_umma_supported(c->geom, k_new, v_new)) {
+    if (c->opt_compress_umma && !c->geom.i8 && compress_umma_supported(c->geom, k_new, v_new)) {
       // tcgen05 path: rows in call order (TMA tile loads), destinations in the same order
       int rc = zero_new_pages(c, new_pages, st);
       if (rc) return rc;
@@ -632,7 +619,7 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
   const uint64_t LH = (uint64_t)c->geom.L * c->geom.H, d = c->geom.d;
   for (const SeqState& S : c->seqs)
     for (int k = 0; k < c->n_classes; ++k)
-      used += (uint64_t)S.count[k] * ((c->geom.i8 ? 2ull * (c->geom.tier_rank[k >> 1] + 1) : 4ull * c->geom.tier_rank[k >> 1]) +
+      used += (uint64_t)S.count[k] * ((c->geom.i8 ? 2ull * (c->geom.tier_rank[k >> 1] + (c->geom.tier_rank[k >> 1] + 31) / 32) : 4ull * c->geom.tier_rank[k >> 1]) +
                                       (k & 1) * 2ull * (d / 2 + d / 8));
   if (used_bytes) *used_bytes = used * LH;
   if (reserved_bytes) *reserved_bytes = (uint64_t)pages_in_use(c) * c->page_bytes;
@@ -661,7 +648,6 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
     // storage format of the coefficient planes: fixed once tokens exist, like the basis (A19)
     if (value != 0 && value != 1) return fail(DWKV_E_INVALID, "coef_int8 must be 0 or 1");
     if (c->total_tokens != 0 || pages_in_use(c) != 0) return fail(DWKV_E_STATE, "coef_int8 cannot change while the cache holds tokens");
-    if (value && c->geom.r > 32) return fail(DWKV_E_INVALID, "coef_int8 needs a basis rank <= 32 (one 32-column block per token)");
     c->geom.i8 = (int32_t)value;
     for (int k = 0; k < c->n_classes; ++k) c->cl[k] = make_class_layout(c->cfg.tier_rank[k >> 1], k & 1, c->cfg.d_head, c->geom.i8);
   }

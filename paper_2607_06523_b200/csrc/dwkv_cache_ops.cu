@@ -1,12 +1,15 @@
 // dwkv_cache_ops.cu -- load / dump auxiliaries of the cache (the append/compress kernel, step a4, is dwkv_compress.cu):
 //   scatter_raw_kernel  load pre-compressed token-ordered entries into the fragment-native pages
 //   gather_kernel       token-ordered dump of stored entries (bit-exact checks of routing and int4 dequantisation)
-//   compress_i8_warp_kernel / compress_i8_kernel   append/compress in 8-bit coefficient mode (option "coef_int8", reading A27)
+//   stats_* kernels     router features of a probe step (per-token attention mass / spike), probe_error_kernel (Eq. 3)
 #include <algorithm>
 #include "dwkv_internal.h"
+#include "dwkv_mma.cuh"
 
 namespace dwkv {
 namespace {
+using dwkv::dev::coef8_exponent;
+using dwkv::dev::coef8_code;
 
 constexpr uint32_t kFull = 0xffffffffu;
 
@@ -49,34 +52,22 @@ __device__ __forceinline__ BlockPtr block_ptr(const uint8_t* arena, const CacheG
   return b;
 }
 
-// 8-bit blockwise coefficient quantiser (reading A27), block = the token's coefficient vector (rank <= 32):
-// e = smallest integer with amax <= 127 * 2^e, clamped to >= -126 (amax == 0 and subnormal amax land on the clamp);
-// code = rint(c / 2^e) in [-127, 127]. Every step is exact in fp32. amax = m * 2^x, m in [0.5, 1): e = x - 7 if m <= 127/128 else x - 6.
-__device__ __forceinline__ int coef8_exponent(float amax) {
-  const uint32_t b = __float_as_uint(amax);
-  const int x = (int)((b >> 23) & 0xffu) - 126;
-  const int e = ((b & 0x7fffffu) <= 0x7e0000u) ? x - 7 : x - 6;
-  return max(e, -126);
-}
-__device__ __forceinline__ int coef8_code(float c, int e) {
-  const float q = rintf(c * __uint_as_float((uint32_t)(127 - e) << 23));     // c / 2^e, exact
-  return (int)fminf(fmaxf(q, -127.f), 127.f);
-}
 __device__ __forceinline__ float warp_max(float a) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) a = fmaxf(a, __shfl_xor_sync(kFull, a, o));
   return a;
 }
-// store one token's coefficient of column col (stored byte = code + 128) and, from column 0, the exponent byte (e + 127)
+// store one token's coefficient of column col (stored byte = code + 128) and, from the first column of a 32-column block, the
+// block's exponent byte (e + 127)
 __device__ __forceinline__ void store_coef8(const BlockPtr& bp, int z, int col, int code, int e) {
   uint8_t* base = bp.blk + (z ? off_coefV(bp.cl) : off_coefK(bp.cl));
   base[z ? vcoef8_elem_off(bp.slot, col, bp.cl.tb) : kcoef8_elem_off(bp.slot, col, bp.cl.tb)] = (uint8_t)(code + 128);
-  if (col == 0) base[coef8_exp_off(bp.slot, bp.cl.nk, bp.cl.tb)] = (uint8_t)(e + 127);
+  if ((col & 31) == 0) base[coef8_exp_off(bp.slot, bp.cl.nk, bp.cl.tb, col >> 5)] = (uint8_t)(e + 127);
 }
 __device__ __forceinline__ float load_coef8(const BlockPtr& bp, int z, int col) {
   const uint8_t* base = bp.blk + (z ? off_coefV(bp.cl) : off_coefK(bp.cl));
   const int u = base[z ? vcoef8_elem_off(bp.slot, col, bp.cl.tb) : kcoef8_elem_off(bp.slot, col, bp.cl.tb)];
-  const uint32_t eb = base[coef8_exp_off(bp.slot, bp.cl.nk, bp.cl.tb)];
+  const uint32_t eb = base[coef8_exp_off(bp.slot, bp.cl.nk, bp.cl.tb, col >> 5)];
   return (float)(u - 128) * __uint_as_float(eb << 23);
 }
 
@@ -99,8 +90,8 @@ __global__ void __launch_bounds__(128) scatter_raw_kernel(const uint8_t* arena, 
   const TokDst td = dst[tok];
   const BlockPtr bp = block_ptr(arena, g, td, lh);
   const size_t row = (size_t)tok * LH + lh;
-  if (g.i8) {                 // quantise the given coefficients (rank <= 32: the vector sits in warp 0)
-    if (tid < 32) {
+  if (g.i8) {                 // quantise the given coefficients: warp b holds the 32-column block b of the vector (rank <= 64)
+    if (tid < 64 && (tid & ~31) < bp.rk) {
       for (int z = 0; z < 2; ++z) {
         const float cf = tid < bp.rk ? __bfloat162float((z ? coefV : coefK)[row * g.r + tid]) : 0.f;
         const int e = coef8_exponent(warp_max(fabsf(cf)));
@@ -148,7 +139,7 @@ __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, Cache
   const BlockPtr bp = block_ptr(arena, g, td, lh);
   const size_t row = (size_t)tok * LH + lh;
   const int d = g.d, ng = d / 16;
-  if (g.i8 && tid < g.r) {     // code * 2^e has <= 7 significant bits: exactly a bf16 value
+  if (g.i8 && tid < g.r) {     // code * 2^e has <= 7 significant bits: exactly a bf16 value (g.r <= 64 < blockDim)
     const __nv_bfloat16 zero = __float2bfloat16_rn(0.f);
     if (o.coefK) o.coefK[row * g.r + tid] = tid < bp.rk ? __float2bfloat16_rn(load_coef8(bp, 0, tid)) : zero;
     if (o.coefV) o.coefV[row * g.r + tid] = tid < bp.rk ? __float2bfloat16_rn(load_coef8(bp, 1, tid)) : zero;
@@ -183,157 +174,6 @@ __global__ void __launch_bounds__(128) gather_kernel(const uint8_t* arena, Cache
   }
 }
 
-// ---------------------------------------------------------------------------------------------------------------
-// Append/compress in 8-bit coefficient mode (step a4 with reading A27 in place of the bf16 rounding): one CTA of 128 threads per
-// (token, layer, head); c = B[:r_t] . (x / g) in fp32, quantised; the residual of a flagged token is taken against the DEQUANTISED
-// coefficients and goes through the A14 quantiser. Plain kernel (not tuned): the tensor-core kernel of dwkv_compress.cu serves bf16 mode.
-__global__ void __launch_bounds__(128) compress_i8_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst, const __nv_bfloat16* k_new,
-                                                          const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
-                                                          const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
-  __shared__ float xn[128], cs[32];
-  const int tok = blockIdx.x, lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const TokDst td = dst[tok];
-  const BlockPtr bp = block_ptr(arena, g, td, lh);
-  const int d = g.d, layer = lh / g.H, h = lh - layer * g.H;
-  const bool fl = (td.cls & 1) != 0;
-  for (int z = 0; z < 2; ++z) {
-    const __nv_bfloat16* B = (z ? BV : BK) + ((size_t)(layer / g.w) * g.H + h) * (size_t)g.r * d;
-    float x = 0.f, gate = 1.f;
-    if (tid < d) {
-      x = __bfloat162float((z ? v_new : k_new)[((size_t)td.src * LH + lh) * d + tid]);
-      gate = __bfloat162float((z ? gV : gK)[(size_t)lh * d + tid]);
-      xn[tid] = __fdiv_rn(x, gate);
-    }
-    __syncthreads();
-    for (int j = warp; j < bp.rk; j += 4) {
-      float acc = 0.f;
-      for (int ch = lane; ch < d; ch += 32) acc = fmaf(__bfloat162float(B[(size_t)j * d + ch]), xn[ch], acc);
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(kFull, acc, o);
-      if (lane == 0) cs[j] = acc;
-    }
-    __syncthreads();
-    if (tid < 32) {
-      const float cf = tid < bp.rk ? cs[tid] : 0.f;
-      const int e = coef8_exponent(warp_max(fabsf(cf)));
-      const int code = coef8_code(cf, e);
-      if (tid < bp.rk) {
-        store_coef8(bp, z, tid, code, e);
-        cs[tid] = (float)code * __uint_as_float((uint32_t)(e + 127) << 23);
-      }
-    }
-    __syncthreads();
-    if (fl && tid < d) {
-      float rec = 0.f;
-      for (int j = 0; j < bp.rk; ++j) rec = fmaf(cs[j], __bfloat162float(B[(size_t)j * d + tid]), rec);
-      const float e = x - gate * rec;
-      __half s;
-      const int code = quant_code(e, group16_amax(fabsf(e)), &s);
-      int wo, bit;
-      if (z == 0) kcode_nibble(bp.slot, tid, d, &wo, &bit); else vcode_nibble(bp.slot, tid, d, &wo, &bit);
-      store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, code);
-      if ((tid & 15) == 0)
-        *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(bp.slot, tid >> 4, d)) = s;
-    }
-    __syncthreads();
-  }
-}
-
-// The same step for d in {64, 128} (the tested shapes), basis staged once per CTA: one CTA of 8 warps per ((layer, head), token
-// chunk); both bases of the (window, head) sit in shared memory as fp32 rows (stride D + 4: conflict-free 128-bit reads), every
-// warp takes one (token, Z) vector at a time. Lane (grp, j) accumulates column j = lane mod rkp of c = B[:r_t] . (x / g) over its
-// channel group (rkp = r_t rounded up to 8 / 16 / 32, 32 / rkp groups), the groups are summed by xor shuffles, the vector is
-// quantised in the warp (A27) and the residual of a flagged token is taken against the dequantised coefficients with lane =
-// channel mod 32 (a 16-lane half-warp = one quantiser group of A14). Same arithmetic per element as compress_i8_kernel except
-// for the summation order of the projection (fp32 either way; parity of dwkv_append_compress is A15 (iii)).
-template <int D>
-__global__ void __launch_bounds__(256) compress_i8_warp_kernel(const uint8_t* arena, CacheGeom g, const TokDst* dst, int n,
-                                                               const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
-                                                               const __nv_bfloat16* BK, const __nv_bfloat16* BV,
-                                                               const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
-  constexpr int ST = D + 4, NC = D / 32;
-  __shared__ __align__(16) float Bs[2][32 * ST];
-  __shared__ __align__(16) float xs[8][D];
-  const int lh = blockIdx.y, LH = g.L * g.H, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int layer = lh / g.H, h = lh - layer * g.H;
-  for (int z = 0; z < 2; ++z) {
-    const __nv_bfloat16* B = (z ? BV : BK) + ((size_t)(layer / g.w) * g.H + h) * (size_t)g.r * D;
-    for (int i = tid; i < 32 * D; i += 256) {
-      const int j = i / D, ch = i - j * D;
-      Bs[z][j * ST + ch] = j < g.r ? __bfloat162float(B[i]) : 0.f;
-    }
-  }
-  float gate[2][NC];
-#pragma unroll
-  for (int k = 0; k < NC; ++k) {
-    gate[0][k] = __bfloat162float(gK[(size_t)lh * D + lane + 32 * k]);
-    gate[1][k] = __bfloat162float(gV[(size_t)lh * D + lane + 32 * k]);
-  }
-  __syncthreads();
-  for (int tok = blockIdx.x * 8 + warp; tok < n; tok += gridDim.x * 8) {
-    const TokDst td = dst[tok];
-    const BlockPtr bp = block_ptr(arena, g, td, lh);
-    const bool fl = (td.cls & 1) != 0;
-    const int rk = bp.rk, rkp = rk <= 8 ? 8 : (rk <= 16 ? 16 : 32);
-    const int j = lane & (rkp - 1), grp = lane / rkp, cpg = D / (32 / rkp);
-    float xkv[2][NC];           // both rows of the token are requested before the first projection starts
-#pragma unroll
-    for (int k = 0; k < NC; ++k) {
-      xkv[0][k] = __bfloat162float(k_new[((size_t)td.src * LH + lh) * D + lane + 32 * k]);
-      xkv[1][k] = __bfloat162float(v_new[((size_t)td.src * LH + lh) * D + lane + 32 * k]);
-    }
-#pragma unroll
-    for (int z = 0; z < 2; ++z) {
-      float x[NC];
-#pragma unroll
-      for (int k = 0; k < NC; ++k) {
-        x[k] = xkv[z][k];
-        xs[warp][lane + 32 * k] = __fdiv_rn(x[k], gate[z][k]);
-      }
-      __syncwarp();
-      const float* brow = &Bs[z][min(j, rk - 1) * ST + grp * cpg];
-      const float* xrow = &xs[warp][grp * cpg];
-      float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;      // four independent chains (channels c mod 4)
-#pragma unroll 4
-      for (int c = 0; c < cpg; c += 4) {
-        const float4 b = *reinterpret_cast<const float4*>(brow + c);
-        const float4 v = *reinterpret_cast<const float4*>(xrow + c);
-        a0 = fmaf(b.x, v.x, a0); a1 = fmaf(b.y, v.y, a1); a2 = fmaf(b.z, v.z, a2); a3 = fmaf(b.w, v.w, a3);
-      }
-      float acc = (a0 + a1) + (a2 + a3);
-      for (int o = rkp; o < 32; o <<= 1) acc += __shfl_xor_sync(kFull, acc, o);
-      const float cf = j < rk ? acc : 0.f;
-      const int e = coef8_exponent(warp_max(fabsf(cf)));
-      const int code = coef8_code(cf, e);
-      if (lane < rk) store_coef8(bp, z, lane, code, e);
-      if (fl) {
-        const float deq = (float)code * __uint_as_float((uint32_t)(e + 127) << 23);   // lane jj < r_t holds column jj
-        float rec[NC];
-#pragma unroll
-        for (int k = 0; k < NC; ++k) rec[k] = 0.f;
-        for (int jj = 0; jj < rk; ++jj) {
-          const float cj = __shfl_sync(kFull, deq, jj);
-#pragma unroll
-          for (int k = 0; k < NC; ++k) rec[k] = fmaf(cj, Bs[z][jj * ST + lane + 32 * k], rec[k]);
-        }
-#pragma unroll
-        for (int k = 0; k < NC; ++k) {
-          const int ch = lane + 32 * k;
-          const float er = x[k] - gate[z][k] * rec[k];
-          __half s;
-          const int rc = quant_code(er, group16_amax(fabsf(er)), &s);
-          int wo, bit;
-          if (z == 0) kcode_nibble(bp.slot, ch, D, &wo, &bit); else vcode_nibble(bp.slot, ch, D, &wo, &bit);
-          store_code(bp.blk + (z ? off_codeV(bp.cl) : off_codeK(bp.cl)), wo, bit, rc);
-          if ((ch & 15) == 0)
-            *reinterpret_cast<__half*>(bp.blk + (z ? off_scaleV(bp.cl) : off_scaleK(bp.cl)) + scale_elem_off(bp.slot, ch >> 4, D)) = s;
-        }
-      }
-      __syncwarp();
-    }
-  }
-}
-
 __global__ void gate_check_kernel(const __nv_bfloat16* g, int64_t n, int* bad) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) {
@@ -350,21 +190,6 @@ int launch_scatter_raw(const uint8_t* arena, const CacheGeom& g, const TokDst* d
   if (n <= 0) return 0;
   dim3 grid(n, g.L * g.H);
   scatter_raw_kernel<<<grid, 128, 0, s>>>(arena, g, dst, coefK, coefV, residK, residV, codeK, codeV, scaleK, scaleV);
-  return 1;
-}
-
-int launch_compress_i8(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const __nv_bfloat16* k_new,
-                       const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK,
-                       const __nv_bfloat16* gV, cudaStream_t s) {
-  if (n <= 0) return 0;
-  if (g.d == 64 || g.d == 128) {      // 64 tokens per CTA (8 per warp), at most 65535 / 8 chunks deep
-    dim3 grid((unsigned)std::min((n + 63) / 64, 8192), g.L * g.H);
-    if (g.d == 128) compress_i8_warp_kernel<128><<<grid, 256, 0, s>>>(arena, g, dst, n, k_new, v_new, BK, BV, gK, gV);
-    else compress_i8_warp_kernel<64><<<grid, 256, 0, s>>>(arena, g, dst, n, k_new, v_new, BK, BV, gK, gV);
-    return 1;
-  }
-  dim3 grid(n, g.L * g.H);
-  compress_i8_kernel<<<grid, 128, 0, s>>>(arena, g, dst, k_new, v_new, BK, BV, gK, gV);
   return 1;
 }
 

@@ -63,35 +63,39 @@ __device__ __forceinline__ __half quant_scale(float amax) {
 
 struct RowDst {          // destination of one token row of the tile for this (layer, head), packed to 4 registers
   uint8_t* blk;          // sub-block base
-  int meta;              // slot inside the sub-block | rank of the token's tier << 8 | valid << 16 | flagged << 17
+  int meta;              // slot inside the sub-block | rank of the token's tier << 8 | valid << 16 | flagged << 17 | 8-bit planes << 18
   int src;               // row of the token in k_new / v_new
   __device__ __forceinline__ int slot() const { return meta & 0xff; }
   __device__ __forceinline__ int rk() const { return (meta >> 8) & 0xff; }
   __device__ __forceinline__ bool valid() const { return (meta >> 16) & 1; }
   __device__ __forceinline__ bool flagged() const { return (meta >> 17) & 1; }
   __device__ __forceinline__ int tb() const { return flagged() ? 2 : 4; }          // tiles per sub-block
-  __device__ __forceinline__ int coef_bytes() const { return rk() * 16 * tb(); }    // bytes of [K coef] (= [V coef])
+  __device__ __forceinline__ bool i8() const { return (meta >> 18) & 1; }
+  // bytes of [K coef] (= [V coef]); 8-bit planes: one byte per coefficient + 8 * tb exponent bytes per 32-column block
+  __device__ __forceinline__ int coef_bytes() const { return i8() ? rk() * 8 * tb() + ((rk() + 31) >> 5) * 8 * tb() : rk() * 16 * tb(); }
 };
 
 // the ClassLayout arithmetic of dwkv_layout.cuh with shifts only (tb is 2 or 4); tier ranks come as 4 bytes of one word
-__device__ __forceinline__ RowDst row_dst_from(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst& td, const bool valid, int lh) {
+__device__ __forceinline__ RowDst row_dst_from(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst& td, const bool valid, int lh,
+                                                const bool i8 = false) {
   RowDst r;
   const int resid = td.cls & 1;
   const int rk = (ranks4 >> (8 * (td.cls >> 1))) & 0xff;
   const int tb = resid ? 2 : 4;
-  const int coef_bytes = rk * 16 * tb;
+  const int coef_bytes = i8 ? rk * 8 * tb + ((rk + 31) >> 5) * 8 * tb : rk * 16 * tb;
   const int sub_bytes = 2 * coef_bytes + (resid ? 2 * 5 * tb * d : 0);
   const int block_bytes = resid ? 2 * sub_bytes : sub_bytes;
   r.src = valid ? td.src : 0;
   r.blk = const_cast<uint8_t*>(arena) + td.page_off + (size_t)lh * kPageLhBytes + (size_t)td.blk * block_bytes +
           ((resid && td.slot >= 16) ? sub_bytes : 0);
-  r.meta = (resid ? (td.slot & 15) : td.slot) | (rk << 8) | ((int)valid << 16) | ((int)(valid && resid) << 17);
+  r.meta = (resid ? (td.slot & 15) : td.slot) | (rk << 8) | ((int)valid << 16) | ((int)(valid && resid) << 17) | ((int)i8 << 18);
   return r;
 }
-__device__ __forceinline__ RowDst row_dst(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst* dst, int tok, int n_tok, int lh) {
+__device__ __forceinline__ RowDst row_dst(const uint8_t* arena, const uint32_t ranks4, const int d, const TokDst* dst, int tok, int n_tok, int lh,
+                                          const bool i8 = false) {
   const bool valid = tok < n_tok;
   const TokDst td = dst[valid ? tok : 0];
-  return row_dst_from(arena, ranks4, d, td, valid, lh);
+  return row_dst_from(arena, ranks4, d, td, valid, lh, i8);
 }
 
 // item position in cost space -> (layer-head, tile). Per layer-head the tiles come in runs of equal cost (CompressRuns).
@@ -151,9 +155,13 @@ template <int D>
 __device__ __forceinline__ uint32_t stage_x(uint32_t stage, int row, int ch) { return lds32(stage + row * (2 * D + 16) + ch * 2); }
 
 // C = X . B'^T for one Z: 3 MMAs (lo, mid, hi term of B') per (k step, rank chunk); returns the rounded coefficients of rows g (ca) and g+8 (cb), columns 8nt + 2t, +1, zero beyond the rank
-template <int D, int NT, int NTM>      // NTM = rank chunks any token of the tile keeps: only those are multiplied
+// 8-bit planes (I8; reading A27): the fp32 coefficients of a row are quantised per 32-column block (exponent from the
+// block's amax over the row's leading r_t columns: the quad's four lanes hold the row), ca / cb then carry the DEQUANTISED values
+// code * 2^e (exactly bf16) so that the residual absorbs the quantisation error, qa / qb the stored bytes (code + 128) of the two
+// columns, xa / xb the exponent bytes (e + 127) of the row's blocks.
+template <int D, int NT, int NTM, bool I8>      // NTM = rank chunks any token of the tile keeps: only those are multiplied
 __device__ __forceinline__ void project_n(const uint4* P4, const uint2* P2, int lane, uint32_t stage, const RowDst& ra, const RowDst& rb,
-                                          uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
+                                          uint32_t (&ca)[NT], uint32_t (&cb)[NT], uint32_t (&qa)[NT], uint32_t (&qb)[NT], uint32_t& xa, uint32_t& xb) {
   // few chunks: one accumulator chain per term of B' (lo, mid, hi) so that the MMAs of a k step are independent
   constexpr int NA = NTM <= 2 ? 3 : 1;
   float c[NA][NTM][4];
@@ -176,6 +184,47 @@ __device__ __forceinline__ void project_n(const uint4* P4, const uint2* P2, int 
       mma16(c[NA == 3 ? 2 : 0][nt], a0, a1, a2, a3, hm.x, hm.y);
     }
   }
+  if constexpr (I8) {
+    constexpr int NB = (NT + 3) / 4;             // 32-column blocks of the basis rank
+    float v[NTM][4];
+    float ama[NB], amb[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) ama[b] = amb[b] = 0.f;
+#pragma unroll
+    for (int nt = 0; nt < NTM; ++nt) {
+#pragma unroll
+      for (int x = 0; x < 4; ++x) v[nt][x] = NA == 3 ? (c[0][nt][x] + c[1][nt][x]) + c[NA - 1][nt][x] : c[0][nt][x];
+      if (8 * nt < ra.rk()) ama[nt >> 2] = fmaxf(ama[nt >> 2], fmaxf(fabsf(v[nt][0]), fabsf(v[nt][1])));
+      if (8 * nt < rb.rk()) amb[nt >> 2] = fmaxf(amb[nt >> 2], fmaxf(fabsf(v[nt][2]), fabsf(v[nt][3])));
+    }
+    int ea[NB], eb[NB];
+    xa = xb = 0u;
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+      ama[b] = fmaxf(ama[b], __shfl_xor_sync(kFull, ama[b], 1)); ama[b] = fmaxf(ama[b], __shfl_xor_sync(kFull, ama[b], 2));
+      amb[b] = fmaxf(amb[b], __shfl_xor_sync(kFull, amb[b], 1)); amb[b] = fmaxf(amb[b], __shfl_xor_sync(kFull, amb[b], 2));
+      ea[b] = coef8_exponent(ama[b]); eb[b] = coef8_exponent(amb[b]);
+      xa |= (uint32_t)(ea[b] + 127) << (8 * b); xb |= (uint32_t)(eb[b] + 127) << (8 * b);
+    }
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) {
+      ca[nt] = cb[nt] = 0u; qa[nt] = qb[nt] = 0u;
+      if (nt < NTM) {
+        if (8 * nt < ra.rk() && ra.valid()) {
+          const int e = ea[nt >> 2], k0 = coef8_code(v[nt][0], e), k1 = coef8_code(v[nt][1], e);
+          const float sc = __uint_as_float((uint32_t)(e + 127) << 23);
+          ca[nt] = pack_bf16x2((float)k0 * sc, (float)k1 * sc);
+          qa[nt] = (uint32_t)(k0 + 128) | ((uint32_t)(k1 + 128) << 8);
+        }
+        if (8 * nt < rb.rk() && rb.valid()) {
+          const int e = eb[nt >> 2], k0 = coef8_code(v[nt][2], e), k1 = coef8_code(v[nt][3], e);
+          const float sc = __uint_as_float((uint32_t)(e + 127) << 23);
+          cb[nt] = pack_bf16x2((float)k0 * sc, (float)k1 * sc);
+          qb[nt] = (uint32_t)(k0 + 128) | ((uint32_t)(k1 + 128) << 8);
+        }
+      }
+    }
+  } else {
 #pragma unroll
   for (int nt = 0; nt < NT; ++nt) {
     ca[nt] = cb[nt] = 0u;
@@ -187,15 +236,40 @@ __device__ __forceinline__ void project_n(const uint4* P4, const uint2* P2, int 
       if (8 * nt < rb.rk() && rb.valid()) cb[nt] = pack_bf16x2(v[2], v[3]);
     }
   }
+  }
 }
 
-template <int D, int NT>
+template <int D, int NT, bool I8>
 __device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int lane, uint32_t stage, const RowDst& ra, const RowDst& rb,
-                                        const int ntmax /* warp-uniform */, uint32_t (&ca)[NT], uint32_t (&cb)[NT]) {
-  if (ntmax <= 1) project_n<D, NT, 1>(P4, P2, lane, stage, ra, rb, ca, cb);
-  else if (NT >= 2 && ntmax == 2) project_n<D, NT, (NT >= 2 ? 2 : NT)>(P4, P2, lane, stage, ra, rb, ca, cb);
-  else if (NT >= 3 && ntmax == 3) project_n<D, NT, (NT >= 3 ? 3 : NT)>(P4, P2, lane, stage, ra, rb, ca, cb);
-  else project_n<D, NT, NT>(P4, P2, lane, stage, ra, rb, ca, cb);
+                                        const int ntmax /* warp-uniform */, uint32_t (&ca)[NT], uint32_t (&cb)[NT], uint32_t (&qa)[NT],
+                                        uint32_t (&qb)[NT], uint32_t& xa, uint32_t& xb) {
+  if (ntmax <= 1) project_n<D, NT, 1, I8>(P4, P2, lane, stage, ra, rb, ca, cb, qa, qb, xa, xb);
+  else if (NT >= 2 && ntmax == 2) project_n<D, NT, (NT >= 2 ? 2 : NT), I8>(P4, P2, lane, stage, ra, rb, ca, cb, qa, qb, xa, xb);
+  else if (NT >= 3 && ntmax == 3) project_n<D, NT, (NT >= 3 ? 3 : NT), I8>(P4, P2, lane, stage, ra, rb, ca, cb, qa, qb, xa, xb);
+  else project_n<D, NT, NT, I8>(P4, P2, lane, stage, ra, rb, ca, cb, qa, qb, xa, xb);
+}
+
+// 8-bit planes: the row's code bytes (two columns per chunk and lane) and, from lane t = 0, the exponent bytes of its blocks
+template <int NT>
+__device__ __forceinline__ void store_coef8(const RowDst& rd, const uint32_t (&q)[NT], const uint32_t xexp, int z, int t) {
+  if (!rd.valid()) return;
+  uint8_t* base = rd.blk + (z ? rd.coef_bytes() : 0);
+#pragma unroll
+  for (int nt = 0; nt < NT; ++nt) {
+    if (8 * nt < rd.rk()) {
+      if (z == 0) {
+        *reinterpret_cast<uint16_t*>(base + kcoef8_elem_off(rd.slot(), 8 * nt + 2 * t, rd.tb())) = (uint16_t)q[nt];
+      } else {
+        base[vcoef8_elem_off(rd.slot(), 8 * nt + 2 * t, rd.tb())] = (uint8_t)(q[nt] & 0xff);
+        base[vcoef8_elem_off(rd.slot(), 8 * nt + 2 * t + 1, rd.tb())] = (uint8_t)(q[nt] >> 8);
+      }
+    }
+  }
+  if (t == 0) {
+#pragma unroll
+    for (int b = 0; b < (NT + 3) / 4; ++b)
+      if (32 * b < rd.rk()) base[coef8_exp_off(rd.slot(), rd.rk() >> 3, rd.tb(), b)] = (uint8_t)(xexp >> (8 * b));
+  }
 }
 
 template <int NT>
@@ -287,7 +361,7 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
   }
 }
 
-template <int D, int NT>      // NT = basis rank / 8
+template <int D, int NT, bool I8>      // NT = basis rank / 8; I8 = 8-bit coefficient planes (option "coef_int8")
 __global__ void __launch_bounds__(kCompressMaxWarps * 32, 1)
 compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, const int n_tok, const CompressRuns runs, const int n_stages,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
@@ -367,8 +441,8 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
     // destination rows of the current tile and (loaded one stage early, so the table read is off the critical path) of the next
     RowDst ra, rb, na, nb;
     if (n > 0) {
-      na = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr, n_tok, lh);
-      nb = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr + 8, n_tok, lh);
+      na = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr, n_tok, lh, I8);
+      nb = row_dst(arena, ranks4, g.d, dst, 16 * (tb + warp) + gr + 8, n_tok, lh, I8);
     }
     bool any_flag = false;
     int ntmax = NT;
@@ -387,13 +461,18 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
         ntmax = __reduce_max_sync(kFull, max(ra.valid() ? ra.rk() : 0, rb.valid() ? rb.rk() : 0)) >> 3;
       } else if (s + 1 < nst) {
         const int tile = tb + warp + W * ((s + 1) >> 1);
-        na = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr, n_tok, lh);
-        nb = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr + 8, n_tok, lh);
+        na = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr, n_tok, lh, I8);
+        nb = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr + 8, n_tok, lh, I8);
       }
-      uint32_t ca[NT], cb[NT];
-      project<D, NT>(P4 + z * NFRAG, P2 + z * NFRAG, lane, stage, ra, rb, ntmax, ca, cb);
-      store_coef<NT>(ra, ca, z, t);
-      store_coef<NT>(rb, cb, z, t);
+      uint32_t ca[NT], cb[NT], qa[NT], qb[NT], xa = 0u, xb = 0u;
+      project<D, NT, I8>(P4 + z * NFRAG, P2 + z * NFRAG, lane, stage, ra, rb, ntmax, ca, cb, qa, qb, xa, xb);
+      if constexpr (I8) {
+        store_coef8<NT>(ra, qa, xa, z, t);
+        store_coef8<NT>(rb, qb, xb, z, t);
+      } else {
+        store_coef<NT>(ra, ca, z, t);
+        store_coef<NT>(rb, cb, z, t);
+      }
       if (any_flag)
         reconstruct_quantise<D, NT>(z, BT + z * D * ldT, ldT, (z ? gV : gK) + (size_t)lh * D + 2 * t, stage, ra, rb, ca, cb, gr, t);
       slot_c = slot_c + 1 == n_stages ? 0 : slot_c + 1;
@@ -870,8 +949,13 @@ int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* 
   bool ok = true;
 #define DWKV_COMPRESS_CASE(DD, NN)                                                                                              \
   case NN:                                                                                                                      \
-    cudaFuncSetAttribute(compress_mma_kernel<DD, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                  \
-    compress_mma_kernel<DD, NN><<<grid, warps * 32, smem, s>>>(arena, g, dst, n, runs, stages, k_new, v_new, BK, BV, gK, gV);     \
+    if (g.i8) {                                                                                                                 \
+      cudaFuncSetAttribute(compress_mma_kernel<DD, NN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);          \
+      compress_mma_kernel<DD, NN, true><<<grid, warps * 32, smem, s>>>(arena, g, dst, n, runs, stages, k_new, v_new, BK, BV, gK, gV); \
+    } else {                                                                                                                    \
+      cudaFuncSetAttribute(compress_mma_kernel<DD, NN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);         \
+      compress_mma_kernel<DD, NN, false><<<grid, warps * 32, smem, s>>>(arena, g, dst, n, runs, stages, k_new, v_new, BK, BV, gK, gV); \
+    }                                                                                                                           \
     break;
   if (g.d == 128) {
     switch (g.r / 8) { DWKV_COMPRESS_CASE(128, 1) DWKV_COMPRESS_CASE(128, 2) DWKV_COMPRESS_CASE(128, 3) DWKV_COMPRESS_CASE(128, 4)

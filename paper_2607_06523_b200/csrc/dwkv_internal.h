@@ -109,10 +109,6 @@ int basis_num_splits(const CacheGeom& g, int n, int n_sms);
 int launch_build_basis(const CacheGeom& g, int n, const __nv_bfloat16* k_dense, const __nv_bfloat16* v_dense, const __nv_bfloat16* omega,
                        int n_sketch, int n_split, float* part, const __nv_bfloat16* gK, const __nv_bfloat16* gV, __nv_bfloat16* BK,
                        __nv_bfloat16* BV, bool use_umma /* tcgen05 sketch kernel (d = 128) instead of the mma.sync one */, cudaStream_t s);
-// 8-bit coefficient mode: straightforward append/compress kernel (one CTA per (token, layer, head)); dst in call order
-int launch_compress_i8(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const __nv_bfloat16* k_new,
-                       const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK,
-                       const __nv_bfloat16* gV, cudaStream_t s);
 struct DumpPtrs {
   __nv_bfloat16 *coefK, *coefV;
   uint8_t *codeK, *codeV;

@@ -25,9 +25,10 @@
 //             half-word) and +1 (high), channel 16*grp + 8*(a&1) + g
 //   [V scale] same arrangement as [K scale]
 //
-// 8-bit coefficient mode ("8-bit blockwise quantized"; reading A27), basis
-// rank <= 32 so that a token's coefficient vector is ONE block: the same fragment order with one BYTE per coefficient
-// (offset-binary code + 128) and, behind the nk code vectors of each of K and V, one exponent byte (e + 127) per slot:
+// 8-bit coefficient mode ("8-bit blockwise quantized"; reading A27): a block
+// is 32 consecutive rank columns of a token's coefficient vector (ranks <= 32: one block, ranks 48 / 64: two): the same fragment
+// order with one BYTE per coefficient (offset-binary code + 128) and, behind the nk code vectors of each of K and V, one
+// exponent byte (e + 127) per slot and block ([K exp] of block 0, then of block 1):
 //   [K coef8] nk vectors of 64*TB B.  vector i, lane (g,t), half-word j : ( uK[slot 8j+g][8i+2t], uK[slot 8j+g][8i+2t+1] )
 //   [K exp]   8*TB B.                 byte (t, j, hi) = exponent byte of slot 8j + 2t + hi   (the C-fragment columns of lane t)
 //   [V coef8] nk vectors of 64*TB B.  vector i, lane (g,t), half-word j : ( uV[slot 8j+2t][8i+g], uV[slot 8j+2t+1][8i+g] )
@@ -54,7 +55,7 @@ struct ClassLayout {
   int i8;            // 8-bit coefficient mode
   int tb;            // tiles (of 8 slots) per sub-block: 4 (unflagged) or 2 (flagged)
   int sub_tok;       // slots per sub-block = 8 * tb
-  int coef_bytes;    // nk * 128 * tb  (per K or V, per sub-block); 8-bit mode: nk * 64 * tb codes + 8 * tb exponent bytes
+  int coef_bytes;    // nk * 128 * tb  (per K or V, per sub-block); 8-bit mode: nk * 64 * tb codes + 8 * tb exponent bytes per 32-column block
   int code_bytes;    // per K or V, per sub-block: tb * 4 * d, 0 if !resid
   int scale_bytes;   // tb * d
   int sub_bytes;     // 2*coef + resid * 2*(code + scale)
@@ -70,7 +71,7 @@ DWKV_HD ClassLayout make_class_layout(int rank, int resid, int d, int i8 = 0) {
   c.i8 = i8;
   c.tb = resid ? 2 : 4;
   c.sub_tok = 8 * c.tb;
-  c.coef_bytes = i8 ? c.nk * 64 * c.tb + 8 * c.tb : c.nk * 128 * c.tb;
+  c.coef_bytes = i8 ? c.nk * 64 * c.tb + ((rank + 31) / 32) * 8 * c.tb : c.nk * 128 * c.tb;
   c.code_bytes = resid ? c.tb * 4 * d : 0;
   c.scale_bytes = resid ? c.tb * d : 0;
   c.sub_bytes = 2 * c.coef_bytes + 2 * (c.code_bytes + c.scale_bytes);
@@ -109,9 +110,9 @@ DWKV_HD int vcoef8_elem_off(int s, int col, int tb) {
   const int j = s >> 3, p = s & 7, t = p >> 1, hi = p & 1, i = col >> 3, g = col & 7;
   return i * 64 * tb + (4 * g + t) * 2 * tb + j * 2 + hi;
 }
-DWKV_HD int coef8_exp_off(int s, int nk, int tb) {
+DWKV_HD int coef8_exp_off(int s, int nk, int tb, int blk = 0) {     // blk = rank column / 32
   const int j = s >> 3, p = s & 7, t = p >> 1, hi = p & 1;
-  return nk * 64 * tb + t * 2 * tb + j * 2 + hi;
+  return nk * 64 * tb + blk * 8 * tb + t * 2 * tb + j * 2 + hi;
 }
 DWKV_HD void kcode_nibble(int s, int ch, int d, int* word_off, int* bit) {   // inside [K code] (s in 0..15)
   const int j = s >> 3, g = s & 7, grp = ch >> 4, wi = ch & 15, b = wi >> 3, t = (wi & 7) >> 1, hi = wi & 1;

@@ -65,6 +65,19 @@ __device__ __forceinline__ float2 h2f2(uint32_t w) {
   return __half22float2(*reinterpret_cast<__half2*>(&w));
 }
 
+// 8-bit blockwise coefficient quantiser (reading A27), block = 32 consecutive rank columns of the token's coefficient vector:
+// e = smallest integer with amax <= 127 * 2^e, clamped to >= -126 (amax == 0 and subnormal amax land on the clamp);
+// code = rint(c / 2^e) in [-127, 127]. Every step is exact in fp32. amax = m * 2^x, m in [0.5, 1): e = x - 7 if m <= 127/128 else x - 6.
+__device__ __forceinline__ int coef8_exponent(float amax) {
+  const uint32_t b = __float_as_uint(amax);
+  const int x = (int)((b >> 23) & 0xffu) - 126;
+  const int e = ((b & 0x7fffffu) <= 0x7e0000u) ? x - 7 : x - 6;
+  return max(e, -126);
+}
+__device__ __forceinline__ int coef8_code(float c, int e) {
+  const float q = rintf(c * __uint_as_float((uint32_t)(127 - e) << 23));     // c / 2^e, exact
+  return (int)fminf(fmaxf(q, -127.f), 127.f);
+}
 
 }  // namespace dev
 }  // namespace dwkv

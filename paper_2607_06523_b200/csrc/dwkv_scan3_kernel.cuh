@@ -201,7 +201,8 @@ template <int NK, bool RESID, int NKB, int D, bool PAIR, bool I8>
 __device__ __forceinline__ void process_stage(State<NKB, D>& st, const uint32_t sp, const int n, const int ntok, const int lane,
                                               const QRegs<NKB, D, PAIR>& q, const float cscale) {
   constexpr int SUBTOK = RESID ? 16 : 32;
-  constexpr int SB1 = I8 ? (RESID ? 2 * (NK * 128 + 16) + 20 * D : 2 * (NK * 256 + 32)) : (RESID ? NK * 512 + 20 * D : NK * 1024);
+  constexpr int NBK = (NK + 3) / 4;      // 8-bit planes: exponent bytes per slot and 32-column block
+  constexpr int SB1 = I8 ? (RESID ? 2 * (NK * 128 + NBK * 16) + 20 * D : 2 * (NK * 256 + NBK * 32)) : (RESID ? NK * 512 + 20 * D : NK * 1024);
   if constexpr (RESID || NK > 2) {
 #pragma unroll 1
     for (int sb = 0; sb < n; ++sb) process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
@@ -410,7 +411,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     const Unit un = load_unit(p.units + f_u);
     const int nk = un.rk >> 3, fl = un.cls & 1;
     f_code = nk | (fl << 8);
-    f_sb1 = I8 ? (fl ? 2 * (nk * 128 + 16) + 20 * D : 2 * (nk * 256 + 32)) : (fl ? nk * 512 + 20 * D : nk * 1024);
+    f_sb1 = I8 ? (fl ? 2 * (nk * 128 + ((nk + 3) >> 2) * 16) + 20 * D : 2 * (nk * 256 + ((nk + 3) >> 2) * 32)) : (fl ? nk * 512 + 20 * D : nk * 1024);
     f_subtok = fl ? 16 : 32;
     f_ntok = un.ntok;
     f_nsub = (un.ntok + f_subtok - 1) / f_subtok;
@@ -621,13 +622,15 @@ bool launch_by_rank(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t
   }
   return false;
 }
-// 8-bit coefficient planes: basis rank <= 32 (one block per token vector)
+// 8-bit coefficient planes (one exponent byte per 32-column block of a token vector)
 template <int D, bool PAIR>
 bool launch_by_rank_i8(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* err) {
   const int nkb = (p.r + 15) / 16 * 2;
   switch (nkb) {
     case 2: *err = launch_instance<2, D, PAIR, true>(p, n_sms, s); return true;
     case 4: *err = launch_instance<4, D, PAIR, true>(p, n_sms, s); return true;
+    case 6: *err = launch_instance<6, D, PAIR, true>(p, n_sms, s); return true;
+    case 8: *err = launch_instance<8, D, PAIR, true>(p, n_sms, s); return true;
   }
   return false;
 }

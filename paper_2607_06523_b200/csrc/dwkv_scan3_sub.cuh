@@ -33,13 +33,14 @@ __device__ __forceinline__ void lds_kcodes(uint32_t (&w)[D / 32], uint32_t base,
 template <int NK, bool RESID, int NKB, int D, bool PAIR, bool I8>
 __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp, const int nv, const int lane,
                                             const QRegs<NKB, D, PAIR>& q, const float cscale) {
-  constexpr int TB = RESID ? 2 : 4, NG = D / 16, COEF = I8 ? NK * 64 * TB + 8 * TB : NK * 128 * TB;
+  constexpr int NBK = (NK + 3) / 4;                // 8-bit planes: 32-column blocks of the class rank, one exponent byte per slot and block
+  constexpr int TB = RESID ? 2 : 4, NG = D / 16, COEF = I8 ? NK * 64 * TB + NBK * 8 * TB : NK * 128 * TB;
   constexpr int NSC = PAIR ? TB / 2 : TB;          // score pairs held by a lane
   const int g = lane >> 2, t = lane & 3;
   const int jt = PAIR ? (g >> 2) : 0;              // PAIR: token tile parity of this lane's row
   const uint32_t mA = (g < 4) ? 0xffffffffu : 0u;  // PAIR: lane belongs to a tile-A row
   uint32_t kw[NK][TB], vw[NK][TB];
-  float ksc[NSC][2], vsc[NSC][2];      // I8: 2^e of the tokens behind s[x][0], s[x][1]
+  float ksc[NBK][NSC][2], vsc[NBK][NSC][2];      // I8: 2^e (per block) of the tokens behind s[x][0], s[x][1]
   if constexpr (I8) {
 #pragma unroll
     for (int i = 0; i < NK; ++i) {
@@ -55,20 +56,23 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
         vw[i][0] = u8pair_to_bf16x2(b, 0); vw[i][1] = u8pair_to_bf16x2(b, 1);
       }
     }
-    uint32_t ek[2], ev[2];               // exponent bytes of lane t: (tile j, hi) at byte 2j + hi
-    if constexpr (TB == 4) {
-      const uint2 a = lds64(sp + NK * 256 + t * 8), b = lds64(sp + COEF + NK * 256 + t * 8);
-      ek[0] = a.x; ek[1] = a.y; ev[0] = b.x; ev[1] = b.y;
-    } else {
-      ek[0] = lds32(sp + NK * 128 + t * 4); ev[0] = lds32(sp + COEF + NK * 128 + t * 4);
-      ek[1] = 0u; ev[1] = 0u;
-    }
 #pragma unroll
-    for (int x = 0; x < NSC; ++x) {      // PAIR: s[x] is tile 2x + jt; FULL: tile x
-      const int wi = PAIR ? x : (x >> 1);
-      const int sh = PAIR ? 16 * jt : 16 * (x & 1);
-      ksc[x][0] = exp_byte_to_scale(ek[wi], sh); ksc[x][1] = exp_byte_to_scale(ek[wi], sh + 8);
-      vsc[x][0] = exp_byte_to_scale(ev[wi], sh); vsc[x][1] = exp_byte_to_scale(ev[wi], sh + 8);
+    for (int bk = 0; bk < NBK; ++bk) {
+      uint32_t ek[2], ev[2];             // exponent bytes of lane t: (tile j, hi) at byte 2j + hi
+      if constexpr (TB == 4) {
+        const uint2 a = lds64(sp + NK * 256 + bk * 32 + t * 8), b = lds64(sp + COEF + NK * 256 + bk * 32 + t * 8);
+        ek[0] = a.x; ek[1] = a.y; ev[0] = b.x; ev[1] = b.y;
+      } else {
+        ek[0] = lds32(sp + NK * 128 + bk * 16 + t * 4); ev[0] = lds32(sp + COEF + NK * 128 + bk * 16 + t * 4);
+        ek[1] = 0u; ev[1] = 0u;
+      }
+#pragma unroll
+      for (int x = 0; x < NSC; ++x) {    // PAIR: s[x] is tile 2x + jt; FULL: tile x
+        const int wi = PAIR ? x : (x >> 1);
+        const int sh = PAIR ? 16 * jt : 16 * (x & 1);
+        ksc[bk][x][0] = exp_byte_to_scale(ek[wi], sh); ksc[bk][x][1] = exp_byte_to_scale(ek[wi], sh + 8);
+        vsc[bk][x][0] = exp_byte_to_scale(ev[wi], sh); vsc[bk][x][1] = exp_byte_to_scale(ev[wi], sh + 8);
+      }
     }
   } else {
 #pragma unroll
@@ -91,30 +95,39 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
   float s[NSC][2];
 #pragma unroll
   for (int x = 0; x < NSC; ++x) {
-    float c[4] = {I8 ? 0.f : cinit, I8 ? 0.f : cinit, 0.f, 0.f};
+    if constexpr (I8) {      // integer-valued code dots per 32-column block, the block's power-of-two scale afterwards
+      s[x][0] = cinit; s[x][1] = cinit;
+#pragma unroll
+      for (int bk = 0; bk < NBK; ++bk) {
+        const int i0 = 4 * bk, i1 = (4 * bk + 4 < NK) ? 4 * bk + 4 : NK;
+        float c[4] = {0.f, 0.f, 0.f, 0.f};
+        if constexpr (PAIR) {
+#pragma unroll
+          for (int i = 0; i < NK; ++i)
+            if (i >= i0 && i < i1) mma16h(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
+        } else {
+#pragma unroll
+          for (int pi = 0; pi < NK / 2; ++pi)
+            if (2 * pi >= i0 && 2 * pi < i1) mma16h(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
+          if constexpr (NK & 1)
+            if (NK - 1 >= i0 && NK - 1 < i1) mma8h(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
+        }
+        s[x][0] = fmaf(ksc[bk][x][0], c[0] + c[2], s[x][0]);
+        s[x][1] = fmaf(ksc[bk][x][1], c[1] + c[3], s[x][1]);
+      }
+    } else {
+    float c[4] = {cinit, cinit, 0.f, 0.f};
     if constexpr (PAIR) {    // k = (tile 2x: 8 rank columns | tile 2x+1: 8 rank columns), block-diagonal A
 #pragma unroll
-      for (int i = 0; i < NK; ++i) {
-        if constexpr (I8) mma16h(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
-        else mma16(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
-      }
+      for (int i = 0; i < NK; ++i) mma16(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
     } else {                 // k = 16 rank columns of tile x
 #pragma unroll
-      for (int pi = 0; pi < NK / 2; ++pi) {
-        if constexpr (I8) mma16h(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
-        else mma16(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
-      }
-      if constexpr (NK & 1) {
-        if constexpr (I8) mma8h(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
-        else mma8(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
-      }
+      for (int pi = 0; pi < NK / 2; ++pi)
+        mma16(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
+      if constexpr (NK & 1) mma8(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
     }
-    if constexpr (I8) {
-      s[x][0] = fmaf(ksc[x][0], c[0] + c[2], cinit);
-      s[x][1] = fmaf(ksc[x][1], c[1] + c[3], cinit);
-    } else {
-      s[x][0] = c[0] + c[2];
-      s[x][1] = c[1] + c[3];
+    s[x][0] = c[0] + c[2];
+    s[x][1] = c[1] + c[3];
     }
   }
   // ---- residual-K term: exact integer-code dot on the tensor cores (biased codes, bias folded into C), fp32 scales ----
@@ -207,26 +220,34 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
   if constexpr (PAIR) {
 #pragma unroll
     for (int x = 0; x < NSC; ++x) {
-      uint32_t ph, pl;
-      if constexpr (I8) split_bf16x2(pr[x][0] * vsc[x][0], pr[x][1] * vsc[x][1], ph, pl);
-      else split_bf16x2(pr[x][0], pr[x][1], ph, pl);
-      const uint32_t a0 = ph & mA, a1 = pl & mA, a2 = ph & ~mA, a3 = pl & ~mA;
 #pragma unroll
-      for (int i = 0; i < NK; ++i) mma16(st.acc[i], a0, a1, a2, a3, vw[i][2 * x], vw[i][2 * x + 1]);
+      for (int bk = 0; bk < (I8 ? NBK : 1); ++bk) {      // 8-bit planes: p * 2^e of the block that the rank chunks belong to
+        uint32_t ph, pl;
+        if constexpr (I8) split_bf16x2(pr[x][0] * vsc[bk][x][0], pr[x][1] * vsc[bk][x][1], ph, pl);
+        else split_bf16x2(pr[x][0], pr[x][1], ph, pl);
+        const uint32_t a0 = ph & mA, a1 = pl & mA, a2 = ph & ~mA, a3 = pl & ~mA;
+#pragma unroll
+        for (int i = 0; i < NK; ++i)
+          if (!I8 || (i >> 2) == bk) mma16(st.acc[i], a0, a1, a2, a3, vw[i][2 * x], vw[i][2 * x + 1]);
+      }
     }
   } else {
 #pragma unroll
     for (int ks = 0; ks < TB / 2; ++ks) {
-      uint32_t a0, a1, a2, a3;
-      if constexpr (I8) {
-        split_bf16x2(pr[2 * ks][0] * vsc[2 * ks][0], pr[2 * ks][1] * vsc[2 * ks][1], a0, a1);
-        split_bf16x2(pr[2 * ks + 1][0] * vsc[2 * ks + 1][0], pr[2 * ks + 1][1] * vsc[2 * ks + 1][1], a2, a3);
-      } else {
-        split_bf16x2(pr[2 * ks][0], pr[2 * ks][1], a0, a1);
-        split_bf16x2(pr[2 * ks + 1][0], pr[2 * ks + 1][1], a2, a3);
-      }
 #pragma unroll
-      for (int i = 0; i < NK; ++i) mma16(st.acc[i], a0, a1, a2, a3, vw[i][2 * ks], vw[i][2 * ks + 1]);
+      for (int bk = 0; bk < (I8 ? NBK : 1); ++bk) {
+        uint32_t a0, a1, a2, a3;
+        if constexpr (I8) {
+          split_bf16x2(pr[2 * ks][0] * vsc[bk][2 * ks][0], pr[2 * ks][1] * vsc[bk][2 * ks][1], a0, a1);
+          split_bf16x2(pr[2 * ks + 1][0] * vsc[bk][2 * ks + 1][0], pr[2 * ks + 1][1] * vsc[bk][2 * ks + 1][1], a2, a3);
+        } else {
+          split_bf16x2(pr[2 * ks][0], pr[2 * ks][1], a0, a1);
+          split_bf16x2(pr[2 * ks + 1][0], pr[2 * ks + 1][1], a2, a3);
+        }
+#pragma unroll
+        for (int i = 0; i < NK; ++i)
+          if (!I8 || (i >> 2) == bk) mma16(st.acc[i], a0, a1, a2, a3, vw[i][2 * ks], vw[i][2 * ks + 1]);
+      }
     }
   }
   // ---- e^T += codeV^T . (P * scaleV): channels on the MMA m dimension, rows/heads on n ----------------------------------

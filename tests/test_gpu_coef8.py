@@ -10,7 +10,7 @@ import torch
 import gen
 from oracle import dwkv_coef8_oracle as c8
 from oracle import dwkv_oracle as orc
-from helpers import f64, check_output, rel_l2
+from helpers import f64, check_output, rel_l2, oracle_slice_from_kept
 from test_gpu_parity import all_lh, compare
 
 pytestmark = pytest.mark.gpu
@@ -132,9 +132,11 @@ def test_llama8b_shape_pair_mode_sampled(mod):
     cache.destroy()
 
 
-@pytest.mark.parametrize("d,G,ranks", [(64, 1, (8,)), (64, 8, (8, 16)), (128, 8, (8, 24)), (128, 2, (16, 32)), (64, 3, (24, 32))])
+@pytest.mark.parametrize("d,G,ranks", [(64, 1, (8,)), (64, 8, (8, 16)), (128, 8, (8, 24)), (128, 2, (16, 32)), (64, 3, (24, 32)),
+                                        (128, 8, (8, 24, 48)), (128, 2, (16, 64)), (64, 4, (8, 48)), (64, 6, (32, 64))])
 def test_kernel_instances(mod, d, G, ranks):
-    """FULL mode (G > 4), odd chunk counts (rank 24), both head dims."""
+    """FULL mode (G > 4), odd chunk counts (rank 24), both head dims; ranks 48 and 64: two 32-column blocks per token vector
+    (two exponent bytes per slot; BASELINE.json configs[3], the 70B shape, has r = 48)."""
     binding, harness = mod
     wl = dataclasses.replace(gen.WORKLOADS["tiny"], d=d, G=G, tier_ranks=ranks, tier_frac=tuple([1.0 / len(ranks)] * len(ranks)), T=(700,))
     routings = [gen.make_routing(wl, 0)]
@@ -145,7 +147,7 @@ def test_kernel_instances(mod, d, G, ranks):
     cache.destroy()
 
 
-@pytest.mark.parametrize("shape", ["tiny", "8b", "r24"])
+@pytest.mark.parametrize("shape", ["tiny", "8b", "r24", "70b", "r64"])
 def test_append_compress_against_oracle(mod, shape):
     """dwkv_append_compress in 8-bit mode from dense K/V: the fp32 projection differs from the oracle's fp64 one in the last bits,
     which can move a code across a rounding boundary (reading A15 iii carried over): coefficients equal on >= 99.5 % of entries and
@@ -156,6 +158,10 @@ def test_append_compress_against_oracle(mod, shape):
     wl = {"tiny": dataclasses.replace(gen.WORKLOADS["tiny"], T=(96,)),
           "8b": dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, w=2, H_kv=2, T=(96, 96)),
           "r24": dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, w=2, H_kv=1, tier_ranks=(8, 24),
+                                     tier_frac=(0.5, 0.5), T=(96, 96)),
+          # two 32-column blocks per token vector: the 70B shape (ranks 8 / 24 / 48, G = 8, w = 4) and a rank-64 basis
+          "70b": dataclasses.replace(gen.WORKLOADS["llama70b_128k_b1"], L=4, H_kv=2, T=(96, 96)),
+          "r64": dataclasses.replace(gen.WORKLOADS["llama8b_16k_b8"], L=2, w=2, H_kv=1, tier_ranks=(16, 64),
                                      tier_frac=(0.5, 0.5), T=(96, 96))}[shape]
     n_t = len(wl.tier_ranks)
     cache, consts = harness.make_cache(wl, n_seqs=2, max_tokens=512, coef_int8=True)
@@ -204,6 +210,39 @@ def test_append_compress_against_oracle(mod, shape):
     cache.destroy()
 
 
+@pytest.mark.parametrize("name", ["llama8b_16k_b8", "llama8b_64k_b1", "llama8b_64k_b8", "llama70b_128k_b1", "ragged32"])
+def test_full_size_sampled_slices_i8(mod, name):
+    """Every BASELINE.json config at full size in the paper's own coefficient format (PAPER.md:56 "8-bit blockwise quantized";
+    the 70B shape has rank 48 = two blocks per token vector): sampled (layer, head) slices of sampled sequences against the oracle
+    fed with the oracle-quantised coefficients, all-layer call and one per-layer call."""
+    binding, harness = mod
+    wl = gen.WORKLOADS[name]
+    routings = [gen.make_routing(wl, s) for s in range(wl.n_seq)]
+    cache, consts = harness.make_cache(wl, arena_bytes=harness.arena_bytes_for(wl, routings, 1), coef_int8=True)
+    keep = [(0, 0), (wl.L - 1, wl.H_kv - 1)]
+    sampled = [0, 1, 3, 4, wl.n_seq - 1] if name == "ragged32" else sorted({0, wl.n_seq - 1})
+    kept = {}
+    for s, (tier, flag) in enumerate(routings):
+        kept[s] = harness.fill_sequence(cache, wl, s, s, tier, flag, chunk=8192, keep=keep if s in sampled else [])
+    keptq = dict(zip(sampled, kept_quantised(wl, [routings[s] for s in sampled], [kept[s] for s in sampled])))
+    ids = list(range(wl.n_seq))
+    q = gen.make_q(wl, device="cuda", gain=2.0)
+    o = cache.decode_attention(-1, ids, q).double().cpu().numpy()
+    l1 = wl.L - 1
+    o_l = cache.decode_attention(l1, ids, q[:, l1].contiguous()).double().cpu().numpy()
+    qn = f64(q)
+    for s in sampled:
+        tier, flag = routings[s]
+        for (l, h) in keep:
+            sl = slice(h * wl.G, (h + 1) * wl.G)
+            o_ref, V, _ = oracle_slice_from_kept(wl, consts, tier, flag, keptq[s][(l, h)], qn[s, l, sl], l, h)
+            check_output(o[s, l, sl], o_ref, float(np.abs(V).max()), f"i8 {name} seq {s} (l,h)=({l},{h})")
+            if l == l1:
+                check_output(o_l[s, sl], o_ref, float(np.abs(V).max()), f"i8 {name} per-layer seq {s} (l,h)=({l},{h})")
+    assert cache.footprint()["used_bytes"] == sum(c8.footprint_bytes_i8(t, f, wl.tier_ranks, wl.d, wl.L, wl.H_kv) for t, f in routings)
+    cache.destroy()
+
+
 def test_option_errors(mod):
     binding, harness = mod
     wl = gen.WORKLOADS["tiny"]
@@ -221,7 +260,9 @@ def test_option_errors(mod):
     cache.destroy()
     wl70 = dataclasses.replace(gen.WORKLOADS["llama70b_128k_b1"], L=4, T=(64,))
     cache, _ = harness.make_cache(wl70, n_seqs=1, max_tokens=64)
-    with pytest.raises(binding.DwkvError) as e:
-        cache.set_option("coef_int8", 1)                      # basis rank 48 > 32: two blocks per token are not built
-    assert e.value.code == binding.DWKV_E_INVALID
+    cache.set_option("coef_int8", 1)                          # basis rank 48: two 32-column blocks per token vector
+    tier = np.full(5, 2, np.uint8); flag = np.zeros(5, np.uint8)
+    cK, cV = gen.make_coef_chunk(wl70, 0, 0, tier, device="cuda")
+    cache.append_raw(0, tier, flag, cK, cV)
+    assert cache.footprint()["used_bytes"] == 5 * 2 * (48 + 2) * wl70.L * wl70.H_kv
     cache.destroy()
