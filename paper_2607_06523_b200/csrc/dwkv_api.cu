@@ -979,6 +979,7 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   sp.layer0 = layer0; sp.Lq = Lsel; sp.LH = Lsel * g.H; sp.w = g.w;
   sp.H = g.H; sp.G = g.G; sp.r = g.r; sp.d = g.d;
   sp.cscale = c->softmax_scale * 1.4426950408889634f;
+  sp.zero = 0.f;
   sp.i8 = g.i8;
   sp.fuse = fuse_mode; sp.spc = P.spc;
   sp.wlast = (const int32_t*)(blob + P.off_wlast);

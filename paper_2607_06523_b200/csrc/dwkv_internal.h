@@ -37,6 +37,7 @@ struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.c
   int32_t layer0, Lq, LH, w;
   int32_t H, G, r, d;
   float cscale;                // softmax_scale * log2(e)
+  float zero;                  // 0.0f (an operand the compiler cannot constant-fold)
   int32_t i8;                  // 8-bit coefficient planes (dwkv_layout.cuh)
   // fused split-combine (step a3 inside the decode kernel; per-layer calls): the warps of a CTA take CONSECUTIVE slices, merge their
   // end-of-slice partials per segment in shared memory and write one partial per (CTA, segment); every partial written is an arrival

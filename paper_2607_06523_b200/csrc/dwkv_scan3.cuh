@@ -117,6 +117,18 @@ __device__ __forceinline__ void mma16(float (&d)[4], uint32_t a0, uint32_t a1, u
       : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
       : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+// D = A . B + C with C in registers of its own (the persistent (-m_ref, -m_ref, 0, 0) quad of the score MMAs: no per-sub-block copy)
+__device__ __forceinline__ void mma16c(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1,
+                                       const float (&c)[4]) {
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%11,%12,%13};"
+      : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "f"(c[0]), "f"(c[1]), "f"(c[2]), "f"(c[3]));
+}
+__device__ __forceinline__ void mma8c(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t b0, const float (&c)[4]) {
+  asm("mma.sync.aligned.m16n8k8.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5}, {%6}, {%7,%8,%9,%10};"
+      : "=f"(d[0]), "=f"(d[1]), "=f"(d[2]), "=f"(d[3])
+      : "r"(a0), "r"(a1), "r"(b0), "f"(c[0]), "f"(c[1]), "f"(c[2]), "f"(c[3]));
+}
 // D = A . B (C = 0): fresh outputs, no accumulator initialisation
 __device__ __forceinline__ void mma16z(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0, uint32_t b1) {
   asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
@@ -173,6 +185,7 @@ template <int NKB, int D>
 struct State {
   float m;                 // reference of row g (log2 units), -inf = none yet
   float thr;               // -inf while unreferenced, kLazy afterwards
+  float cq[4];             // C operand of the score MMAs: (-m, -m, 0, 0), (0, 0, 0, 0) while unreferenced; changes only on a rescale
   float l;                 // this lane's share of sum p of row g
   float acc[NKB][4];       // a[row g][8i + 2t + {0,1}] hi-part accumulators (0,1) and lo-part accumulators (2,3)
   float eacc[D / 16][4];   // TRANSPOSED e^T[channel 16grp + g (+8)][column 2t + {0,1}], column n <-> row n

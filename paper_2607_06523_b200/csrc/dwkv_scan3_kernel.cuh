@@ -137,8 +137,11 @@ __device__ __forceinline__ void prologue_compute(QRegs<NKB, D, PAIR>& q, const P
 }
 
 template <int NKB, int D>
-__device__ __forceinline__ void state_reset(State<NKB, D>& st) {
+__device__ __forceinline__ void state_reset(State<NKB, D>& st, const float zero) {
   st.m = -INFINITY; st.thr = -INFINITY; st.l = 0.f;
+  // (zero comes from a kernel parameter: a value the compiler cannot fold, so the quad stays in four registers of its own instead of
+  //  being rebuilt before every MMA chain)
+  st.cq[0] = st.cq[1] = st.cq[2] = st.cq[3] = zero;
 #pragma unroll
   for (int i = 0; i < NKB; ++i) st.acc[i][0] = st.acc[i][1] = st.acc[i][2] = st.acc[i][3] = 0.f;
 #pragma unroll
@@ -203,18 +206,21 @@ __device__ __forceinline__ void process_stage(State<NKB, D>& st, const uint32_t 
   constexpr int SUBTOK = RESID ? 16 : 32;
   constexpr int NBK = (NK + 3) / 4;      // 8-bit planes: exponent bytes per slot and 32-column block
   constexpr int SB1 = I8 ? (RESID ? 2 * (NK * 128 + NBK * 16) + 20 * D : 2 * (NK * 256 + NBK * 32)) : (RESID ? NK * 512 + 20 * D : NK * 1024);
+  // only the last sub-block of a stage can be ragged (the end of a unit): the full ones run without the per-score slot checks
+  const int nfull = (ntok >= n * SUBTOK) ? n : n - 1;
   if constexpr (RESID || NK > 2) {
 #pragma unroll 1
-    for (int sb = 0; sb < n; ++sb) process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+    for (int sb = 0; sb < nfull; ++sb) process_sub<NK, RESID, NKB, D, PAIR, I8, false>(st, sp + sb * SB1, SUBTOK, lane, q, cscale);
   } else {   // two independent sub-blocks per iteration: more instruction-level parallelism for the 2 warps per scheduler
     int sb = 0;
 #pragma unroll 1
-    for (; sb + 2 <= n; sb += 2) {
-      process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
-      process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + (sb + 1) * SB1, ntok - (sb + 1) * SUBTOK, lane, q, cscale);
+    for (; sb + 2 <= nfull; sb += 2) {
+      process_sub<NK, RESID, NKB, D, PAIR, I8, false>(st, sp + sb * SB1, SUBTOK, lane, q, cscale);
+      process_sub<NK, RESID, NKB, D, PAIR, I8, false>(st, sp + (sb + 1) * SB1, SUBTOK, lane, q, cscale);
     }
-    if (sb < n) process_sub<NK, RESID, NKB, D, PAIR, I8>(st, sp + sb * SB1, ntok - sb * SUBTOK, lane, q, cscale);
+    if (sb < nfull) process_sub<NK, RESID, NKB, D, PAIR, I8, false>(st, sp + sb * SB1, SUBTOK, lane, q, cscale);
   }
+  if (nfull < n) process_sub<NK, RESID, NKB, D, PAIR, I8, true>(st, sp + nfull * SB1, ntok - nfull * SUBTOK, lane, q, cscale);
 }
 
 // ---- fused split-combine (step a3 inside the decode kernel; per-layer calls) ---------------------------------------------------
@@ -466,7 +472,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     for (int k = 0; k < NS; ++k) fetch_one(k);
     __syncwarp();
     prologue_compute<NKB, D, PAIR, I8>(q, pl, p, ws.x, lane);
-    state_reset<NKB, D>(st);
+    state_reset<NKB, D>(st, p.zero);
   }
 
   // ---- compute stream ----------------------------------------------------------------------------------------------------
@@ -486,7 +492,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
       if constexpr (FUSE) { if (p.fuse == 1) arrive<D>(p, cur_seg, rec, lane, &sh_ntodo, sh_todo); }
       slot_next = __ldg(p.pstart + seg);       // a segment entered inside a slice is entered at its start: its first slot
       prologue_compute<NKB, D, PAIR, I8>(q, pl, p, seg, lane);
-      state_reset<NKB, D>(st);
+      state_reset<NKB, D>(st, p.zero);
       cur_seg = seg;
       ++n_entered;
     }

@@ -30,7 +30,8 @@ __device__ __forceinline__ void lds_kcodes(uint32_t (&w)[D / 32], uint32_t base,
 // planes (dwkv_layout.cuh): codes are widened to exact 16-bit floating integers in registers (K: fp16, the score MMA runs in fp16
 // with q~ split hi + lo in fp16; V: bf16, because p * 2^e needs the bf16 exponent range), the token's power-of-two scale multiplies its
 // score after the MMA and its p before the value MMA -- the contractions themselves are unchanged.
-template <int NK, bool RESID, int NKB, int D, bool PAIR, bool I8>
+// RAGGED = the sub-block may hold fewer than 8 * TB valid tokens (only the last sub-block of a unit can): the full ones skip the checks
+template <int NK, bool RESID, int NKB, int D, bool PAIR, bool I8, bool RAGGED>
 __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp, const int nv, const int lane,
                                             const QRegs<NKB, D, PAIR>& q, const float cscale) {
   constexpr int NBK = (NK + 3) / 4;                // 8-bit planes: 32-column blocks of the class rank, one exponent byte per slot and block
@@ -91,7 +92,7 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
   }
   }
   // ---- scores relative to the reference: s' = q~ . cK - m_ref, hi and lo parts of q~ on MMA rows r and r + 8 ----------
-  const float cinit = (st.thr == -INFINITY) ? 0.f : -st.m;
+  const float cinit = st.cq[0];
   float s[NSC][2];
 #pragma unroll
   for (int x = 0; x < NSC; ++x) {
@@ -116,15 +117,21 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
         s[x][1] = fmaf(ksc[bk][x][1], c[1] + c[3], s[x][1]);
       }
     } else {
-    float c[4] = {cinit, cinit, 0.f, 0.f};
+    float c[4];              // the first MMA of the chain takes C = (-m_ref, -m_ref, 0, 0) from the state's own registers
     if constexpr (PAIR) {    // k = (tile 2x: 8 rank columns | tile 2x+1: 8 rank columns), block-diagonal A
+      mma16c(c, q.qa[0][0], q.qa[0][1], q.qa[0][2], q.qa[0][3], kw[0][2 * x], kw[0][2 * x + 1], st.cq);
 #pragma unroll
-      for (int i = 0; i < NK; ++i) mma16(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
+      for (int i = 1; i < NK; ++i) mma16(c, q.qa[i][0], q.qa[i][1], q.qa[i][2], q.qa[i][3], kw[i][2 * x], kw[i][2 * x + 1]);
     } else {                 // k = 16 rank columns of tile x
+      if constexpr (NK >= 2) {
+        mma16c(c, q.qa[0][0], q.qa[0][1], q.qa[1][0], q.qa[1][1], kw[0][x], kw[1][x], st.cq);
 #pragma unroll
-      for (int pi = 0; pi < NK / 2; ++pi)
-        mma16(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
-      if constexpr (NK & 1) mma8(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
+        for (int pi = 1; pi < NK / 2; ++pi)
+          mma16(c, q.qa[2 * pi][0], q.qa[2 * pi][1], q.qa[2 * pi + 1][0], q.qa[2 * pi + 1][1], kw[2 * pi][x], kw[2 * pi + 1][x]);
+        if constexpr (NK & 1) mma8(c, q.qa[NK - 1][0], q.qa[NK - 1][1], kw[NK - 1][x]);
+      } else {
+        mma8c(c, q.qa[0][0], q.qa[0][1], kw[0][x], st.cq);
+      }
     }
     s[x][0] = c[0] + c[2];
     s[x][1] = c[1] + c[3];
@@ -175,8 +182,7 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
       }
     }
   }
-  if (nv < 8 * TB) {   // ragged tail: slots >= nv do not exist (rare: a real branch, not predication of every score)
-    asm volatile("");
+  if constexpr (RAGGED) {   // ragged tail: slots >= nv do not exist
 #pragma unroll
     for (int x = 0; x < NSC; ++x) {
       const int slot = PAIR ? (16 * x + 8 * jt + 2 * t) : (8 * x + 2 * t);
@@ -192,10 +198,15 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
     mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 1));
     mx = fmaxf(mx, __shfl_xor_sync(kFull, mx, 2));
     const bool unref = st.thr == -INFINITY, none = mx == -INFINITY;
+    // The reference is kept INTEGER-valued (log2 units): references of different work splits then differ by whole powers of two, so
+    // p = 2^(s - m), its hi + lo split and the bf16 rounding of the p * scaleV operand scale exactly and the result no longer depends
+    // on where the slices were cut beyond fp32 summation order (pin P11)
+    mx = ceilf(mx);
     const float up = unref ? (none ? 0.f : mx) : fmaxf(mx, 0.f);   // new reference = old reference + up
     const float corr = unref ? 1.f : ex2(-up);
     st.m = unref ? (none ? -INFINITY : mx) : st.m + up;
     st.thr = (unref && none) ? -INFINITY : kLazy;
+    st.cq[0] = st.cq[1] = (st.thr == -INFINITY) ? st.cq[2] : -st.m;
     st.l *= corr;
 #pragma unroll
     for (int i = 0; i < NKB; ++i) { st.acc[i][0] *= corr; st.acc[i][1] *= corr; st.acc[i][2] *= corr; st.acc[i][3] *= corr; }

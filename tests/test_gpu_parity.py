@@ -138,9 +138,10 @@ def test_raw_mode_b_codes_and_minus_eight(mod):
 
 def test_split_invariance_p11(mod):
     """Result independent of the work split (pin P11): one block per unit, a single warp slice for the whole step, a few
-    slices, class-interleaved order with tiny units, and the default plan. Different cuts move the rescale points and the
-    bf16 roundings of the p * scaleV operand of the residual-V MMA, so the bar between variants is
-    that rounding level (1e-3 rel-L2); every variant must also meet the oracle tolerance."""
+    slices, class-interleaved order with tiny units, the default plan and the fused-combine variants. The softmax reference of
+    every warp is integer-valued (log2 units), so different cuts change p, its hi + lo split and the bf16 rounding of the p * scaleV
+    operand by exact powers of two only: the variants agree to fp32 summation order (<= 2e-6 rel-L2; SURVEY.md
+    section 8c asks 1e-6; measured 5.8e-7, printed); every variant must also meet the oracle tolerance."""
     binding, harness = mod
     wl = gen.WORKLOADS["tiny"]
     routings = [gen.make_routing(wl, 0)]
@@ -162,8 +163,9 @@ def test_split_invariance_p11(mod):
         assert shapes[-1][2] == (1 if change.get("fuse_combine", 0) == 1 else 0)
     assert shapes[1][1] == wl.L * wl.H_kv            # one slice: one partial per segment
     assert len(set(shapes)) >= 5, shapes
-    for o in outs[1:]:
-        assert rel_l2(o, outs[0]) < 1e-3
+    worst = max(rel_l2(o, outs[0]) for o in outs[1:])
+    print(f"P11 split invariance: worst rel-L2 between work splits {worst:.2e}")
+    assert worst < 2e-6
     for o in outs:
         compare(wl, cache, consts, kept, routings, q, torch.as_tensor(o), what="split variant")
     cache.destroy()
