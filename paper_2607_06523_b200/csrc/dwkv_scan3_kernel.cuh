@@ -422,7 +422,7 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     f_ntok = un.ntok;
     f_nsub = (un.ntok + f_subtok - 1) / f_subtok;
     f_per = SLOT / f_sb1;
-    if (f_per > 2) f_per &= ~1;       // even stages: the unflagged low-rank classes are processed two sub-blocks at a time
+    if (!fl && nk <= 2) f_per &= ~1;  // even stages: the unflagged low-rank classes are processed two sub-blocks at a time
     f_base = p.arena + un.page_off + (size_t)(p.layer0 * p.H + f_lh) * kPageLhBytes + (size_t)un.blk0 * (size_t)(f_sb1 * (kBlockTok / f_subtok));
   };
   unit_setup();

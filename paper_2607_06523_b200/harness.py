@@ -17,8 +17,9 @@ def class_block_bytes(rank: int, flag: int, d: int) -> int:
     return 2 * (rank // 8) * 512 + flag * 40 * d
 
 
-def arena_bytes_for(wl: gen.Workload, routings, slack_pages_per_class: int = 1) -> int:
-    """Pages needed for the given per-sequence (tier, flag) routings, plus slack for appended tokens."""
+def arena_bytes_for(wl: gen.Workload, routings, slack_pages_per_class: int = 1, slack_tokens: int = 0) -> int:
+    """Pages needed for the given per-sequence (tier, flag) routings, plus slack for appended tokens: `slack_pages_per_class` pages
+    per (sequence, class), and room for `slack_tokens` more tokens per sequence in whichever class they fall."""
     page = wl.L * wl.H_kv * PAGE_LH_BYTES
     pages = 0
     for tier, flag in routings:
@@ -26,7 +27,7 @@ def arena_bytes_for(wl: gen.Workload, routings, slack_pages_per_class: int = 1) 
         for k in range(2 * len(wl.tier_ranks)):
             tpp = (PAGE_LH_BYTES // class_block_bytes(wl.tier_ranks[k >> 1], k & 1, wl.d)) * 32
             n = int((cls == k).sum())
-            pages += (n + tpp - 1) // tpp + slack_pages_per_class
+            pages += (n + tpp - 1) // tpp + slack_pages_per_class + (slack_tokens + tpp - 1) // tpp
     return pages * page
 
 
