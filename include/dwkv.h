@@ -182,7 +182,6 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *   "time_scan"       1 = bracket the fused decode kernel and the append/compress kernel with CUDA events
  *                     (dwkv_get_stat "scan_ms" / "compress_ms")
  *   "sketch_umma"     dwkv_build_basis: 1 (default) = TMA + tcgen05 sketch kernel for d = 128, 0 = mma.sync kernel
- *   "compress_umma"   dwkv_append_compress: 1 = TMA + tcgen05 kernel (d = 128, r <= 48; experimental, slower), 0 (default) = mma.sync kernel
  *   "max_unit_blocks" planner: blocks (of 32 token slots) per work unit, 0 = by "unit_kb"
  *   "unit_kb"         planner: target size of a work unit per (layer, head), KB (default 64 = one page stripe)
  *   "n_slices"        planner: number of warp slices the step is cut into, 0 (default) = one per warp of the persistent grid,

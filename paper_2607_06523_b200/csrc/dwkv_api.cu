@@ -164,7 +164,6 @@ struct dwkv_cache {
   int64_t opt_time_scan = 0;
   int64_t opt_combine_warps = 0;     // combine kernel: warps per (segment, head): 1 / 4 / 16, 0 = by partials per segment
   int64_t opt_fuse_combine = 0;      // 0 = separate combine kernel (default), 1 = split-combine fused into the decode kernel, 2 = CTA merge + combine kernel
-  int64_t opt_compress_umma = 0;     // append/compress: 1 = tcgen05 kernel (d = 128, r <= 64), 0 = mma.sync kernel
   int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
   static constexpr int kScanRing = 64;   // "time_scan": the last 64 decode kernels are bracketed, read back without a sync in between
   cudaEvent_t ev_scan0[kScanRing] = {}, ev_scan1[kScanRing] = {}, ev_app0 = nullptr, ev_app1 = nullptr;
@@ -458,12 +457,13 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
   cudaStream_t st = (cudaStream_t)stream;
   // Large (prefill-sized) calls go in chunks of kChunk tokens of the call's row order: the host routes chunk i + 1 while the GPU
   // compresses chunk i. Rows keep their global index (TokDst::src), so every launch reads k_new / v_new in place.
-  constexpr int64_t kChunk = 16384;
+  // (the first chunk is short, so that the GPU starts while the host still routes)
+  constexpr int64_t kChunk = 16384, kFirst = 4096;
   std::vector<TokDst> dst, sorted;
   std::vector<int32_t> new_pages;
   int ridx = 0;
-  for (int64_t g0 = 0; g0 < total; g0 += kChunk) {
-    const int64_t g1 = std::min(total, g0 + kChunk);
+  for (int64_t g0 = 0, g1 = 0; g0 < total; g0 = g1) {
+    g1 = std::min(total, g0 + ((g0 == 0 && total > kChunk) ? kFirst : kChunk));
     dst.clear();
     new_pages.clear();
     int64_t off = 0;
@@ -475,23 +475,6 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
         for (size_t k = first; k < dst.size(); ++k) dst[k].src = (int32_t)(lo + (int64_t)(k - first));
       }
       off += n_new[i];
-    }
-    if (c->opt_compress_umma && !c->geom.i8 && compress_umma_supported(c->geom, k_new, v_new)) {
-      // tcgen05 path: rows in call order (TMA tile loads), destinations in the same order
-      int rc = zero_new_pages(c, new_pages, st);
-      if (rc) return rc;
-      rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
-      if (rc) return rc;
-      if (c->opt_time_scan && g0 == 0) {
-        if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
-        CU_OK(cudaEventRecord(c->ev_app0, st));
-      }
-      const int launched = launch_compress_umma(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)dst.size(), (int)g0, total,
-                                                (const __nv_bfloat16*)k_new, (const __nv_bfloat16*)v_new, c->BK, c->BV, c->gK, c->gV,
-                                                c->n_sms, st);
-      if (launched) { c->launches += launched; continue; }
-      // no tensor-map entry point: fall through to the mma.sync kernel (pages are zeroed and the table is re-uploaded sorted)
-      new_pages.clear();
     }
     // flagged tokens first, then by descending rank: only the flagged 16-token tiles run the reconstruction + int4 quantiser
     // part of the kernel, and a tile multiplies only the rank chunks its tokens keep. Counting sort, stable.
@@ -634,7 +617,6 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   else if (!strcmp(key, "combine_warps")) c->opt_combine_warps = value;
   else if (!strcmp(key, "fuse_combine")) c->opt_fuse_combine = value;
   else if (!strcmp(key, "sketch_umma")) c->opt_sketch_umma = value;
-  else if (!strcmp(key, "compress_umma")) c->opt_compress_umma = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
   else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
   else if (!strcmp(key, "interleave")) c->opt_interleave = value;

@@ -32,16 +32,50 @@ __global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Co
   __shared__ float sh_e[S][D];
   const int seg = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ws = SPLIT ? warp : 0;                  // this warp's offset in the split
-  // programmatic dependent launch: this grid may start while the decode kernel drains; wait for its completion and flush
-  cudaGridDependencySynchronize();
-  cudaTriggerProgrammaticLaunchCompletion();        // the next decode kernel of the stream may become resident; it waits for this grid's end
   const int b = seg / p.LH, lh = seg - b * p.LH;
   const int layer = p.layer0 + lh / p.H, h = lh % p.H;
   const int G = p.G, r = p.r, PR = 2 + p.r + D;
   const int P0 = __ldg(p.pstart + seg), n = __ldg(p.pstart + seg + 1) - P0;
   const size_t stride = (size_t)G * PR;
+  // The merge is a chain of dependent L2 round trips (~0.8 us each), so everything that does not depend on an earlier load is
+  // requested up front. The basis rows and the gate of the back-projection (the same for every query head of the segment) and the
+  // plan are constants: they are requested BEFORE the grid dependency resolves, i.e. while the decode kernel still drains.
+  const bool finisher = !SPLIT || warp == 0;
+  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
+  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
+  uint2 bw[32];                                     // rows 0..31 of the basis block (CPL = 2: .y unused)
+  uint2 gw = make_uint2(0u, 0u);
+  if (finisher) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      if constexpr (CPL == 4) bw[j] = (j < r) ? __ldg(reinterpret_cast<const uint2*>(BV + (size_t)j * D)) : make_uint2(0u, 0u);
+      else bw[j] = make_uint2((j < r) ? __ldg(reinterpret_cast<const uint32_t*>(BV + (size_t)j * D)) : 0u, 0u);
+    }
+    if constexpr (CPL == 4) gw = __ldg(reinterpret_cast<const uint2*>(gVp));
+    else gw.x = __ldg(reinterpret_cast<const uint32_t*>(gVp));
+  }
+  // programmatic dependent launch: this grid may start while the decode kernel drains; wait for its completion and flush
+  cudaGridDependencySynchronize();
+  cudaTriggerProgrammaticLaunchCompletion();        // the next decode kernel of the stream may become resident; it waits for this grid's end
   for (int gq = SPLIT ? (int)blockIdx.y : warp; gq < G; gq += SPLIT ? G : 4) {
   const float* part = p.part + ((size_t)P0 * G + gq) * PR;       // partial k of this head: part + k * stride
+  // (the maxima of all partials and the first batch of this warp's partial records are requested together: the weights need m*, the
+  //  loads do not)
+  const int nw = (n > ws) ? (n - ws + S - 1) / S : 0;            // partials of this warp: ws, ws + S, ...
+  // first batch of this warp's partials (8), requested before m* is known
+  float va0[8], va1[8], ml0[8], ml1[8];
+  float2 ve[8][CPL / 2];
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    const float* rec = part + (size_t)(ws + S * min(u, max(nw - 1, 0))) * stride;
+    const bool ok = u < nw;
+    const float2 ml = ok ? *reinterpret_cast<const float2*>(rec) : make_float2(-INFINITY, 0.f);
+    ml0[u] = ml.x; ml1[u] = ml.y;
+    va0[u] = (ok && lane < r) ? rec[2 + lane] : 0.f;
+    va1[u] = (ok && lane + 32 < r) ? rec[2 + lane + 32] : 0.f;
+#pragma unroll
+    for (int c = 0; c < CPL / 2; ++c) ve[u][c] = ok ? *reinterpret_cast<const float2*>(rec + 2 + r + lane * CPL + 2 * c) : make_float2(0.f, 0.f);
+  }
   // pass 1: m* over all partials (every warp computes it: n is small, the loads hit L2)
   float mstar = -INFINITY;
   for (int k0 = lane; k0 < n; k0 += 32 * 8) {       // 8 independent loads in flight per lane
@@ -53,46 +87,42 @@ __global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Co
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) mstar = fmaxf(mstar, __shfl_xor_sync(kFull, mstar, o));
-  // pass 2: this warp's partials w, w+4, ...; lane j of a 32-batch owns the weight of the batch's j-th partial
+  // pass 2: weighted sums; lanes hold rank columns (a*) and channels (e*); every lane computes the weights of the batch itself
   float lsum = 0.f, a0 = 0.f, a1 = 0.f, e[CPL];
 #pragma unroll
   for (int c = 0; c < CPL; ++c) e[c] = 0.f;
-  const int nw = (n > ws) ? (n - ws + S - 1) / S : 0;            // partials of this warp
-  for (int i0 = 0; i0 < nw; i0 += 32) {
-    const int i = i0 + lane;
-    float wk = 0.f;
-    if (i < nw) {
-      const float2 ml = *reinterpret_cast<const float2*>(part + (size_t)(ws + S * i) * stride);
-      wk = (ml.x == -INFINITY) ? 0.f : ex2(ml.x - mstar);
-      lsum = fmaf(wk, ml.y, lsum);
+#pragma unroll
+  for (int u = 0; u < 8; ++u) {
+    const float wu = (ml0[u] == -INFINITY) ? 0.f : ex2(ml0[u] - mstar);
+    lsum = fmaf(wu, ml1[u], lsum);
+    a0 = fmaf(wu, va0[u], a0);
+    a1 = fmaf(wu, va1[u], a1);
+#pragma unroll
+    for (int c = 0; c < CPL / 2; ++c) { e[2 * c] = fmaf(wu, ve[u][c].x, e[2 * c]); e[2 * c + 1] = fmaf(wu, ve[u][c].y, e[2 * c + 1]); }
+  }
+  for (int i0 = 8; i0 < nw; i0 += 8) {               // further batches (more than 8 partials per warp: rare)
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const bool ok = i0 + u < nw;
+      const float* rec = part + (size_t)(ws + S * min(i0 + u, nw - 1)) * stride;
+      const float2 ml = ok ? *reinterpret_cast<const float2*>(rec) : make_float2(-INFINITY, 0.f);
+      ml0[u] = ml.x; ml1[u] = ml.y;
+      va0[u] = (ok && lane < r) ? rec[2 + lane] : 0.f;
+      va1[u] = (ok && lane + 32 < r) ? rec[2 + lane + 32] : 0.f;
+#pragma unroll
+      for (int c = 0; c < CPL / 2; ++c) ve[u][c] = ok ? *reinterpret_cast<const float2*>(rec + 2 + r + lane * CPL + 2 * c) : make_float2(0.f, 0.f);
     }
-    const int nc = min(32, nw - i0);
-    for (int k0 = 0; k0 < nc; k0 += 8) {              // explicit batches of 8 partials: all loads issued before any use
-      float w[8], va0[8], va1[8];
-      float2 ve[8][CPL / 2];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        const int k = k0 + u;
-        w[u] = __shfl_sync(kFull, wk, k & 31);          // lanes >= nc hold weight 0
-        const float* rec = part + (size_t)(ws + S * (i0 + min(k, nc - 1))) * stride + 2;
-        va0[u] = (lane < r) ? rec[lane] : 0.f;
-        va1[u] = (lane + 32 < r) ? rec[lane + 32] : 0.f;
+    for (int u = 0; u < 8; ++u) {
+      const float wu = (ml0[u] == -INFINITY) ? 0.f : ex2(ml0[u] - mstar);
+      lsum = fmaf(wu, ml1[u], lsum);
+      a0 = fmaf(wu, va0[u], a0);
+      a1 = fmaf(wu, va1[u], a1);
 #pragma unroll
-        for (int c = 0; c < CPL / 2; ++c) ve[u][c] = *reinterpret_cast<const float2*>(rec + r + lane * CPL + 2 * c);   // 8-byte aligned
-      }
-#pragma unroll
-      for (int u = 0; u < 8; ++u) {
-        const float wu = (k0 + u < nc) ? w[u] : 0.f;
-        a0 = fmaf(wu, va0[u], a0);
-        a1 = fmaf(wu, va1[u], a1);
-#pragma unroll
-        for (int c = 0; c < CPL / 2; ++c) { e[2 * c] = fmaf(wu, ve[u][c].x, e[2 * c]); e[2 * c + 1] = fmaf(wu, ve[u][c].y, e[2 * c + 1]); }
-      }
+      for (int c = 0; c < CPL / 2; ++c) { e[2 * c] = fmaf(wu, ve[u][c].x, e[2 * c]); e[2 * c + 1] = fmaf(wu, ve[u][c].y, e[2 * c + 1]); }
     }
   }
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) lsum += __shfl_xor_sync(kFull, lsum, o);
-  float lstar = lsum;
+  float lstar = lsum;                                // (every lane accumulated every partial of the warp: no lane reduction needed)
   if constexpr (SPLIT) {
     if (lane == 0) sh_l[warp] = lsum;
     sh_a[warp][lane] = a0; sh_a[warp][lane + 32] = a1;
@@ -110,36 +140,40 @@ __global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Co
       for (int c = 0; c < CPL; ++c) e[c] += sh_e[w][lane * CPL + c];
     }
   }
-  // back-projection o = (gV * (BV^T a*) + e*) / l*: basis rows as coalesced loads, a*_j broadcast by shuffle
-  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
-  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
+  // back-projection o = (gV * (BV^T a*) + e*) / l*: basis rows already in registers, a*_j broadcast by shuffle
   float acc[CPL];
 #pragma unroll
   for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
-#pragma unroll 8
-  for (int j = 0; j < r; ++j) {
-    const float aj = __shfl_sync(kFull, j < 32 ? a0 : a1, j & 31);
-    if constexpr (CPL == 4) {
-      const uint2 bw = __ldg(reinterpret_cast<const uint2*>(BV + (size_t)j * D));
-      acc[0] = fmaf(aj, __uint_as_float(bw.x << 16), acc[0]); acc[1] = fmaf(aj, __uint_as_float(bw.x & 0xffff0000u), acc[1]);
-      acc[2] = fmaf(aj, __uint_as_float(bw.y << 16), acc[2]); acc[3] = fmaf(aj, __uint_as_float(bw.y & 0xffff0000u), acc[3]);
-    } else {
-      const uint32_t bw = __ldg(reinterpret_cast<const uint32_t*>(BV + (size_t)j * D));
-      acc[0] = fmaf(aj, __uint_as_float(bw << 16), acc[0]); acc[1] = fmaf(aj, __uint_as_float(bw & 0xffff0000u), acc[1]);
+#pragma unroll
+  for (int j = 0; j < 32; ++j) {
+    const float aj = __shfl_sync(kFull, a0, j);
+    acc[0] = fmaf(aj, __uint_as_float(bw[j].x << 16), acc[0]); acc[1] = fmaf(aj, __uint_as_float(bw[j].x & 0xffff0000u), acc[1]);
+    if constexpr (CPL == 4) { acc[2] = fmaf(aj, __uint_as_float(bw[j].y << 16), acc[2]); acc[3] = fmaf(aj, __uint_as_float(bw[j].y & 0xffff0000u), acc[3]); }
+  }
+  if (r > 32) {                                      // basis ranks 48 / 64: the second half of the rows
+    uint2 bw2[32];
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      if constexpr (CPL == 4) bw2[j] = (32 + j < r) ? __ldg(reinterpret_cast<const uint2*>(BV + (size_t)(32 + j) * D)) : make_uint2(0u, 0u);
+      else bw2[j] = make_uint2((32 + j < r) ? __ldg(reinterpret_cast<const uint32_t*>(BV + (size_t)(32 + j) * D)) : 0u, 0u);
+    }
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const float aj = __shfl_sync(kFull, a1, j);
+      acc[0] = fmaf(aj, __uint_as_float(bw2[j].x << 16), acc[0]); acc[1] = fmaf(aj, __uint_as_float(bw2[j].x & 0xffff0000u), acc[1]);
+      if constexpr (CPL == 4) { acc[2] = fmaf(aj, __uint_as_float(bw2[j].y << 16), acc[2]); acc[3] = fmaf(aj, __uint_as_float(bw2[j].y & 0xffff0000u), acc[3]); }
     }
   }
   const float inv = 1.f / lstar;
   float* out = p.out + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * G) + (size_t)h * G + gq) * D + lane * CPL;
   if constexpr (CPL == 4) {
-    const uint2 gw = __ldg(reinterpret_cast<const uint2*>(gVp));
     float4 o;
     o.x = (__uint_as_float(gw.x << 16) * acc[0] + e[0]) * inv; o.y = (__uint_as_float(gw.x & 0xffff0000u) * acc[1] + e[1]) * inv;
     o.z = (__uint_as_float(gw.y << 16) * acc[2] + e[2]) * inv; o.w = (__uint_as_float(gw.y & 0xffff0000u) * acc[3] + e[3]) * inv;
     *reinterpret_cast<float4*>(out) = o;
   } else {
-    const uint32_t gw = __ldg(reinterpret_cast<const uint32_t*>(gVp));
     float2 o;
-    o.x = (__uint_as_float(gw << 16) * acc[0] + e[0]) * inv; o.y = (__uint_as_float(gw & 0xffff0000u) * acc[1] + e[1]) * inv;
+    o.x = (__uint_as_float(gw.x << 16) * acc[0] + e[0]) * inv; o.y = (__uint_as_float(gw.x & 0xffff0000u) * acc[1] + e[1]) * inv;
     *reinterpret_cast<float2*>(out) = o;
   }
   }   // heads of this warp

@@ -17,8 +17,6 @@
 // V-code byte and scale is owned by exactly one (token, lane), so no atomics are needed (pages are zeroed when allocated).
 #include <algorithm>
 
-#include <cuda.h>
-
 #include "dwkv_internal.h"
 #include "dwkv_mma.cuh"
 
@@ -481,455 +479,7 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
   }
 }
 
-// =====================================================================================================================================
-// tcgen05 variant (d = 128): the projection and the reconstruction as UMMA tiles of 128 tokens, accumulators in TMEM.
-//   tile   = 128 consecutive rows of the call (no sorting: a thread of the epilogue owns one token row = one TMEM lane)
-//   MMA 1  : acc[128 x N1] = X[128 x 128] . B1^T, B1 = the three bf16 terms of B' = B / g as separate output columns, ordered
-//            [chunk b][term][8 columns] so that one chunk's lo / mid / hi partial sums are three 8-column TMEM loads; N1 = 3r (to 16)
-//   epi 1  : c = bf16((lo + mid) + hi), tier mask, fragment-native coefficient stores; the rows of FLAGGED tokens join a batch:
-//            coefficients into the A operand of MMA 2, token row and destination into side buffers. The batch (<= 128 rows, gathered
-//            over the tiles of one (layer, head, Z) run) is flushed when the run ends or the next tile's flagged rows would not fit
-//   MMA 2  : rec[p x 128] = c[p x 64] . B2^T, B2 = the transposed basis padded to 64 ranks
-//   epi 2  : thread p < batch rows: e = x - g * rec, int4 quantiser A14, code / scale stores (one thread per row: batching over
-//            tiles is what keeps all 128 threads busy -- a single tile has only a handful of flagged rows)
-// Warps 0-3: epilogue (and the per-(layer, head) staging of B1 / B2); warp 4 lane 0: TMA producer (two 64-channel halves of 128
-// token rows per (tile, Z), hardware 128-byte swizzle); warp 5 lane 0: MMA issuer. mbarrier rings: x_full / x_empty (token
-// stages), acc_full / acc_empty (two accumulators), a2_ready / rec_full (second product), basis_ready (operands of a new (l, h)).
-constexpr int kCuS = 3;                               // token stages of 32 KB
-constexpr int kCuXBytes = 32768;
-constexpr int kCuAccCols = 192;                       // columns reserved per projection accumulator (N1 <= 192)
-
-__device__ __forceinline__ void cu_mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void cu_mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void cu_mbar_wait(uint32_t bar, uint32_t parity) {
-  // bounded (about 10 s with the back-off): a protocol error traps instead of hanging the GPU
-  for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
-    uint32_t ok;
-    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    if (ok) return;
-    if (spin > 4096) __nanosleep(128);
-  }
-  __trap();
-}
-__device__ __forceinline__ uint64_t cu_desc(uint32_t saddr) {     // K-major, SWIZZLE_128B, 8-row groups 1024 bytes apart, version 1
-  return (uint64_t)((saddr >> 4) & 0x3fff) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
-}
-__device__ __forceinline__ void cu_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t acc) {
-  asm volatile("{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p; }"
-               ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(acc) : "memory");
-}
-__device__ __forceinline__ void cu_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void cu_tma_3d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1, int c2) {
-  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-               ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
-}
-__device__ __forceinline__ void cu_tmem_ld8(uint32_t taddr, float (&v)[8]) {
-  uint32_t r[8];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr));
-#pragma unroll
-  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
-}
-constexpr int kCuEpiGroups = 2;                       // epilogue warpgroups (each 4 warps = the 4 TMEM lane quadrants)
-constexpr int kCuEpi = 128 * kCuEpiGroups, kCuThreads = kCuEpi + 64;
-__device__ __forceinline__ void cu_bar_epi() { asm volatile("bar.sync 1, %0;" ::"n"(kCuEpi) : "memory"); }      // the epilogue threads
-
-// the steps of a CTA: its (layer-head, tile) items [item0, item1), per layer-head first all tiles for K, then all for V
-struct CuIter {
-  int n_tiles, left, lh, z, tile, ta, tb;
-  __device__ CuIter(int item0, int item1, int nt) : n_tiles(nt), left(item1 - item0), lh(item0 / nt), z(0) {
-    ta = item0 - lh * nt; tb = min(nt, ta + left); tile = ta;
-  }
-  __device__ bool last_of_run() const { return tile == tb - 1; }
-  __device__ void next() {
-    if (++tile < tb) return;
-    if (z == 0) { z = 1; tile = ta; return; }
-    left -= tb - ta; ++lh; z = 0; ta = 0; tb = min(n_tiles, left); tile = 0;
-  }
-};
-
-struct CuParams {
-  const uint8_t* arena;
-  const TokDst* dst;            // row order of the call's chunk (unsorted): row i of the chunk = global row row0 + i
-  const __nv_bfloat16 *BK, *BV, *gK, *gV, *k_new, *v_new;
-  int n_rows;                   // rows of this chunk
-  int row0;                     // first global row of the chunk in k_new / v_new
-  int N1;                       // 3 r rounded up to 16
-  uint32_t ranks4;
-  CacheGeom g;
-};
-
-__global__ void __launch_bounds__(kCuThreads, 1) compress_umma_kernel(const __grid_constant__ CUtensorMap mapK, const __grid_constant__ CUtensorMap mapV,
-                                                               const CuParams p) {
-  constexpr int D = 128;
-  extern __shared__ __align__(1024) uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t bars[2 * kCuS + 8];
-  __shared__ uint32_t tmem_base_sh;
-  __shared__ int nflag_sh[2], wcount_sh[8];
-  const CacheGeom& g = p.g;
-  const int r = g.r, N1 = p.N1, LH = g.L * g.H, NC = r / 8;
-  const uint32_t sm = ((uint32_t)__cvta_generic_to_shared(smem_raw) + 1023u) & ~1023u;
-  // shared-memory map (all 1024-aligned): token stages | B1[z][atom] | B2[z] | A2 | gate[z][128] floats | flagged-row list
-  const uint32_t xs0 = sm, b1_0 = xs0 + kCuS * kCuXBytes, b1_atom = (uint32_t)N1 * 128, b2_0 = b1_0 + 4 * b1_atom, a2 = b2_0 + 2 * 16384,
-                 gam = a2 + 16384, flist = gam + 1024;
-  const uint32_t bar0 = (uint32_t)__cvta_generic_to_shared(bars);
-  // a2_ready is a pair (step parity): the epilogue can post two steps before the MMA thread has looked at the first, and a waiter
-  // may lag an mbarrier by one phase only
-  const uint32_t x_full = bar0, x_empty = bar0 + 8 * kCuS, acc_full = bar0 + 16 * kCuS, acc_empty = acc_full + 16, a2_ready = acc_empty + 16,
-                 rec_full = a2_ready + 16, basis_ready = rec_full + 8;
-  const int tid_all = threadIdx.x, lane = tid_all & 31, warp = tid_all >> 5;
-  const int tid = tid_all & 127, grp_e = tid_all >> 7;       // epilogue: row / TMEM lane of the thread, and its warpgroup (splits chunks)
-  const int n_tiles = (p.n_rows + 127) >> 7;
-  const long long items = (long long)LH * n_tiles;
-  const int item0 = (int)(items * blockIdx.x / gridDim.x), item1 = (int)(items * (blockIdx.x + 1) / gridDim.x);
-  const int n_idx = 2 * (item1 - item0);                     // (item, Z) steps of this CTA
-  if (tid_all == 0) {
-    for (int i = 0; i < 2 * kCuS + 8; ++i) cu_mbar_init(bar0 + 8 * i, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&mapK) : "memory");
-    asm volatile("prefetch.tensormap [%0];" ::"l"(&mapV) : "memory");
-  }
-  if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((uint32_t)__cvta_generic_to_shared(&tmem_base_sh)) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  }
-  for (int i = tid_all; i < 3 * 16384 / 16; i += kCuThreads)            // B2 (both Z) and A2: the ranks >= r stay zero for the whole kernel
-    asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(b2_0 + 16 * i), "r"(0u) : "memory");
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
-  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-  const uint32_t tmem = tmem_base_sh;
-  const uint32_t idesc1 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N1 >> 3) << 17) | ((128u >> 4) << 24);      // both operands K-major
-  const uint32_t idesc2 = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
-  if (warp == 4 * kCuEpiGroups) {
-    // ===== TMA producer =========================================================================================================
-    if (lane == 0) {
-      CuIter it(item0, item1, n_tiles);
-      for (int idx = 0; idx < n_idx; ++idx, it.next()) {
-        const int s = idx % kCuS;
-        if (idx >= kCuS) cu_mbar_wait(x_empty + 8 * s, (uint32_t)(((idx / kCuS) - 1) & 1));
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(x_full + 8 * s), "r"((uint32_t)kCuXBytes) : "memory");
-        const CUtensorMap* map = it.z ? &mapV : &mapK;
-        cu_tma_3d(xs0 + s * kCuXBytes, map, x_full + 8 * s, 0, it.lh, p.row0 + 128 * it.tile);
-        cu_tma_3d(xs0 + s * kCuXBytes + 16384, map, x_full + 8 * s, 64, it.lh, p.row0 + 128 * it.tile);
-      }
-    }
-  } else if (warp == 4 * kCuEpiGroups + 1) {
-    // ===== MMA issuer ===========================================================================================================
-    if (lane == 0) {
-      int n_seg = 0, cur_lh = -1;
-      CuIter it(item0, item1, n_tiles);          // the step MMA 1 is issued for next
-      auto mma1 = [&](int idx) {
-        const int s = idx % kCuS, buf = idx & 1;
-        if (it.lh != cur_lh) { cu_mbar_wait(basis_ready, (uint32_t)(n_seg & 1)); ++n_seg; cur_lh = it.lh; }
-        cu_mbar_wait(x_full + 8 * s, (uint32_t)((idx / kCuS) & 1));
-        if (idx >= 2) cu_mbar_wait(acc_empty + 8 * buf, (uint32_t)(((idx >> 1) - 1) & 1));
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t xs = xs0 + s * kCuXBytes, b1 = b1_0 + (uint32_t)(2 * it.z) * b1_atom;
-#pragma unroll
-        for (int k = 0; k < 8; ++k)       // channels 16k .. 16k+15: atom k / 4, 32 bytes per step inside the swizzled 128-byte rows
-          cu_mma(tmem + buf * kCuAccCols, cu_desc(xs + (k >> 2) * 16384 + 32 * (k & 3)), cu_desc(b1 + (k >> 2) * b1_atom + 32 * (k & 3)), idesc1, k > 0);
-        cu_commit(acc_full + 8 * buf);
-        cu_commit(x_empty + 8 * s);           // the token stage is free as soon as these products have read it
-        it.next();
-      };
-      int z_cur = 0;
-      if (n_idx > 0) { z_cur = it.z; mma1(0); }
-      for (int idx = 0; idx < n_idx; ++idx) {
-        const int z_this = z_cur;
-        const bool more = idx + 1 < n_idx, same_lh = more && it.lh == cur_lh;
-        if (same_lh) { z_cur = it.z; mma1(idx + 1); }      // run ahead into the other accumulator while the epilogue of idx works
-        cu_mbar_wait(a2_ready + 8 * (idx & 1), (uint32_t)((idx >> 1) & 1));
-        if (nflag_sh[idx & 1] > 0) {                       // the epilogue flushes its batch of flagged rows: rec = c . B2^T
-          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-          const uint32_t b2 = b2_0 + (uint32_t)z_this * 16384;
-#pragma unroll
-          for (int k = 0; k < 4; ++k) cu_mma(tmem + 2 * kCuAccCols, cu_desc(a2 + 32 * k), cu_desc(b2 + 32 * k), idesc2, k > 0);
-          cu_commit(rec_full);
-        }
-        if (!same_lh && more) { z_cur = it.z; mma1(idx + 1); }     // a new (layer, head): staged only after idx is finished
-      }
-    }
-  } else {
-    // ===== epilogue warps (128 threads = TMEM lanes) ============================================================================
-    const uint32_t rows_sh = flist + 256;                       // RowDst (16 bytes) of the batch of flagged rows
-    int cur_lh = -1, n_rec = 0, nb = 0;                         // nb = flagged rows waiting in the batch (CTA-uniform)
-    const int wq = warp & 3;                                    // TMEM lane quadrant of this warp
-    const uint32_t lane_taddr = (uint32_t)(32 * wq) << 16;
-    CuIter it(item0, item1, n_tiles);
-    // destination of my row in the current and in the next step (the table read of the next step is off the critical path)
-    RowDst rd = row_dst(p.arena, p.ranks4, D, p.dst, 128 * it.tile + tid, p.n_rows, it.lh);
-    for (int idx = 0; idx < n_idx; ++idx) {
-      const int z = it.z, lh = it.lh, tile_cur = it.tile, buf = idx & 1;
-      const bool last_of_run = it.last_of_run();
-      it.next();
-      // the table row of the next step: the load is issued here, its first use is at the end of this step
-      const bool more = idx + 1 < n_idx, vn = more && 128 * it.tile + tid < p.n_rows;
-      const TokDst tdn = p.dst[vn ? 128 * it.tile + tid : 0];
-      const int lh_next = it.lh;
-      if (lh != cur_lh) {
-        // ---- operands of this (layer, head): B1 = three-term split of B / g in [chunk][term][8] row order, B2 = B^T, gates ------
-        const int l = lh / g.H, h = lh - l * g.H;
-        for (int zz = 0; zz < 2; ++zz) {
-          const __nv_bfloat16* B = (zz ? p.BV : p.BK) + ((size_t)(l / g.w) * g.H + h) * (size_t)r * D;
-          const __nv_bfloat16* gz = (zz ? p.gV : p.gK) + (size_t)lh * D;
-          const uint32_t b1 = b1_0 + (uint32_t)(2 * zz) * b1_atom, b2 = b2_0 + (uint32_t)zz * 16384;
-          for (int i0 = tid_all; i0 < r * 64; i0 += kCuEpi * 8) {       // 8 (rank, channel pair) items per thread with all loads issued first
-            uint32_t bwv[8], gwv[8];
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-              const int i = i0 + kCuEpi * u, j = i >> 6, ch = (i & 63) * 2;
-              const bool ok = i < r * 64;
-              bwv[u] = ok ? __ldg(reinterpret_cast<const uint32_t*>(B + (size_t)j * D + ch)) : 0u;
-              gwv[u] = ok ? __ldg(reinterpret_cast<const uint32_t*>(gz + ch)) : 0x3f803f80u;
-            }
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-              const int i = i0 + kCuEpi * u, j = i >> 6, ch = (i & 63) * 2;
-              if (i >= r * 64) break;
-              const uint32_t bw = bwv[u];
-              const float2 bb = bf2(bw), gg = bf2(gwv[u]);
-              uint32_t t3[3];
-              split3(__fdiv_rn(bb.x, gg.x), __fdiv_rn(bb.y, gg.y), t3[0], t3[1], t3[2]);
-              const uint32_t col = (uint32_t)(ch >> 6) * b1_atom + (uint32_t)(ch & 7) * 2, chunk = (uint32_t)(ch & 63) >> 3;
-#pragma unroll
-              for (int term = 0; term < 3; ++term) {
-                const uint32_t nrow = (uint32_t)(j >> 3) * 24 + 8 * term + (j & 7);
-                asm volatile("st.shared.u32 [%0], %1;" ::"r"(b1 + col + nrow * 128 + ((chunk ^ (nrow & 7)) << 4)), "r"(t3[term]) : "memory");
-              }
-              // B2[ch][j] = B[j][ch]
-              asm volatile("st.shared.u16 [%0], %1;" ::"r"(b2 + (uint32_t)ch * 128 + ((((uint32_t)j >> 3) ^ (ch & 7)) << 4) + (j & 7) * 2), "h"((uint16_t)(bw & 0xffff)) : "memory");
-              asm volatile("st.shared.u16 [%0], %1;" ::"r"(b2 + (uint32_t)(ch + 1) * 128 + ((((uint32_t)j >> 3) ^ ((ch + 1) & 7)) << 4) + (j & 7) * 2), "h"((uint16_t)(bw >> 16)) : "memory");
-            }
-          }
-          for (int i = tid_all; i < (N1 - 3 * r) * 16; i += kCuEpi) {     // padding rows 3r .. N1-1 of both atoms
-            const uint32_t nrow = 3 * r + (i >> 4) % (N1 - 3 * r), c16 = i & 15;
-            asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(b1 + (c16 >> 3) * b1_atom + nrow * 128 + ((c16 & 7) << 4)), "r"(0u) : "memory");
-          }
-          for (int i = tid_all; i < D; i += kCuEpi) {
-            const float gv = __bfloat162float(gz[i]);
-            asm volatile("st.shared.f32 [%0], %1;" ::"r"(gam + (uint32_t)(zz * 128 + i) * 4), "f"(gv) : "memory");
-          }
-        }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        cu_bar_epi();
-        if (tid_all == 0) cu_mbar_arrive(basis_ready);
-        cur_lh = lh;
-      }
-      // ---- positions of this tile's flagged rows in the batch, and the flagged count of the next tile ---------------------------
-      const unsigned bal = __ballot_sync(kFull, rd.flagged());
-      if (lane == 0 && grp_e == 0) wcount_sh[wq] = __popc(bal);
-      cu_bar_epi();
-      int pre = 0, n_flag = 0;
-#pragma unroll
-      for (int ww = 0; ww < 4; ++ww) { const int cnt = wcount_sh[ww]; pre += ww < wq ? cnt : 0; n_flag += cnt; }
-      const int my_p = nb + pre + __popc(bal & ((1u << lane) - 1u));      // nb + n_flag <= 128 by the flush rule below
-      // ---- epilogue 1: coefficients ---------------------------------------------------------------------------------------------
-      cu_mbar_wait(acc_full + 8 * buf, (uint32_t)((idx >> 1) & 1));
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      {
-        const uint32_t taddr = tmem + buf * kCuAccCols + lane_taddr;
-        const bool valid = rd.valid(), fl = rd.flagged();
-        const int rk = rd.rk(), slot = rd.slot(), tb = rd.tb();
-        uint8_t* base = rd.blk + (z ? rd.coef_bytes() : 0);
-#pragma unroll 1
-        for (int b = grp_e; b < NC; b += kCuEpiGroups) {       // the warpgroups split the rank chunks
-          float hi[8], mid[8], lo[8];
-          cu_tmem_ld8(taddr + 24 * b, hi);
-          cu_tmem_ld8(taddr + 24 * b + 8, mid);
-          cu_tmem_ld8(taddr + 24 * b + 16, lo);
-          asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-          const bool keep = valid && 8 * b < rk;
-          uint32_t wv[4];
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-            wv[k] = keep ? pack_bf16x2((lo[2 * k] + mid[2 * k]) + hi[2 * k], (lo[2 * k + 1] + mid[2 * k + 1]) + hi[2 * k + 1]) : 0u;
-          if (keep) {
-            if (z == 0) {
-#pragma unroll
-              for (int k = 0; k < 4; ++k) *reinterpret_cast<uint32_t*>(base + kcoef_elem_off(slot, 8 * b + 2 * k, tb)) = wv[k];
-            } else {
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                *reinterpret_cast<uint16_t*>(base + vcoef_elem_off(slot, 8 * b + 2 * k, tb)) = (uint16_t)(wv[k] & 0xffff);
-                *reinterpret_cast<uint16_t*>(base + vcoef_elem_off(slot, 8 * b + 2 * k + 1, tb)) = (uint16_t)(wv[k] >> 16);
-              }
-            }
-          }
-          if (fl)
-            asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a2 + (uint32_t)my_p * 128 + (((uint32_t)b ^ (my_p & 7)) << 4)),
-                         "r"(wv[0]), "r"(wv[1]), "r"(wv[2]), "r"(wv[3]) : "memory");
-        }
-        if (fl && grp_e == 0)        // a flagged row joins the batch: its destination and its row index in k_new / v_new (re-read from L2 at the flush)
-          asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(rows_sh + 16 * my_p), "r"((uint32_t)(uintptr_t)rd.blk),
-                       "r"((uint32_t)((uintptr_t)rd.blk >> 32)), "r"((uint32_t)rd.meta), "r"((uint32_t)(p.row0 + 128 * tile_cur + tid)) : "memory");
-      }
-      nb += n_flag;
-      {   // flagged rows of the next tile (first use of the table row loaded at the top of the step)
-        const unsigned baln = __ballot_sync(kFull, vn && tdn.ridx >= 0);
-        if (lane == 0 && grp_e == 0) wcount_sh[4 + wq] = __popc(baln);
-      }
-      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      cu_bar_epi();
-      // flush the batch through MMA 2 when the (layer, head, Z) run ends or the next tile's flagged rows would not fit
-      const int n_flag_next = wcount_sh[4] + wcount_sh[5] + wcount_sh[6] + wcount_sh[7];
-      const int flush = (nb > 0 && (last_of_run || nb + n_flag_next > 128)) ? nb : 0;
-      if (tid_all == 0) {
-        cu_mbar_arrive(acc_empty + 8 * buf);
-        nflag_sh[idx & 1] = flush;
-        cu_mbar_arrive(a2_ready + 8 * (idx & 1));
-      }
-      // ---- epilogue 2: residuals of the batch (thread p owns batch row p; its rec is in TMEM lane p) ------------------------------
-      if (flush > 0) {
-        cu_mbar_wait(rec_full, (uint32_t)(n_rec & 1));
-        ++n_rec;
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        if (32 * wq < flush) {                                   // warp-uniform: this warp's lanes hold batch rows
-          const bool act = tid < flush;
-          RowDst rq = rd;
-          if (act) {
-            uint32_t b0, b1w, mt, sr;
-            asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(b0), "=r"(b1w), "=r"(mt), "=r"(sr) : "r"(rows_sh + 16 * tid));
-            rq.blk = reinterpret_cast<uint8_t*>((uintptr_t)b0 | ((uintptr_t)b1w << 32)); rq.meta = (int)mt; rq.src = (int)sr;
-          }
-          const uint4* xg = reinterpret_cast<const uint4*>((z ? p.v_new : p.k_new) + ((size_t)(act ? rq.src : 0) * LH + lh) * D);
-          const uint32_t taddr = tmem + 2 * kCuAccCols + lane_taddr;
-          const int slot = rq.slot(), sj = slot >> 3, sg = slot & 7;
-          uint8_t* res = rq.blk + 2 * rq.coef_bytes();            // [K code | K scale | V code | V scale], sub-block of 16 slots
-          uint4 xn[4];
-#pragma unroll
-          for (int c = 0; c < 4; ++c) xn[c] = __ldg(xg + 4 * grp_e + c);
-#pragma unroll 1
-          for (int gp = grp_e; gp < D / 32; gp += kCuEpiGroups) {  // pairs of 16-channel groups (split over the warpgroups): channels 32 gp .. + 31
-            uint4 xc[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) { xc[c] = xn[c]; xn[c] = __ldg(xg + 4 * min(gp + kCuEpiGroups, D / 32 - 1) + c); }     // next pair's row chunks in flight
-            float rec[32];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) cu_tmem_ld8(taddr + 32 * gp + 8 * c, *reinterpret_cast<float(*)[8]>(rec + 8 * c));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-            if (act) {
-              int code[32];
-              __half sc[2];
-#pragma unroll
-              for (int gg = 0; gg < 2; ++gg) {
-                float e[16];
-                float amax = 0.f;
-#pragma unroll
-                for (int c = 0; c < 2; ++c) {                      // two 8-channel chunks of the group
-                  const int ch0 = 32 * gp + 16 * gg + 8 * c;
-                  uint4 xv, g0, g1;
-                  xv = xc[2 * gg + c];
-                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g0.x), "=r"(g0.y), "=r"(g0.z), "=r"(g0.w) : "r"(gam + (uint32_t)(z * 128 + ch0) * 4));
-                  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(g1.x), "=r"(g1.y), "=r"(g1.z), "=r"(g1.w) : "r"(gam + (uint32_t)(z * 128 + ch0 + 4) * 4));
-                  const uint32_t xw[4] = {xv.x, xv.y, xv.z, xv.w};
-                  const float gm[8] = {__uint_as_float(g0.x), __uint_as_float(g0.y), __uint_as_float(g0.z), __uint_as_float(g0.w),
-                                       __uint_as_float(g1.x), __uint_as_float(g1.y), __uint_as_float(g1.z), __uint_as_float(g1.w)};
-#pragma unroll
-                  for (int k = 0; k < 4; ++k) {
-                    const float2 xx = bf2(xw[k]);
-                    e[8 * c + 2 * k] = fmaf(-gm[2 * k], rec[16 * gg + 8 * c + 2 * k], xx.x);
-                    e[8 * c + 2 * k + 1] = fmaf(-gm[2 * k + 1], rec[16 * gg + 8 * c + 2 * k + 1], xx.y);
-                    amax = fmaxf(amax, fmaxf(fabsf(e[8 * c + 2 * k]), fabsf(e[8 * c + 2 * k + 1])));
-                  }
-                }
-                sc[gg] = quant_scale(amax);
-                const float sf = __half2float(sc[gg]);
-#pragma unroll
-                for (int i = 0; i < 16; ++i) code[16 * gg + i] = (quant_code(e[i], sf) + 8) & 15;     // offset binary
-              }
-              if (z == 0) {
-                // K codes: word (slot, t) of group pair gp holds, for gg, b, hi: channel 32gp + 16gg + 8b + 2t + hi at bit 4(2gg + b) + 16hi
-#pragma unroll
-                for (int t = 0; t < 4; ++t) {
-                  uint32_t wd = 0u;
-#pragma unroll
-                  for (int gg = 0; gg < 2; ++gg)
-#pragma unroll
-                    for (int b = 0; b < 2; ++b)
-#pragma unroll
-                      for (int hi = 0; hi < 2; ++hi) wd |= (uint32_t)code[16 * gg + 8 * b + 2 * t + hi] << (4 * (2 * gg + b) + 16 * hi);
-                  *reinterpret_cast<uint32_t*>(res + sj * 4 * D + (4 * sg + t) * (D / 8) + 4 * gp) = wd;
-                }
-#pragma unroll
-                for (int gg = 0; gg < 2; ++gg) *reinterpret_cast<__half*>(res + 8 * D + scale_elem_off(slot, 2 * gp + gg, D)) = sc[gg];
-              } else {
-                // V codes: byte (2 * hi + tile) of word (4 * gch + ts) * (D / 4) + 4 * grp holds channels gch (low nibble) and gch + 8
-                const int ts = sg >> 1, hs = sg & 1;
-#pragma unroll
-                for (int gg = 0; gg < 2; ++gg) {
-                  uint8_t* cv = res + 10 * D + 4 * (2 * gp + gg) + 2 * hs + sj;
-#pragma unroll
-                  for (int gch = 0; gch < 8; ++gch) cv[(4 * gch + ts) * (D / 4)] = (uint8_t)(code[16 * gg + gch] | (code[16 * gg + 8 + gch] << 4));
-                  *reinterpret_cast<__half*>(res + 18 * D + scale_elem_off(slot, 2 * gp + gg, D)) = sc[gg];
-                }
-              }
-            }
-          }
-        }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        cu_bar_epi();                                               // the batch buffers and the rec columns are free again
-        nb = 0;
-      }
-      if (more) rd = row_dst_from(p.arena, p.ranks4, D, tdn, vn, lh_next);
-    }
-  }
-  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-  __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem) : "memory");
-}
-
-typedef CUresult (*CuEncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
-                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-bool cu_make_row_map(CUtensorMap* m, const void* base, uint64_t LH, uint64_t rows) {     // dims (128 channels, LH, rows), box (64, 1, 128)
-  static CuEncodeTiledFn fn = [] {
-    void* q = nullptr;
-    cudaDriverEntryPointQueryResult st;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &q, cudaEnableDefault, &st) != cudaSuccess || st != cudaDriverEntryPointSuccess) q = nullptr;
-    return (CuEncodeTiledFn)q;
-  }();
-  if (!fn) return false;
-  const cuuint64_t dims[3] = {128, LH, rows}, strides[2] = {256, LH * 256};
-  const cuuint32_t box[3] = {64, 1, 128}, es[3] = {1, 1, 1};
-  return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 }  // namespace
-
-bool compress_umma_supported(const CacheGeom& g, const void* k_new, const void* v_new) {
-  return g.d == 128 && g.r <= 48 && ((((uintptr_t)k_new | (uintptr_t)v_new) & 15) == 0);
-}
-
-// rows [row0, row0 + n_rows) of k_new / v_new (total_rows rows in all), dst = their destinations in row order (not sorted)
-int launch_compress_umma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n_rows, int row0, long long total_rows,
-                         const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
-                         const __nv_bfloat16* gK, const __nv_bfloat16* gV, int n_sms, cudaStream_t s) {
-  if (n_rows <= 0) return 0;
-  CUtensorMap mapK, mapV;
-  const uint64_t LH = (uint64_t)g.L * g.H;
-  if (!cu_make_row_map(&mapK, k_new, LH, (uint64_t)total_rows) || !cu_make_row_map(&mapV, v_new, LH, (uint64_t)total_rows)) return 0;
-  CuParams p;
-  p.arena = arena; p.dst = dst; p.BK = BK; p.BV = BV; p.gK = gK; p.gV = gV; p.k_new = k_new; p.v_new = v_new; p.n_rows = n_rows; p.row0 = row0;
-  p.N1 = (3 * g.r + 15) / 16 * 16;
-  p.ranks4 = (uint32_t)g.tier_rank[0] | ((uint32_t)g.tier_rank[1] << 8) | ((uint32_t)g.tier_rank[2] << 16) | ((uint32_t)g.tier_rank[3] << 24);
-  p.g = g;
-  const size_t smem = 1024 + (size_t)kCuS * kCuXBytes + (size_t)4 * p.N1 * 128 + 2 * 16384 + 16384 + 1024 + 256 + 2048;
-  const long long items = (long long)LH * ((n_rows + 127) / 128);
-  const int grid = (int)std::max<long long>(1, std::min<long long>(n_sms, items));
-  cudaFuncSetAttribute(compress_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  compress_umma_kernel<<<grid, kCuThreads, smem, s>>>(mapK, mapV, p);
-  return 1;
-}
 
 int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n, const CompressRuns& runs, const __nv_bfloat16* k_new,
                         const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK,

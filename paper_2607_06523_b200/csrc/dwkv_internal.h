@@ -99,11 +99,6 @@ int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* 
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new,
                     const __nv_bfloat16* BK, const __nv_bfloat16* BV, const __nv_bfloat16* gK, const __nv_bfloat16* gV,
                     int n_sms, cudaStream_t s);
-// tcgen05 / TMEM / TMA variant of append/compress (d = 128, basis rank <= 64): rows are taken in call order, dst is NOT sorted
-bool compress_umma_supported(const CacheGeom& g, const void* k_new, const void* v_new);
-int launch_compress_umma(const uint8_t* arena, const CacheGeom& g, const TokDst* dst, int n_rows, int row0, long long total_rows,
-                         const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
-                         const __nv_bfloat16* gK, const __nv_bfloat16* gV, int n_sms, cudaStream_t s);
 // basis construction (dwkv_basis.cu): sketch GEMM + one-sided Jacobi; returns the number of kernels launched (0 = no instance)
 size_t basis_scratch_bytes(const CacheGeom& g, int n_sketch, int n_split);
 int basis_num_splits(const CacheGeom& g, int n, int n_sms);

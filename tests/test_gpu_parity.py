@@ -340,9 +340,8 @@ def test_kernel_instances_small_shapes(mod, d, G, ranks):
     cache.destroy()
 
 
-@pytest.mark.parametrize("umma", [0, 1])
 @pytest.mark.parametrize("shape", ["8b", "70b", "odd", "8b_all_layers", "r64"])
-def test_append_compress_tensor_core_tiles(mod, shape, umma):
+def test_append_compress_tensor_core_tiles(mod, shape):
     """dwkv_append_compress on the shapes of the big configs: d = 128 with three tiers (8B: r = 32, 70B: r = 48, G = 8) and a basis of
     rank 24 (odd number of 8-column chunks, d = 64); token counts that are not multiples of the 16-token tile, several
     sequences per call, a second call that continues the slots. Same bars as the tiny append test (reading A15 iii)."""
@@ -358,10 +357,7 @@ def test_append_compress_tensor_core_tiles(mod, shape, umma):
     else:
         wl = dataclasses.replace(gen.WORKLOADS["tiny"], tier_ranks=(8, 24), T=(64, 64, 64))
     calls = ([700, 333, 64], [1, 30, 0]) if shape == "8b_all_layers" else ([37, 5, 64], [1, 30, 0])
-    if umma and wl.d != 128:
-        pytest.skip("the tcgen05 append/compress kernel is instantiated for d = 128")
     cache, consts = harness.make_cache(wl, n_seqs=3, max_tokens=1024)
-    cache.set_option("compress_umma", umma)      # 1: TMA + tcgen05 + TMEM kernel, 0: mma.sync kernel
     BK, BV, gK, gV = consts
     oc = orc.OracleCache(wl.L, wl.w, wl.H_kv, wl.G, wl.d, wl.tier_ranks, f64(BK), f64(BV), f64(gK), f64(gV))
     rng = np.random.default_rng(11)
