@@ -387,7 +387,7 @@ def test_append_compress_tensor_core_tiles(mod, shape):
             # reading A15 (iii): one bf16 ulp of the oracle's value, or -- for dot products that cancel to almost nothing --
             # the fp32 accumulation error of a d-term dot product, 2^-20 of the token's largest coefficient
             ulp = np.maximum(np.abs(want) * 2.0 ** -7, np.abs(want).max(axis=-1, keepdims=True) * 2.0 ** -20)
-            assert np.all(np.abs(got - want) <= ulp) and np.mean(got != want) < 5e-3
+            assert np.all(np.abs(got - want) <= ulp) and np.mean(got != want) < 1e-3      # measured: <= 3.3e-4 (typically 1e-4)
             gc = dump["code" + z].cpu().numpy()
             lo = (gc & 15).astype(np.int8); hi = (gc >> 4).astype(np.int8)
             lo = np.where(lo > 7, lo - 16, lo); hi = np.where(hi > 7, hi - 16, hi)
@@ -398,7 +398,9 @@ def test_append_compress_tensor_core_tiles(mod, shape):
             # reconstructions must agree to within one quantisation step; everywhere else the scales are identical or adjacent fp16 values
             same = np.all(got == want, axis=-1)                                   # [T, L, H]
             rows = same & fl[:, None, None]                                       # flagged rows with identical coefficients
-            assert diff[rows].max(initial=0) <= 1 and (not rows.any() or np.mean(diff[rows] != 0) <= 2e-3)
+            assert diff[rows].max(initial=0) <= 1 and (not rows.any() or np.mean(diff[rows] != 0) <= 1e-3)      # S:§8c A15 (iii): 0.1 %; measured <= 3e-6
+            print(f"A15(iii) {shape} seq {s_} {z}: coefficients differing from the fp64 oracle {np.mean(got != want):.2e}, "
+                  f"codes differing (rows with equal coefficients) {np.mean(diff[rows] != 0) if rows.any() else 0.0:.2e}")
             gsf = dump["scale" + z].cpu().numpy(); wsf = S["scale" + z]
             gs = gsf.view(np.uint16).astype(np.int32); ws = wsf.view(np.uint16).astype(np.int32)
             assert np.abs(gs - ws)[same].max() <= 1 and np.mean((gs != ws)[same]) <= 5e-3
