@@ -99,7 +99,8 @@ int dwkv_set_gates(dwkv_cache* c, const void* gK, const void* gV, void* stream);
  * (tier, flag); slot = number of earlier tokens of the sequence in that class.
  *   seq_ids, n_new : host int32 [n_seqs]      k_new, v_new : dev bf16 [sum(n_new), L, H_kv, d], sequences in call order
  *   tier, flag     : host uint8 [sum(n_new)]  (tier index 0..n_tiers-1, residual flag 0/1)
- * Errors: INVALID, STATE (basis/gates not set), CAPACITY (state is unchanged when CAPACITY is returned). */
+ * Errors: INVALID, STATE (basis/gates not set), CAPACITY (state is unchanged when INVALID / STATE / CAPACITY is returned), CUDA (a CUDA
+ * call failed after the routing was committed: the handle is then poisoned, every later append / decode returns STATE; destroy it). */
 int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, const int32_t* n_new,
                          const void* k_new, const void* v_new, const uint8_t* tier, const uint8_t* flag, void* stream);
 

@@ -170,11 +170,25 @@ struct dwkv_cache {
   int64_t scan_samples = 0;              // decode kernels timed since "time_scan" was last set
   bool app_timed = false;
   int64_t launches = 0;
+  // set when a CUDA call failed AFTER the host had committed the routing of an append (slots, pages, counts): the host index and
+  // the pages may then disagree, so every later append / decode / probe call refuses with DWKV_E_STATE until the handle is destroyed
+  bool poisoned = false;
 };
 
 namespace {
 
 int check_seq(const dwkv_cache* c, int32_t s) { return (s >= 0 && s < c->cfg.max_seqs) ? 0 : -1; }
+
+// armed once an append has committed host state; a return before disarm() (a failed upload, memset or launch) poisons the handle
+struct PoisonGuard {
+  dwkv_cache* c;
+  bool armed = false;
+  explicit PoisonGuard(dwkv_cache* cache) : c(cache) {}
+  ~PoisonGuard() { if (armed) c->poisoned = true; }
+  void arm() { armed = true; }
+  void disarm() { armed = false; }
+};
+const char* kPoisonMsg = "an earlier append failed after its routing was committed: the cache is inconsistent, destroy the handle";
 
 int64_t pages_in_use(const dwkv_cache* c) { return c->n_pages - (int64_t)c->free_pages.size(); }
 
@@ -437,6 +451,8 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
                          const void* v_new, const uint8_t* tier, const uint8_t* flag, void* stream) {
   if (!c || n_seqs < 0 || (n_seqs > 0 && (!seq_ids || !n_new))) return fail(DWKV_E_INVALID, "NULL argument");
   if (!c->basis_set || !c->gates_set) return fail(DWKV_E_STATE, "basis and gates must be set before append");
+  if (c->poisoned) return fail(DWKV_E_STATE, kPoisonMsg);
+  PoisonGuard guard(c);
   int64_t total = 0, need = 0;
   if (c->seq_stamp.size() != (size_t)c->cfg.max_seqs) c->seq_stamp.assign(c->cfg.max_seqs, 0u);
   if (++c->stamp_gen == 0) { std::fill(c->seq_stamp.begin(), c->seq_stamp.end(), 0u); c->stamp_gen = 1; }
@@ -471,6 +487,7 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
       const int64_t lo = std::max(off, g0), hi = std::min(off + n_new[i], g1);
       if (lo < hi) {
         const size_t first = dst.size();
+        guard.arm();
         route_commit(c, seq_ids[i], (int32_t)(hi - lo), tier + lo, flag + lo, &ridx, &dst, &new_pages);
         for (size_t k = first; k < dst.size(); ++k) dst[k].src = (int32_t)(lo + (int64_t)(k - first));
       }
@@ -508,6 +525,7 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
   }
   if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_app1, st)); c->app_timed = true; }
   CU_OK(cudaGetLastError());
+  guard.disarm();
   return DWKV_OK;
 }
 
@@ -516,6 +534,7 @@ int dwkv_append_raw(dwkv_cache* c, int32_t seq_id, int32_t n, const uint8_t* tie
   if (!c || n < 0) return fail(DWKV_E_INVALID, "NULL cache or negative n");
   if (check_seq(c, seq_id)) return fail(DWKV_E_INVALID, "bad sequence id");
   if (!c->basis_set || !c->gates_set) return fail(DWKV_E_STATE, "basis and gates must be set before append");
+  if (c->poisoned) return fail(DWKV_E_STATE, kPoisonMsg);
   if (n == 0) return DWKV_OK;
   if (!tier || !flag || !data || !data->coefK || !data->coefV) return fail(DWKV_E_INVALID, "NULL argument");
   int64_t need = 0;
@@ -534,6 +553,8 @@ int dwkv_append_raw(dwkv_cache* c, int32_t seq_id, int32_t n, const uint8_t* tie
   dst.reserve(n);
   std::vector<int32_t> new_pages;
   int ridx = 0;
+  PoisonGuard guard(c);
+  guard.arm();
   route_commit(c, seq_id, n, tier, flag, &ridx, &dst, &new_pages);
   rc = zero_new_pages(c, new_pages, st);
   if (rc) return rc;
@@ -545,6 +566,7 @@ int dwkv_append_raw(dwkv_cache* c, int32_t seq_id, int32_t n, const uint8_t* tie
                                     modeA ? data->residV : nullptr, modeA ? nullptr : data->codeK, modeA ? nullptr : data->codeV,
                                     modeA ? nullptr : (const __half*)data->scaleK, modeA ? nullptr : (const __half*)data->scaleV, st);
   CU_OK(cudaGetLastError());
+  guard.disarm();
   return DWKV_OK;
 }
 
@@ -998,6 +1020,7 @@ extern "C" int dwkv_decode_attention(dwkv_cache* c, int32_t layer, int32_t n_seq
   if (!c || !seq_ids || !q || !out || n_seqs <= 0) return fail(DWKV_E_INVALID, "NULL argument or n_seqs <= 0");
   if (layer < -1 || layer >= c->geom.L) return fail(DWKV_E_INVALID, "layer out of range");
   if (!c->basis_set || !c->gates_set) return fail(DWKV_E_STATE, "basis and gates must be set before decode");
+  if (c->poisoned) return fail(DWKV_E_STATE, kPoisonMsg);
   if (n_seqs > 32767) return fail(DWKV_E_INVALID, "too many sequences in one call");
   if (c->seq_stamp.size() != (size_t)c->cfg.max_seqs) c->seq_stamp.assign(c->cfg.max_seqs, 0u);
   if (++c->stamp_gen == 0) { std::fill(c->seq_stamp.begin(), c->seq_stamp.end(), 0u); c->stamp_gen = 1; }

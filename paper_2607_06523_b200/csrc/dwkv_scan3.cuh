@@ -197,8 +197,12 @@ struct QRegs {
   // PAIR: qa[i] = {selA ? hi : 0, selA ? lo : 0, selA ? 0 : hi, selA ? 0 : lo}  (selA = lane's row is a tile-A row)
   // FULL: qa[i] = {hi, lo} of chunk i
   uint32_t qa[NKB][PAIR ? 4 : 2];
-  // raw q (residual-K term), group grp: PAIR {selA ? q0 : 0, selA ? q2 : 0, selA ? 0 : q0, selA ? 0 : q2}; FULL {q0, q2}
-  uint32_t qr[D / 16][PAIR ? 4 : 2];
+  // raw q (residual-K term) as ready-made A-operand quads (a0, a1, a2, a3) = (row g | row g+8) x (channels +0 | +8). Rows g+8 of these
+  // MMAs are "don't care" rows for one of the two products that share a quad, so no register is spent on zeros and none is moved:
+  // PAIR, group grp:      qr[grp]   = {selA ? q0 : 0, selA ? 0 : q0, selA ? q2 : 0, selA ? 0 : q2}: the tile-A product reads rows g,
+  //                                   the tile-B product (same quad, tile B codes) reads rows g+8
+  // FULL, groups 2p, 2p+1: qr[p]    = {q0(2p), q0(2p+1), q2(2p), q2(2p+1)}: group 2p reads rows g, group 2p+1 rows g+8
+  uint32_t qr[PAIR ? D / 16 : D / 32][4];
   float qbias[D / 16];     // -136 * sum_{i in grp} q[head][i]: removes the offset of the biased codes
 };
 

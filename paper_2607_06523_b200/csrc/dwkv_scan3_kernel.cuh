@@ -89,9 +89,9 @@ __device__ __forceinline__ void prologue_compute(QRegs<NKB, D, PAIR>& q, const P
     split_bf16x2(x0.x * g0.x, x0.y * g0.y, af[kk][0], af[kk][1]);
     split_bf16x2(x2.x * g2.x, x2.y * g2.y, af[kk][2], af[kk][3]);
     if constexpr (PAIR) {
-      q.qr[kk][0] = pl.qv[kk][0] & mA; q.qr[kk][1] = pl.qv[kk][1] & mA; q.qr[kk][2] = pl.qv[kk][0] & ~mA; q.qr[kk][3] = pl.qv[kk][1] & ~mA;
+      q.qr[kk][0] = pl.qv[kk][0] & mA; q.qr[kk][1] = pl.qv[kk][0] & ~mA; q.qr[kk][2] = pl.qv[kk][1] & mA; q.qr[kk][3] = pl.qv[kk][1] & ~mA;
     } else {
-      q.qr[kk][0] = pl.qv[kk][0]; q.qr[kk][1] = pl.qv[kk][1];
+      q.qr[kk >> 1][kk & 1] = pl.qv[kk][0]; q.qr[kk >> 1][2 + (kk & 1)] = pl.qv[kk][1];
     }
     float sum = (x0.x + x0.y) + (x2.x + x2.y);
     sum += __shfl_xor_sync(kFull, sum, 1);

@@ -149,14 +149,14 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
 #pragma unroll
       for (int grp = 0; grp < NG; ++grp) {
         const int qq = 2 * grp;
-        float c[4];
-        mma16z(c, q.qr[grp][0], 0u, q.qr[grp][1], 0u, nib_to_bf16x2_biased(wA[qq >> 2], qq & 3),
+        float c1[4], c2[4];     // one A quad for both products: tile A reads rows g (c1[0..1]), tile B rows g+8 (c2[2..3])
+        mma16z(c1, q.qr[grp][0], q.qr[grp][1], q.qr[grp][2], q.qr[grp][3], nib_to_bf16x2_biased(wA[qq >> 2], qq & 3),
                nib_to_bf16x2_biased(wA[qq >> 2], (qq & 3) + 1));
-        mma16(c, q.qr[grp][2], 0u, q.qr[grp][3], 0u, nib_to_bf16x2_biased(wB[qq >> 2], qq & 3),
-              nib_to_bf16x2_biased(wB[qq >> 2], (qq & 3) + 1));
+        mma16z(c2, q.qr[grp][0], q.qr[grp][1], q.qr[grp][2], q.qr[grp][3], nib_to_bf16x2_biased(wB[qq >> 2], qq & 3),
+               nib_to_bf16x2_biased(wB[qq >> 2], (qq & 3) + 1));
         const float2 f = h2f2(sc[grp]);
-        sr0 = fmaf(c[0] + q.qbias[grp], f.x, sr0);      // the -136 * sum(q) offset of the biased codes
-        sr1 = fmaf(c[1] + q.qbias[grp], f.y, sr1);
+        sr0 = fmaf((c1[0] + c2[2]) + q.qbias[grp], f.x, sr0);      // the -136 * sum(q) offset of the biased codes
+        sr1 = fmaf((c1[1] + c2[3]) + q.qbias[grp], f.y, sr1);
       }
       s[0][0] = fmaf(cscale, sr0, s[0][0]);
       s[0][1] = fmaf(cscale, sr1, s[0][1]);
@@ -170,12 +170,12 @@ __device__ __forceinline__ void process_sub(State<NKB, D>& st, const uint32_t sp
 #pragma unroll
         for (int grp = 0; grp < NG; ++grp) {
           const int qq = 2 * grp;
-          float c[4];
-          mma16z(c, q.qr[grp][0], 0u, q.qr[grp][1], 0u, nib_to_bf16x2_biased(w[qq >> 2], qq & 3),
+          float c[4];             // the quad holds groups 2p (rows g) and 2p + 1 (rows g+8): take the rows of this group
+          mma16z(c, q.qr[grp >> 1][0], q.qr[grp >> 1][1], q.qr[grp >> 1][2], q.qr[grp >> 1][3], nib_to_bf16x2_biased(w[qq >> 2], qq & 3),
                  nib_to_bf16x2_biased(w[qq >> 2], (qq & 3) + 1));
           const float2 f = h2f2(sc[grp]);
-          sr0 = fmaf(c[0] + q.qbias[grp], f.x, sr0);
-          sr1 = fmaf(c[1] + q.qbias[grp], f.y, sr1);
+          sr0 = fmaf(c[2 * (grp & 1)] + q.qbias[grp], f.x, sr0);
+          sr1 = fmaf(c[2 * (grp & 1) + 1] + q.qbias[grp], f.y, sr1);
         }
         s[j][0] = fmaf(cscale, sr0, s[j][0]);
         s[j][1] = fmaf(cscale, sr1, s[j][1]);
