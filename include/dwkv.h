@@ -291,6 +291,24 @@ int dwkv_dense_decode_attention(const void* K, const void* V, const void* q, flo
                                 int32_t n_seqs, int32_t n_layers, int32_t n_kv_heads, int32_t n_q_heads, int32_t d_head,
                                 int64_t T, float softmax_scale, void* stream);
 
+/* Allocation-free variant of dwkv_dense_decode_attention for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it): same kernels, same arguments minus `workspace`; the split-T partial records go to
+ * a file-scope device array of DWKV_DENSE_STATIC_SCRATCH_BYTES inside the library (every GPU that loads the library holds it until
+ * the process exits). The call allocates and frees nothing; the first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress, with the caller's current device), so make that first call outside a stream capture.
+ *   K, V, q, out: device pointers, layouts as above (caller-owned).
+ * A call needs n_seqs * n_layers * n_kv_heads * n_splits * G * (2 + d_head) * 4 bytes, n_splits = min(ceil(1776 / (n_seqs * n_layers
+ * * n_kv_heads)), ceil(T / 256)) rounded as dwkv_dense_decode_attention does; e.g. the 8B shape (32 layers, 8 kv heads, G = 4,
+ * d = 128) at batch 8 and any T needs 4.3 MB. A call that needs more returns DWKV_E_INVALID and dwkv_last_error() names both sizes.
+ * All calls on a device share the array and it keeps the last call's contents. Nothing in it has to be cleared (every record a call
+ * reads was written by that call), but two calls that overlap on the GPU (different streams, or graphs replayed concurrently) RACE
+ * on it: serialise them, or use dwkv_dense_decode_attention with one workspace per stream.
+ * Errors: INVALID (NULL, shapes, scratch too small, device ordinal > 63), CUDA. */
+#define DWKV_DENSE_STATIC_SCRATCH_BYTES (16u << 20)
+int dwkv_dense_decode_attention_static(const void* K, const void* V, const void* q, float* out, int32_t n_seqs, int32_t n_layers,
+                                       int32_t n_kv_heads, int32_t n_q_heads, int32_t d_head, int64_t T, float softmax_scale,
+                                       void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,7 +24,7 @@ EXPORTED = [
     "dwkv_launch_count", "dwkv_get_stat", "dwkv_last_error", "dwkv_dense_workspace_bytes", "dwkv_dense_decode_attention",
     "dwkv_build_basis", "dwkv_export_basis", "dwkv_probe_error", "dwkv_route_tokens", "dwkv_router_thresholds",
     "dwkv_probe_token_stats", "dwkv_controller_create", "dwkv_controller_destroy", "dwkv_controller_step", "dwkv_controller_state",
-    "dwkv_controller_thresholds",
+    "dwkv_controller_thresholds", "dwkv_dense_decode_attention_static",
 ]
 
 
@@ -95,6 +95,7 @@ def _load() -> C.CDLL:
     lib.dwkv_dense_workspace_bytes.argtypes = [i32, i32, i32, i32, i64]
     lib.dwkv_dense_workspace_bytes.restype = u64
     lib.dwkv_dense_decode_attention.argtypes = [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, i64, C.c_float, vp]
+    lib.dwkv_dense_decode_attention_static.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, i64, C.c_float, vp]
     for name in EXPORTED:
         getattr(lib, name)
     return lib
@@ -264,6 +265,19 @@ def dense_decode_attention(K: torch.Tensor, V: torch.Tensor, q: torch.Tensor, n_
     _check(lib.dwkv_dense_decode_attention(_ptr(K, torch.bfloat16), _ptr(V, torch.bfloat16), _ptr(q, torch.bfloat16),
                                            _ptr(out, torch.float32), _ptr(workspace), n_seqs, L, H, Hq, d, T,
                                            softmax_scale, _stream()))
+    return out
+
+
+DENSE_STATIC_SCRATCH_BYTES = 16 << 20      # DWKV_DENSE_STATIC_SCRATCH_BYTES of include/dwkv.h
+
+
+def dense_decode_attention_static(K: torch.Tensor, V: torch.Tensor, q: torch.Tensor, n_kv_heads: int, out: torch.Tensor,
+                                  softmax_scale: float = 0.0) -> torch.Tensor:
+    """dwkv_dense_decode_attention_static: the dense kernel with its split partials in the library's static device array; the
+    call allocates nothing (so `out` is the caller's). Calls that overlap on the GPU race on that array."""
+    n_seqs, L, H, T, d = K.shape
+    _check(lib.dwkv_dense_decode_attention_static(_ptr(K, torch.bfloat16), _ptr(V, torch.bfloat16), _ptr(q, torch.bfloat16),
+                                                  _ptr(out, torch.float32), n_seqs, L, H, q.shape[2], d, T, softmax_scale, _stream()))
     return out
 
 

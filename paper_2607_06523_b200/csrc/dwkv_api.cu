@@ -21,6 +21,14 @@ int fail(int code, const std::string& msg) {
   return code;
 }
 
+}  // namespace
+
+namespace dwkv {
+int set_error(int code, const std::string& msg) { return fail(code, msg); }
+}  // namespace dwkv
+
+namespace {
+
 #define CU_OK(call)                                                                             \
   do {                                                                                          \
     cudaError_t e__ = (call);                                                                   \

@@ -2,6 +2,9 @@
 // step a5 (BASELINE.json north_star: "the same figures for a from-scratch dense-bf16-cache decode kernel").
 // Plain softmax attention over K, V [n_seqs, L, H_kv, T, d] bf16 (row-major, no special packing), split-T with a
 // log-sum-exp combine, all G query heads of a kv head share every cache load, mma.sync bf16 contractions.
+#include <mutex>
+#include <string>
+
 #include "dwkv_internal.h"
 #include "../../include/dwkv.h"
 
@@ -228,3 +231,68 @@ extern "C" int dwkv_dense_decode_attention(const void* K, const void* V, const v
   }
   return cudaGetLastError() == cudaSuccess ? DWKV_OK : DWKV_E_CUDA;
 }
+
+// ---- allocation-free variant (include/dwkv.h: dwkv_dense_decode_attention_static) --------------------------------------------
+// The split-T partial records live in a file-scope device array instead of a caller workspace, for callers that cannot allocate
+// (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc). Every GPU that loads the library holds the array until the
+// process exits. In host code `g_dense_static_scratch` is only the host-side stand-in of the symbol, never a device address: the
+// address is resolved once per device with cudaGetSymbolAddress (that device current) and that pointer is what the kernels get.
+namespace dwkv {
+namespace {
+constexpr size_t kDenseStaticBytes = DWKV_DENSE_STATIC_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_dense_static_scratch[kDenseStaticBytes];
+
+constexpr int kMaxDevices = 64;
+std::mutex g_dense_static_mu;
+void* g_dense_static_ptr[kMaxDevices] = {};
+
+// device address of the array on the current device; resolved on the first call per device
+int dense_static_ptr(void** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return set_error(DWKV_E_CUDA, std::string("cudaGetDevice: ") + cudaGetErrorString(e));
+  if (dev < 0 || dev >= kMaxDevices) return set_error(DWKV_E_INVALID, "dwkv_dense_decode_attention_static: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lock(g_dense_static_mu);
+  if (!g_dense_static_ptr[dev]) {
+    void* ptr = nullptr;
+    e = cudaGetSymbolAddress(&ptr, g_dense_static_scratch);
+    if (e != cudaSuccess || !ptr)
+      return set_error(DWKV_E_CUDA, std::string("cudaGetSymbolAddress(g_dense_static_scratch): ") + cudaGetErrorString(e));
+    g_dense_static_ptr[dev] = ptr;
+  }
+  *out = g_dense_static_ptr[dev];
+  return DWKV_OK;
+}
+}  // namespace
+}  // namespace dwkv
+
+extern "C" int dwkv_dense_decode_attention_static(const void* K, const void* V, const void* q, float* out, int32_t n_seqs,
+                                                  int32_t n_layers, int32_t n_kv_heads, int32_t n_q_heads, int32_t d_head,
+                                                  int64_t T, float softmax_scale, void* stream) {
+  using namespace dwkv;
+  if (!K || !V || !q || !out || n_seqs <= 0 || n_layers <= 0 || n_kv_heads <= 0 || n_q_heads <= 0 || T <= 0)
+    return set_error(DWKV_E_INVALID, "dwkv_dense_decode_attention_static: NULL pointer or non-positive size");
+  if (n_q_heads % n_kv_heads != 0 || n_q_heads / n_kv_heads > 8 || (d_head != 64 && d_head != 128))
+    return set_error(DWKV_E_INVALID, "dwkv_dense_decode_attention_static: needs H_q = G * H_kv with G <= 8 and d_head 64 or 128");
+  const int64_t n_lhb = (int64_t)n_seqs * n_layers * n_kv_heads;
+  if (n_lhb > 65535) return set_error(DWKV_E_INVALID, "dwkv_dense_decode_attention_static: n_seqs * n_layers * n_kv_heads > 65535");
+  // the partial records the launch below will write: [n_lhb][n_splits][G][2 + d] fp32, n_splits as dwkv_dense_decode_attention cuts T
+  const int64_t steps = (T + 15) / 16;
+  int64_t n_splits = dense_splits((int)n_lhb, T);
+  const int64_t per = (steps + n_splits - 1) / n_splits;
+  n_splits = (steps + per - 1) / per;
+  const uint64_t need = (uint64_t)n_lhb * (uint64_t)n_splits * (uint64_t)(n_q_heads / n_kv_heads) * (uint64_t)(2 + d_head) * 4ull;
+  if (need > kDenseStaticBytes)
+    return set_error(DWKV_E_INVALID, "dwkv_dense_decode_attention_static: the call needs " + std::to_string(need) +
+                                         " bytes of split partials, the static scratch holds " + std::to_string(kDenseStaticBytes) +
+                                         " (DWKV_DENSE_STATIC_SCRATCH_BYTES); use dwkv_dense_decode_attention with a caller workspace");
+  void* scratch = nullptr;
+  const int rc = dense_static_ptr(&scratch);
+  if (rc) return rc;
+  // nothing in the array has to start at zero: the scan kernel writes every record of this launch in full before the combine
+  // kernel of the same stream reads them, and records of earlier calls beyond this launch's extent are never read
+  const int rc2 = dwkv_dense_decode_attention(K, V, q, out, scratch, n_seqs, n_layers, n_kv_heads, n_q_heads, d_head, T, softmax_scale, stream);
+  if (rc2) return set_error(rc2, "dwkv_dense_decode_attention_static: kernel launch failed");
+  return DWKV_OK;
+}
+

@@ -5,6 +5,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <string>
+
 #include "dwkv_layout.cuh"
 
 namespace dwkv {
@@ -77,6 +79,9 @@ struct CacheGeom {
   int32_t tier_rank[4];
   int32_t i8;         // 8-bit coefficient mode (option "coef_int8"; dwkv_layout.cuh)
 };
+
+// records the message dwkv_last_error() returns (thread-local, dwkv_api.cu) and returns `code`
+int set_error(int code, const std::string& msg);
 
 // kernel launchers (dwkv_combine3.cu, dwkv_cache_ops.cu, dwkv_dense.cu); each returns the number of kernels launched
 int scan3_num_slices(int n_sms);
