@@ -46,12 +46,34 @@ __device__ __forceinline__ void split3(float x, float y, uint32_t& hi, uint32_t&
   lo = pack_bf16x2(rx - __uint_as_float(mid << 16), ry - __uint_as_float(mid & 0xffff0000u));
 }
 
-// Reading A14: fp32 IEEE, round-to-nearest-even, no FMA contraction, no reciprocal.
-__device__ __forceinline__ int quant_code(float e, float sf) {
-  if (sf == 0.f) return 0;
-  float r = rintf(__fdiv_rn(e, sf));
-  r = fminf(fmaxf(r, -7.f), 7.f);
-  return (int)r;
+// Reading A14: fp32 IEEE, round-to-nearest-even, no FMA contraction: code = clamp(rint(RN(e / sf)), -7, 7).
+// The quotient is first formed with the approximate reciprocal of sf (one MUFU.RCP per group, shared by the group's codes):
+// qa = e * rinv differs from the real e / sf by less than 2^-21 relative, and so does the correctly rounded RN(e / sf); for
+// |e / sf| < 8 both therefore lie within 2^-17 of each other, and if qa is further than 2^-16 from every half-integer the two
+// round to the same integer (beyond 7.6 both clamp to 7). Only a code whose qa sits inside that margin (a few per million) takes
+// the IEEE division. The result is bit-identical to the plain form for every input.
+__device__ __forceinline__ float rcp_approx(float x) {
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// (Further than 7.6 from zero both clamp to 7, so the margin test needs no range check: a code that takes the division there
+// ends at the same clamp.) quant_codes4 does the four codes a lane owns of one group, with one branch for the rare case.
+static __device__ __noinline__ float quant_quotient_exact(float e, float sf) { return rintf(__fdiv_rn(e, sf)); }   // one copy, cold
+__device__ __forceinline__ void quant_codes4(const float (&e)[4], float sf, float rinv /* 0 if sf == 0 */, int (&code)[4]) {
+  float r[4], margin = 1.f;
+#pragma unroll
+  for (int x = 0; x < 4; ++x) {
+    const float qa = e[x] * rinv;
+    r[x] = rintf(qa);
+    margin = fminf(margin, 0.5f - fabsf(qa - r[x]));
+  }
+  if (margin < 0x1p-16f) {                 // rare: a quotient next to a rounding boundary
+#pragma unroll
+    for (int x = 0; x < 4; ++x) r[x] = quant_quotient_exact(e[x], sf);
+  }
+#pragma unroll
+  for (int x = 0; x < 4; ++x) code[x] = (int)fminf(fmaxf(r[x] + 8.f, 1.f), 15.f);      // offset binary: clamp(r, -7, 7) + 8
 }
 __device__ __forceinline__ __half quant_scale(float amax) {
   float s32 = __fdiv_rn(amax, 7.0f);
@@ -289,14 +311,26 @@ __device__ __forceinline__ void store_coef(const RowDst& rd, const uint32_t (&cw
 
 // rec = c . B, e = x - g * rec, int4 quantiser (A14), fragment-native code / scale stores: tiles with a flagged token only.
 // x is read from the shared-memory stage in the unpermuted channel order of the reconstruction's n dimension; the loop is kept
-// rolled so the kernel stays inside the instruction cache.
+// rolled so the kernel stays inside the instruction cache. The store positions of a row depend on (z, slot, t) only: they are
+// formed once, as 32-bit offsets from the row's sub-block base, and advance by 4 bytes per group.
 template <int D, int NT>
 __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfloat16* BTz, const int ldT, const __nv_bfloat16* gt,
                                                      const uint32_t stage, const RowDst& ra, const RowDst& rb,
                                                      const uint32_t (&ca)[NT], const uint32_t (&cb)[NT], const int gr, const int t) {
+  // residual planes of a sub-block of 16 slots, behind the two coefficient planes: [K code 8D | K scale 2D | V code 8D | V scale 2D]
+  int code_off[2], scale_off[2];
+#pragma unroll
+  for (int row = 0; row < 2; ++row) {
+    const RowDst& rd = row ? rb : ra;
+    const int sl = rd.slot(), j = sl >> 3, p = sl & 7, res = 2 * rd.coef_bytes();
+    // K: 16-byte code row of (slot, t): word wx at + 4 wx.  V: byte (2 hi + j) of word (4 gch + ts) * (D / 4) + 4 grp, gch = 2t, 2t + 1
+    code_off[row] = z == 0 ? res + j * 4 * D + (4 * p + t) * (D / 8) : res + 10 * D + 2 * (p & 1) + j + (8 * t + (p >> 1)) * (D / 4);
+    scale_off[row] = res + (z == 0 ? 8 * D : 18 * D) + scale_elem_off(sl, 0, D);
+  }
+  const bool fa = ra.flagged(), fb = rb.flagged();
 #pragma unroll 1
   for (int wx = 0; wx < D / 32; ++wx) {     // K code word wx of a row = groups 2wx, 2wx+1 (registers q = 4wx .. 4wx+3)
-    uint32_t kwa = 0u, kwb = 0u;
+    uint32_t kw[2] = {0u, 0u};
 #pragma unroll
     for (int gg = 0; gg < 2; ++gg) {
       const int grp = 2 * wx + gg;
@@ -319,7 +353,6 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
       const float2 g0 = bf2(__ldg(reinterpret_cast<const uint32_t*>(gt + 16 * grp))), g2 = bf2(__ldg(reinterpret_cast<const uint32_t*>(gt + 16 * grp + 8)));
 #pragma unroll
       for (int row = 0; row < 2; ++row) {
-        const RowDst& rd = row ? rb : ra;
         const float2 x0 = bf2(stage_x<D>(stage, gr + 8 * row, 16 * grp + 2 * t));          // rows beyond n_tok were zero-filled
         const float2 x2 = bf2(stage_x<D>(stage, gr + 8 * row, 16 * grp + 8 + 2 * t));
         float e[4];
@@ -328,33 +361,28 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
         float amax = fmaxf(fmaxf(fabsf(e[0]), fabsf(e[1])), fmaxf(fabsf(e[2]), fabsf(e[3])));
         amax = fmaxf(amax, __shfl_xor_sync(kFull, amax, 1));
         amax = fmaxf(amax, __shfl_xor_sync(kFull, amax, 2));
-        if (rd.flagged()) {
+        if (row ? fb : fa) {
+          uint8_t* blk = row ? rb.blk : ra.blk;
           const __half s = quant_scale(amax);
           const float sf = __half2float(s);
+          const float rinv = sf == 0.f ? 0.f : rcp_approx(sf);
           int code[4];
-#pragma unroll
-          for (int x = 0; x < 4; ++x) code[x] = (quant_code(e[x], sf) + 8) & 15;     // offset binary
-          uint8_t* res = rd.blk + 2 * rd.coef_bytes();          // [K code | K scale | V code | V scale], sub-block of 16 slots
-          const int j = rd.slot() >> 3, p = rd.slot() & 7;
+          quant_codes4(e, sf, rinv, code);
           if (z == 0) {
-            const uint32_t bits = ((uint32_t)code[0] << (8 * gg)) | ((uint32_t)code[1] << (16 + 8 * gg)) |
-                                  ((uint32_t)code[2] << (8 * gg + 4)) | ((uint32_t)code[3] << (16 + 8 * gg + 4));
-            if (row) kwb |= bits; else kwa |= bits;
-            if (t == 0) *reinterpret_cast<__half*>(res + 8 * D + scale_elem_off(rd.slot(), grp, D)) = s;
+            kw[row] |= ((uint32_t)code[0] << (8 * gg)) | ((uint32_t)code[1] << (16 + 8 * gg)) |
+                       ((uint32_t)code[2] << (8 * gg + 4)) | ((uint32_t)code[3] << (16 + 8 * gg + 4));
           } else {
-            // V codes: byte (2*hi + tile) of word (4*gch + ts)*(D/4) + 4*grp holds channels gch (low nibble) and gch + 8
-            const int ts = p >> 1, hi = p & 1;
-            uint8_t* cv = res + 10 * D + 4 * grp + 2 * hi + j;
-            cv[(4 * (2 * t) + ts) * (D / 4)] = (uint8_t)(code[0] | (code[2] << 4));
-            cv[(4 * (2 * t + 1) + ts) * (D / 4)] = (uint8_t)(code[1] | (code[3] << 4));
-            if (t == 0) *reinterpret_cast<__half*>(res + 18 * D + scale_elem_off(rd.slot(), grp, D)) = s;
+            uint8_t* cv = blk + code_off[row] + 4 * grp;
+            cv[0] = (uint8_t)(code[0] | (code[2] << 4));
+            cv[D] = (uint8_t)(code[1] | (code[3] << 4));
           }
+          if (t == 0) *reinterpret_cast<__half*>(blk + scale_off[row] + 4 * grp) = s;
         }
       }
     }
     if (z == 0) {
-      if (ra.flagged()) *reinterpret_cast<uint32_t*>(ra.blk + 2 * ra.coef_bytes() + (ra.slot() >> 3) * 4 * D + (4 * (ra.slot() & 7) + t) * (D / 8) + 4 * wx) = kwa;
-      if (rb.flagged()) *reinterpret_cast<uint32_t*>(rb.blk + 2 * rb.coef_bytes() + (rb.slot() >> 3) * 4 * D + (4 * (rb.slot() & 7) + t) * (D / 8) + 4 * wx) = kwb;
+      if (fa) *reinterpret_cast<uint32_t*>(ra.blk + code_off[0] + 4 * wx) = kw[0];
+      if (fb) *reinterpret_cast<uint32_t*>(rb.blk + code_off[1] + 4 * wx) = kw[1];
     }
   }
 }
