@@ -132,10 +132,15 @@ __device__ __forceinline__ void cost_to_item(long long pos, const CompressRuns& 
 }
 
 // ---- per-warp shared-memory ring of token-row stages -------------------------------------------------------------------------
-// A stage holds the 16 token rows of one tile for one Z, row-major with a row pitch of 2 * D + 16 bytes (ldmatrix and 4-byte
-// reads of 8 consecutive rows are then bank-conflict free). Lane (g, t) copies channels 32u + 8t .. +7 of rows g and g + 8 with
-// 16-byte cp.async (zero-filled for rows beyond n_tok); one ldmatrix.x4 per k step returns the A fragment of the projection as
-// an aligned register quad. A stage is complete for the warp after cp.async.wait_group + __syncwarp.
+// A stage holds the 16 token rows of one tile for one Z, row-major with a row pitch of 2 * D bytes and the 16-byte chunks of a
+// row XOR-swizzled: chunk c of row r sits at chunk c ^ f(r), f(r) = ((r & 1) << 2) | ((r >> 1) & 3) (a bijection of r mod 8 whose
+// bit 2 is the row's parity). Lane (g, t) copies channels 32u + 8t .. +7 of rows g and g + 8 with 16-byte cp.async (zero-filled
+// for rows beyond n_tok): a quarter warp writes two neighbouring rows, which the swizzle sends to different 64-byte halves of the
+// banks; ldmatrix (8 rows, one chunk) and the reconstruction's 4-byte reads (8 rows x 4 words of one chunk) see 8 distinct chunk
+// positions: all three patterns are conflict-free (the padded layout this replaces cost 2 - 3 wavefronts per cp.async quarter).
+// One ldmatrix.x4 per k step returns the A fragment of the projection as an aligned register quad. A stage is complete for the
+// warp after cp.async.wait_group + __syncwarp. Stages are 256-byte aligned (the swizzle is applied by XOR on the address).
+__device__ __forceinline__ uint32_t stage_swz(int row) { return (uint32_t)(((row & 1) << 2) | ((row >> 1) & 3)); }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
@@ -156,23 +161,26 @@ __device__ __forceinline__ void ldmatrix_x4(uint32_t a, uint32_t& r0, uint32_t& 
 }
 
 template <int D>
-__device__ __forceinline__ void issue_rows(uint32_t stage, const __nv_bfloat16* X, int2 src, int LH, int lh, int lane) {
-  constexpr int PITCH = 2 * D + 16;
+__device__ __forceinline__ void issue_rows(uint32_t stage, const char* xlh /* X + (lh * D + 8t) elements */, int2 src, uint32_t row_bytes,
+                                           int lane) {
+  constexpr int PITCH = 2 * D;
   const int g = lane >> 2, t = lane & 3;
-  const char* pa = reinterpret_cast<const char*>(X + ((size_t)max(src.x, 0) * LH + lh) * D + 8 * t);
-  const char* pb = reinterpret_cast<const char*>(X + ((size_t)max(src.y, 0) * LH + lh) * D + 8 * t);
+  const char* pa = xlh + (size_t)(uint32_t)max(src.x, 0) * row_bytes;
+  const char* pb = xlh + (size_t)(uint32_t)max(src.y, 0) * row_bytes;
   const int sa = src.x >= 0 ? 16 : 0, sb = src.y >= 0 ? 16 : 0;
-  const uint32_t da = stage + g * PITCH + 16 * t, db = da + 8 * PITCH;
+  const uint32_t da = (stage + g * PITCH) | (16u * ((uint32_t)t ^ stage_swz(g))), db = da + 8 * PITCH;     // f(g + 8) = f(g)
 #pragma unroll
   for (int u = 0; u < D / 32; ++u) {
-    cp_async16(da + 64 * u, pa + 64 * u, sa);
-    cp_async16(db + 64 * u, pb + 64 * u, sb);
+    cp_async16(da ^ (64u * u), pa + 64 * u, sa);
+    cp_async16(db ^ (64u * u), pb + 64 * u, sb);
   }
 }
 
 // bf16 pair (channels ch, ch+1; ch even) of row `row` of a stage
 template <int D>
-__device__ __forceinline__ uint32_t stage_x(uint32_t stage, int row, int ch) { return lds32(stage + row * (2 * D + 16) + ch * 2); }
+__device__ __forceinline__ uint32_t stage_x(uint32_t stage, int row, int ch) {
+  return lds32((stage + row * (2 * D)) | ((((uint32_t)ch >> 3) ^ stage_swz(row)) << 4) | ((ch & 7) * 2));
+}
 
 // C = X . B'^T for one Z: 3 MMAs (lo, mid, hi term of B') per (k step, rank chunk); returns the rounded coefficients of rows g (ca) and g+8 (cb), columns 8nt + 2t, +1, zero beyond the rank
 // 8-bit planes (I8; reading A27): the fp32 coefficients of a row are quantised per 32-column block (exponent from the
@@ -190,11 +198,12 @@ __device__ __forceinline__ void project_n(const uint4* P4, const uint2* P2, int 
 #pragma unroll
     for (int nt = 0; nt < NTM; ++nt) c[a][nt][0] = c[a][nt][1] = c[a][nt][2] = c[a][nt][3] = 0.f;
   // ldmatrix: lanes 8i .. 8i+7 address the rows of matrix i = (rows 0-7 | 8-15) x (channels +0 | +8) of the k step
-  const uint32_t am = stage + ((lane & 7) + 8 * ((lane >> 3) & 1)) * (2 * D + 16) + 16 * (lane >> 4);
+  const int arow = (lane & 7) + 8 * ((lane >> 3) & 1);
+  const uint32_t am = (stage + arow * (2 * D)) | (16u * ((uint32_t)(lane >> 4) ^ stage_swz(arow)));       // chunk 2kk + (lane >> 4), swizzled
 #pragma unroll
   for (int kk = 0; kk < D / 16; ++kk) {
     uint32_t a0, a1, a2, a3;
-    ldmatrix_x4(am + 32 * kk, a0, a1, a2, a3);
+    ldmatrix_x4(am ^ (32u * kk), a0, a1, a2, a3);
 #pragma unroll
     for (int nt = 0; nt < NTM; ++nt) {
       const uint4 hm = P4[(kk * NT + nt) * 32 + lane];
@@ -269,44 +278,64 @@ __device__ __forceinline__ void project(const uint4* P4, const uint2* P2, int la
   else project_n<D, NT, NT, I8>(P4, P2, lane, stage, ra, rb, ca, cb, qa, qb, xa, xb);
 }
 
+// Coefficient stores of one row: the position of (slot, lane) inside the class plane is formed once, the rank chunks follow at a
+// constant stride (kcoef_elem_off / vcoef_elem_off of dwkv_layout.cuh with col = 8 nt + 2t, TB = tiles per sub-block: 2 if the
+// token is flagged, else 4; compile-time so that the chunk offsets are immediates).
 // 8-bit planes: the row's code bytes (two columns per chunk and lane) and, from lane t = 0, the exponent bytes of its blocks
-template <int NT>
-__device__ __forceinline__ void store_coef8(const RowDst& rd, const uint32_t (&q)[NT], const uint32_t xexp, int z, int t) {
-  if (!rd.valid()) return;
-  uint8_t* base = rd.blk + (z ? rd.coef_bytes() : 0);
+template <int NT, int TB>
+__device__ __forceinline__ void store_coef8_tb(const RowDst& rd, const uint32_t (&q)[NT], const uint32_t xexp, int z, int t) {
+  const int sl = rd.slot(), rk = rd.rk();
+  uint8_t* plane = rd.blk + (z ? rd.coef_bytes() : 0);
+  if (z == 0) {
+    uint8_t* p = plane + (4 * (sl & 7) + t) * 2 * TB + (sl >> 3) * 2;
 #pragma unroll
-  for (int nt = 0; nt < NT; ++nt) {
-    if (8 * nt < rd.rk()) {
-      if (z == 0) {
-        *reinterpret_cast<uint16_t*>(base + kcoef8_elem_off(rd.slot(), 8 * nt + 2 * t, rd.tb())) = (uint16_t)q[nt];
-      } else {
-        base[vcoef8_elem_off(rd.slot(), 8 * nt + 2 * t, rd.tb())] = (uint8_t)(q[nt] & 0xff);
-        base[vcoef8_elem_off(rd.slot(), 8 * nt + 2 * t + 1, rd.tb())] = (uint8_t)(q[nt] >> 8);
+    for (int nt = 0; nt < NT; ++nt)
+      if (8 * nt < rk) *reinterpret_cast<uint16_t*>(p + nt * 64 * TB) = (uint16_t)q[nt];
+  } else {
+    uint8_t* p = plane + (8 * t + ((sl & 7) >> 1)) * 2 * TB + (sl >> 3) * 2 + (sl & 1);
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+      if (8 * nt < rk) {
+        p[nt * 64 * TB] = (uint8_t)(q[nt] & 0xff);
+        p[nt * 64 * TB + 8 * TB] = (uint8_t)(q[nt] >> 8);
       }
-    }
   }
   if (t == 0) {
 #pragma unroll
     for (int b = 0; b < (NT + 3) / 4; ++b)
-      if (32 * b < rd.rk()) base[coef8_exp_off(rd.slot(), rd.rk() >> 3, rd.tb(), b)] = (uint8_t)(xexp >> (8 * b));
+      if (32 * b < rk) plane[coef8_exp_off(sl, rk >> 3, TB, b)] = (uint8_t)(xexp >> (8 * b));
   }
 }
+template <int NT>
+__device__ __forceinline__ void store_coef8(const RowDst& rd, const uint32_t (&q)[NT], const uint32_t xexp, int z, int t) {
+  if (!rd.valid()) return;
+  if (rd.flagged()) store_coef8_tb<NT, 2>(rd, q, xexp, z, t);
+  else store_coef8_tb<NT, 4>(rd, q, xexp, z, t);
+}
 
+template <int NT, int TB>
+__device__ __forceinline__ void store_coef_tb(const RowDst& rd, const uint32_t (&cw)[NT], int z, int t) {
+  const int sl = rd.slot(), rk = rd.rk();
+  if (z == 0) {
+    uint8_t* p = rd.blk + (4 * (sl & 7) + t) * 4 * TB + (sl >> 3) * 4;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+      if (8 * nt < rk) *reinterpret_cast<uint32_t*>(p + nt * 128 * TB) = cw[nt];
+  } else {
+    uint8_t* p = rd.blk + rd.coef_bytes() + (8 * t + ((sl & 7) >> 1)) * 4 * TB + (sl >> 3) * 4 + (sl & 1) * 2;
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt)
+      if (8 * nt < rk) {
+        *reinterpret_cast<uint16_t*>(p + nt * 128 * TB) = (uint16_t)(cw[nt] & 0xffff);
+        *reinterpret_cast<uint16_t*>(p + nt * 128 * TB + 16 * TB) = (uint16_t)(cw[nt] >> 16);
+      }
+  }
+}
 template <int NT>
 __device__ __forceinline__ void store_coef(const RowDst& rd, const uint32_t (&cw)[NT], int z, int t) {
   if (!rd.valid()) return;
-  uint8_t* base = rd.blk + (z ? rd.coef_bytes() : 0);
-#pragma unroll
-  for (int nt = 0; nt < NT; ++nt) {
-    if (8 * nt < rd.rk()) {
-      if (z == 0) {
-        *reinterpret_cast<uint32_t*>(base + kcoef_elem_off(rd.slot(), 8 * nt + 2 * t, rd.tb())) = cw[nt];
-      } else {
-        *reinterpret_cast<uint16_t*>(base + vcoef_elem_off(rd.slot(), 8 * nt + 2 * t, rd.tb())) = (uint16_t)(cw[nt] & 0xffff);
-        *reinterpret_cast<uint16_t*>(base + vcoef_elem_off(rd.slot(), 8 * nt + 2 * t + 1, rd.tb())) = (uint16_t)(cw[nt] >> 16);
-      }
-    }
-  }
+  if (rd.flagged()) store_coef_tb<NT, 2>(rd, cw, z, t);
+  else store_coef_tb<NT, 4>(rd, cw, z, t);
 }
 
 // rec = c . B, e = x - g * rec, int4 quantiser (A14), fragment-native code / scale stores: tiles with a flagged token only.
@@ -392,8 +421,8 @@ __global__ void __launch_bounds__(kCompressMaxWarps * 32, 1)
 compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, const int n_tok, const CompressRuns runs, const int n_stages,
                     const __nv_bfloat16* k_new, const __nv_bfloat16* v_new, const __nv_bfloat16* BK, const __nv_bfloat16* BV,
                     const __nv_bfloat16* gK, const __nv_bfloat16* gV) {
-  constexpr int NKK = D / 16, r = 8 * NT, ldT = r + 8, NFRAG = NKK * NT * 32, STAGE = 16 * (2 * D + 16);
-  extern __shared__ __align__(16) uint8_t smem_raw[];
+  constexpr int NKK = D / 16, r = 8 * NT, ldT = r + 8, NFRAG = NKK * NT * 32, STAGE = 16 * (2 * D);
+  extern __shared__ __align__(256) uint8_t smem_raw[];
   uint4* P4 = reinterpret_cast<uint4*>(smem_raw);                        // [2][NFRAG]  (hi.b0, hi.b1, mid.b0, mid.b1) of B'
   uint2* P2 = reinterpret_cast<uint2*>(P4 + 2 * NFRAG);                  // [2][NFRAG]  (lo.b0, lo.b1)
   __nv_bfloat16* BT = reinterpret_cast<__nv_bfloat16*>(P2 + 2 * NFRAG);  // [2][D][ldT] transposed basis (reconstruction B operand)
@@ -416,6 +445,9 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
     const int n = (te - tb - warp + W - 1) / W;                          // tiles of this warp (may be <= 0)
     const int nst = 2 * n;                                               // stages: (tile 0, K), (tile 0, V), (tile 1, K), ...
     int issued = 0, slot_i = 0;
+    const char* xk = reinterpret_cast<const char*>(k_new + (size_t)lh * D + 8 * t);      // row 0 of this (layer, head), this lane's channels
+    const char* xv = reinterpret_cast<const char*>(v_new + (size_t)lh * D + 8 * t);
+    const uint32_t row_bytes = (uint32_t)LH * D * 2;
     int2 src_cur = make_int2(-1, -1), src_nxt = make_int2(-1, -1);       // source rows (-1: beyond n_tok) of the tile being issued / the next
     auto fetch_src = [&](int i) {
       const int tok = 16 * (tb + warp + W * i) + gr;
@@ -423,7 +455,7 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
     };
     auto issue_one = [&]() {
       if (issued < nst) {
-        issue_rows<D>(ring + slot_i * STAGE, (issued & 1) ? v_new : k_new, src_cur, LH, lh, lane);
+        issue_rows<D>(ring + slot_i * STAGE, (issued & 1) ? xv : xk, src_cur, row_bytes, lane);
         if (issued & 1) {
           src_cur = src_nxt;
           const int ni = (issued >> 1) + 2;
@@ -485,10 +517,16 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
         ra = na; rb = nb;
         any_flag = __any_sync(kFull, ra.flagged() || rb.flagged());
         ntmax = __reduce_max_sync(kFull, max(ra.valid() ? ra.rk() : 0, rb.valid() ? rb.rk() : 0)) >> 3;
-      } else if (s + 1 < nst) {
-        const int tile = tb + warp + W * ((s + 1) >> 1);
-        na = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr, n_tok, lh, I8);
-        nb = row_dst(arena, ranks4, g.d, dst, 16 * tile + gr + 8, n_tok, lh, I8);
+      }
+      // table entries of the next tile: requested here, turned into destinations after this stage's arithmetic (the conversion is
+      // a chain of dependent integer operations: placed right behind the loads it was the kernel's largest single stall)
+      TokDst tda, tdb;
+      bool va = false, vb = false;
+      const bool fetch_next = z == 1 && s + 1 < nst;
+      if (fetch_next) {
+        const int tok = 16 * (tb + warp + W * ((s + 1) >> 1)) + gr;
+        va = tok < n_tok; vb = tok + 8 < n_tok;
+        tda = dst[va ? tok : 0]; tdb = dst[vb ? tok + 8 : 0];
       }
       uint32_t ca[NT], cb[NT], qa[NT], qb[NT], xa = 0u, xb = 0u;
       project<D, NT, I8>(P4 + z * NFRAG, P2 + z * NFRAG, lane, stage, ra, rb, ntmax, ca, cb, qa, qb, xa, xb);
@@ -501,6 +539,10 @@ compress_mma_kernel(const uint8_t* arena, const CacheGeom g, const TokDst* dst, 
       }
       if (any_flag)
         reconstruct_quantise<D, NT>(z, BT + z * D * ldT, ldT, (z ? gV : gK) + (size_t)lh * D + 2 * t, stage, ra, rb, ca, cb, gr, t);
+      if (fetch_next) {
+        na = row_dst_from(arena, ranks4, g.d, tda, va, lh, I8);
+        nb = row_dst_from(arena, ranks4, g.d, tdb, vb, lh, I8);
+      }
       slot_c = slot_c + 1 == n_stages ? 0 : slot_c + 1;
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");                 // only empty groups are left
@@ -514,7 +556,7 @@ int launch_compress_mma(const uint8_t* arena, const CacheGeom& g, const TokDst* 
                         const __nv_bfloat16* gV, int n_sms, cudaStream_t s) {
   if (n <= 0) return 0;
   const int nfrag = (g.d / 16) * (g.r / 8) * 32;
-  const size_t fixed = (size_t)2 * nfrag * 24 + (size_t)2 * g.d * (g.r + 8) * 2, stage = (size_t)16 * (2 * g.d + 16);
+  const size_t fixed = (size_t)2 * nfrag * 24 + (size_t)2 * g.d * (g.r + 8) * 2, stage = (size_t)16 * (2 * g.d);
   const size_t cap = 227 * 1024;
   // warps per CTA and ring stages per warp: 16 warps (the kernel is latency-bound: 4 warps per scheduler) if they can have 2
   // stages each, else 8 warps
