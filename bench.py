@@ -122,7 +122,7 @@ def time_steps(fn, steps, warmup):
 def prefill_compress(wl, harness, local, reps=3):
     """Batched (prefill-sized) dwkv_append_compress: all tokens of one sequence of the workload's length (capped at 64K) in ONE
     call on a cache of its own -- the TTFT side of the method (PAPER.md:74 'during prefill ... projects keys and values into
-    shared coefficient space, stores quantized residuals'). Returns ms per call (host routing + page zeroing + kernel, the
+    shared coefficient space, stores quantized residuals'). Returns ms per call (host routing + kernel, the
     GPU idle at the start) and the dense bytes read."""
     import dataclasses
     n = min(max(wl.T), 65536)
@@ -162,7 +162,7 @@ def prefill_compress(wl, harness, local, reps=3):
     best = min(ms[1:])
     return {"tokens": n, "ms_per_call": best, "dense_bytes_read": dense_bytes, "dense_GBps": dense_bytes / best / 1e6,
             "tokens_per_s": n / best * 1e3, "build_basis_ms": min(bms[1:]), "build_basis_sketch_rows": n_sketch,
-            "build_basis_dense_GBps": 2 * k_new[:n8].numel() * 2 / min(bms[1:]) / 1e6, "note": "one dwkv_append_compress call, timed from an idle GPU: host routing + page zeroing + kernel"}
+            "build_basis_dense_GBps": 2 * k_new[:n8].numel() * 2 / min(bms[1:]) / 1e6, "note": "one dwkv_append_compress call, timed from an idle GPU: host routing + table upload + kernels (free pages are kept cleared: nothing is zeroed in the call)"}
 
 
 def reconstruct_dense(cache, wl, consts, seq, K_out, V_out, chunk=2048):

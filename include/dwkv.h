@@ -58,7 +58,7 @@ typedef struct {
   int64_t max_tokens_per_seq;        /* capacity per sequence                                                  */
   float softmax_scale;               /* 0 => 1/sqrt(d_head)  (reading A9)                                      */
   int32_t device;                    /* CUDA device ordinal                                                    */
-  void* arena;                       /* optional caller-owned device memory for the cache pages (256-B aligned) */
+  void* arena;                       /* optional caller-owned device memory for the cache pages (256-B aligned; cleared by dwkv_create) */
   uint64_t arena_bytes;              /* size of `arena`; if arena == NULL: bytes to cudaMalloc (0 => worst case) */
 } dwkv_config;
 
@@ -153,7 +153,8 @@ typedef struct {
 
 int dwkv_export_tokens(dwkv_cache* c, int32_t seq_id, int64_t t0, int64_t n, const dwkv_token_dump* out, void* stream);
 
-/* Drop all tokens of a sequence and return its pages to the pool. */
+/* Drop all tokens of a sequence and return its pages to the pool (cleared: free pages are always all zero, so appends never
+ * clear memory; the whole arena, caller-owned or not, is cleared once by dwkv_create). Synchronises the device. */
 int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id);
 
 /* Attention-output probe, Eq. (3) (reading A25): for one sequence and

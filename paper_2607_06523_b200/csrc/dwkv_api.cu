@@ -295,7 +295,10 @@ void stored_token_table(const dwkv_cache* c, const SeqState& S, int64_t t0, int6
   }
 }
 
-int zero_new_pages(dwkv_cache* c, const std::vector<int32_t>& pages, cudaStream_t st) {
+// Invariant: every page in `free_pages` is all zero (the kernels rely on unused slots of a page being zero). The arena is cleared
+// once at dwkv_create and a page is cleared again when dwkv_reset_seq returns it to the pool, so the append path never clears
+// anything (a prefill-sized call used to spend ~0.3 ms on 1 GB of cudaMemsetAsync, a configs[4] step several 16 MB ones).
+int zero_pages(dwkv_cache* c, const std::vector<int32_t>& pages, cudaStream_t st) {
   for (int32_t pg : pages) CU_OK(cudaMemsetAsync(c->arena + (size_t)pg * c->page_bytes, 0, c->page_bytes, st));
   return DWKV_OK;
 }
@@ -361,6 +364,11 @@ int dwkv_create(const dwkv_config* cfg, dwkv_cache** out) {
   if (c->n_pages < 1) { if (c->own_arena) cudaFree(c->arena); delete c; return fail(DWKV_E_INVALID, "arena smaller than one page"); }
   c->free_pages.resize(c->n_pages);
   for (int64_t i = 0; i < c->n_pages; ++i) c->free_pages[i] = (int32_t)(c->n_pages - 1 - i);   // pop -> ascending ids
+  {   // free pages are all zero (see zero_pages): clear the arena once, here
+    cudaError_t ez = cudaMemset(c->arena, 0, (size_t)c->n_pages * c->page_bytes);
+    if (ez == cudaSuccess) ez = cudaDeviceSynchronize();
+    if (ez != cudaSuccess) { dwkv_destroy(c); return fail(DWKV_E_CUDA, std::string("cudaMemset(arena): ") + cudaGetErrorString(ez)); }
+  }
 
   const size_t nb = (size_t)(f.n_layers / f.group_size) * f.n_kv_heads * c->geom.r * f.d_head * sizeof(__nv_bfloat16);
   const size_t ng = (size_t)f.n_layers * f.n_kv_heads * f.d_head * sizeof(__nv_bfloat16);
@@ -520,9 +528,7 @@ int dwkv_append_compress(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, 
       runs.count[runs.n - 1]++;
       runs.per_lh += cost;
     }
-    int rc = zero_new_pages(c, new_pages, st);
-    if (rc) return rc;
-    rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
+    int rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
     if (rc) return rc;
     if (c->opt_time_scan && g0 == 0) {       // "compress_ms": from the first kernel of the call to the end of the last
       if (!c->ev_app0) { CU_OK(cudaEventCreate(&c->ev_app0)); CU_OK(cudaEventCreate(&c->ev_app1)); }
@@ -564,8 +570,6 @@ int dwkv_append_raw(dwkv_cache* c, int32_t seq_id, int32_t n, const uint8_t* tie
   PoisonGuard guard(c);
   guard.arm();
   route_commit(c, seq_id, n, tier, flag, &ridx, &dst, &new_pages);
-  rc = zero_new_pages(c, new_pages, st);
-  if (rc) return rc;
   rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
   if (rc) return rc;
   const bool modeA = data->residK && data->residV;
@@ -610,10 +614,16 @@ int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id) {
   cudaDeviceSynchronize();     // pages may still be read by kernels in flight
   SeqState& S = c->seqs[seq_id];
   c->total_tokens -= (int64_t)S.tier.size();
+  std::vector<int32_t> returned;
   for (int k = 0; k < kMaxClasses; ++k) {
-    for (auto it = S.pages[k].rbegin(); it != S.pages[k].rend(); ++it) c->free_pages.push_back(*it);
+    for (auto it = S.pages[k].rbegin(); it != S.pages[k].rend(); ++it) { c->free_pages.push_back(*it); returned.push_back(*it); }
     S.pages[k].clear();
     S.count[k] = 0;
+  }
+  if (!returned.empty()) {     // pages go back to the pool cleared; nothing may be in flight on them, before or after
+    int rc = zero_pages(c, returned, 0);
+    if (rc) { c->poisoned = true; return rc; }
+    CU_OK(cudaDeviceSynchronize());
   }
   S.tier.clear(); S.flag.clear(); S.slot.clear();
   c->version++;

@@ -14,7 +14,7 @@
 // Every warp streams its token rows through a private shared-memory ring filled by cp.async 2-4 stages ahead (a stage = the 16
 // rows of one tile and one Z) and reads the A fragments back with ldmatrix. Results go straight
 // to their fragment-native positions in the class pages (dwkv_layout.cuh): every 32-bit coefficient word, 16-byte K-code row,
-// V-code byte and scale is owned by exactly one (token, lane), so no atomics are needed (pages are zeroed when allocated).
+// V-code byte and scale is owned by exactly one (token, lane), so no atomics are needed (free pages are always all zero: dwkv_api.cu, zero_pages).
 #include <algorithm>
 
 #include "dwkv_internal.h"
