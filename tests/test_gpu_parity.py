@@ -493,6 +493,31 @@ def test_dense_bf16_kernel_against_oracle_softmax(mod):
                 check_output(out[s, l], ref, float(np.abs(Vn[s, l]).max()), f"dense {(n_seq, L, H, G, d, T)}")
 
 
+def test_reset_returns_cleared_pages(mod):
+    """Free pages are always all zero (dwkv_api.cu, zero_pages): a sequence of fat records (every token top tier + flagged, two
+    pages) is dropped and a shorter sequence of another class mix is appended; the free list is a stack, so it gets the same two
+    pages first, and its ragged page tails would hold the old bytes if they had not been cleared. Decode against the oracle."""
+    binding, harness = mod
+    wl_a = dataclasses.replace(gen.WORKLOADS["tiny"], T=(600,), patterns=("all_top_flag",))      # 448 tokens of that class per page
+    tier_a, flag_a = gen.make_routing(wl_a, 0)
+    page = wl_a.L * wl_a.H_kv * harness.PAGE_LH_BYTES
+    cache, consts = harness.make_cache(wl_a, n_seqs=1, max_tokens=1024, arena_bytes=2 * len(wl_a.tier_ranks) * page)   # one page per class
+    for rep, T in enumerate((77, 33)):
+        harness.fill_sequence(cache, wl_a, 0, 0, tier_a, flag_a, chunk=128)
+        assert cache.footprint()["reserved_bytes"] == 2 * page
+        cache.reset_seq(0)
+        assert cache.seq_len(0) == 0 and cache.footprint()["reserved_bytes"] == 0
+        wl_b = dataclasses.replace(gen.WORKLOADS["tiny"], T=(T,), patterns=("",))
+        rt_b = [gen.make_routing(wl_b, 0)]
+        kept = [harness.fill_sequence(cache, wl_b, 0, 0, *rt_b[0], chunk=64, keep=all_lh(wl_b))]
+        assert cache.footprint()["reserved_bytes"] >= 2 * page            # the two returned pages are in use again
+        q = gen.make_q(wl_b, step=rep, device="cuda")
+        out = cache.decode_attention(-1, [0], q)
+        compare(wl_b, cache, consts, kept, rt_b, q, out, what=f"after reset, T = {T}")
+        cache.reset_seq(0)
+    cache.destroy()
+
+
 @pytest.mark.parametrize("name", ["tiny", "8b"])
 def test_probe_error_eq3(mod, name):
     """dwkv_probe_error (Eq. 3, reading A25): the compressed cache against a higher-fidelity dense cache of the same tokens
