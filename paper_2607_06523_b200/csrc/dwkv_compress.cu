@@ -46,34 +46,38 @@ __device__ __forceinline__ void split3(float x, float y, uint32_t& hi, uint32_t&
   lo = pack_bf16x2(rx - __uint_as_float(mid << 16), ry - __uint_as_float(mid & 0xffff0000u));
 }
 
-// Reading A14: fp32 IEEE, round-to-nearest-even, no FMA contraction: code = clamp(rint(RN(e / sf)), -7, 7).
-// The quotient is first formed with the approximate reciprocal of sf (one MUFU.RCP per group, shared by the group's codes):
-// qa = e * rinv differs from the real e / sf by less than 2^-21 relative, and so does the correctly rounded RN(e / sf); for
-// |e / sf| < 8 both therefore lie within 2^-17 of each other, and if qa is further than 2^-16 from every half-integer the two
-// round to the same integer (beyond 7.6 both clamp to 7). Only a code whose qa sits inside that margin (a few per million) takes
-// the IEEE division. The result is bit-identical to the plain form for every input.
+// Reading A14: fp32 IEEE, round-to-nearest-even, no FMA contraction: code = clamp(rint(RN(e / sf)), -7, 7), stored as code + 8.
+// Fast path, for a scale that is a normal fp16 number below the fp16 maximum (then |e / sf| <= 7 (1 + 2^-24) / (1 - 2^-11) < 7.004
+// for every element of the group and the clamp can never act): ONE approximate reciprocal per group and per code
+//     s8 = fma(e, rinv, 8)      r8 = rint(s8)      code + 8 = (int) r8
+// s8 differs from e / sf + 8 by less than 2^-19 (reciprocal: 2^-22 relative of a value below 8) + 2^-21 (one rounding in [8, 16)),
+// and RN(e / sf) differs from e / sf by at most 2^-21; so if s8 is further than 2^-16 from every half-integer, r8 - 8 is the
+// correctly rounded quotient's integer. Only a group with a code inside that margin (a few per 10^5), or with a subnormal / saturated
+// scale, takes the IEEE divisions (one cold non-inlined copy). The result is bit-identical to the plain form for every input.
 __device__ __forceinline__ float rcp_approx(float x) {
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-// (Further than 7.6 from zero both clamp to 7, so the margin test needs no range check: a code that takes the division there
-// ends at the same clamp.) quant_codes4 does the four codes a lane owns of one group, with one branch for the rare case.
-static __device__ __noinline__ float quant_quotient_exact(float e, float sf) { return rintf(__fdiv_rn(e, sf)); }   // one copy, cold
-__device__ __forceinline__ void quant_codes4(const float (&e)[4], float sf, float rinv /* 0 if sf == 0 */, int (&code)[4]) {
-  float r[4], margin = 1.f;
+static __device__ __noinline__ float quant_code_exact(float e, float sf) {      // cold: clamp(rint(RN(e / sf)), -7, 7) + 8
+  return fminf(fmaxf(rintf(__fdiv_rn(e, sf)), -7.f), 7.f) + 8.f;
+}
+// the four codes (+ 8) a lane owns of one group; sf != 0
+__device__ __forceinline__ void quant_codes4(const float (&e)[4], float sf, int (&code)[4]) {
+  const float rinv = rcp_approx(sf);
+  float r8[4], dev = 0.f;
 #pragma unroll
   for (int x = 0; x < 4; ++x) {
-    const float qa = e[x] * rinv;
-    r[x] = rintf(qa);
-    margin = fminf(margin, 0.5f - fabsf(qa - r[x]));
+    const float s8 = fmaf(e[x], rinv, 8.f);
+    r8[x] = rintf(s8);
+    dev = fmaxf(dev, fabsf(s8 - r8[x]));
   }
-  if (margin < 0x1p-16f) {                 // rare: a quotient next to a rounding boundary
+  if (dev > 0.5f - 0x1p-16f || sf < 0x1p-14f || sf >= 65504.f) {        // rare
 #pragma unroll
-    for (int x = 0; x < 4; ++x) r[x] = quant_quotient_exact(e[x], sf);
+    for (int x = 0; x < 4; ++x) r8[x] = quant_code_exact(e[x], sf);
   }
 #pragma unroll
-  for (int x = 0; x < 4; ++x) code[x] = (int)fminf(fmaxf(r[x] + 8.f, 1.f), 15.f);      // offset binary: clamp(r, -7, 7) + 8
+  for (int x = 0; x < 4; ++x) code[x] = (int)r8[x];
 }
 __device__ __forceinline__ __half quant_scale(float amax) {
   float s32 = __fdiv_rn(amax, 7.0f);
@@ -394,9 +398,8 @@ __device__ __forceinline__ void reconstruct_quantise(const int z, const __nv_bfl
           uint8_t* blk = row ? rb.blk : ra.blk;
           const __half s = quant_scale(amax);
           const float sf = __half2float(s);
-          const float rinv = sf == 0.f ? 0.f : rcp_approx(sf);
-          int code[4];
-          quant_codes4(e, sf, rinv, code);
+          int code[4] = {8, 8, 8, 8};                  // sf == 0 (amax / 7 rounds to zero in fp16): codes 0
+          if (sf != 0.f) quant_codes4(e, sf, code);
           if (z == 0) {
             kw[row] |= ((uint32_t)code[0] << (8 * gg)) | ((uint32_t)code[1] << (16 + 8 * gg)) |
                        ((uint32_t)code[2] << (8 * gg + 4)) | ((uint32_t)code[3] << (16 + 8 * gg + 4));
