@@ -157,6 +157,17 @@ int dwkv_export_tokens(dwkv_cache* c, int32_t seq_id, int64_t t0, int64_t n, con
  * clear memory; the whole arena, caller-owned or not, is cleared once by dwkv_create). Synchronises the device. */
 int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id);
 
+/* Re-tiering of the stored tokens of one sequence (SURVEY.md section 8f NEXT-4 "re-tiering"; "adaptive threshold chosen
+ * to satisfy the current memory budget"; reading A29): every token gets the class (new_tier[t], new_flag[t]), which
+ * may only LOWER it: new_tier[t] <= tier[t] and new_flag[t] <= flag[t]. A stored coefficient vector is the leading-r_t part of
+ * B (x / gate) (reading A13), so a lower tier is the truncation to its leading r' entries -- bit for bit what an append at that tier
+ * would have stored -- and a cleared flag drops the int4 residual; raising a token would need its original vector, which is gone.
+ * The tokens keep their order; slots are renumbered per class, the records move to pages of their new classes (device-side gather +
+ * scatter of the stored bytes, 8-bit coefficient planes re-blocked exactly) and the old pages return to the pool. Enqueues on
+ * `stream`. new_tier, new_flag: HOST uint8 [dwkv_seq_len]. Needs free pages for the whole new layout while the old one is still
+ * held (CAPACITY otherwise, nothing changed). Errors: INVALID (NULL, a raised tier / flag), STATE (poisoned handle), CAPACITY, CUDA. */
+int dwkv_retier_seq(dwkv_cache* c, int32_t seq_id, const uint8_t* new_tier /*host*/, const uint8_t* new_flag /*host*/, void* stream);
+
 /* Attention-output probe, Eq. (3) (reading A25): for one sequence and
  * layer and n_q probed query positions, the attention output over the compressed cache is compared with the output over a
  * "temporarily materialized higher-fidelity cache" the caller provides for that layer:

@@ -20,8 +20,9 @@ What it computes (plain definition, fp64, token-ordered storage, no blocking / f
   Routing (reading A15): class = 2*tier + flag, slot = number of earlier tokens of the sequence in that class.
 
 Inputs are the stored numbers (bf16 / fp16 / int4 values held exactly in float64 / float16 / int8 arrays).
-Pins: tests/test_oracle_pins.py (P1-P10, P12, P13 of SURVEY.md §8c) and tests/test_oracle_pins_windows.py (P14 hand-derived
-append case with two depth windows, P15 / P16 multi-window decode and append against loop-built references). The paper prints no worked numeric example
+Pins: tests/test_oracle_pins.py (P1-P10, P12, P13 of SURVEY.md §8c), tests/test_oracle_pins_windows.py (P14 hand-derived
+append case with two depth windows, P15 / P16 multi-window decode and append against loop-built references) and tests/test_retier.py
+(OracleCache.retier, reading A29: against a fresh append at the lower tier, a closed form of the change of K-hat, brute-force slots). The paper prints no worked numeric example
 of this path, so Eq. (3)'s 0.027 and the 72.8 tok/s are *parity unpinned* (out of scope, need real activations).
 """
 from __future__ import annotations
@@ -228,6 +229,25 @@ class OracleCache:
                         residV=resid["V"][fidx] if len(fidx) else None)
 
     # -- reconstruction and attention ------------------------------------------------------------------------
+    # -- re-tiering of stored tokens (reading A29): lowering only ---------------------------
+    def retier(self, s, new_tier, new_flag):
+        """Every token of sequence s gets the class (new_tier[t], new_flag[t]) <= its stored one. The stored coefficient vector is
+        the leading-r_t part of B (x / gate), so the lower tier keeps its leading r' entries; a cleared flag drops the residual.
+        Token order is kept and the slots are renumbered per class (route_slots from an empty sequence)."""
+        S = self._seq(s)
+        new_tier = np.asarray(new_tier, np.uint8)
+        new_flag = np.asarray(new_flag, np.uint8)
+        assert len(new_tier) == len(S["tier"]) == len(new_flag)
+        assert np.all(new_tier <= S["tier"]) and np.all(new_flag <= S["flag"]), "re-tiering only lowers a token"
+        ranks = np.asarray(self.tier_ranks)[new_tier]                                    # [n]
+        keep = np.arange(self.r)[None, :] < ranks[:, None]                                # [n, r]
+        for z in "KV":
+            S["c" + z] = np.where(keep[:, None, None, :], S["c" + z], 0.0)
+            S["code" + z] = np.where(new_flag[:, None, None, None] != 0, S["code" + z], 0).astype(np.int8)
+            S["scale" + z] = np.where(new_flag[:, None, None, None] != 0, S["scale" + z], 0).astype(np.float16)
+        S["tier"], S["flag"] = new_tier, new_flag
+        S["cls"], S["slot"], S["counts"] = route_slots(new_tier, new_flag, len(self.tier_ranks), None)
+
     def khat_vhat(self, s, l, h):
         """K-hat, V-hat in R^{T x d} for sequence s, layer l, kv head h (Eq. 1)."""
         S = self._seq(s)

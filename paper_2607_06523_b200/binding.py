@@ -24,7 +24,7 @@ EXPORTED = [
     "dwkv_launch_count", "dwkv_get_stat", "dwkv_last_error", "dwkv_dense_workspace_bytes", "dwkv_dense_decode_attention",
     "dwkv_build_basis", "dwkv_export_basis", "dwkv_probe_error", "dwkv_route_tokens", "dwkv_router_thresholds",
     "dwkv_probe_token_stats", "dwkv_controller_create", "dwkv_controller_destroy", "dwkv_controller_step", "dwkv_controller_state",
-    "dwkv_controller_thresholds", "dwkv_dense_decode_attention_static",
+    "dwkv_controller_thresholds", "dwkv_dense_decode_attention_static", "dwkv_retier_seq",
 ]
 
 
@@ -83,6 +83,7 @@ def _load() -> C.CDLL:
     lib.dwkv_append_raw.argtypes = [vp, i32, i32, vp, vp, C.POINTER(dwkv_raw_tokens), vp]
     lib.dwkv_export_tokens.argtypes = [vp, i32, i64, i64, C.POINTER(dwkv_token_dump), vp]
     lib.dwkv_reset_seq.argtypes = [vp, i32]
+    lib.dwkv_retier_seq.argtypes = [vp, i32, vp, vp, vp]
     lib.dwkv_seq_len.argtypes = [vp, i32]
     lib.dwkv_seq_len.restype = i64
     lib.dwkv_footprint.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
@@ -231,6 +232,14 @@ class DwkvCache:
 
     def reset_seq(self, seq_id: int):
         _check(lib.dwkv_reset_seq(self._h, seq_id))
+
+    def retier_seq(self, seq_id: int, new_tier, new_flag):
+        """Lower the class of stored tokens (dwkv_retier_seq): new_tier / new_flag host uint8 [seq_len], element-wise <= the stored ones."""
+        t, f = _u8(new_tier), _u8(new_flag)
+        n = self.seq_len(seq_id)
+        if len(t) != n or len(f) != n:
+            raise ValueError(f"retier_seq needs {n} tiers and flags")
+        _check(lib.dwkv_retier_seq(self._h, seq_id, t.ctypes.data, f.ctypes.data, _stream()))
 
     def seq_len(self, seq_id: int) -> int:
         n = lib.dwkv_seq_len(self._h, seq_id)

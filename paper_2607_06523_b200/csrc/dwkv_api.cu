@@ -153,7 +153,7 @@ struct dwkv_cache {
   int64_t total_tokens = 0;
   uint64_t version = 0;
   // scratch
-  DevBuf part, plan3_dev, tokdst_dev, basis_scratch, probe_ws, segcnt;
+  DevBuf part, plan3_dev, tokdst_dev, basis_scratch, probe_ws, segcnt, retier_ws;
   size_t segcnt_zeroed = 0;          // leading bytes of segcnt known to be zero (the finishing CTAs reset what they use)
   uint64_t opt_epoch = 0;            // bumped by every dwkv_set_option: a cached plan is reused only under the options it was built with
   std::vector<uint32_t> seq_stamp;   // duplicate-id check of a call in O(n): stamp per sequence slot
@@ -392,7 +392,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gK) cudaFree(c->gK);
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
-  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release(); c->segcnt.release();
+  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release(); c->segcnt.release(); c->retier_ws.release();
   c->ring.release();
   for (int i = 0; i < dwkv_cache::kScanRing; ++i) {
     if (c->ev_scan0[i]) cudaEventDestroy(c->ev_scan0[i]);
@@ -627,6 +627,80 @@ int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id) {
   }
   S.tier.clear(); S.flag.clear(); S.slot.clear();
   c->version++;
+  return DWKV_OK;
+}
+
+int dwkv_retier_seq(dwkv_cache* c, int32_t seq_id, const uint8_t* new_tier, const uint8_t* new_flag, void* stream) {
+  if (!c || !new_tier || !new_flag) return fail(DWKV_E_INVALID, "NULL argument");
+  if (check_seq(c, seq_id)) return fail(DWKV_E_INVALID, "bad sequence id");
+  if (c->poisoned) return fail(DWKV_E_STATE, kPoisonMsg);
+  cudaSetDevice(c->cfg.device);
+  SeqState& S = c->seqs[seq_id];
+  const int64_t n = (int64_t)S.tier.size();
+  if (n == 0) return DWKV_OK;
+  if (n > 0x7fffffff) return fail(DWKV_E_INVALID, "too many tokens");
+  bool same = true;
+  int64_t add[kMaxClasses] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (int64_t i = 0; i < n; ++i) {
+    if (new_tier[i] > S.tier[i] || new_flag[i] > S.flag[i])
+      return fail(DWKV_E_INVALID, "re-tiering only lowers a token: new_tier <= tier and new_flag <= flag (the original vector is gone)");
+    same = same && new_tier[i] == S.tier[i] && new_flag[i] == S.flag[i];
+    add[2 * new_tier[i] + new_flag[i]]++;
+  }
+  if (same) return DWKV_OK;
+  int64_t need = 0;
+  for (int k = 0; k < c->n_classes; ++k) need += (add[k] + c->cl[k].tokens_per_page - 1) / c->cl[k].tokens_per_page;
+  if (need > (int64_t)c->free_pages.size())      // the old pages are released only after the move
+    return fail(DWKV_E_CAPACITY, "re-tiering needs " + std::to_string(need) + " free pages for the new layout, " +
+                                     std::to_string(c->free_pages.size()) + " are free");
+  cudaStream_t st = (cudaStream_t)stream;
+  const CacheGeom& g = c->geom;
+  const size_t LH = (size_t)g.L * g.H;
+  const int64_t kChunkTok = 1024;
+  const size_t per_tok = LH * ((size_t)g.r * 2 * 2 + (size_t)(g.d / 2) * 2 + (size_t)(g.d / 16) * 2 * 2);
+  CU_OK(c->retier_ws.reserve((size_t)std::min<int64_t>(n, kChunkTok) * per_tok));
+  CU_OK(c->tokdst_dev.reserve((size_t)std::min<int64_t>(n, kChunkTok) * sizeof(TokDst)));
+
+  PoisonGuard guard(c);
+  guard.arm();
+  SeqState old = std::move(S);
+  S = SeqState();
+  c->total_tokens -= n;
+  std::vector<TokDst> dst_new, dst_old;
+  std::vector<int32_t> new_pages;
+  int ridx = 0;
+  route_commit(c, seq_id, (int32_t)n, new_tier, new_flag, &ridx, &dst_new, &new_pages);
+  for (int64_t t0 = 0; t0 < n; t0 += kChunkTok) {
+    const int64_t m = std::min(kChunkTok, n - t0);
+    uint8_t* w = (uint8_t*)c->retier_ws.p;
+    DumpPtrs o;
+    o.coefK = (__nv_bfloat16*)w; w += (size_t)m * LH * g.r * 2;
+    o.coefV = (__nv_bfloat16*)w; w += (size_t)m * LH * g.r * 2;
+    o.codeK = w; w += (size_t)m * LH * (g.d / 2);
+    o.codeV = w; w += (size_t)m * LH * (g.d / 2);
+    o.scaleK = (__half*)w; w += (size_t)m * LH * (g.d / 16) * 2;
+    o.scaleV = (__half*)w;
+    o.deqK = o.deqV = nullptr;
+    stored_token_table(c, old, t0, m, &dst_old);
+    int rc = upload(c, c->tokdst_dev, dst_old.data(), dst_old.size() * sizeof(TokDst), st);
+    if (rc) return rc;
+    c->launches += launch_gather(c->arena, g, (const TokDst*)c->tokdst_dev.p, (int)m, o, st);
+    for (int64_t i = 0; i < m; ++i) dst_new[(size_t)(t0 + i)].ridx = new_flag[t0 + i] ? (int32_t)i : -1;    // row of the chunk's dump
+    rc = upload(c, c->tokdst_dev, dst_new.data() + t0, (size_t)m * sizeof(TokDst), st);
+    if (rc) return rc;
+    c->launches += launch_scatter_raw(c->arena, g, (const TokDst*)c->tokdst_dev.p, (int)m, o.coefK, o.coefV, nullptr, nullptr, o.codeK,
+                                      o.codeV, o.scaleK, o.scaleV, st);
+    CU_OK(cudaGetLastError());
+  }
+  // the old pages go back to the pool, cleared, in stream order behind the reads above
+  std::vector<int32_t> returned;
+  for (int k = 0; k < kMaxClasses; ++k)
+    for (auto it = old.pages[k].rbegin(); it != old.pages[k].rend(); ++it) returned.push_back(*it);
+  int rc = zero_pages(c, returned, st);
+  if (rc) return rc;
+  for (int32_t pg : returned) c->free_pages.push_back(pg);
+  c->version++;
+  guard.disarm();
   return DWKV_OK;
 }
 
