@@ -292,7 +292,9 @@ int dwkv_controller_thresholds(const dwkv_controller* ctl, int32_t n_tiers, cons
  *     mass[t]  += sum_hq p[hq, t]                 spike[t] = max(spike[t], max_hq p[hq, t])
  * so that calling it on every probe step accumulates phi_0 and phi_1 of Eq. (2) on the device. Token order = append order.
  *   q     dev bf16 [H_q, d]        mass, spike   dev fp32 [T], T = dwkv_seq_len (read-modify-write; zero them before the first probe)
- * Enqueues on `stream`; scratch is owned by the handle. Errors: INVALID, STATE (no basis / gates), EMPTY (T = 0), CUDA. */
+ * Enqueues on `stream`; scratch is owned by the handle, and so is the sequence's device-resident token table (where each token lives
+ * and its class id), of which a call uploads only the entries of tokens appended since the last probe.
+ * Errors: INVALID, STATE (no basis / gates), EMPTY (T = 0), CUDA. */
 int dwkv_probe_token_stats(dwkv_cache* c, int32_t layer, int32_t seq_id, const void* q, float* mass, float* spike, void* stream);
 
 /* ---- dense bf16 comparison kernel (BASELINE.json "from-scratch dense-bf16-cache decode kernel")

@@ -51,6 +51,20 @@ struct DevBuf {
     if (e == cudaSuccess) cap = want;
     return e;
   }
+  // grow to at least `bytes`, keeping the first `keep` bytes (device-to-device copy on `st`, then the old block is freed:
+  // cudaFree waits for the copy)
+  cudaError_t grow_keep(size_t bytes, size_t keep, cudaStream_t st) {
+    if (bytes <= cap) return cudaSuccess;
+    size_t want = std::max(std::max(bytes, 2 * cap), (size_t)4096);
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, want);
+    if (e != cudaSuccess) return e;
+    if (p && keep) e = cudaMemcpyAsync(q, p, keep, cudaMemcpyDeviceToDevice, st);
+    if (p) cudaFree(p);
+    p = q;
+    cap = want;
+    return e;
+  }
   void release() {
     if (p) cudaFree(p);
     p = nullptr;
@@ -112,6 +126,11 @@ struct SeqState {
   std::vector<int32_t> slot;
   int64_t count[kMaxClasses] = {0, 0, 0, 0, 0, 0, 0, 0};
   std::vector<int32_t> pages[kMaxClasses];
+  // device-resident token table: entry t = where token t lives (page, block, slot) and its class id (2 * tier + flag), in append
+  // order; the probe kernels walk it. Maintained incrementally: a probe uploads only the entries of the tokens appended since the
+  // last one (stored tokens never move, except through dwkv_retier_seq / dwkv_reset_seq, which invalidate it).
+  DevBuf tok_dev;
+  int64_t tok_dev_n = 0;
 };
 
 struct Plan3 {                    // plan of the fused persistent decode kernel (dwkv_scan3*.cuh)
@@ -277,6 +296,16 @@ int upload(dwkv_cache* c, DevBuf& dst, const void* src, size_t bytes, cudaStream
   return DWKV_OK;
 }
 
+int upload_to(dwkv_cache* c, void* dptr, const void* src, size_t bytes, cudaStream_t st) {      // through the pinned staging ring
+  void* h;
+  int slot;
+  CU_OK(c->ring.acquire(bytes, &h, &slot));
+  memcpy(h, src, bytes);
+  CU_OK(cudaMemcpyAsync(dptr, h, bytes, cudaMemcpyHostToDevice, st));
+  CU_OK(c->ring.mark(slot, st));
+  return DWKV_OK;
+}
+
 // where the stored tokens [t0, t0 + n) of a sequence live: the table the gather / token-statistics kernels walk
 void stored_token_table(const dwkv_cache* c, const SeqState& S, int64_t t0, int64_t n, std::vector<TokDst>* out) {
   out->resize((size_t)n);
@@ -392,6 +421,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gK) cudaFree(c->gK);
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
+  for (SeqState& S : c->seqs) S.tok_dev.release();
   c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release(); c->segcnt.release(); c->retier_ws.release();
   c->ring.release();
   for (int i = 0; i < dwkv_cache::kScanRing; ++i) {
@@ -626,6 +656,7 @@ int dwkv_reset_seq(dwkv_cache* c, int32_t seq_id) {
     CU_OK(cudaDeviceSynchronize());
   }
   S.tier.clear(); S.flag.clear(); S.slot.clear();
+  S.tok_dev_n = 0;
   c->version++;
   return DWKV_OK;
 }
@@ -665,6 +696,8 @@ int dwkv_retier_seq(dwkv_cache* c, int32_t seq_id, const uint8_t* new_tier, cons
   guard.arm();
   SeqState old = std::move(S);
   S = SeqState();
+  S.tok_dev = old.tok_dev;          // the device token table's block moves to the new state; its entries are rebuilt by the next probe
+  old.tok_dev = DevBuf();
   c->total_tokens -= n;
   std::vector<TokDst> dst_new, dst_old;
   std::vector<int32_t> new_pages;
@@ -1131,17 +1164,21 @@ extern "C" int dwkv_probe_token_stats(dwkv_cache* c, int32_t layer, int32_t seq_
   if (layer < 0 || layer >= c->geom.L) return fail(DWKV_E_INVALID, "layer out of range");
   if (check_seq(c, seq_id)) return fail(DWKV_E_INVALID, "bad sequence id");
   if (!c->basis_set || !c->gates_set) return fail(DWKV_E_STATE, "basis and gates must be set before the probe");
-  const SeqState& S = c->seqs[seq_id];
+  SeqState& S = c->seqs[seq_id];
   const int64_t T = (int64_t)S.tier.size();
   if (T == 0) return fail(DWKV_E_EMPTY, "token statistics of an empty sequence");
   if (T > 0x7fffffff) return fail(DWKV_E_INVALID, "sequence too long");
   cudaStream_t st = (cudaStream_t)stream;
-  std::vector<TokDst> dst;
-  stored_token_table(c, S, 0, T, &dst);
-  int rc = upload(c, c->tokdst_dev, dst.data(), dst.size() * sizeof(TokDst), st);
-  if (rc) return rc;
+  if (S.tok_dev_n < T) {        // bring the device-resident token table up to date: only the tokens appended since the last probe
+    std::vector<TokDst> dst;
+    stored_token_table(c, S, S.tok_dev_n, T - S.tok_dev_n, &dst);
+    CU_OK(S.tok_dev.grow_keep((size_t)T * sizeof(TokDst), (size_t)S.tok_dev_n * sizeof(TokDst), st));
+    int rc = upload_to(c, (uint8_t*)S.tok_dev.p + (size_t)S.tok_dev_n * sizeof(TokDst), dst.data(), dst.size() * sizeof(TokDst), st);
+    if (rc) return rc;
+    S.tok_dev_n = T;
+  }
   CU_OK(c->probe_ws.reserve(token_stats_scratch_bytes(c->geom, T)));
-  c->launches += launch_token_stats(c->arena, c->geom, (const TokDst*)c->tokdst_dev.p, (int)T, layer, (const __nv_bfloat16*)q, c->BK, c->gK,
+  c->launches += launch_token_stats(c->arena, c->geom, (const TokDst*)S.tok_dev.p, (int)T, layer, (const __nv_bfloat16*)q, c->BK, c->gK,
                                     c->softmax_scale * 1.4426950408889634f, (float*)c->probe_ws.p, mass, spike, st);
   CU_OK(cudaGetLastError());
   return DWKV_OK;

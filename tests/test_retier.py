@@ -139,6 +139,10 @@ def test_gpu_retier_against_oracle(mod, name):
     oc = oracle_from_kept(wl, consts, routings, kept)
     rng = np.random.default_rng(5)
     used0 = cache.footprint()["used_bytes"]
+    q0 = gen.make_q(wl, device="cuda")
+    for s, (tier, flag) in enumerate(routings):       # a probe before the move: the device-resident token table now holds the old places
+        m = torch.zeros(len(tier), dtype=torch.float32, device="cuda"); sp = torch.zeros_like(m)
+        cache.probe_token_stats(0, s, q0[s, 0].contiguous(), m, sp)
     for s, (tier, flag) in enumerate(routings):
         nt = np.minimum(tier, rng.integers(0, len(wl.tier_ranks), len(tier))).astype(np.uint8)
         nf = (flag & (rng.random(len(flag)) < 0.5)).astype(np.uint8)
@@ -162,6 +166,13 @@ def test_gpu_retier_against_oracle(mod, name):
     for s in ids:
         for l in range(wl.L):
             check_output(out[s, l], ref[s, l], oc.max_abs_vhat(s, l), f"retier {name} seq {s} layer {l}")
+    from test_gpu_controller import oracle_stats
+    for s, (tier, flag) in enumerate(routings):       # ... and after it the table is rebuilt: statistics of the moved records
+        m = torch.zeros(len(tier), dtype=torch.float32, device="cuda"); sp = torch.zeros_like(m)
+        cache.probe_token_stats(wl.L - 1, s, q0[s, wl.L - 1].contiguous(), m, sp)
+        m_o, sp_o = oracle_stats(oc, wl, s, wl.L - 1, f64(q0[s, wl.L - 1]))
+        np.testing.assert_allclose(m.double().cpu().numpy(), m_o, rtol=3e-3, atol=1e-7)
+        np.testing.assert_allclose(sp.double().cpu().numpy(), sp_o, rtol=3e-3, atol=1e-7)
     # a raised tier is refused and changes nothing; an identity call is a no-op
     tier0 = oc.seqs[0]["tier"].copy()
     if tier0.min() < len(wl.tier_ranks) - 1:
