@@ -200,11 +200,6 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *   "n_slices"        planner: number of warp slices the step is cut into, 0 (default) = one per warp of the persistent grid,
  *                     fewer (2..7 per SM) when the call is so small that a slice would stream less than ~40 KB
  *   "combine_warps"   combine kernel: warps per (segment, query head): 1, 4 or 16; 0 (default) = by the partials per segment
- *   "fuse_combine"    where the split-combine (step a3) runs: 0 (default) = the separate combine kernel; 1 = fused into the decode
- *                     kernel (the warps of a CTA take consecutive slices and merge their partials in shared memory, every record
- *                     written is an arrival on its segment's counter, the CTA of the last arrival merges, back-projects and writes
- *                     `out`: one launch per call); 2 = the CTA-level merge + the combine kernel. 1 and 2 are parity-tested but
- *                     measured slower than 0 on B200 for all-layer and per-layer calls
  *   "interleave"      planner: 1 = interleave the classes of a sequence in the work order, 0 = class after class,
  *                     -1 (default) = interleave when G > 4 or the call lists one sequence
  *   "cost_coef_pct", "cost_tok", "cost_resid_pct", "flag_cost_pct"   planner cost model (byte-equivalents per coefficient
@@ -229,7 +224,7 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value);
  * calls timed since "time_scan" was last set (at most the last 64), "scan_samples" = how many those are, "scan_ms@i" = sample i of them (0 = oldest). "compress_ms" is the
  * bracket of the append/compress kernel (step a4) of the last dwkv_append_compress. */
 /* Plan of the last dwkv_decode_attention (tests): "plan_slices" = warp slices the work was cut into, "plan_slots" = partial records,
- * "plan_segments" = (sequence, layer, kv head) segments, "plan_fused" = 1 if the call ran with "fuse_combine" = 1. */
+ * "plan_segments" = (sequence, layer, kv head) segments. */
 double dwkv_get_stat(dwkv_cache* c, const char* key);
 
 /* Kernels launched by this handle since creation (bench's gpu_launches claim). */

@@ -138,10 +138,8 @@ struct Plan3 {                    // plan of the fused persistent decode kernel 
   int n_lsel = 0;
   uint64_t version = ~0ull;
   int n_units = 0, n_slices = 0, n_segs = 0, n_slots = 0;
-  size_t off_ustart = 0, off_wentry = 0, off_pstart = 0, off_wlast = 0;
+  size_t off_ustart = 0, off_wentry = 0, off_pstart = 0;
   bool valid = false;
-  bool fuse = false;              // fused split-combine: CTA-contiguous slices, one partial per (CTA, segment), arrival counters
-  int spc = 0;                    // fuse: slices per CTA
   uint64_t opt_epoch = ~0ull;     // planner options the plan was built with (dwkv_set_option bumps the cache's epoch)
   // structure of the cached plan (units without their token counts, sub-blocks per unit): an append that opens no new sub-block
   // leaves the slices, the partial slots and the unit list as they are -- only Unit::ntok changes
@@ -172,8 +170,7 @@ struct dwkv_cache {
   int64_t total_tokens = 0;
   uint64_t version = 0;
   // scratch
-  DevBuf part, plan3_dev, tokdst_dev, basis_scratch, probe_ws, segcnt, retier_ws;
-  size_t segcnt_zeroed = 0;          // leading bytes of segcnt known to be zero (the finishing CTAs reset what they use)
+  DevBuf part, plan3_dev, tokdst_dev, basis_scratch, probe_ws, retier_ws;
   uint64_t opt_epoch = 0;            // bumped by every dwkv_set_option: a cached plan is reused only under the options it was built with
   std::vector<uint32_t> seq_stamp;   // duplicate-id check of a call in O(n): stamp per sequence slot
   uint32_t stamp_gen = 0;
@@ -190,7 +187,6 @@ struct dwkv_cache {
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
   int64_t opt_combine_warps = 0;     // combine kernel: warps per (segment, head): 1 / 4 / 16, 0 = by partials per segment
-  int64_t opt_fuse_combine = 0;      // 0 = separate combine kernel (default), 1 = split-combine fused into the decode kernel, 2 = CTA merge + combine kernel
   int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
   static constexpr int kScanRing = 64;   // "time_scan": the last 64 decode kernels are bracketed, read back without a sync in between
   cudaEvent_t ev_scan0[kScanRing] = {}, ev_scan1[kScanRing] = {}, ev_app0 = nullptr, ev_app1 = nullptr;
@@ -422,7 +418,7 @@ void dwkv_destroy(dwkv_cache* c) {
   if (c->gV) cudaFree(c->gV);
   if (c->d_flag) cudaFree(c->d_flag);
   for (SeqState& S : c->seqs) S.tok_dev.release();
-  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release(); c->segcnt.release(); c->retier_ws.release();
+  c->part.release(); c->plan3_dev.release(); c->tokdst_dev.release(); c->basis_scratch.release(); c->probe_ws.release(); c->retier_ws.release();
   c->ring.release();
   for (int i = 0; i < dwkv_cache::kScanRing; ++i) {
     if (c->ev_scan0[i]) cudaEventDestroy(c->ev_scan0[i]);
@@ -762,7 +758,6 @@ int dwkv_set_option(dwkv_cache* c, const char* key, int64_t value) {
   if (!strcmp(key, "max_unit_blocks")) c->opt_max_unit_blocks = value;
   else if (!strcmp(key, "time_scan")) { c->opt_time_scan = value; c->scan_samples = 0; }
   else if (!strcmp(key, "combine_warps")) c->opt_combine_warps = value;
-  else if (!strcmp(key, "fuse_combine")) c->opt_fuse_combine = value;
   else if (!strcmp(key, "sketch_umma")) c->opt_sketch_umma = value;
   else if (!strcmp(key, "n_slices")) c->opt_n_slices = value;
   else if (!strcmp(key, "flag_cost_pct")) c->opt_flag_cost_pct = value;
@@ -793,7 +788,6 @@ double dwkv_get_stat(dwkv_cache* c, const char* key) {
   if (!strcmp(key, "plan_slices")) return c->plan3.valid ? (double)c->plan3.n_slices : -1.0;     // of the last decode call
   if (!strcmp(key, "plan_slots")) return c->plan3.valid ? (double)c->plan3.n_slots : -1.0;
   if (!strcmp(key, "plan_segments")) return c->plan3.valid ? (double)c->plan3.n_segs : -1.0;
-  if (!strcmp(key, "plan_fused")) return c->plan3.valid ? (double)(c->plan3.fuse ? 1 : 0) : -1.0;
   if (!strcmp(key, "scan_samples")) return (double)(c->scan_samples < dwkv_cache::kScanRing ? c->scan_samples : dwkv_cache::kScanRing);
   if (!strncmp(key, "scan_ms@", 8)) {                  // "scan_ms@i": sample i (0 = oldest kept) of the calls timed since "time_scan" was set
     const int64_t n = c->scan_samples < dwkv_cache::kScanRing ? c->scan_samples : dwkv_cache::kScanRing;
@@ -842,13 +836,13 @@ namespace {
 // COST (bytes, flagged bytes weighted by opt_flag_cost_pct) at sub-block granularity, one per warp. A slice touches one or a
 // few segments (b, lh); every (slice, segment) contact yields one partial, numbered contiguously per segment (pstart).
 // Depends on the sequence set, the token counts, the layer count and the options only.
-int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel, bool fuse, cudaStream_t st) {
+int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lsel, cudaStream_t st) {
   Plan3& P = c->plan3;
-  if (P.valid && P.version == c->version && P.n_lsel == n_lsel && P.fuse == fuse && (int)P.seq_ids.size() == n_seqs &&
+  if (P.valid && P.version == c->version && P.n_lsel == n_lsel && (int)P.seq_ids.size() == n_seqs &&
       std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids))
     return DWKV_OK;
   // (the fast path below keeps the old slice cut: only under the same planner options)
-  const bool same_call = P.valid && P.n_lsel == n_lsel && P.fuse == fuse && P.opt_epoch == c->opt_epoch && (int)P.seq_ids.size() == n_seqs &&
+  const bool same_call = P.valid && P.n_lsel == n_lsel && P.opt_epoch == c->opt_epoch && (int)P.seq_ids.size() == n_seqs &&
                          std::equal(P.seq_ids.begin(), P.seq_ids.end(), seq_ids);
   P.valid = false;
   const int LH = n_lsel * c->geom.H;
@@ -856,8 +850,7 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   const double seg_ovh = (double)c->opt_cost_seg;
   // class order inside a sequence: interleaved, every slice sees the sequence's class mix and the cost model drops out of the
   // balance; measured -1.2 % at G = 8 (70B shape) and -1.7 % on a single sequence, neutral (+-0.3 %) on batches at G = 4
-  // (fused combine: the 8 warps of an SM take consecutive slices, so a class-by-class order would give an SM one class only)
-  const bool interleave = c->opt_interleave >= 0 ? c->opt_interleave != 0 : (c->geom.G > 4 || n_seqs == 1 || fuse);
+  const bool interleave = c->opt_interleave >= 0 ? c->opt_interleave != 0 : (c->geom.G > 4 || n_seqs == 1);
   // per-token and per-residual-byte work grows with the query heads per kv head (fits at G = 4: 24 / 235 %, G = 8: 48 / 265 %)
   const double cost_tok = c->opt_cost_tok >= 0 ? (double)c->opt_cost_tok : 6.0 * c->geom.G;
   const double cost_resid_pct = c->opt_cost_resid_pct >= 0 ? (double)c->opt_cost_resid_pct : 205.0 + 7.5 * c->geom.G;
@@ -954,15 +947,8 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   // small calls (one layer of one 64K sequence: 33 MB) are latency bound: with one slice per warp a warp streams < 30 KB and
   // every segment collects ~150 partials; fewer, longer slices (~85 K cost units = ~55 KB each, the same number of warps on
   // every SM) shorten both the scan and the combine (measured: 707 -> 635 us per 32 per-layer calls at batch 1)
-  int W = Wmax, spc = 0;
-  if (fuse) {
-    // fused combine: the 8 warps of a CTA take consecutive slices and merge their partials in shared memory, so the partials per
-    // segment do not grow with the slice count: one slice per warp unless a slice would stream less than ~8 KB
-    spc = Wmax / c->n_sms;
-    if (c->opt_n_slices > 0) spc = (int)std::min<int64_t>(spc, std::max<int64_t>(1, c->opt_n_slices / c->n_sms));
-    else spc = std::min(spc, std::max(1, (int)std::ceil(C / (12e3 * (double)c->n_sms))));
-    W = spc * c->n_sms;
-  } else if (c->opt_n_slices > 0) W = (int)std::min<int64_t>(c->opt_n_slices, Wmax);
+  int W = Wmax;
+  if (c->opt_n_slices > 0) W = (int)std::min<int64_t>(c->opt_n_slices, Wmax);
   else if (C >= 8e6 && C < 50e3 * (double)Wmax && Wmax % c->n_sms == 0) {      // (below ~6 MB everything is launch latency)
     const int per_sm = std::min(Wmax / c->n_sms, std::max(2, (int)std::floor(C / (85e3 * (double)c->n_sms) + 0.5)));
     W = per_sm * c->n_sms;
@@ -1006,58 +992,31 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
     const int b = e.seg / LH;
     return (e.u == ustart[b] && e.sub == 0) ? e.seg - 1 : e.seg;
   };
-  std::vector<int32_t> wentry(4 * (size_t)(NSL + 1), 0), wlast(NSL, 0);
+  std::vector<int32_t> wentry(4 * (size_t)(NSL + 1), 0);
   for (int w = 0; w <= NSL; ++w) {
     wentry[4 * w + 0] = pos[w].seg; wentry[4 * w + 1] = pos[w].u; wentry[4 * w + 2] = pos[w].sub; wentry[4 * w + 3] = 0;
   }
-  if (!fuse) {
-    for (int w = 0; w < NSL; ++w) {
-      if (!less(pos[w], pos[w + 1])) continue;
-      for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) pstart[s + 1]++;
-    }
-    for (int s = 0; s < S_total; ++s) pstart[s + 1] += pstart[s];
-    for (int w = 0; w < NSL; ++w) {
-      if (!less(pos[w], pos[w + 1])) continue;
-      wentry[4 * w + 3] = pstart[pos[w].seg] + seen[pos[w].seg];
-      for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) seen[s]++;
-    }
-  } else {
-    // fused combine: a slice flushes every segment it LEAVES straight to global memory (one arrival each); its last segment goes
-    // to the CTA's shared-memory merge, and the consecutive slices of a CTA that end in the same segment share one record
-    for (int pass = 0; pass < 2; ++pass) {
-      int prev_cta = -1, prev_last = -1, prev_slot = 0;
-      for (int w = 0; w < NSL; ++w) {
-        if (!less(pos[w], pos[w + 1])) continue;
-        const int s0 = pos[w].seg, s1 = last_seg(pos[w + 1]), cta = w / spc;
-        const bool new_group = cta != prev_cta || s1 != prev_last;
-        if (pass == 0) {
-          for (int s = s0; s < s1; ++s) pstart[s + 1]++;
-          if (new_group) pstart[s1 + 1]++;
-        } else {
-          if (s0 < s1) wentry[4 * w + 3] = pstart[s0] + seen[s0]++;
-          for (int s = s0 + 1; s < s1; ++s) seen[s]++;          // the kernel uses the segment's first slot (it is the only contributor)
-          if (new_group) prev_slot = pstart[s1] + seen[s1]++;
-          wlast[w] = prev_slot;
-        }
-        prev_cta = cta; prev_last = s1;
-      }
-      if (pass == 0)
-        for (int s = 0; s < S_total; ++s) pstart[s + 1] += pstart[s];
-    }
+  for (int w = 0; w < NSL; ++w) {
+    if (!less(pos[w], pos[w + 1])) continue;
+    for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) pstart[s + 1]++;
   }
-  // one blob: units | ustart | wentry | pstart | wlast
+  for (int s = 0; s < S_total; ++s) pstart[s + 1] += pstart[s];
+  for (int w = 0; w < NSL; ++w) {
+    if (!less(pos[w], pos[w + 1])) continue;
+    wentry[4 * w + 3] = pstart[pos[w].seg] + seen[pos[w].seg];
+    for (int s = pos[w].seg, s1 = last_seg(pos[w + 1]); s <= s1; ++s) seen[s]++;
+  }
+  // one blob: units | ustart | wentry | pstart
   const size_t sz_units = units.size() * sizeof(Unit);
   P.off_ustart = (sz_units + 15) & ~(size_t)15;
   P.off_wentry = (P.off_ustart + ustart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
   P.off_pstart = (P.off_wentry + wentry.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  P.off_wlast = (P.off_pstart + pstart.size() * sizeof(int32_t) + 15) & ~(size_t)15;
-  const size_t total = P.off_wlast + wlast.size() * sizeof(int32_t);
+  const size_t total = P.off_pstart + pstart.size() * sizeof(int32_t);
   std::vector<uint8_t> blob(total, 0);
   memcpy(blob.data(), units.data(), sz_units);
   memcpy(blob.data() + P.off_ustart, ustart.data(), ustart.size() * sizeof(int32_t));
   memcpy(blob.data() + P.off_wentry, wentry.data(), wentry.size() * sizeof(int32_t));
   memcpy(blob.data() + P.off_pstart, pstart.data(), pstart.size() * sizeof(int32_t));
-  memcpy(blob.data() + P.off_wlast, wlast.data(), wlast.size() * sizeof(int32_t));
   int rc = upload(c, c->plan3_dev, blob.data(), total, st);
   if (rc) return rc;
   P.n_units = n_units; P.n_slices = NSL; P.n_segs = S_total; P.n_slots = pstart[S_total];
@@ -1065,7 +1024,6 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   P.unsub.swap(unsub);
   P.seq_ids.assign(seq_ids, seq_ids + n_seqs);
   P.n_lsel = n_lsel;
-  P.fuse = fuse; P.spc = spc;
   P.opt_epoch = c->opt_epoch;
   P.version = c->version;
   P.valid = true;
@@ -1075,25 +1033,13 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
 int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids, const void* q, float* out, cudaStream_t st) {
   const CacheGeom& g = c->geom;
   const int Lsel = layer < 0 ? g.L : 1, layer0 = layer < 0 ? 0 : layer;
-  // per-layer calls (what a decoder issues) are latency-bound: one launch with the split-combine fused in; an all-layer
-  // call has thousands of segments finishing all through the kernel and keeps the separate combine kernel
-  // 0 = warp partials + combine kernel (default: measured fastest for all-layer AND per-layer calls),
-  // 1 = split-combine fused into the decode kernel (last-arrival epilogue), 2 = CTA-level merge of the partials + combine kernel
-  const int fuse_mode = c->opt_fuse_combine > 0 ? (int)std::min<int64_t>(c->opt_fuse_combine, 2) : 0;
-  const bool fuse = fuse_mode != 0;
-  int rc = build_plan3(c, n_seqs, seq_ids, Lsel, fuse, st);
+  // warp partials + a separate combine kernel, for all-layer and per-layer calls alike: the variants with the split-combine fused
+  // into the decode kernel (last-arrival epilogue, CTA-level merge of the partials) were built, parity-tested and measured slower
+  // (git history before this line's commit holds them)
+  int rc = build_plan3(c, n_seqs, seq_ids, Lsel, st);
   if (rc) return rc;
   const Plan3& P = c->plan3;
   CU_OK(c->part.reserve((size_t)P.n_slots * g.G * (2 + g.r + g.d) * sizeof(float)));
-  if (fuse_mode == 1) {
-    const size_t need = (size_t)P.n_segs * sizeof(int32_t);
-    if (need > c->segcnt.cap) c->segcnt_zeroed = 0;
-    CU_OK(c->segcnt.reserve(need));
-    if (c->segcnt_zeroed < c->segcnt.cap) {      // counters are zero between calls: the CTA that finishes a segment resets its counter
-      CU_OK(cudaMemsetAsync(c->segcnt.p, 0, c->segcnt.cap, st));
-      c->segcnt_zeroed = c->segcnt.cap;
-    }
-  }
   const uint8_t* blob = (const uint8_t*)c->plan3_dev.p;
   Scan3Params sp;
   sp.arena = c->arena;
@@ -1110,10 +1056,6 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   sp.cscale = c->softmax_scale * 1.4426950408889634f;
   sp.zero = 0.f;
   sp.i8 = g.i8;
-  sp.fuse = fuse_mode; sp.spc = P.spc;
-  sp.wlast = (const int32_t*)(blob + P.off_wlast);
-  sp.segcnt = (int32_t*)c->segcnt.p;
-  sp.BV = c->BV; sp.gV = c->gV; sp.out = out;
   const int ev_i = (int)(c->scan_samples % dwkv_cache::kScanRing);
   if (c->opt_time_scan) {
     if (!c->ev_scan0[ev_i]) { CU_OK(cudaEventCreate(&c->ev_scan0[ev_i])); CU_OK(cudaEventCreate(&c->ev_scan1[ev_i])); }
@@ -1125,7 +1067,6 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   CU_OK(lerr);
   c->launches += n;
   if (c->opt_time_scan) { CU_OK(cudaEventRecord(c->ev_scan1[ev_i], st)); ++c->scan_samples; }
-  if (fuse_mode == 1) { CU_OK(cudaGetLastError()); return DWKV_OK; }
   Combine3Params cp;
   cp.pstart = sp.pstart; cp.part = sp.part; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
   cp.layer0 = layer0; cp.Lq = Lsel; cp.LH = sp.LH; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;

@@ -41,16 +41,6 @@ struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.c
   float cscale;                // softmax_scale * log2(e)
   float zero;                  // 0.0f (an operand the compiler cannot constant-fold)
   int32_t i8;                  // 8-bit coefficient planes (dwkv_layout.cuh)
-  // fused split-combine (step a3 inside the decode kernel; per-layer calls): the warps of a CTA take CONSECUTIVE slices, merge their
-  // end-of-slice partials per segment in shared memory and write one partial per (CTA, segment); every partial written is an arrival
-  // on the segment's counter, and the CTA of the last arrival merges the segment's partials, back-projects and writes `out`.
-  int32_t fuse;                // 1 = fused combine (no combine3 launch), 0 = partials only
-  int32_t spc;                 // fuse: slices per CTA (1..8); slice of warp w of CTA c = c * spc + w
-  const int32_t* wlast;        // fuse: [n_slices] partial slot of the slice's last segment (shared by the warps of a CTA that end in it)
-  int32_t* segcnt;             // fuse: [n_segs] arrival counters, zero between calls (the finishing CTA resets them)
-  const __nv_bfloat16* BV;     // fuse: [M][H][r][d]
-  const __nv_bfloat16* gV;     // fuse: [L][H][d]
-  float* out;                  // fuse: [n_seqs][Lq][Hq][d]
 };
 
 struct Combine3Params {

@@ -223,165 +223,11 @@ __device__ __forceinline__ void process_stage(State<NKB, D>& st, const uint32_t 
   if (nfull < n) process_sub<NK, RESID, NKB, D, PAIR, I8, true>(st, sp + nfull * SB1, ntok - nfull * SUBTOK, lane, q, cscale);
 }
 
-// ---- fused split-combine (step a3 inside the decode kernel; per-layer calls) ---------------------------------------------------
-// Every partial record written to global memory is one ARRIVAL on its segment's counter; a segment expects pstart[seg + 1] -
-// pstart[seg] arrivals. The CTA that brings the last one merges the segment's partials (log-sum-exp), back-projects through B_V and
-// the gate and writes the output (the classic fence + counter pattern: writers fence before the atomic, the finisher after it).
-constexpr int kTodoCap = 32;     // segments a CTA can have to finish: <= 2 shared segments per slice + one per end-of-slice group
-
-__device__ __forceinline__ void seg_coords(const Scan3Params& p, const int seg, int& b, int& layer, int& h) {
-  b = seg / p.LH;
-  const int lh = seg - b * p.LH;
-  layer = p.layer0 + lh / p.H; h = lh % p.H;
-}
-
-// o = (gV * (BV^T a) + e) / l for the G query heads of a segment with ONE partial record (at `rec`), by one warp. Used when the
-// warp (or its CTA group) is the segment's only contributor: no counter, no shared memory.
-template <int D>
-__device__ __noinline__ void finalize_single(const Scan3Params& p, const int seg, const float* rec, const int lane) {
-  constexpr int CPL = D / 32;
-  int b, layer, h;
-  seg_coords(p, seg, b, layer, h);
-  const int r = p.r, PR = 2 + p.r + D;
-  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D + lane * CPL;
-  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D + lane * CPL;
-  float gv[CPL];
-#pragma unroll
-  for (int c = 0; c < CPL; c += 2) { const float2 f = bf2(ldg32(gVp + c)); gv[c] = f.x; gv[c + 1] = f.y; }
-  for (int gq = 0; gq < p.G; ++gq) {
-    const float* rc = rec + (size_t)gq * PR;
-    const float inv = 1.f / __ldcg(rc + 1);
-    float acc[CPL];
-#pragma unroll
-    for (int c = 0; c < CPL; ++c) acc[c] = 0.f;
-#pragma unroll 8
-    for (int j = 0; j < r; ++j) {
-      const float aj = __ldcg(rc + 2 + j);
-#pragma unroll
-      for (int c = 0; c < CPL; c += 2) {
-        const float2 f = bf2(ldg32(BV + (size_t)j * D + c));
-        acc[c] = fmaf(aj, f.x, acc[c]); acc[c + 1] = fmaf(aj, f.y, acc[c + 1]);
-      }
-    }
-    float* o = p.out + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * p.G) + (size_t)h * p.G + gq) * D + lane * CPL;
-#pragma unroll
-    for (int c = 0; c < CPL; c += 2) {
-      const float2 e = __ldcg(reinterpret_cast<const float2*>(rc + 2 + r + lane * CPL + c));
-      *reinterpret_cast<float2*>(o + c) = make_float2((gv[c] * acc[c] + e.x) * inv, (gv[c + 1] * acc[c + 1] + e.y) * inv);
-    }
-  }
-}
-
-// The same for a segment with n >= 1 partials, by the 256 threads of a CTA. This code runs once per segment at the very end of the
-// kernel, so it is COLD: every new 128-byte line of instructions costs an L2 round trip (~0.14 us measured), and a dependent
-// global load another ~0.8 us. It is therefore written as a few short rolled loops: the partial records, the basis block and the
-// gate row are brought into the (drained) ring memory by fire-and-forget cp.async copies, everything else works from shared memory.
-// `scratch`: the CTA's dynamic shared memory (16-byte aligned), `scratch_bytes` long. All 256 threads must call it.
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-template <int D>
-__device__ __noinline__ void finalize_cta(const Scan3Params& p, const int seg, uint8_t* scratch, const int scratch_bytes) {
-  constexpr int NT = kWarps * 32;
-  const int tid = threadIdx.x;
-  int b, layer, h;
-  seg_coords(p, seg, b, layer, h);
-  const int G = p.G, r = p.r, PR = 2 + p.r + D, GPR = G * PR;
-  const int P0 = __ldg(p.pstart + seg), n = __ldg(p.pstart + seg + 1) - P0;
-  // shared memory: [basis r x D bf16][gate D bf16][m* G (8)][weights n x G][merged record G x PR][partial records, 16-byte image]
-  __nv_bfloat16* sm_B = reinterpret_cast<__nv_bfloat16*>(scratch);
-  __nv_bfloat16* sm_g = sm_B + r * D;
-  float* sm_star = reinterpret_cast<float*>(sm_g + D);
-  float* sm_w = sm_star + 8;
-  float* sm_rec = sm_w + ((n * G + 3) & ~3);
-  uint8_t* sm_part = reinterpret_cast<uint8_t*>(sm_rec + ((GPR + 3) & ~3));
-  const int room = scratch_bytes - (int)(sm_part - scratch) - 32;
-  const int cap_n = max(1, room / (GPR * 4));                   // partial records per round
-  const __nv_bfloat16* BV = p.BV + ((size_t)(layer / p.w) * p.H + h) * (size_t)r * D;
-  const __nv_bfloat16* gVp = p.gV + ((size_t)layer * p.H + h) * D;
-  const uint8_t* gpart = reinterpret_cast<const uint8_t*>(p.part + (size_t)P0 * GPR);
-  auto copy_round = [&](const int k0, const int nr) -> int {      // records [k0, k0 + nr) -> sm_part; returns the image's byte offset
-    const uint8_t* lo = gpart + (size_t)k0 * GPR * 4;
-    const int mis = (int)(reinterpret_cast<uintptr_t>(lo) & 15);
-    const int nchunk = (mis + nr * GPR * 4 + 15) >> 4;
-    for (int i = tid; i < nchunk; i += NT) cp_async16(smem_u32(sm_part) + 16 * i, lo - mis + 16 * (size_t)i);
-    return mis;
-  };
-  int mis = copy_round(0, min(n, cap_n));
-  for (int i = tid; i < (r * D + D) / 8; i += NT) {             // basis block + gate row (16-byte chunks)
-    const bool isg = i >= r * D / 8;
-    cp_async16(smem_u32(sm_B) + 16 * i, isg ? (const void*)(gVp + 8 * (i - r * D / 8)) : (const void*)(BV + 8 * i));
-  }
-  asm volatile("cp.async.commit_group;" ::: "memory");
-  if (tid < G) sm_star[tid] = __int_as_float((int)0x80800000u);      // order-preserving integer key of -inf
-  __syncthreads();
-  for (int i = tid; i < n * G; i += NT) {                        // maxima of all partials (one load each), m* per head
-    const int k = i / G, hq = i - k * G;
-    const float m = __ldcg(p.part + (size_t)(P0 + k) * GPR + hq * PR);
-    sm_w[i] = m;
-    atomicMax(reinterpret_cast<int*>(sm_star + hq), __float_as_int(m) >= 0 ? __float_as_int(m) : (int)(0x80000000u - (uint32_t)__float_as_int(m)));
-  }
-  __syncthreads();
-  for (int i = tid; i < n * G; i += NT) {                        // weights 2^(m_k - m*)
-    const int ik = __float_as_int(sm_star[i % G]);
-    const float mstar = __int_as_float(ik >= 0 ? ik : (int)(0x80000000u - (uint32_t)ik));
-    const float m = sm_w[i];
-    sm_w[i] = (m == -INFINITY) ? 0.f : ex2(m - mstar);
-  }
-  for (int c = tid; c < GPR; c += NT) sm_rec[c] = 0.f;
-  for (int k0 = 0; k0 < n; k0 += cap_n) {
-    const int nr = min(cap_n, n - k0);
-    if (k0 > 0) { mis = copy_round(k0, nr); asm volatile("cp.async.commit_group;" ::: "memory"); }
-    asm volatile("cp.async.wait_all;" ::: "memory");
-    __syncthreads();
-    const float* img = reinterpret_cast<const float*>(sm_part + mis);
-    for (int c = tid; c < GPR; c += NT) {                        // element c of the flat record: head c / PR
-      const int hq = c / PR;
-      float acc = sm_rec[c];
-      for (int k = 0; k < nr; ++k) acc = fmaf(sm_w[(k0 + k) * G + hq], img[k * GPR + c], acc);
-      sm_rec[c] = acc;
-    }
-    __syncthreads();
-  }
-  float* out = p.out + (((size_t)b * p.Lq + (p.Lq == 1 ? 0 : layer)) * (size_t)(p.H * G) + (size_t)h * G) * D;
-  for (int pp = tid; pp < G * (D / 2); pp += NT) {               // back-projection: channel pairs over the threads
-    const int gq = pp / (D / 2), ch = 2 * (pp - gq * (D / 2));
-    const float* rc = sm_rec + gq * PR;
-    float a0 = 0.f, a1 = 0.f;
-    for (int j = 0; j < r; ++j) {
-      const float2 f = bf2(*reinterpret_cast<const uint32_t*>(sm_B + j * D + ch));
-      a0 = fmaf(rc[2 + j], f.x, a0); a1 = fmaf(rc[2 + j], f.y, a1);
-    }
-    const float inv = 1.f / rc[1];                               // element 0 of a head (the weighted sum of the m's) is not used
-    const float2 gv = bf2(*reinterpret_cast<const uint32_t*>(sm_g + ch));
-    *reinterpret_cast<float2*>(out + (size_t)gq * D + ch) = make_float2((gv.x * a0 + rc[2 + r + ch]) * inv, (gv.y * a1 + rc[2 + r + ch + 1]) * inv);
-  }
-  if (tid == 0) p.segcnt[seg] = 0;       // ready for the next call (which starts after this grid has completed)
-  __syncthreads();
-}
-
-// one arrival on `seg` by a warp that has just written the record at `rec` (all lanes call); a sole contributor finishes the
-// segment at once, the last of several queues it for the CTA
-template <int D>
-__device__ __forceinline__ void arrive(const Scan3Params& p, const int seg, const float* rec, const int lane, int* sh_ntodo, int* sh_todo) {
-  const int expect = __ldg(p.pstart + seg + 1) - __ldg(p.pstart + seg);
-  __syncwarp();
-  if (expect == 1) { finalize_single<D>(p, seg, rec, lane); return; }
-  __threadfence();
-  __syncwarp();
-  if (lane == 0 && atomicAdd(p.segcnt + seg, 1) == expect - 1) {
-    __threadfence();
-    const int i = atomicAdd(sh_ntodo, 1);
-    if (i < kTodoCap) sh_todo[i] = seg;
-  }
-}
-
-template <int NKB, int D, bool PAIR, bool I8, bool FUSE>
+template <int NKB, int D, bool PAIR, bool I8>
 __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_constant__ Scan3Params p) {
   using RG = Ring<NKB, D>;
   constexpr int SLOT = RG::SLOT, NS = RG::NS;
   extern __shared__ __align__(128) uint8_t smem[];
-  __shared__ int sh_seg[kWarps], sh_ntodo, sh_todo[kTodoCap];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t ring = smem_u32(smem) + warp * kWarpSmem;
   const uint32_t descs = ring + kRingBytes, bars = descs + kMaxSlots * 16;
@@ -390,22 +236,19 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  if (threadIdx.x == 0) sh_ntodo = 0;
-  if constexpr (FUSE) __syncthreads(); else __syncwarp();
-  // fuse: the warps of a CTA take consecutive slices (their partials meet in shared memory); else consecutive slices go to different SMs
-  const int gw = FUSE ? (warp < p.spc ? (int)blockIdx.x * p.spc + warp : p.n_slices) : warp * (int)gridDim.x + (int)blockIdx.x;
+  __syncwarp();
+  const int gw = warp * (int)gridDim.x + (int)blockIdx.x;       // consecutive slices go to different SMs
   int4 ws = make_int4(0, 0, 0, 0), we = ws;
   bool active = gw < p.n_slices;
   if (active) {
     ws = __ldg(p.wentry + gw); we = __ldg(p.wentry + gw + 1);
     active = !(ws.x == we.x && ws.y == we.y && ws.z == we.z);
   }
-  if (!FUSE && !active) { cudaGridDependencySynchronize(); return; }
+  if (!active) { cudaGridDependencySynchronize(); return; }
 
   State<NKB, D> st;
   int cur_seg = -1, slot_next = 0, n_entered = 0;
   const int PRG = p.G * (2 + p.r + D);
-  if (active) {
   // ---- fetch cursor (warp-uniform) over the slice [ws, we) of the linear order ----------------------------------------------
   int f_seg = ws.x, f_u = ws.y, f_sub = ws.z;
   int f_b = f_seg / p.LH, f_lh = f_seg - f_b * p.LH;
@@ -489,7 +332,6 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
       prologue_load<NKB, D, PAIR>(pl, p, seg, lane);       // L2 hits: the fetch cursor prefetched them when it crossed over
       float* rec = p.part + (size_t)slot_next * (size_t)PRG;
       flush_partial<NKB, D, PAIR>(st, p, rec, lane);
-      if constexpr (FUSE) { if (p.fuse == 1) arrive<D>(p, cur_seg, rec, lane, &sh_ntodo, sh_todo); }
       slot_next = __ldg(p.pstart + seg);       // a segment entered inside a slice is entered at its start: its first slot
       prologue_compute<NKB, D, PAIR, I8>(q, pl, p, seg, lane);
       state_reset<NKB, D>(st, p.zero);
@@ -520,81 +362,25 @@ __global__ void __launch_bounds__(kWarps * 32, 1) scan3_kernel(const __grid_cons
     __syncwarp();
     k_c = (k_c + 1 == NS) ? 0 : k_c + 1;
   }
-  if constexpr (!FUSE) flush_partial<NKB, D, PAIR>(st, p, p.part + (size_t)slot_next * (size_t)PRG, lane);
+  flush_partial<NKB, D, PAIR>(st, p, p.part + (size_t)slot_next * (size_t)PRG, lane);
   if (p.stamps && lane == 0) {       // measurement aid: when did this warp finish (planner cost-model fits)
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     p.stamps[gw] = t;
     p.stamps[p.n_slices + gw] = (unsigned long long)n_entered;     // segments this slice touched
   }
-  } else {
-    cudaGridDependencySynchronize();
-  }
-  if constexpr (!FUSE) return;
-
-  // ---- fused combine: end-of-slice partials meet in the (drained) rings, one record per (CTA, segment) goes to global memory ------
-  float* ent = reinterpret_cast<float*>(smem + (size_t)warp * kWarpSmem);
-  if (active) flush_partial<NKB, D, PAIR>(st, p, ent, lane);
-  if (lane == 0) sh_seg[warp] = active ? cur_seg : -1;
-  __syncthreads();
-  {   // every run of warps that ended in the same segment: all 256 threads merge its records (float2 columns of the flat G * PR
-      // record) and write ONE record to global memory; thread 0 brings the arrival
-    const int PR = 2 + p.r + D, GPR = p.G * PR, ncol = GPR / 2, tid = threadIdx.x;
-    for (int w0 = 0; w0 < kWarps; ++w0) {
-      const int sg = sh_seg[w0];
-      if (sg < 0) continue;
-      bool first = true;
-      for (int w2 = 0; w2 < w0; ++w2) first = first && (sh_seg[w2] != sg);
-      if (!first) continue;
-      const int slot = __ldg(p.wlast + ((int)blockIdx.x * p.spc + w0));
-      float* rec = p.part + (size_t)slot * (size_t)GPR;
-      for (int c = tid; c < ncol; c += kWarps * 32) {
-        const int hq = (2 * c) / PR;
-        const bool ml = 2 * c == hq * PR;
-        float mstar = -INFINITY;
-        for (int w2 = w0; w2 < kWarps; ++w2)
-          if (sh_seg[w2] == sg) mstar = fmaxf(mstar, reinterpret_cast<const float*>(smem + (size_t)w2 * kWarpSmem)[hq * PR]);
-        float2 acc = make_float2(0.f, 0.f);
-        for (int w2 = w0; w2 < kWarps; ++w2) {
-          if (sh_seg[w2] != sg) continue;
-          const float* e2 = reinterpret_cast<const float*>(smem + (size_t)w2 * kWarpSmem);
-          const float mk = e2[hq * PR];
-          const float wk = (mk == -INFINITY) ? 0.f : ex2(mk - mstar);
-          const float2 v = *reinterpret_cast<const float2*>(e2 + 2 * c);
-          acc.x = fmaf(wk, ml ? 0.f : v.x, acc.x);
-          acc.y = fmaf(wk, v.y, acc.y);
-        }
-        if (ml) acc.x = mstar;
-        *reinterpret_cast<float2*>(rec + 2 * c) = acc;
-      }
-      if (p.fuse != 1) continue;       // CTA merge only: the separate combine kernel finishes the segments
-      __threadfence();
-      __syncthreads();
-      if (tid == 0) {
-        const int expect = __ldg(p.pstart + sg + 1) - __ldg(p.pstart + sg);
-        if (expect == 1 || atomicAdd(p.segcnt + sg, 1) == expect - 1) {
-          __threadfence();
-          const int i = atomicAdd(&sh_ntodo, 1);
-          if (i < kTodoCap) sh_todo[i] = sg;
-        }
-      }
-    }
-  }
-  __syncthreads();
-  const int n_todo = min(sh_ntodo, kTodoCap);
-  for (int i = 0; i < n_todo; ++i) finalize_cta<D>(p, sh_todo[i], smem, kWarps * kWarpSmem);
 }
 
 // cudaFuncSetAttribute is per device: remember which devices this instance has been prepared on
-template <int NKB, int D, bool PAIR, bool I8, bool FUSE>
-cudaError_t launch_instance2(const Scan3Params& p, int n_sms, cudaStream_t s) {
+template <int NKB, int D, bool PAIR, bool I8>
+cudaError_t launch_instance(const Scan3Params& p, int n_sms, cudaStream_t s) {
   const int smem = kWarps * kWarpSmem;
   static bool attr_set[64] = {};
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-    e = cudaFuncSetAttribute(scan3_kernel<NKB, D, PAIR, I8, FUSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    e = cudaFuncSetAttribute(scan3_kernel<NKB, D, PAIR, I8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     if (e != cudaSuccess) return e;
     if (dev >= 0 && dev < 64) attr_set[dev] = true;
   }
@@ -608,12 +394,7 @@ cudaError_t launch_instance2(const Scan3Params& p, int n_sms, cudaStream_t s) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, scan3_kernel<NKB, D, PAIR, I8, FUSE>, p);
-}
-
-template <int NKB, int D, bool PAIR, bool I8>
-cudaError_t launch_instance(const Scan3Params& p, int n_sms, cudaStream_t s) {
-  return p.fuse ? launch_instance2<NKB, D, PAIR, I8, true>(p, n_sms, s) : launch_instance2<NKB, D, PAIR, I8, false>(p, n_sms, s);
+  return cudaLaunchKernelEx(&cfg, scan3_kernel<NKB, D, PAIR, I8>, p);
 }
 
 // returns false if no instance exists for the basis rank; *err receives the launch status otherwise
