@@ -199,7 +199,7 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *   "unit_kb"         planner: target size of a work unit per (layer, head), KB (default 64 = one page stripe)
  *   "n_slices"        planner: number of warp slices the step is cut into, 0 (default) = one per warp of the persistent grid,
  *                     fewer (2..7 per SM) when the call is so small that a slice would stream less than ~40 KB
- *   "combine_warps"   combine kernel: warps per (segment, query head): 1, 4 or 16; 0 (default) = by the partials per segment
+ *   "combine_warps"   combine kernel: warps per (segment, query head): 1 or 4; 0 (default) = by the partials per segment
  *   "interleave"      planner: 1 = interleave the classes of a sequence in the work order, 0 = class after class,
  *                     -1 (default) = interleave when G > 4 or the call lists one sequence
  *   "cost_coef_pct", "cost_tok", "cost_resid_pct", "flag_cost_pct"   planner cost model (byte-equivalents per coefficient

@@ -186,7 +186,7 @@ struct dwkv_cache {
   int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
-  int64_t opt_combine_warps = 0;     // combine kernel: warps per (segment, head): 1 / 4 / 16, 0 = by partials per segment
+  int64_t opt_combine_warps = 0;     // combine kernel: warps per (segment, head): 1 / 4, 0 = by partials per segment
   int64_t opt_sketch_umma = 1;       // basis sketch: 1 = tcgen05 kernel (d = 128), 0 = mma.sync kernel
   static constexpr int kScanRing = 64;   // "time_scan": the last 64 decode kernels are bracketed, read back without a sync in between
   cudaEvent_t ev_scan0[kScanRing] = {}, ev_scan1[kScanRing] = {}, ev_app0 = nullptr, ev_app1 = nullptr;
@@ -1070,9 +1070,11 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   Combine3Params cp;
   cp.pstart = sp.pstart; cp.part = sp.part; cp.BV = c->BV; cp.gV = c->gV; cp.out = out;
   cp.layer0 = layer0; cp.Lq = Lsel; cp.LH = sp.LH; cp.w = g.w; cp.H = g.H; cp.G = g.G; cp.r = g.r; cp.d = g.d;
-  const int split = (c->opt_combine_warps == 1 || c->opt_combine_warps == 4 || c->opt_combine_warps == 16)
-                        ? (int)c->opt_combine_warps
-                        : (P.n_slots > 64LL * P.n_segs ? 16 : (P.n_slots > 8LL * P.n_segs ? 4 : 1));
+  // more than ~8 partials per segment (per-layer calls): the 4 warps of a CTA share one head's partial list; a 16-warp shape was
+  // carried until the combine's dependent round trips were cut to two, after which it lost everywhere (per-layer step at batch 1:
+  // 614 us against 582 us with 4 warps) and was removed
+  const int split = (c->opt_combine_warps == 1 || c->opt_combine_warps == 4) ? (int)c->opt_combine_warps
+                                                                             : (P.n_slots > 8LL * P.n_segs ? 4 : 1);
   c->launches += launch_combine3(cp, P.n_segs, split, st, &lerr);
   CU_OK(lerr);
   CU_OK(cudaGetLastError());

@@ -23,8 +23,8 @@ using namespace dwkv::dev;
 // dozen (segment, head) pairs: the merge is a chain of dependent L2 round trips, so its time is set by the partials per warp. !SPLIT: one CTA per segment, warp w merges
 // heads w, w+4 on its own -- for all-layer steps (1-6 partials per segment, thousands of segments). Lanes run over rank
 // columns for a*, over channels (D / 32 each) for e* and the back-projection.
-template <int D, int S>      // S = warps sharing one head's partial list: 1 (no split), 4 or 16
-__global__ void __launch_bounds__(S > 4 ? 32 * S : 128) combine3_kernel(const Combine3Params p) {
+template <int D, int S>      // S = warps sharing one head's partial list: 1 (no split) or 4
+__global__ void __launch_bounds__(128) combine3_kernel(const Combine3Params p) {
   constexpr bool SPLIT = S > 1;
   constexpr int CPL = D / 32;                       // channels per lane
   __shared__ float sh_l[S];
@@ -197,8 +197,8 @@ int launch_scan3(const Scan3Params& p, int n_sms, cudaStream_t s, cudaError_t* e
 
 int launch_combine3(const Combine3Params& p, int n_segs, int split, cudaStream_t s, cudaError_t* err) {
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = split > 1 ? dim3(n_segs, p.G) : dim3(n_segs);       // split: 16 warps share the partial list of one head
-  cfg.blockDim = dim3(split > 4 ? 32 * split : 128);
+  cfg.gridDim = split > 1 ? dim3(n_segs, p.G) : dim3(n_segs);       // split: the CTA's 4 warps share the partial list of one head
+  cfg.blockDim = dim3(128);
   cfg.dynamicSmemBytes = 0;
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
@@ -207,12 +207,10 @@ int launch_combine3(const Combine3Params& p, int n_segs, int split, cudaStream_t
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if (p.d == 128) {
-    if (split == 16) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 16>, p);
-    else if (split == 4) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 4>, p);
+    if (split == 4) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 4>, p);
     else *err = cudaLaunchKernelEx(&cfg, combine3_kernel<128, 1>, p);
   } else {
-    if (split == 16) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 16>, p);
-    else if (split == 4) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 4>, p);
+    if (split == 4) *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 4>, p);
     else *err = cudaLaunchKernelEx(&cfg, combine3_kernel<64, 1>, p);
   }
   return 1;

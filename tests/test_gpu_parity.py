@@ -150,7 +150,7 @@ def test_split_invariance_p11(mod):
     outs, shapes = [], []
     base = {"max_unit_blocks": 0, "n_slices": 0, "interleave": 0, "unit_kb": 64, "combine_warps": 0}
     for change in ({"max_unit_blocks": 1}, {"n_slices": 1}, {"n_slices": 7}, {"interleave": 1, "unit_kb": 1}, {"interleave": -1},
-                   {"n_slices": 296, "combine_warps": 16}, {"combine_warps": 4}, {"combine_warps": 1, "n_slices": 592},
+                   {"n_slices": 296, "combine_warps": 4}, {"combine_warps": 4}, {"combine_warps": 1, "n_slices": 592},
                    {"n_slices": 148, "max_unit_blocks": 1}, {}):
         for k, v in {**base, **change}.items():
             cache.set_option(k, v)
