@@ -179,7 +179,7 @@ struct dwkv_cache {
   Plan3 plan3;
   // options
   int64_t opt_max_unit_blocks = 0;   // 0 = adaptive
-  int64_t opt_cost_coef_pct = 80, opt_cost_tok = -1, opt_cost_resid_pct = -1, opt_cost_seg = 40000;   // planner cost model (-1 = by G)
+  int64_t opt_cost_coef_pct = 80, opt_cost_tok = -1, opt_cost_resid_pct = -1, opt_cost_seg = 65000;   // planner cost model (-1 = by G)
   int64_t opt_interleave = -1;       // planner: 1 = interleave the classes of a sequence, 0 = class after class, -1 = by shape
   int64_t opt_stamps_ptr = 0;        // device pointer [2 * n_slices] u64 for per-warp end stamps + segment counts (measurement aid), 0 = off
   int64_t opt_unit_kb = 64;          // planner: target bytes of a work unit (per layer-head), KB
