@@ -1056,6 +1056,7 @@ int decode3(dwkv_cache* c, int32_t layer, int32_t n_seqs, const int32_t* seq_ids
   sp.cscale = c->softmax_scale * 1.4426950408889634f;
   sp.zero = 0.f;
   sp.i8 = g.i8;
+  sp.rot = (n_seqs == 1 && Lsel > 1) ? 53 : 0;
   const int ev_i = (int)(c->scan_samples % dwkv_cache::kScanRing);
   if (c->opt_time_scan) {
     if (!c->ev_scan0[ev_i]) { CU_OK(cudaEventCreate(&c->ev_scan0[ev_i])); CU_OK(cudaEventCreate(&c->ev_scan1[ev_i])); }

@@ -41,6 +41,7 @@ struct Scan3Params {            // fused persistent decode kernel (dwkv_scan3*.c
   float cscale;                // softmax_scale * log2(e)
   float zero;                  // 0.0f (an operand the compiler cannot constant-fold)
   int32_t i8;                  // 8-bit coefficient planes (dwkv_layout.cuh)
+  int32_t rot;                 // rotation of the block index per warp in the slice numbering (0, or 53 for single-sequence all-layer calls)
 };
 
 struct Combine3Params {
