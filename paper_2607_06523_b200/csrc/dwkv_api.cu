@@ -183,7 +183,7 @@ struct dwkv_cache {
   int64_t opt_interleave = -1;       // planner: 1 = interleave the classes of a sequence, 0 = class after class, -1 = by shape
   int64_t opt_stamps_ptr = 0;        // device pointer [2 * n_slices] u64 for per-warp end stamps + segment counts (measurement aid), 0 = off
   int64_t opt_unit_kb = 64;          // planner: target bytes of a work unit (per layer-head), KB
-  int64_t opt_flag_cost_pct = 100;   // planner weight of flagged-class bytes, percent
+  int64_t opt_flag_cost_pct = 85;    // planner weight of flagged-class bytes, percent (100 until the residual-K products shared their A operand)
   int64_t opt_n_slices = 0;          // 0 = one slice per warp of the persistent grid
   int64_t opt_time_scan = 0;
   int64_t opt_combine_warps = 0;     // combine kernel: warps per (segment, head): 1 / 4, 0 = by partials per segment
