@@ -201,7 +201,7 @@ int dwkv_footprint(const dwkv_cache* c, uint64_t* used_bytes, uint64_t* reserved
  *                     fewer (2..7 per SM) when the call is so small that a slice would stream less than ~40 KB
  *   "combine_warps"   combine kernel: warps per (segment, query head): 1 or 4; 0 (default) = by the partials per segment
  *   "interleave"      planner: 1 = interleave the classes of a sequence in the work order, 0 = class after class,
- *                     -1 (default) = interleave when G > 4 or the call lists one sequence
+ *                     -1 (default) = interleave when G > 4 or the call lists at most four sequences
  *   "cost_coef_pct", "cost_tok", "cost_resid_pct", "flag_cost_pct"   planner cost model (byte-equivalents per coefficient
  *                     byte in %, per token, per residual byte in %, extra weight of flagged classes in %)
  *   "coef_int8"       1 = store the coefficients "in 8-bit blockwise quantized form" (

@@ -850,7 +850,8 @@ int build_plan3(dwkv_cache* c, int32_t n_seqs, const int32_t* seq_ids, int n_lse
   const double seg_ovh = (double)c->opt_cost_seg;
   // class order inside a sequence: interleaved, every slice sees the sequence's class mix and the cost model drops out of the
   // balance; measured -1.2 % at G = 8 (70B shape) and -1.7 % on a single sequence, neutral (+-0.3 %) on batches at G = 4
-  const bool interleave = c->opt_interleave >= 0 ? c->opt_interleave != 0 : (c->geom.G > 4 || n_seqs == 1);
+  // (re-measured at the end of round 2 on per-layer calls: -2 % at batch 2, -4 % at batch 4, +2 % at batch 8; all-layer -0.3 % throughout)
+  const bool interleave = c->opt_interleave >= 0 ? c->opt_interleave != 0 : (c->geom.G > 4 || n_seqs <= 4);
   // per-token and per-residual-byte work grows with the query heads per kv head (fits at G = 4: 24 / 235 %, G = 8: 48 / 265 %)
   const double cost_tok = c->opt_cost_tok >= 0 ? (double)c->opt_cost_tok : 6.0 * c->geom.G;
   const double cost_resid_pct = c->opt_cost_resid_pct >= 0 ? (double)c->opt_cost_resid_pct : 205.0 + 7.5 * c->geom.G;
